@@ -1,0 +1,126 @@
+/*
+ * dfjk.h -- C ABI of the B200-native density-fitted Coulomb/exchange (JK) build.
+ *
+ * The operation is the "JK call" of arxiv 2505.03755, section 2.D.i:
+ *   "the input is a density matrix and the AO ... Cholesky vectors and the output is J and K"
+ *   (PAPER.md:148), with
+ *      rho_P     = sum_{mu,nu} b^P_{mu nu} D_{mu nu}                        Eq. 14
+ *      J_{mu nu} = sum_P rho_P b^P_{mu nu}                                  Eq. 15
+ *      X^P_{mu i} = sum_lam b^P_{mu lam} C_{lam i}      Eq. 16 with gamma = C n C^T;
+ *                                                       the half-transform of Eq. 18
+ *      K_{mu nu} = sum_P sum_i n_i X^P_{mu i} X^P_{nu i}                    Eq. 17
+ *   for every density set s, D_s = C_s diag(n_s) C_s^T.  The Cholesky vectors are "stored in
+ *   triangular form of size Naux*Nao(Nao+1)/2" and unpacked on the GPU; they are
+ *   kept resident on the GPU across calls; a call allocates nothing and never
+ *   blocks the host; init/destroy pair as in PAPER.md:227,242.
+ *
+ * Everything is fp64.  All matrices are row-major (C order).  Every step runs in hand-written
+ * CUDA kernels for sm_100a; there is no CPU fallback and no library GEMM.
+ *
+ * Threading: one in-flight call per handle (calls on one handle must be stream-ordered);
+ * different handles are independent.  No function throws, aborts or prints.
+ */
+#ifndef DFJK_H
+#define DFJK_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dfjk_ctx* dfjk_handle; /* opaque */
+
+/* CUDA stream, passed as an opaque pointer so that this header needs no CUDA include
+ * (it is a cudaStream_t / CUstream; NULL is the legacy default stream). */
+typedef void* dfjk_stream;
+
+enum {
+  DFJK_OK = 0,
+  DFJK_ERR_INVALID_ARG = 1,      /* NULL / shape / nocc[s] outside [0,nao] / capacity exceeded / misaligned B */
+  DFJK_ERR_ALLOC = 2,            /* device or host allocation failed (create only) */
+  DFJK_ERR_CUDA = 3,             /* a CUDA call or launch failed; text via dfjk_last_error() */
+  DFJK_ERR_UNSUPPORTED_ARCH = 4  /* the current device is not compute capability 10.x */
+};
+
+/* All fields optional; zero = default.  Pass NULL for all defaults. */
+typedef struct {
+  size_t workspace_cap_bytes; /* cap for the half-transformed block X (step a8);
+                                 default 1 GiB.  nblk = floor(cap / bytes of one aux row of X) >= 1 */
+  int nblk;                   /* force the aux block size N_blk; 0 = derive from cap */
+  int max_nocc_total;         /* capacity for sum_s nocc[s]; 0 = nao */
+  int max_nset;               /* capacity for nset; 0 = 8 */
+  int copy_B;                 /* 0 = borrow the caller's device pointer (default); 1 = private copy */
+  int ksplit;                 /* force the split-K factor of the SYRK; 0 = automatic */
+} dfjk_options;
+
+/*
+ * dfjk_create -- bind a resident packed tensor and allocate every scratch buffer (step a0).
+ *   naux, nao   sizes, naux >= 0, nao >= 1.
+ *   B_packed    DEVICE pointer, naux * nao(nao+1)/2 doubles, 16-byte aligned.  Aux index P slowest,
+ *               then the row-major lower triangle: B[P][mu(mu+1)/2 + nu], mu >= nu.
+ *               Borrowed unless opt->copy_B: it must stay valid and unchanged until dfjk_destroy.
+ *   opt         options or NULL.
+ *   out         receives the handle.
+ * Allocates on the CURRENT device; may synchronise.  Returns DFJK_OK or an error code (then
+ * *out = NULL).
+ */
+int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* opt, dfjk_handle* out);
+
+/*
+ * dfjk_get_jk -- J and K of nset densities D_s = C_s diag(occ_s) C_s^T (steps a1-a9).
+ *   nset     number of sets, 1 <= nset <= max_nset.
+ *   nocc     HOST array, length nset; 0 <= nocc[s] <= nao, sum <= max_nocc_total.
+ *            nocc[s] = 0 gives J_s = K_s = 0.
+ *   C        DEVICE, blocks [C_0 | C_1 | ...] one after another; block s is row-major
+ *            nao x nocc[s].  Columns need not be orthonormal.
+ *   occ      DEVICE, concatenated occupations, length sum nocc[s]; must be >= 0
+ *            (a negative occupation yields NaN in K_s; J_s is unaffected).
+ *   J_out    DEVICE, nset x nao x nao, or NULL to skip J.
+ *   K_out    DEVICE, nset x nao x nao, or NULL to skip K.
+ *   stream   all work is enqueued on this stream.
+ * Outputs are overwritten (not accumulated), full squares, both triangles, bitwise symmetric, raw
+ * J[D_s], K[D_s] (no factor 1/2, no subtraction: Eq. 13 is the caller's).  The call only
+ * enqueues: it never allocates and never synchronises the host.  Results are deterministic
+ * (bitwise equal from run to run for equal inputs and options).
+ */
+int dfjk_get_jk(dfjk_handle h, int nset, const int* nocc, const double* C, const double* occ,
+                double* J_out, double* K_out, dfjk_stream stream);
+
+/*
+ * dfjk_get_jk_host -- the same call with HOST buffers, as the paper states it: the density
+ * (here C, occ) is pushed, J and K are pulled back ("transfer them back to the
+ * CPU"); B stays resident.  C, occ, J_out, K_out are HOST pointers (pinned memory makes the
+ * copies asynchronous).  Copies in, runs dfjk_get_jk on the handle's staging
+ * buffers, copies out and synchronises `stream` before returning.
+ */
+int dfjk_get_jk_host(dfjk_handle h, int nset, const int* nocc, const double* C, const double* occ,
+                     double* J_out, double* K_out, dfjk_stream stream);
+
+/* Frees everything the handle owns.  dfjk_destroy(NULL) is a no-op returning DFJK_OK. */
+int dfjk_destroy(dfjk_handle h);
+
+/* Static text for an error code. */
+const char* dfjk_strerror(int code);
+
+/* Text of the last CUDA failure seen on this handle ("" if none).  Valid until the next call. */
+const char* dfjk_last_error(dfjk_handle h);
+
+/* Bytes of device scratch the handle owns (excluding a private copy of B). */
+size_t dfjk_workspace_bytes(dfjk_handle h);
+
+/* Plan of the last/next call, for tests and the bench: aux block size, number of aux blocks,
+ * SYRK split-K factor, padded column count of X.  Any pointer may be NULL. */
+int dfjk_get_plan(dfjk_handle h, int* nblk, int* ksplit, int* nocc_pad_capacity);
+
+/* Number of kernel launches dfjk_get_jk enqueued in its last call on this handle. */
+int dfjk_last_launch_count(dfjk_handle h);
+
+/* 1-warp self-test of the DMMA.8x8x4 fragment mapping against a scalar loop on the device
+ * (synchronises).  Returns DFJK_OK if the mapping assumed by the kernels holds. */
+int dfjk_selftest_dmma(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DFJK_H */

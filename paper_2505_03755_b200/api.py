@@ -1,0 +1,201 @@
+"""ctypes binding of include/dfjk.h (same names, marshalling only).
+
+There is no CPU fallback: if libdfjk.so is missing or no CUDA device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as ct
+import os
+from typing import List, Optional, Sequence, Tuple
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_NAME = "libdfjk.so"
+_lib = None
+
+EXPORTS = ["dfjk_create", "dfjk_get_jk", "dfjk_get_jk_host", "dfjk_destroy", "dfjk_strerror",
+           "dfjk_last_error", "dfjk_workspace_bytes", "dfjk_get_plan", "dfjk_last_launch_count",
+           "dfjk_selftest_dmma"]
+
+
+class DFJKError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"dfjk error {code}: {msg}")
+        self.code = code
+
+
+class dfjk_options(ct.Structure):
+    _fields_ = [("workspace_cap_bytes", ct.c_size_t), ("nblk", ct.c_int), ("max_nocc_total", ct.c_int),
+                ("max_nset", ct.c_int), ("copy_B", ct.c_int), ("ksplit", ct.c_int)]
+
+
+def lib_path() -> str:
+    return os.path.join(HERE, _LIB_NAME)
+
+
+def load_library():
+    """Load libdfjk.so (built in-tree by paper_2505_03755_b200.build); fail loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = lib_path()
+    if not os.path.exists(path):
+        raise FileNotFoundError(f"{path} is missing: run `python -m paper_2505_03755_b200.build` "
+                                "(there is no CPU fallback)")
+    lib = ct.CDLL(path)
+    vp, ip, dp = ct.c_void_p, ct.POINTER(ct.c_int), ct.c_void_p
+    lib.dfjk_create.argtypes = [ct.c_int, ct.c_int, dp, ct.POINTER(dfjk_options), ct.POINTER(vp)]
+    lib.dfjk_create.restype = ct.c_int
+    for name in ("dfjk_get_jk", "dfjk_get_jk_host"):
+        fn = getattr(lib, name)
+        fn.argtypes = [vp, ct.c_int, ip, dp, dp, dp, dp, vp]
+        fn.restype = ct.c_int
+    lib.dfjk_destroy.argtypes = [vp]
+    lib.dfjk_destroy.restype = ct.c_int
+    lib.dfjk_strerror.argtypes = [ct.c_int]
+    lib.dfjk_strerror.restype = ct.c_char_p
+    lib.dfjk_last_error.argtypes = [vp]
+    lib.dfjk_last_error.restype = ct.c_char_p
+    lib.dfjk_workspace_bytes.argtypes = [vp]
+    lib.dfjk_workspace_bytes.restype = ct.c_size_t
+    lib.dfjk_get_plan.argtypes = [vp, ip, ip, ip]
+    lib.dfjk_get_plan.restype = ct.c_int
+    lib.dfjk_last_launch_count.argtypes = [vp]
+    lib.dfjk_last_launch_count.restype = ct.c_int
+    lib.dfjk_selftest_dmma.argtypes = []
+    lib.dfjk_selftest_dmma.restype = ct.c_int
+    _lib = lib
+    return lib
+
+
+def _check(lib, code: int, handle=None):
+    if code != 0:
+        msg = lib.dfjk_strerror(code).decode()
+        if handle is not None:
+            extra = lib.dfjk_last_error(handle).decode()
+            if extra:
+                msg += f" ({extra})"
+        raise DFJKError(code, msg)
+
+
+def selftest_dmma() -> None:
+    lib = load_library()
+    _check(lib, lib.dfjk_selftest_dmma())
+
+
+class DFJK:
+    """Handle on a resident packed tensor B (torch CUDA float64, shape (naux, nao(nao+1)/2))."""
+
+    def __init__(self, B_packed, nao: int, *, workspace_cap_bytes: int = 0, nblk: int = 0,
+                 max_nocc_total: int = 0, max_nset: int = 0, copy_B: bool = False, ksplit: int = 0):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("dfjk needs a CUDA device (sm_100); there is no CPU fallback")
+        self._lib = load_library()
+        if not (B_packed.is_cuda and B_packed.dtype == torch.float64 and B_packed.is_contiguous()):
+            raise ValueError("B_packed must be a contiguous CUDA float64 tensor")
+        npair = nao * (nao + 1) // 2
+        if B_packed.dim() != 2 or B_packed.shape[1] != npair:
+            raise ValueError(f"B_packed must have shape (naux, {npair})")
+        self.naux, self.nao, self.npair = int(B_packed.shape[0]), int(nao), npair
+        self._B = None if copy_B else B_packed      # borrowed: keep it alive
+        self._device = B_packed.device
+        opt = dfjk_options(workspace_cap_bytes, nblk, max_nocc_total, max_nset, int(copy_B), ksplit)
+        h = ct.c_void_p()
+        with torch.cuda.device(self._device):
+            code = self._lib.dfjk_create(self.naux, self.nao, ct.c_void_p(B_packed.data_ptr() if self.naux else 0),
+                                         ct.byref(opt), ct.byref(h))
+        _check(self._lib, code)
+        self._h = h
+
+    # -- marshalling helpers
+    @staticmethod
+    def _concat(Cs, occs, nao, device, torch):
+        nocc = [int(o.shape[0]) for o in occs]
+        for c, n in zip(Cs, nocc):
+            if tuple(c.shape) != (nao, n):
+                raise ValueError(f"C block has shape {tuple(c.shape)}, expected {(nao, n)}")
+        if sum(nocc) == 0:
+            z = torch.zeros(1, dtype=torch.float64, device=device)
+            return nocc, z, z
+        C = torch.cat([c.to(device=device, dtype=torch.float64).contiguous().reshape(-1) for c in Cs])
+        occ = torch.cat([o.to(device=device, dtype=torch.float64).reshape(-1) for o in occs])
+        return nocc, C, occ
+
+    def get_jk(self, Cs: Sequence, occs: Sequence, with_j: bool = True, with_k: bool = True,
+               out_j=None, out_k=None, stream=None):
+        """J, K (nset, nao, nao) of D_s = C_s diag(occ_s) C_s^T; enqueue-only on `stream`."""
+        import torch
+        nset = len(Cs)
+        nocc, C, occ = self._concat(Cs, occs, self.nao, self._device, torch)
+        return self.get_jk_raw(nocc, C, occ, with_j, with_k, out_j, out_k, stream)
+
+    def get_jk_raw(self, nocc: List[int], C, occ, with_j=True, with_k=True, out_j=None, out_k=None, stream=None):
+        """Same, with C/occ already concatenated on the device (no torch ops in the call path)."""
+        import torch
+        nset = len(nocc)
+        with torch.cuda.device(self._device):
+            st = stream if stream is not None else torch.cuda.current_stream()
+            J = out_j if out_j is not None else (torch.empty((nset, self.nao, self.nao), dtype=torch.float64, device=self._device) if with_j else None)
+            K = out_k if out_k is not None else (torch.empty((nset, self.nao, self.nao), dtype=torch.float64, device=self._device) if with_k else None)
+            arr = (ct.c_int * max(nset, 1))(*nocc)
+            code = self._lib.dfjk_get_jk(self._h, nset, arr, ct.c_void_p(C.data_ptr()), ct.c_void_p(occ.data_ptr()),
+                                         ct.c_void_p(J.data_ptr() if J is not None else 0),
+                                         ct.c_void_p(K.data_ptr() if K is not None else 0),
+                                         ct.c_void_p(st.cuda_stream))
+        _check(self._lib, code, self._h)
+        return J, K
+
+    def get_jk_host(self, nocc: List[int], C_host, occ_host, J_host=None, K_host=None, stream=None):
+        """dfjk_get_jk_host: C/occ/J/K are HOST (ideally pinned) float64 tensors; synchronises."""
+        import torch
+        nset = len(nocc)
+        with torch.cuda.device(self._device):
+            st = stream if stream is not None else torch.cuda.current_stream()
+            arr = (ct.c_int * max(nset, 1))(*nocc)
+            code = self._lib.dfjk_get_jk_host(self._h, nset, arr, ct.c_void_p(C_host.data_ptr()),
+                                              ct.c_void_p(occ_host.data_ptr()),
+                                              ct.c_void_p(J_host.data_ptr() if J_host is not None else 0),
+                                              ct.c_void_p(K_host.data_ptr() if K_host is not None else 0),
+                                              ct.c_void_p(st.cuda_stream))
+        _check(self._lib, code, self._h)
+        return J_host, K_host
+
+    def plan(self) -> dict:
+        a, b, c = ct.c_int(), ct.c_int(), ct.c_int()
+        _check(self._lib, self._lib.dfjk_get_plan(self._h, ct.byref(a), ct.byref(b), ct.byref(c)))
+        return dict(nblk=a.value, ksplit=b.value, nocc_pad_capacity=c.value)
+
+    @property
+    def workspace_bytes(self) -> int:
+        return int(self._lib.dfjk_workspace_bytes(self._h))
+
+    @property
+    def last_launch_count(self) -> int:
+        return int(self._lib.dfjk_last_launch_count(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.dfjk_destroy(self._h)
+            self._h = None
+            self._B = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+
+def get_jk(B_packed, nao: int, Cs, occs, **kw) -> Tuple:
+    """One-shot convenience: create, get_jk, destroy."""
+    import torch
+    with DFJK(B_packed, nao) as h:
+        J, K = h.get_jk(Cs, occs, **kw)
+        torch.cuda.current_stream().synchronize()
+    return J, K

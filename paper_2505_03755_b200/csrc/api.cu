@@ -1,0 +1,246 @@
+// C ABI of the DF-JK library (include/dfjk.h): handle, validation, planning, enqueue.
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "common.cuh"
+#include "ctx.h"
+
+using namespace dfjk;
+
+namespace {
+
+void set_err(dfjk_ctx* h, const char* where, cudaError_t e) {
+  if (h) snprintf(h->last_error, sizeof(h->last_error), "%s: %s", where, cudaGetErrorString(e));
+}
+
+template <typename T>
+bool dev_alloc(dfjk_ctx* h, T** p, size_t count) {
+  *p = nullptr;
+  if (count == 0) count = 1;
+  cudaError_t e = cudaMalloc((void**)p, count * sizeof(T));
+  if (e != cudaSuccess) {
+    set_err(h, "cudaMalloc", e);
+    cudaGetLastError();
+    return false;
+  }
+  h->workspace_bytes += count * sizeof(T);
+  return true;
+}
+
+void free_all(dfjk_ctx* h) {
+  cudaFree(h->B_owned); cudaFree(h->Ct); cudaFree(h->Dw); cudaFree(h->rho_part); cudaFree(h->rho);
+  cudaFree(h->Jp_part); cudaFree(h->X); cudaFree(h->Kpart);
+  cudaFree(h->C_stage); cudaFree(h->occ_stage); cudaFree(h->J_stage); cudaFree(h->K_stage);
+}
+
+// validate nocc and lay out the padded columns of C'/X
+int build_setinfo(const dfjk_ctx* h, int nset, const int* nocc, SetInfo* si) {
+  if (nset < 1 || nset > h->max_nset || !nocc) return DFJK_ERR_INVALID_ARG;
+  si->nset = nset;
+  long long coff = 0;
+  int ooff = 0, col = 0;
+  for (int s = 0; s < nset; s++) {
+    if (nocc[s] < 0 || nocc[s] > h->nao) return DFJK_ERR_INVALID_ARG;
+    si->col0[s] = col;
+    si->nocc[s] = nocc[s];
+    si->coff[s] = coff;
+    si->ooff[s] = ooff;
+    col += round_up(nocc[s], 8);
+    coff += (long long)h->nao * nocc[s];
+    ooff += nocc[s];
+  }
+  si->col0[nset] = col;
+  si->nocc_pad = col;
+  if (ooff > h->max_nocc_total || col > h->nocc_pad_cap) return DFJK_ERR_INVALID_ARG;
+  return DFJK_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* dfjk_strerror(int code) {
+  switch (code) {
+    case DFJK_OK: return "ok";
+    case DFJK_ERR_INVALID_ARG: return "invalid argument";
+    case DFJK_ERR_ALLOC: return "allocation failed";
+    case DFJK_ERR_CUDA: return "CUDA error";
+    case DFJK_ERR_UNSUPPORTED_ARCH: return "unsupported device architecture (needs sm_100)";
+    default: return "unknown error code";
+  }
+}
+
+int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* opt, dfjk_handle* out) {
+  if (!out) return DFJK_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (naux < 0 || nao < 1 || nao > 32768) return DFJK_ERR_INVALID_ARG;
+  if (naux > 0 && !B_packed) return DFJK_ERR_INVALID_ARG;
+  if (((uintptr_t)B_packed & 15u) != 0) return DFJK_ERR_INVALID_ARG;
+  dfjk_options o;
+  memset(&o, 0, sizeof(o));
+  if (opt) o = *opt;
+  if (o.nblk < 0 || o.max_nocc_total < 0 || o.max_nset < 0 || o.max_nset > kMaxSets || o.ksplit < 0)
+    return DFJK_ERR_INVALID_ARG;
+
+  int dev = 0;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+    cudaGetLastError();
+    return DFJK_ERR_CUDA;
+  }
+  if (prop.major != 10) return DFJK_ERR_UNSUPPORTED_ARCH;
+
+  dfjk_ctx* h = new (std::nothrow) dfjk_ctx;
+  if (!h) return DFJK_ERR_ALLOC;
+  memset(h, 0, sizeof(*h));
+  h->naux = naux; h->nao = nao; h->device = dev;
+  h->npair = (size_t)nao * (nao + 1) / 2;
+  h->nao_k = round_up(nao, kBK);
+  h->max_nset = o.max_nset ? o.max_nset : 8;
+  h->max_nocc_total = o.max_nocc_total ? o.max_nocc_total : nao;
+  h->nocc_pad_cap = round_up(h->max_nocc_total + 7 * h->max_nset, 8);
+  h->n_mtiles = cdiv(nao, 128);
+  h->nblk_forced = o.nblk;
+  h->ksplit_forced = o.ksplit;
+  // split-K partial slots: enough to fill the SMs about three times with one set's tiles
+  {
+    const int ntiles = h->n_mtiles * (h->n_mtiles + 1) / 2;
+    h->ksplit = o.ksplit ? o.ksplit : cdiv(3 * 148, ntiles);
+    if (h->ksplit > 64 && !o.ksplit) h->ksplit = 64;
+  }
+  // X capacity: the cap, but at least one aux row at full column capacity
+  {
+    const size_t cap = o.workspace_cap_bytes ? o.workspace_cap_bytes : ((size_t)1 << 30);
+    const size_t one_row = (size_t)nao * h->nocc_pad_cap;
+    size_t dbl = cap / sizeof(double);
+    if (o.nblk > 0) dbl = (size_t)o.nblk * one_row;
+    if (dbl < one_row) dbl = one_row;
+    const size_t all_rows = (size_t)(naux > 0 ? naux : 1) * one_row;
+    if (dbl > all_rows) dbl = all_rows;
+    h->X_doubles = dbl;
+    h->nblk = (int)(dbl / one_row);
+  }
+  h->j1_chunks = (int)((h->npair + kJ1Chunk - 1) / kJ1Chunk);
+  {
+    const long long xcols = (long long)((h->npair + 2 * kJ2Threads - 1) / (2 * kJ2Threads));
+    long long g = (148LL * 32 + xcols - 1) / xcols;
+    if (g < 1) g = 1;
+    if (g > 16) g = 16;
+    if (g > (naux + 7) / 8) g = (naux + 7) / 8 > 0 ? (naux + 7) / 8 : 1;
+    h->j2_splits = (int)g;
+  }
+  const int naux_pad = round_up(naux > 0 ? naux : 1, kJ1Rows);
+  const size_t n2 = (size_t)nao * nao;
+  bool ok = true;
+  ok = ok && dev_alloc(h, &h->Ct, (size_t)h->nocc_pad_cap * h->nao_k);
+  ok = ok && dev_alloc(h, &h->Dw, (size_t)h->max_nset * h->npair);
+  ok = ok && dev_alloc(h, &h->rho_part, (size_t)h->j1_chunks * 8 * naux_pad);
+  ok = ok && dev_alloc(h, &h->rho, (size_t)h->max_nset * (naux > 0 ? naux : 1));
+  ok = ok && dev_alloc(h, &h->Jp_part, (size_t)h->j2_splits * h->max_nset * h->npair);
+  ok = ok && dev_alloc(h, &h->X, h->X_doubles);
+  ok = ok && dev_alloc(h, &h->Kpart, (size_t)h->ksplit * h->max_nset * n2);
+  ok = ok && dev_alloc(h, &h->C_stage, (size_t)nao * h->max_nocc_total);
+  ok = ok && dev_alloc(h, &h->occ_stage, (size_t)h->max_nocc_total);
+  ok = ok && dev_alloc(h, &h->J_stage, (size_t)h->max_nset * n2);
+  ok = ok && dev_alloc(h, &h->K_stage, (size_t)h->max_nset * n2);
+  if (ok && o.copy_B && naux > 0) {
+    size_t ws = h->workspace_bytes;
+    ok = dev_alloc(h, &h->B_owned, (size_t)naux * h->npair);
+    h->workspace_bytes = ws;
+    if (ok) {
+      cudaError_t e = cudaMemcpy(h->B_owned, B_packed, (size_t)naux * h->npair * sizeof(double), cudaMemcpyDeviceToDevice);
+      if (e != cudaSuccess) { free_all(h); delete h; cudaGetLastError(); return DFJK_ERR_CUDA; }
+    }
+  }
+  if (!ok) { free_all(h); delete h; return DFJK_ERR_ALLOC; }
+  h->B = h->B_owned ? h->B_owned : B_packed;
+  *out = h;
+  return DFJK_OK;
+}
+
+int dfjk_get_jk(dfjk_handle h, int nset, const int* nocc, const double* C, const double* occ, double* J_out,
+                double* K_out, dfjk_stream stream) {
+  if (!h) return DFJK_ERR_INVALID_ARG;
+  SetInfo si;
+  int rc = build_setinfo(h, nset, nocc, &si);
+  if (rc != DFJK_OK) return rc;
+  int ntot = 0;
+  for (int s = 0; s < nset; s++) ntot += nocc[s];
+  if (ntot > 0 && (!C || !occ)) return DFJK_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  h->last_launches = 0;
+  h->last_error[0] = 0;
+  if (!J_out && !K_out) return DFJK_OK;
+  int n = 0, k;
+  n += launch_prep_ct(h, si, C, occ, st);
+  if (J_out) {
+    n += launch_prep_dw(h, si, st);
+    n += launch_j_passes(h, si, J_out, st);
+  }
+  if (K_out) {
+    k = launch_k_path(h, si, K_out, st);
+    if (k < 0) { set_err(h, "k path launch", cudaGetLastError()); return DFJK_ERR_CUDA; }
+    n += k;
+  }
+  h->last_launches = n;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { set_err(h, "kernel launch", e); return DFJK_ERR_CUDA; }
+  return DFJK_OK;
+}
+
+int dfjk_get_jk_host(dfjk_handle h, int nset, const int* nocc, const double* C, const double* occ, double* J_out,
+                     double* K_out, dfjk_stream stream) {
+  if (!h) return DFJK_ERR_INVALID_ARG;
+  SetInfo si;
+  int rc = build_setinfo(h, nset, nocc, &si);
+  if (rc != DFJK_OK) return rc;
+  size_t ntot = 0;
+  for (int s = 0; s < nset; s++) ntot += (size_t)nocc[s];
+  if (ntot > 0 && (!C || !occ)) return DFJK_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaError_t e = cudaSuccess;
+  if (ntot > 0) {
+    e = cudaMemcpyAsync(h->C_stage, C, ntot * h->nao * sizeof(double), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h->occ_stage, occ, ntot * sizeof(double), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) { set_err(h, "H2D copy", e); cudaGetLastError(); return DFJK_ERR_CUDA; }
+  }
+  rc = dfjk_get_jk(h, nset, nocc, h->C_stage, h->occ_stage, J_out ? h->J_stage : nullptr,
+                   K_out ? h->K_stage : nullptr, stream);
+  if (rc != DFJK_OK) return rc;
+  const size_t bytes = (size_t)nset * h->nao * h->nao * sizeof(double);
+  if (J_out) e = cudaMemcpyAsync(J_out, h->J_stage, bytes, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && K_out) e = cudaMemcpyAsync(K_out, h->K_stage, bytes, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) { set_err(h, "D2H copy / sync", e); cudaGetLastError(); return DFJK_ERR_CUDA; }
+  return DFJK_OK;
+}
+
+int dfjk_destroy(dfjk_handle h) {
+  if (!h) return DFJK_OK;
+  free_all(h);
+  delete h;
+  return DFJK_OK;
+}
+
+const char* dfjk_last_error(dfjk_handle h) { return h ? h->last_error : ""; }
+
+size_t dfjk_workspace_bytes(dfjk_handle h) { return h ? h->workspace_bytes : 0; }
+
+int dfjk_get_plan(dfjk_handle h, int* nblk, int* ksplit, int* nocc_pad_capacity) {
+  if (!h) return DFJK_ERR_INVALID_ARG;
+  if (nblk) *nblk = h->plan_nblk ? h->plan_nblk : h->nblk;
+  if (ksplit) *ksplit = h->plan_ksplit ? h->plan_ksplit : h->ksplit;
+  if (nocc_pad_capacity) *nocc_pad_capacity = h->nocc_pad_cap;
+  return DFJK_OK;
+}
+
+int dfjk_last_launch_count(dfjk_handle h) { return h ? h->last_launches : 0; }
+
+int dfjk_selftest_dmma(void) {
+  const int bad = run_dmma_selftest();
+  if (bad < 0) return DFJK_ERR_CUDA;
+  return bad == 0 ? DFJK_OK : DFJK_ERR_UNSUPPORTED_ARCH;
+}
+
+}  // extern "C"

@@ -1,0 +1,70 @@
+// Internal context and kernel-launch prototypes of the DF-JK library (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+
+#include "../../include/dfjk.h"
+
+namespace dfjk {
+
+constexpr int kMaxSets = 32;       // hard upper bound for options.max_nset
+constexpr int kBK = 32;            // k-chunk (doubles) of the DMMA tile pipelines
+constexpr int kJ1Rows = 64;        // aux rows per J-pass-1 work item (8 DMMA row groups per warp)
+constexpr int kJ1SubChunk = 2048;  // pairs per warp per J-pass-1 work item
+constexpr int kJ1Warps = 8;
+constexpr int kJ1Chunk = kJ1SubChunk * kJ1Warps;  // pairs per CTA work item
+constexpr int kJ2Threads = 256;
+
+// Column bookkeeping of one get_jk call: set s owns padded columns [col0[s], col0[s+1]) of C'/X,
+// of which the first nocc[s] are real and the rest zero.
+struct SetInfo {
+  int nset;
+  int nocc_pad;             // col0[nset]
+  int col0[kMaxSets + 1];
+  int nocc[kMaxSets];
+  long long coff[kMaxSets];  // offset of block s inside the caller's C
+  int ooff[kMaxSets];        // offset of set s inside the caller's occ
+};
+
+}  // namespace dfjk
+
+struct dfjk_ctx {
+  int naux, nao;
+  size_t npair;
+  int nao_k;                 // nao rounded up to kBK (k extent of the half-transform)
+  int device;
+  const double* B;           // packed tensor (borrowed or owned)
+  double* B_owned;
+  // options / plan
+  int max_nset, max_nocc_total, nocc_pad_cap;
+  int nblk, ksplit;          // capacities: aux rows of X at nocc_pad_cap columns; split-K partial slots
+  int nblk_forced, ksplit_forced;
+  int plan_nblk, plan_ksplit, plan_nblocks;  // what the last get_jk actually used
+  int n_mtiles;              // 128-row tiles along nao
+  int j1_chunks, j2_splits;
+  // scratch (all allocated at create)
+  double* Ct;                // [nocc_pad_cap][nao_k]     C' transposed, sqrt(occ) folded, zero padded
+  double* Dw;                // [max_nset][npair]         packed density, off-diagonal weight 2
+  double* rho_part;          // [j1_chunks][8][naux_pad]
+  double* rho;               // [max_nset][naux]
+  double* Jp_part;           // [j2_splits][max_nset][npair]
+  double* X;                 // [plan_nblk][nao][nocc_pad] half-transformed block
+  size_t X_doubles;          // capacity of X
+  double* Kpart;             // [ksplit][max_nset][nao][nao]
+  // staging for dfjk_get_jk_host
+  double *C_stage, *occ_stage, *J_stage, *K_stage;
+  size_t workspace_bytes;
+  int last_launches;
+  char last_error[256];
+};
+
+namespace dfjk {
+
+// Each launcher enqueues on `st` and returns the number of kernels it launched.
+int launch_prep_ct(const dfjk_ctx* h, const SetInfo& si, const double* C, const double* occ, cudaStream_t st);
+int launch_prep_dw(const dfjk_ctx* h, const SetInfo& si, cudaStream_t st);
+int launch_j_passes(const dfjk_ctx* h, const SetInfo& si, double* J_out, cudaStream_t st);
+int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, cudaStream_t st);
+int run_dmma_selftest();
+
+}  // namespace dfjk

@@ -1,0 +1,257 @@
+// Steps a2-a4, the Coulomb build (Eq. 14-15), HBM-bandwidth bound:
+//   pass 1  rho[s][P]  = sum_pair B[P][pair] Dw_s[pair]        (one stream over packed B)
+//   pass 2  Jp_s[pair] = sum_P rho[s][P] B[P][pair]            (second stream over packed B)
+//   epilogue: fixed-order sum of the P-split partials and unpack to the full symmetric square.
+// Pass 1 is a (64 aux rows) x (<=8 sets) x (pairs) contraction per warp on DMMA.8x8x4: the
+// row x set accumulators fall out of the MMA fragments, so no per-row shuffle reduction exists,
+// and one Dw fragment is reused against 8 row groups (Dw traffic from L2 = 1/8 of the B stream).
+// The k index of an MMA is free to permute, so each lane reads 16 contiguous bytes (LDG.128).
+#include "common.cuh"
+#include "ctx.h"
+
+namespace dfjk {
+
+template <bool VEC>
+__device__ __forceinline__ double2 load_pair(const double* p) {
+  if (VEC) return ldg_stream2(p);
+  double2 v;
+  v.x = ldg_stream1(p);
+  v.y = ldg_stream1(p + 1);
+  return v;
+}
+
+// grid.x = pair chunk (kJ1Chunk pairs), grid.y = block of 64 aux rows; 8 warps, warp w streams
+// pairs [chunk*kJ1Chunk + w*kJ1SubChunk, +kJ1SubChunk) of its 64 rows.
+template <bool VEC>
+__global__ void __launch_bounds__(kJ1Warps * 32, 2)
+k_j1(const double* __restrict__ B, size_t npair, int naux, const double* __restrict__ Dw, int nsetg,
+     double* __restrict__ part, int naux_pad) {
+  __shared__ double red[kJ1Warps][kJ1Rows][8];
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31, r = l >> 2, j = l & 3;
+  const int p0 = blockIdx.y * kJ1Rows;
+  const size_t kbeg = (size_t)blockIdx.x * kJ1Chunk + (size_t)w * kJ1SubChunk;
+  size_t kend = kbeg + kJ1SubChunk;
+  if (kend > npair) kend = npair;
+
+  const double* rowp[8];
+#pragma unroll
+  for (int g = 0; g < 8; g++) {
+    int row = p0 + 8 * g + r;
+    if (row > naux - 1) row = naux - 1;  // clamped rows land in accumulator rows nobody reads
+    rowp[g] = B + (size_t)row * npair + 2 * j;
+  }
+  const bool dw_on = r < nsetg;          // lane's column of the MMA B operand = set index r
+  const double* dwp = Dw + (size_t)(dw_on ? r : 0) * npair + 2 * j;
+
+  double acc[8][2];
+#pragma unroll
+  for (int g = 0; g < 8; g++) acc[g][0] = acc[g][1] = 0.0;
+
+  size_t kk = kbeg;
+  for (; kk + 16 <= kend; kk += 16) {
+    double2 b[2][8], d[2];
+#pragma unroll
+    for (int u = 0; u < 2; u++)
+#pragma unroll
+      for (int g = 0; g < 8; g++) b[u][g] = load_pair<VEC>(rowp[g] + kk + 8 * u);
+#pragma unroll
+    for (int u = 0; u < 2; u++) {
+      d[u] = make_double2(0.0, 0.0);
+      if (dw_on) {
+        if (VEC) d[u] = *reinterpret_cast<const double2*>(dwp + kk + 8 * u);
+        else { d[u].x = dwp[kk + 8 * u]; d[u].y = dwp[kk + 8 * u + 1]; }
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 2; u++)
+#pragma unroll
+      for (int g = 0; g < 8; g++) {
+        dmma884(acc[g][0], acc[g][1], b[u][g].x, d[u].x);
+        dmma884(acc[g][0], acc[g][1], b[u][g].y, d[u].y);
+      }
+  }
+  for (; kk < kend; kk += 8) {  // guarded tail steps
+    const bool ok0 = kk + 2 * j < kend, ok1 = kk + 2 * j + 1 < kend;
+    double2 d = make_double2(0.0, 0.0);
+    if (dw_on && ok0) d.x = dwp[kk];
+    if (dw_on && ok1) d.y = dwp[kk + 1];
+#pragma unroll
+    for (int g = 0; g < 8; g++) {
+      double2 b = make_double2(0.0, 0.0);
+      if (ok0) b.x = ldg_stream1(rowp[g] + kk);
+      if (ok1) b.y = ldg_stream1(rowp[g] + kk + 1);
+      dmma884(acc[g][0], acc[g][1], b.x, d.x);
+      dmma884(acc[g][0], acc[g][1], b.y, d.y);
+    }
+  }
+  // fixed-order combine of the 8 warps, one partial per CTA
+#pragma unroll
+  for (int g = 0; g < 8; g++) {
+    red[w][8 * g + r][2 * j] = acc[g][0];
+    red[w][8 * g + r][2 * j + 1] = acc[g][1];
+  }
+  __syncthreads();
+  for (int e = threadIdx.x; e < kJ1Rows * 8; e += kJ1Warps * 32) {
+    const int s = e / kJ1Rows, row = e % kJ1Rows;
+    double t = 0.0;
+#pragma unroll
+    for (int ww = 0; ww < kJ1Warps; ww++) t += red[ww][row][s];
+    part[((size_t)blockIdx.x * 8 + s) * naux_pad + p0 + row] = t;
+  }
+}
+
+// rho[s][P] = sum over chunks in ascending order
+__global__ void k_j1_reduce(const double* __restrict__ part, int nchunks, int naux_pad, int naux, int nsetg,
+                            double* __restrict__ rho) {
+  const int P = blockIdx.x * blockDim.x + threadIdx.x, s = blockIdx.y;
+  if (P >= naux || s >= nsetg) return;
+  double t = 0.0;
+  for (int c = 0; c < nchunks; c++) t += part[((size_t)c * 8 + s) * naux_pad + P];
+  rho[(size_t)s * naux + P] = t;
+}
+
+// Pass 2: a thread owns two adjacent pairs and NS accumulators each; rows stream 8 at a time.
+template <int NS, bool VEC>
+__global__ void __launch_bounds__(kJ2Threads)
+k_j2(const double* __restrict__ B, size_t npair, int naux, const double* __restrict__ rho,
+     double* __restrict__ part, size_t split_stride, int rows_per_split) {
+  __shared__ __align__(16) double rs[NS][128];
+  const size_t col = ((size_t)blockIdx.x * kJ2Threads + threadIdx.x) * 2;
+  const bool ok0 = col < npair, ok1 = col + 1 < npair;
+  const int p_beg = blockIdx.y * rows_per_split;
+  int p_end = p_beg + rows_per_split;
+  if (p_end > naux) p_end = naux;
+  double acc[NS][2];
+#pragma unroll
+  for (int s = 0; s < NS; s++) acc[s][0] = acc[s][1] = 0.0;
+
+  for (int pt = p_beg; pt < p_end; pt += 128) {
+    const int n = min(128, p_end - pt);
+    for (int e = threadIdx.x; e < NS * 128; e += kJ2Threads) {
+      const int s = e >> 7, q = e & 127;
+      rs[s][q] = q < n ? rho[(size_t)s * naux + pt + q] : 0.0;
+    }
+    __syncthreads();
+    if (ok0) {
+      const double* bp = B + (size_t)pt * npair + col;
+      int q0 = 0;
+      for (; q0 + 8 <= n; q0 += 8) {
+        double2 b[8];
+#pragma unroll
+        for (int u = 0; u < 8; u++) {
+          const double* p = bp + (size_t)(q0 + u) * npair;
+          if (VEC) b[u] = ldg_stream2(p);
+          else { b[u].x = ldg_stream1(p); b[u].y = ok1 ? ldg_stream1(p + 1) : 0.0; }
+        }
+#pragma unroll
+        for (int s = 0; s < NS; s++)
+#pragma unroll
+          for (int u = 0; u < 8; u += 2) {
+            const double2 rr = *reinterpret_cast<const double2*>(&rs[s][q0 + u]);
+            acc[s][0] = fma(rr.x, b[u].x, acc[s][0]);
+            acc[s][1] = fma(rr.x, b[u].y, acc[s][1]);
+            acc[s][0] = fma(rr.y, b[u + 1].x, acc[s][0]);
+            acc[s][1] = fma(rr.y, b[u + 1].y, acc[s][1]);
+          }
+      }
+      for (; q0 < n; q0++) {
+        const double* p = bp + (size_t)q0 * npair;
+        const double bx = ldg_stream1(p), by = ok1 ? ldg_stream1(p + 1) : 0.0;
+#pragma unroll
+        for (int s = 0; s < NS; s++) {
+          acc[s][0] = fma(rs[s][q0], bx, acc[s][0]);
+          acc[s][1] = fma(rs[s][q0], by, acc[s][1]);
+        }
+      }
+    }
+    __syncthreads();
+  }
+  if (ok0) {
+    double* out = part + (size_t)blockIdx.y * split_stride + col;
+#pragma unroll
+    for (int s = 0; s < NS; s++) {
+      out[(size_t)s * npair] = acc[s][0];
+      if (ok1) out[(size_t)s * npair + 1] = acc[s][1];
+    }
+  }
+}
+
+// Step a4: J_s[mu][nu] = J_s[nu][mu] = sum_g part[g][s][tri(mu)+nu] (g ascending), 32x32 tiles,
+// the mirrored tile goes through shared memory so both global writes are row-contiguous.
+__global__ void __launch_bounds__(256)
+k_j_epilogue(const double* __restrict__ part, int nsplit, size_t split_stride, size_t npair, int nao,
+             double* __restrict__ J) {
+  const int bi = blockIdx.x, bj = blockIdx.y, s = blockIdx.z;
+  if (bj > bi) return;
+  __shared__ double t[32][33];
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  const double* src = part + (size_t)s * npair;
+  for (int r = ty; r < 32; r += 8) {
+    const int mu = bi * 32 + r, nu = bj * 32 + tx;
+    double v = 0.0;
+    if (mu < nao && nu <= mu) {
+      const size_t idx = tri(mu) + nu;
+      for (int g = 0; g < nsplit; g++) v += src[(size_t)g * split_stride + idx];
+    }
+    t[r][tx] = v;
+  }
+  __syncthreads();
+  double* Js = J + (size_t)s * nao * nao;
+  for (int r = ty; r < 32; r += 8) {
+    const int mu = bi * 32 + r, nu = bj * 32 + tx;  // lower tile (bi,bj)
+    if (mu < nao && nu < nao) {
+      if (bi != bj) Js[(size_t)mu * nao + nu] = t[r][tx];
+      else Js[(size_t)mu * nao + nu] = (nu <= mu) ? t[r][tx] : t[tx][r];
+    }
+    if (bi != bj) {  // mirrored tile (bj,bi): row nu' = bj*32 + r, col mu' = bi*32 + tx
+      const int row = bj * 32 + r, colm = bi * 32 + tx;
+      if (row < nao && colm < nao) Js[(size_t)row * nao + colm] = t[tx][r];
+    }
+  }
+}
+
+template <bool VEC>
+static void launch_j2(int ns, dim3 grid, cudaStream_t st, const double* B, size_t npair, int naux,
+                      const double* rho, double* part, size_t split_stride, int rows_per_split) {
+  switch (ns) {
+#define DFJK_J2_CASE(N)                                                                               \
+  case N:                                                                                             \
+    k_j2<N, VEC><<<grid, kJ2Threads, 0, st>>>(B, npair, naux, rho, part, split_stride, rows_per_split); \
+    break;
+    DFJK_J2_CASE(1) DFJK_J2_CASE(2) DFJK_J2_CASE(3) DFJK_J2_CASE(4)
+    DFJK_J2_CASE(5) DFJK_J2_CASE(6) DFJK_J2_CASE(7) DFJK_J2_CASE(8)
+#undef DFJK_J2_CASE
+    default: break;
+  }
+}
+
+int launch_j_passes(const dfjk_ctx* h, const SetInfo& si, double* J_out, cudaStream_t st) {
+  int launches = 0;
+  const int naux = h->naux, nao = h->nao;
+  const size_t npair = h->npair;
+  const bool vec = (npair % 2 == 0);
+  const int naux_pad = round_up(naux > 0 ? naux : 1, kJ1Rows);
+  const size_t split_stride = (size_t)h->max_nset * npair;
+  const int rows_per_split = round_up(cdiv(naux > 0 ? naux : 1, h->j2_splits), 8);
+  for (int s0 = 0; s0 < si.nset; s0 += 8) {  // the MMA N dimension holds 8 sets per pass
+    const int ns = si.nset - s0 < 8 ? si.nset - s0 : 8;
+    if (naux > 0) {
+      dim3 g1(h->j1_chunks, naux_pad / kJ1Rows);
+      if (vec) k_j1<true><<<g1, kJ1Warps * 32, 0, st>>>(h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad);
+      else k_j1<false><<<g1, kJ1Warps * 32, 0, st>>>(h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad);
+      dim3 gr(cdiv(naux, 128), ns);
+      k_j1_reduce<<<gr, 128, 0, st>>>(h->rho_part, h->j1_chunks, naux_pad, naux, ns, h->rho + (size_t)s0 * naux);
+      launches += 2;
+    }
+    dim3 g2((unsigned)((npair + 2 * kJ2Threads - 1) / (2 * kJ2Threads)), h->j2_splits);
+    if (vec) launch_j2<true>(ns, g2, st, h->B, npair, naux, h->rho + (size_t)s0 * naux, h->Jp_part + (size_t)s0 * npair, split_stride, rows_per_split);
+    else launch_j2<false>(ns, g2, st, h->B, npair, naux, h->rho + (size_t)s0 * naux, h->Jp_part + (size_t)s0 * npair, split_stride, rows_per_split);
+    launches += 1;
+  }
+  const int nb = cdiv(nao, 32);
+  dim3 ge(nb, nb, si.nset), be(32, 8);
+  k_j_epilogue<<<ge, be, 0, st>>>(h->Jp_part, h->j2_splits, split_stride, npair, nao, J_out);
+  return launches + 1;
+}
+
+}  // namespace dfjk

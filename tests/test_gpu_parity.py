@@ -1,0 +1,184 @@
+"""GPU parity: the CUDA path (through the C ABI binding) against the CPU oracle, element by element.
+
+Bar (BASELINE.json north_star): max|dJ|/max|J| and max|dK|/max|K| <= 1e-10 per set.  fp64 DMMA/DFMA
+sums differ from the oracle only in the order of additions, so the observed errors are ~1e-15..1e-13.
+"""
+import numpy as np
+import pytest
+
+import dfjk_inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device; there is no CPU fallback")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def dfjk(torch_cuda):
+    import paper_2505_03755_b200 as pkg
+    pkg.load_library()
+    return pkg
+
+
+def to_dev(torch, inp):
+    B = torch.from_numpy(inp.B_packed).cuda()
+    Cs = [torch.from_numpy(c).cuda() for c in inp.C]
+    occs = [torch.from_numpy(o).cuda() for o in inp.occ]
+    return B, Cs, occs
+
+
+def rel(a, b):
+    return float(np.abs(a - b).max() / max(np.abs(b).max(), 1e-300))
+
+
+def check_against_oracle(torch, dfjk, inp, **opts):
+    import oracle
+    Jo, Ko = oracle.get_jk_inputs(inp)
+    B, Cs, occs = to_dev(torch, inp)
+    with dfjk.DFJK(B, inp.nao, **opts) as h:
+        J, K = h.get_jk(Cs, occs)
+        torch.cuda.synchronize()
+        plan = h.plan()
+        assert h.last_launch_count > 0
+    J, K = J.cpu().numpy(), K.cpu().numpy()
+    for s in range(inp.nset):
+        if np.abs(Jo[s]).max() == 0:
+            assert not J[s].any() and not K[s].any()
+            continue
+        ej, ek = rel(J[s], Jo[s]), rel(K[s], Ko[s])
+        assert ej <= TOL and ek <= TOL, (inp.name, s, ej, ek, plan)
+        assert np.array_equal(J[s], J[s].T) and np.array_equal(K[s], K[s].T)   # bitwise symmetric
+    return J, K
+
+
+def test_dmma_fragment_mapping(dfjk):
+    dfjk.selftest_dmma()
+
+
+def test_tiny_config(torch_cuda, dfjk):
+    check_against_oracle(torch_cuda, dfjk, dfjk_inputs.make_config("tiny"))
+
+
+def test_small_config(torch_cuda, dfjk):
+    check_against_oracle(torch_cuda, dfjk, dfjk_inputs.make_config("small"))
+
+
+@pytest.mark.parametrize("nao,naux,nocc,seed", [
+    (5, 3, [2], 101),            # npair odd: scalar load paths
+    (6, 7, [6], 102),            # npair odd, nocc = nao
+    (67, 45, [23, 7], 103),      # ragged everything, two sets
+    (129, 70, [33], 104),        # one row past a 128 tile
+    (130, 9, [5, 0, 12], 105),   # empty middle set
+    (200, 130, [9, 8, 8, 1, 40, 3, 17, 2], 106),  # eight sets
+    (257, 33, [64], 107),        # three m-tiles: direct, crossing and transposed chunks all occur
+    (48, 1, [12], 108),          # single aux row
+])
+def test_ragged_shapes(torch_cuda, dfjk, nao, naux, nocc, seed):
+    inp = dfjk_inputs.make_random(nao, naux, nocc, seed, L=max(4.0, nao / 6))
+    check_against_oracle(torch_cuda, dfjk, inp)
+
+
+def test_more_than_eight_sets(torch_cuda, dfjk):
+    inp = dfjk_inputs.make_random(40, 21, [3, 1, 4, 1, 5, 9, 2, 6, 5, 3, 5], 109)
+    check_against_oracle(torch_cuda, dfjk, inp, max_nset=12, max_nocc_total=44)
+
+
+@pytest.mark.parametrize("opts", [dict(nblk=1), dict(nblk=7), dict(nblk=16, ksplit=5), dict(ksplit=1),
+                                  dict(workspace_cap_bytes=1 << 20), dict(copy_B=True)])
+def test_blocking_and_split_k_do_not_change_the_result(torch_cuda, dfjk, opts):
+    """N_blk and split-K are memory/parallelism knobs, not part of the result."""
+    inp = dfjk_inputs.make_random(150, 61, [37, 10], 110, L=20.0)
+    check_against_oracle(torch_cuda, dfjk, inp, **opts)
+
+
+def test_j_only_k_only_and_batching(torch_cuda, dfjk):
+    torch = torch_cuda
+    inp = dfjk_inputs.make_random(90, 50, [20, 11, 6], 111, L=15.0)
+    B, Cs, occs = to_dev(torch, inp)
+    with dfjk.DFJK(B, inp.nao) as h:
+        J, K = h.get_jk(Cs, occs)
+        Jonly, none_k = h.get_jk(Cs, occs, with_k=False)
+        none_j, Konly = h.get_jk(Cs, occs, with_j=False)
+        assert none_k is None and none_j is None
+        torch.cuda.synchronize()
+        assert torch.equal(J, Jonly) and torch.equal(K, Konly)
+        for s in range(3):                      # nset-batched == one at a time, bit for bit in J
+            J1, K1 = h.get_jk([Cs[s]], [occs[s]])
+            torch.cuda.synchronize()
+            assert rel(J1[0].cpu().numpy(), J[s].cpu().numpy()) < 1e-13
+            assert rel(K1[0].cpu().numpy(), K[s].cpu().numpy()) < 1e-13
+
+
+def test_repeat_calls_are_bitwise_deterministic_and_stream_ordered(torch_cuda, dfjk):
+    torch = torch_cuda
+    inp = dfjk_inputs.make_random(140, 77, [31, 9], 112, L=12.0)
+    B, Cs, occs = to_dev(torch, inp)
+    with dfjk.DFJK(B, inp.nao) as h:
+        J0, K0 = h.get_jk(Cs, occs)
+        torch.cuda.synchronize()
+        st = torch.cuda.Stream()
+        st.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(st):
+            J1, K1 = h.get_jk(Cs, occs)
+            J2, K2 = h.get_jk(Cs, occs, stream=st)
+        st.synchronize()
+        assert torch.equal(J0, J1) and torch.equal(K0, K1)
+        assert torch.equal(J0, J2) and torch.equal(K0, K2)
+
+
+def test_outputs_are_overwritten_not_accumulated(torch_cuda, dfjk):
+    torch = torch_cuda
+    inp = dfjk_inputs.make_random(33, 12, [7], 113)
+    B, Cs, occs = to_dev(torch, inp)
+    with dfjk.DFJK(B, inp.nao) as h:
+        J, K = h.get_jk(Cs, occs)
+        junk_j = torch.full_like(J, 1e300)
+        junk_k = torch.full_like(K, float("nan"))
+        h.get_jk(Cs, occs, out_j=junk_j, out_k=junk_k)
+        torch.cuda.synchronize()
+        assert torch.equal(J, junk_j) and torch.equal(K, junk_k)
+
+
+def test_host_buffer_entry_point(torch_cuda, dfjk):
+    torch = torch_cuda
+    import oracle
+    inp = dfjk_inputs.make_random(70, 40, [15, 6], 114, L=10.0)
+    Jo, Ko = oracle.get_jk_inputs(inp)
+    B = torch.from_numpy(inp.B_packed).cuda()
+    C = torch.from_numpy(inp.C_concat()).pin_memory()
+    occ = torch.from_numpy(inp.occ_concat()).pin_memory()
+    J = torch.empty((2, 70, 70), dtype=torch.float64).pin_memory()
+    K = torch.empty((2, 70, 70), dtype=torch.float64).pin_memory()
+    with dfjk.DFJK(B, inp.nao) as h:
+        h.get_jk_host(inp.nocc, C, occ, J, K)     # synchronises before returning
+    for s in range(2):
+        assert rel(J[s].numpy(), Jo[s]) <= TOL and rel(K[s].numpy(), Ko[s]) <= TOL
+
+
+def test_error_codes(torch_cuda, dfjk):
+    torch = torch_cuda
+    inp = dfjk_inputs.make_random(20, 6, [4], 115)
+    B, Cs, occs = to_dev(torch, inp)
+    with pytest.raises(ValueError):
+        dfjk.DFJK(B[:, :-1].contiguous(), 20)
+    with dfjk.DFJK(B, 20, max_nset=2, max_nocc_total=10) as h:
+        with pytest.raises(dfjk.DFJKError) as e:   # nset beyond capacity
+            h.get_jk([Cs[0]] * 3, [occs[0]] * 3)
+        assert e.value.code == 1
+        with pytest.raises(dfjk.DFJKError):        # nocc total beyond capacity
+            big = torch.zeros((20, 11), dtype=torch.float64, device="cuda")
+            h.get_jk([big], [torch.ones(11, dtype=torch.float64, device="cuda")])
+        J, K = h.get_jk(Cs, occs)                  # the handle is still usable afterwards
+        torch.cuda.synchronize()
+        assert torch.isfinite(J).all() and torch.isfinite(K).all()
+    lib = dfjk.load_library()
+    assert lib.dfjk_destroy(None) == 0
+    assert lib.dfjk_strerror(4).decode().startswith("unsupported")
