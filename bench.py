@@ -1,0 +1,368 @@
+#!/usr/bin/env python
+"""bench.py -- DF get_jk milliseconds at nao=1200 / naux=4000 on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config large] [--impl reference]
+
+A step is one pass of the whole hot path: one dfjk_get_jk producing J
+and K of the `large` config (nao=1200, naux=4000, nocc=300, ~23 GB packed B resident in HBM).
+`value` is the device-timed milliseconds per step with inputs resident; `e2e` is the same call
+through dfjk_get_jk_host with pinned HOST buffers for C, occ, J, K (copies inside the timed
+region; B stays resident as the paper prescribes).  `roofline` describes the
+dominant kernel (the DMMA half-transform), `cpu_baseline` the oracle on the host cores on a
+bounded sample of aux rows.  The path does not shard in this build ("replicas only"):
+with --gpus N every rank runs an independent replica and the max over ranks is reported.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import dfjk_inputs  # noqa: E402
+
+METRIC = "DF get_jk ms at nao=1200/naux=4000; K FP64 TFLOP/s & J HBM GB/s vs peak"
+# measured on this pool (profiles/r01_ubench.md): DMMA.8x8x4 issue-rate peak, burst == sustained
+FP64_DMMA_PEAK_TFLOPS = 37.1
+FP64_CUBLAS_TFLOPS = 35.47
+HBM_READ_STREAM_GBS = 7430.0
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return dict(hbm_gbs=float(d["hbm_gbs"]), bf16=float(d["bf16_tflops"]),
+                    bf16_sustained=float(d.get("bf16_tflops_sustained", d["bf16_tflops"])), source="measured")
+    return dict(hbm_gbs=6650.0, bf16=1590.0, bf16_sustained=1400.0, source="fallback")
+
+
+def flops_bytes(cfg):
+    nao, naux = cfg["nao"], cfg["naux"]
+    nocc_tot, nset = sum(cfg["nocc"]), len(cfg["nocc"])
+    npair = nao * (nao + 1) // 2
+    ht = 2.0 * naux * nao * nao * nocc_tot
+    syrk = 1.0 * naux * nao * (nao + 1) * nocc_tot
+    jbytes = 2.0 * naux * npair * 8 + nset * (2 * npair + 2 * naux) * 8.0
+    return dict(ht=ht, syrk=syrk, k=ht + syrk, j_bytes=jbytes, j_flops=4.0 * naux * npair * nset,
+                b_bytes=naux * npair * 8.0)
+
+
+class ClockSampler:
+    """nvidia-smi clock / throttle-reason sampler running during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[], samples=0, power_w_max=None)
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, smax, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f:
+            t = [x.strip() for x in line.split(",")]
+            if len(t) < 7:
+                continue
+            try:
+                sm.append(float(t[0])); smax.append(float(t[1])); pw.append(float(t[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, t[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(smax)), reasons=sorted(reasons),
+                       samples=len(sm), power_w_max=float(max(pw)))
+        return out
+
+
+def upload_B(torch, cfg, keep_host: bool):
+    """Generate packed B on the host in row chunks (the canonical recipe) and upload it."""
+    nao, naux, L, k = cfg["nao"], cfg["naux"], cfg["L"], cfg["k"]
+    npair = dfjk_inputs.npair_of(nao)
+    Bd = torch.empty((naux, npair), dtype=torch.float64, device="cuda")
+    env = dfjk_inputs.gen.decay_envelope(nao, naux, L)
+    rng = np.random.default_rng(1000 + k)
+    Bh = np.empty((naux, npair)) if keep_host else None
+    rows = max(1, min(naux, (1 << 28) // npair))          # ~2 GiB chunks
+    stage = torch.empty((rows, npair), dtype=torch.float64).pin_memory()
+    sv = stage.numpy()
+    for r0 in range(0, naux, rows):
+        r1 = min(naux, r0 + rows)
+        torch.cuda.synchronize()                           # the previous async copy has left `stage`
+        rng.standard_normal(out=sv[: r1 - r0])
+        sv[: r1 - r0] *= env
+        if keep_host:
+            Bh[r0:r1] = sv[: r1 - r0]
+        Bd[r0:r1].copy_(stage[: r1 - r0], non_blocking=True)
+    torch.cuda.synchronize()
+    return Bd, Bh
+
+
+def oracle_sample_time(cfg, C, occ, Bh_rows, target_s: float):
+    """Time the oracle (as it stands) on a bounded sample: the first R aux rows of the workload.
+    Returns (seconds, R).  R is calibrated from a 2-row probe to land near target_s."""
+    import oracle
+    nao = cfg["nao"]
+    t0 = time.perf_counter()
+    oracle.get_jk(Bh_rows[:2], nao, C, occ)
+    per_row = (time.perf_counter() - t0) / 2
+    R = int(max(2, min(Bh_rows.shape[0], target_s / max(per_row, 1e-9))))
+    t0 = time.perf_counter()
+    oracle.get_jk(Bh_rows[:R], nao, C, occ)
+    return time.perf_counter() - t0, R
+
+
+def run_reference(args, cfg, name):
+    """--impl reference: the CPU oracle on the host cores, bounded sample per step (rank 0 only)."""
+    import oracle
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    C, occ = dfjk_inputs.make_orbitals(name)
+    nao, naux = cfg["nao"], cfg["naux"]
+    probe_rows = min(naux, 64)
+    Bh = dfjk_inputs.make_B_packed(nao, naux, cfg["L"], 1000 + cfg["k"], rows=probe_rows)
+    t0 = time.perf_counter()
+    oracle.get_jk(Bh[:2], nao, C, occ)
+    per_row = (time.perf_counter() - t0) / 2
+    R = int(max(2, min(probe_rows, 4.0 / max(per_row, 1e-9))))      # ~4 s of CPU work per step
+    for _ in range(args.warmup):
+        oracle.get_jk(Bh[:2], nao, C, occ)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.get_jk(Bh[:R], nao, C, occ)
+    dt = (time.perf_counter() - t0) / args.steps
+    ms_full = dt * 1e3 * naux / R
+    sample = f"first {R} of {naux} aux rows per step, time scaled by {naux}/{R} (cost is linear in aux rows)"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": ms_full, "unit": "ms", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_full, "higher_is_better": False,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": name, "nao": nao, "naux": naux, "nocc": cfg["nocc"], "sample": sample},
+        "cpu_baseline": {"value": ms_full, "unit": "ms", "cores": oracle.num_threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": ms_full, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="large", choices=list(dfjk_inputs.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-parity", action="store_true", help="skip the sampled parity check")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    args = ap.parse_args()
+    name = args.config
+    cfg = dfjk_inputs.CONFIGS[name]
+    if args.impl == "reference":
+        run_reference(args, cfg, name)
+        return
+
+    import torch
+    import paper_2505_03755_b200 as dfjk          # raises if libdfjk.so is missing: no CPU fallback
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (B200); there is no CPU fallback")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    nao, naux, nocc = cfg["nao"], cfg["naux"], cfg["nocc"]
+    nset = len(nocc)
+    fb = flops_bytes(cfg)
+    lead = rank == 0
+    want_host_B = lead and world == 1 and not (args.no_parity and args.no_cpu_baseline)
+    t_gen = time.perf_counter()
+    Bd, Bh = upload_B(torch, cfg, keep_host=want_host_B)
+    t_gen = time.perf_counter() - t_gen
+    C_list, occ_list = dfjk_inputs.make_orbitals(name)
+    C_host = torch.from_numpy(np.concatenate([c.ravel() for c in C_list])).pin_memory()
+    occ_host = torch.from_numpy(np.concatenate(occ_list)).pin_memory()
+    C_dev, occ_dev = C_host.cuda(), occ_host.cuda()
+    J = torch.empty((nset, nao, nao), dtype=torch.float64, device="cuda")
+    K = torch.empty_like(J)
+    J_host = torch.empty((nset, nao, nao), dtype=torch.float64).pin_memory()
+    K_host = torch.empty_like(J_host).pin_memory()
+
+    h = dfjk.DFJK(Bd, nao)
+    stream = torch.cuda.current_stream()
+
+    def timed(fn, steps):
+        """device milliseconds per step over exactly `steps` calls, events on the launching stream"""
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record(stream)
+        for _ in range(steps):
+            fn()
+        e1.record(stream)
+        barrier()
+        return e0.elapsed_time(e1) / steps
+
+    full = lambda: h.get_jk_raw(nocc, C_dev, occ_dev, out_j=J, out_k=K, stream=stream)
+    j_only = lambda: h.get_jk_raw(nocc, C_dev, occ_dev, with_k=False, out_j=J, stream=stream)
+    k_only = lambda: h.get_jk_raw(nocc, C_dev, occ_dev, with_j=False, out_k=K, stream=stream)
+    host = lambda: h.get_jk_host(nocc, C_host, occ_host, J_host, K_host, stream=stream)
+
+    for _ in range(args.warmup):
+        full()
+    barrier()
+
+    # ---- the timed region: exactly K steps of the whole path, clocks sampled meanwhile
+    h.set_profiling(True)
+    phases = {p: [0.0, 0] for p in dfjk.api.PHASES}
+    launches = 0
+    clocks = ClockSampler(local)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        full()
+        launches += h.last_launch_count
+        for p, (ms, n) in h.profile().items():     # waits for this step's last event only
+            phases[p][0] += ms
+            phases[p][1] += n
+    e1.record(stream)
+    barrier()
+    ms_step = max_over_ranks(e0.elapsed_time(e1) / args.steps)
+    clk = clocks.stop()
+    h.set_profiling(False)
+    plan = h.plan()
+
+    # ---- the same call through the host-buffer entry point (H2D of C/occ, D2H of J/K inside)
+    for _ in range(2):
+        host()
+    t0 = time.perf_counter()
+    ms_e2e_dev = timed(host, args.steps)
+    ms_e2e_wall = (time.perf_counter() - t0) * 1e3 / args.steps
+    ms_e2e = max_over_ranks(max(ms_e2e_dev, ms_e2e_wall))
+    h2d = int(C_host.numel() * 8 + occ_host.numel() * 8)
+    d2h = int(2 * J_host.numel() * 8)
+
+    # ---- J pass and K path alone (K_out = NULL / J_out = NULL), for the two rooflines
+    nrep = max(3, min(args.steps, 5))
+    j_only(); k_only()
+    ms_j = max_over_ranks(timed(j_only, nrep))
+    ms_k = max_over_ranks(timed(k_only, nrep))
+
+    if not lead:
+        return
+    pk = measured_peaks()
+    ht_ms, ht_n = phases["half_transform"]
+    sy_ms, sy_n = phases["syrk"]
+    ht_tflops = fb["ht"] * args.steps / (ht_ms * 1e-3) * 1e-12 if ht_ms > 0 else 0.0
+    sy_tflops = fb["syrk"] * args.steps / (sy_ms * 1e-3) * 1e-12 if sy_ms > 0 else 0.0
+    j1_ms, j2_ms = phases["j1"][0] / args.steps, phases["j2"][0] / args.steps
+    line = {
+        "metric": METRIC, "value": ms_step, "unit": "ms", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": name, "nao": nao, "naux": naux, "nset": nset, "nocc": nocc,
+                   "B_packed_GB": fb["b_bytes"] * 1e-9, "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "l2": "inputs (packed B) far larger than the 126 MB L2, no flush needed" if fb["b_bytes"] > 1e9
+                         else "L2-warm (inputs fit the L2)",
+                   "plan": plan, "input_gen_s": round(t_gen, 1)},
+        "clocks": {"sm_mhz": clk["sm_mhz"], "sm_max_mhz": clk["sm_max_mhz"], "reasons": clk["reasons"],
+                   "samples": clk["samples"], "power_w_max": clk["power_w_max"]},
+        "e2e": {"value": ms_e2e, "unit": "ms", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "api": "dfjk_get_jk_host (pinned C, occ, J, K; B resident)"},
+        "gpu_launches": launches,
+        "roofline": {"kernel": "k_half_transform", "bound": "tensor", "achieved": ht_tflops,
+                     "peak": FP64_DMMA_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ht_tflops / FP64_DMMA_PEAK_TFLOPS,
+                     "traffic": None, "launches": ht_n, "avg_launch_ms": ht_ms / max(ht_n, 1),
+                     "algorithmic_flops_per_step": fb["ht"],
+                     "peak_source": "measured DMMA.8x8x4 issue-rate peak on this pool (profiles/r01_ubench.md); "
+                                    "cuBLAS fp64 8192^3 reaches %.2f; MEASURED_PEAKS bf16 %.1f x nominal 45/2250 = %.1f"
+                                    % (FP64_CUBLAS_TFLOPS, pk["bf16"], pk["bf16"] * 45.0 / 2250.0)},
+        "k_path": {"ms": ms_k, "tflops": fb["k"] / (ms_k * 1e-3) * 1e-12,
+                   "frac_of_fp64_peak": fb["k"] / (ms_k * 1e-3) * 1e-12 / FP64_DMMA_PEAK_TFLOPS,
+                   "half_transform_tflops": ht_tflops, "syrk_tflops": sy_tflops,
+                   "algorithmic_flops": fb["k"]},
+        "j_pass": {"ms": ms_j, "gbs": fb["j_bytes"] / (ms_j * 1e-3) * 1e-9,
+                   "frac_of_measured_hbm": fb["j_bytes"] / (ms_j * 1e-3) * 1e-9 / pk["hbm_gbs"],
+                   "frac_of_8TBs": fb["j_bytes"] / (ms_j * 1e-3) * 1e-9 / 8000.0,
+                   "pass1_gbs": fb["b_bytes"] / (j1_ms * 1e-3) * 1e-9 if j1_ms > 0 else None,
+                   "pass2_gbs": fb["b_bytes"] / (j2_ms * 1e-3) * 1e-9 if j2_ms > 0 else None,
+                   "algorithmic_bytes": fb["j_bytes"], "hbm_peak_source": pk["source"]},
+        "phases_ms_per_step": {p: v[0] / args.steps for p, v in phases.items()},
+    }
+
+    if Bh is not None and not args.no_parity:
+        import oracle
+        torch.cuda.synchronize()
+        rs = np.random.default_rng(7)
+        samples = [(int(rs.integers(nset)), int(rs.integers(nao)), int(rs.integers(nao))) for _ in range(4)]
+        samples += [(0, 0, 0), (nset - 1, nao - 1, nao - 1), (0, nao - 1, 0), (0, 127, 128)]
+        t0 = time.perf_counter()
+        Jv, Kv = oracle.sample(Bh, nao, C_list, occ_list, samples)
+        Jg, Kg = J.cpu().numpy(), K.cpu().numpy()
+        ej = max(abs(Jg[s, m, n] - Jv[t]) / np.abs(Jg[s]).max() for t, (s, m, n) in enumerate(samples))
+        ek = max(abs(Kg[s, m, n] - Kv[t]) / np.abs(Kg[s]).max() for t, (s, m, n) in enumerate(samples))
+        line["parity"] = {"kind": "oracle.sample on %d elements" % len(samples), "max_rel_err_J": float(ej),
+                          "max_rel_err_K": float(ek), "tolerance": 1e-10, "ok": bool(ej <= 1e-10 and ek <= 1e-10),
+                          "seconds": round(time.perf_counter() - t0, 1)}
+    if Bh is not None and not args.no_cpu_baseline:
+        import oracle
+        secs, R = oracle_sample_time(cfg, C_list, occ_list, Bh, args.cpu_seconds)
+        line["cpu_baseline"] = {"value": secs * 1e3 * naux / R, "unit": "ms", "cores": oracle.num_threads(),
+                                "kind": "oracle",
+                                "sample": f"first {R} of {naux} aux rows in {secs:.1f} s, scaled by {naux}/{R} "
+                                          "(the oracle's cost is linear in aux rows)"}
+    print(json.dumps(line), flush=True)
+    h.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -116,6 +116,26 @@ int dfjk_get_plan(dfjk_handle h, int* nblk, int* ksplit, int* nocc_pad_capacity)
 /* Number of kernel launches dfjk_get_jk enqueued in its last call on this handle. */
 int dfjk_last_launch_count(dfjk_handle h);
 
+/*
+ * Optional per-phase profile with CUDA events recorded on the launching stream (the paper used
+ * wall-clock timers per stage and Nsight timelines).  Off by default.
+ * dfjk_set_profiling(h, 1) makes every later dfjk_get_jk record an event at each phase boundary
+ * (a few microseconds each).  dfjk_get_profile synchronises on the last event of the last call and
+ * returns, per phase, the summed milliseconds and the number of kernel-launch groups.
+ */
+enum {
+  DFJK_PHASE_PREP = 0,           /* a1: C' and packed weighted density */
+  DFJK_PHASE_J1 = 1,             /* a2: rho = <B_P, D>   (includes the tiny chunk reduce) */
+  DFJK_PHASE_J2 = 2,             /* a3: Jp = sum_P rho_P B_P */
+  DFJK_PHASE_J_EPILOGUE = 3,     /* a4 */
+  DFJK_PHASE_HALF_TRANSFORM = 4, /* a5+a6 */
+  DFJK_PHASE_SYRK = 5,           /* a7 */
+  DFJK_PHASE_K_EPILOGUE = 6,     /* a9 (and zero fills) */
+  DFJK_NUM_PHASES = 7
+};
+int dfjk_set_profiling(dfjk_handle h, int on);
+int dfjk_get_profile(dfjk_handle h, double* ms /* [DFJK_NUM_PHASES] */, int* groups /* [DFJK_NUM_PHASES] */);
+
 /* 1-warp self-test of the DMMA.8x8x4 fragment mapping against a scalar loop on the device
  * (synchronises).  Returns DFJK_OK if the mapping assumed by the kernels holds. */
 int dfjk_selftest_dmma(void);

@@ -14,7 +14,9 @@ _lib = None
 
 EXPORTS = ["dfjk_create", "dfjk_get_jk", "dfjk_get_jk_host", "dfjk_destroy", "dfjk_strerror",
            "dfjk_last_error", "dfjk_workspace_bytes", "dfjk_get_plan", "dfjk_last_launch_count",
-           "dfjk_selftest_dmma"]
+           "dfjk_selftest_dmma", "dfjk_set_profiling", "dfjk_get_profile"]
+
+PHASES = ["prep", "j1", "j2", "j_epilogue", "half_transform", "syrk", "k_epilogue"]
 
 
 class DFJKError(RuntimeError):
@@ -61,6 +63,10 @@ def load_library():
     lib.dfjk_get_plan.restype = ct.c_int
     lib.dfjk_last_launch_count.argtypes = [vp]
     lib.dfjk_last_launch_count.restype = ct.c_int
+    lib.dfjk_set_profiling.argtypes = [vp, ct.c_int]
+    lib.dfjk_set_profiling.restype = ct.c_int
+    lib.dfjk_get_profile.argtypes = [vp, ct.POINTER(ct.c_double), ip]
+    lib.dfjk_get_profile.restype = ct.c_int
     lib.dfjk_selftest_dmma.argtypes = []
     lib.dfjk_selftest_dmma.restype = ct.c_int
     _lib = lib
@@ -164,6 +170,16 @@ class DFJK:
         a, b, c = ct.c_int(), ct.c_int(), ct.c_int()
         _check(self._lib, self._lib.dfjk_get_plan(self._h, ct.byref(a), ct.byref(b), ct.byref(c)))
         return dict(nblk=a.value, ksplit=b.value, nocc_pad_capacity=c.value)
+
+    def set_profiling(self, on: bool) -> None:
+        _check(self._lib, self._lib.dfjk_set_profiling(self._h, int(on)), self._h)
+
+    def profile(self) -> dict:
+        """{phase: (ms, launch groups)} of the last get_jk (synchronises on its last event)."""
+        ms = (ct.c_double * len(PHASES))()
+        n = (ct.c_int * len(PHASES))()
+        _check(self._lib, self._lib.dfjk_get_profile(self._h, ms, n), self._h)
+        return {p: (ms[i], n[i]) for i, p in enumerate(PHASES)}
 
     @property
     def workspace_bytes(self) -> int:

@@ -32,6 +32,9 @@ void free_all(dfjk_ctx* h) {
   cudaFree(h->B_owned); cudaFree(h->Ct); cudaFree(h->Dw); cudaFree(h->rho_part); cudaFree(h->rho);
   cudaFree(h->Jp_part); cudaFree(h->X); cudaFree(h->Kpart);
   cudaFree(h->C_stage); cudaFree(h->occ_stage); cudaFree(h->J_stage); cudaFree(h->K_stage);
+  for (int i = 0; i < h->ev_cap; i++) cudaEventDestroy(h->ev[i]);
+  delete[] h->ev;
+  delete[] h->ev_phase;
 }
 
 // validate nocc and lay out the padded columns of C'/X
@@ -171,6 +174,7 @@ int dfjk_get_jk(dfjk_handle h, int nset, const int* nocc, const double* C, const
   cudaStream_t st = (cudaStream_t)stream;
   h->last_launches = 0;
   h->last_error[0] = 0;
+  h->ev_n = 0;
   if (!J_out && !K_out) return DFJK_OK;
   int n = 0, k;
   n += launch_prep_ct(h, si, C, occ, st);
@@ -183,6 +187,7 @@ int dfjk_get_jk(dfjk_handle h, int nset, const int* nocc, const double* C, const
     if (k < 0) { set_err(h, "k path launch", cudaGetLastError()); return DFJK_ERR_CUDA; }
     n += k;
   }
+  prof_mark(h, -1, st);
   h->last_launches = n;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { set_err(h, "kernel launch", e); return DFJK_ERR_CUDA; }
@@ -236,6 +241,40 @@ int dfjk_get_plan(dfjk_handle h, int* nblk, int* ksplit, int* nocc_pad_capacity)
 }
 
 int dfjk_last_launch_count(dfjk_handle h) { return h ? h->last_launches : 0; }
+
+int dfjk_set_profiling(dfjk_handle h, int on) {
+  if (!h) return DFJK_ERR_INVALID_ARG;
+  if (on && !h->ev) {
+    const int cap = 8192;
+    h->ev = new (std::nothrow) cudaEvent_t[cap];
+    h->ev_phase = new (std::nothrow) int[cap];
+    if (!h->ev || !h->ev_phase) return DFJK_ERR_ALLOC;
+    for (int i = 0; i < cap; i++) {
+      if (cudaEventCreate(&h->ev[i]) != cudaSuccess) { cudaGetLastError(); return DFJK_ERR_CUDA; }
+      h->ev_cap = i + 1;
+    }
+  }
+  h->profiling = on ? 1 : 0;
+  h->ev_n = 0;
+  return DFJK_OK;
+}
+
+int dfjk_get_profile(dfjk_handle h, double* ms, int* groups) {
+  if (!h || !ms || !groups) return DFJK_ERR_INVALID_ARG;
+  for (int p = 0; p < DFJK_NUM_PHASES; p++) { ms[p] = 0.0; groups[p] = 0; }
+  if (h->ev_n < 2) return DFJK_OK;
+  cudaError_t e = cudaEventSynchronize(h->ev[h->ev_n - 1]);
+  if (e != cudaSuccess) { set_err(h, "event sync", e); cudaGetLastError(); return DFJK_ERR_CUDA; }
+  for (int i = 0; i + 1 < h->ev_n; i++) {
+    const int p = h->ev_phase[i];
+    if (p < 0 || p >= DFJK_NUM_PHASES) continue;
+    float t = 0.f;
+    if (cudaEventElapsedTime(&t, h->ev[i], h->ev[i + 1]) != cudaSuccess) { cudaGetLastError(); continue; }
+    ms[p] += t;
+    groups[p] += 1;
+  }
+  return DFJK_OK;
+}
 
 int dfjk_selftest_dmma(void) {
   const int bad = run_dmma_selftest();

@@ -55,15 +55,26 @@ struct dfjk_ctx {
   double *C_stage, *occ_stage, *J_stage, *K_stage;
   size_t workspace_bytes;
   int last_launches;
+  // optional per-phase CUDA-event profile of the last call (dfjk_set_profiling)
+  int profiling, ev_cap, ev_n;
+  cudaEvent_t* ev;
+  int* ev_phase;
   char last_error[256];
 };
 
 namespace dfjk {
 
+// Phase marker of the event profile: the phase lasts until the next marker on the stream.
+inline void prof_mark(dfjk_ctx* h, int phase, cudaStream_t st) {
+  if (!h->profiling || h->ev_n >= h->ev_cap) return;
+  cudaEventRecord(h->ev[h->ev_n], st);
+  h->ev_phase[h->ev_n++] = phase;
+}
+
 // Each launcher enqueues on `st` and returns the number of kernels it launched.
-int launch_prep_ct(const dfjk_ctx* h, const SetInfo& si, const double* C, const double* occ, cudaStream_t st);
-int launch_prep_dw(const dfjk_ctx* h, const SetInfo& si, cudaStream_t st);
-int launch_j_passes(const dfjk_ctx* h, const SetInfo& si, double* J_out, cudaStream_t st);
+int launch_prep_ct(dfjk_ctx* h, const SetInfo& si, const double* C, const double* occ, cudaStream_t st);
+int launch_prep_dw(dfjk_ctx* h, const SetInfo& si, cudaStream_t st);
+int launch_j_passes(dfjk_ctx* h, const SetInfo& si, double* J_out, cudaStream_t st);
 int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, cudaStream_t st);
 int run_dmma_selftest();
 

@@ -225,7 +225,7 @@ static void launch_j2(int ns, dim3 grid, cudaStream_t st, const double* B, size_
   }
 }
 
-int launch_j_passes(const dfjk_ctx* h, const SetInfo& si, double* J_out, cudaStream_t st) {
+int launch_j_passes(dfjk_ctx* h, const SetInfo& si, double* J_out, cudaStream_t st) {
   int launches = 0;
   const int naux = h->naux, nao = h->nao;
   const size_t npair = h->npair;
@@ -236,6 +236,7 @@ int launch_j_passes(const dfjk_ctx* h, const SetInfo& si, double* J_out, cudaStr
   for (int s0 = 0; s0 < si.nset; s0 += 8) {  // the MMA N dimension holds 8 sets per pass
     const int ns = si.nset - s0 < 8 ? si.nset - s0 : 8;
     if (naux > 0) {
+      prof_mark(h, DFJK_PHASE_J1, st);
       dim3 g1(h->j1_chunks, naux_pad / kJ1Rows);
       if (vec) k_j1<true><<<g1, kJ1Warps * 32, 0, st>>>(h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad);
       else k_j1<false><<<g1, kJ1Warps * 32, 0, st>>>(h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad);
@@ -243,11 +244,13 @@ int launch_j_passes(const dfjk_ctx* h, const SetInfo& si, double* J_out, cudaStr
       k_j1_reduce<<<gr, 128, 0, st>>>(h->rho_part, h->j1_chunks, naux_pad, naux, ns, h->rho + (size_t)s0 * naux);
       launches += 2;
     }
+    prof_mark(h, DFJK_PHASE_J2, st);
     dim3 g2((unsigned)((npair + 2 * kJ2Threads - 1) / (2 * kJ2Threads)), h->j2_splits);
     if (vec) launch_j2<true>(ns, g2, st, h->B, npair, naux, h->rho + (size_t)s0 * naux, h->Jp_part + (size_t)s0 * npair, split_stride, rows_per_split);
     else launch_j2<false>(ns, g2, st, h->B, npair, naux, h->rho + (size_t)s0 * naux, h->Jp_part + (size_t)s0 * npair, split_stride, rows_per_split);
     launches += 1;
   }
+  prof_mark(h, DFJK_PHASE_J_EPILOGUE, st);
   const int nb = cdiv(nao, 32);
   dim3 ge(nb, nb, si.nset), be(32, 8);
   k_j_epilogue<<<ge, be, 0, st>>>(h->Jp_part, h->j2_splits, split_stride, npair, nao, J_out);

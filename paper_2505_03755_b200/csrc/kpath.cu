@@ -295,6 +295,7 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, cudaStream_t st
   const int nb32 = cdiv(nao, 32);
   const int ldx = si.nocc_pad;
   // sets without columns (or no aux rows at all): K_s = 0
+  prof_mark(h, DFJK_PHASE_K_EPILOGUE, st);
   for (int s = 0; s < si.nset; s++)
     if (naux == 0 || si.col0[s + 1] == si.col0[s]) {
       k_zero<<<148, 256, 0, st>>>(K_out + n2 * s, n2);
@@ -332,9 +333,11 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, cudaStream_t st
   for (int p0 = 0; p0 < naux; p0 += (int)nblk, nblocks++) {
     const int nb = (int)(naux - p0 < nblk ? naux - p0 : nblk);
     dim3 gh(ntn, ntm, nb);
+    prof_mark(h, DFJK_PHASE_HALF_TRANSFORM, st);
     if (dispatch_ht(wn, gh, st, h->B, h->npair, nao, h->nao_k, h->Ct, ldx, h->X, p0) != cudaSuccess) return -1;
     launches++;
     const int rps = cdiv(nb, ksplit);
+    prof_mark(h, DFJK_PHASE_SYRK, st);
     for (int s = 0; s < si.nset; s++) {
       if (si.col0[s + 1] == si.col0[s]) continue;
       k_syrk<<<ntiles * ksplit, 256, syrk_smem_bytes(), st>>>(h->X, nao, ldx, si.col0[s], si.col0[s + 1], nb, rps,
@@ -342,6 +345,7 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, cudaStream_t st
       launches++;
     }
   }
+  prof_mark(h, DFJK_PHASE_K_EPILOGUE, st);
   for (int s = 0; s < si.nset; s++) {
     if (si.col0[s + 1] == si.col0[s]) continue;
     dim3 ge(nb32, nb32, 1), be(32, 8);

@@ -88,14 +88,16 @@ k_prep_dw(const __grid_constant__ SetInfo si, const double* __restrict__ Ct, dou
   }
 }
 
-int launch_prep_ct(const dfjk_ctx* h, const SetInfo& si, const double* C, const double* occ, cudaStream_t st) {
+int launch_prep_ct(dfjk_ctx* h, const SetInfo& si, const double* C, const double* occ, cudaStream_t st) {
   if (si.nocc_pad == 0) return 0;
+  prof_mark(h, DFJK_PHASE_PREP, st);
   dim3 grid(cdiv(h->nao_k, 32), cdiv(si.nocc_pad, 32)), block(32, 8);
   k_prep_ct<<<grid, block, 0, st>>>(si, C, occ, h->Ct, h->nao, h->nao_k);
   return 1;
 }
 
-int launch_prep_dw(const dfjk_ctx* h, const SetInfo& si, cudaStream_t st) {
+int launch_prep_dw(dfjk_ctx* h, const SetInfo& si, cudaStream_t st) {
+  prof_mark(h, DFJK_PHASE_PREP, st);
   const int nb = cdiv(h->nao, 64);
   dim3 grid(nb, nb, si.nset);
   k_prep_dw<<<grid, 256, 0, st>>>(si, h->Ct, h->Dw, h->nao, h->nao_k, h->npair);
