@@ -99,23 +99,26 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   memset(h, 0, sizeof(*h));
   h->naux = naux; h->nao = nao; h->device = dev;
   h->npair = (size_t)nao * (nao + 1) / 2;
-  h->nao_k = round_up(nao, kBK);
+  h->nck = cdiv(nao, kHtBK);
+  h->mu_pad = round_up(nao, 128);
   h->max_nset = o.max_nset ? o.max_nset : 8;
   h->max_nocc_total = o.max_nocc_total ? o.max_nocc_total : nao;
   h->nocc_pad_cap = round_up(h->max_nocc_total + 7 * h->max_nset, 8);
+  h->ct_rows = h->nocc_pad_cap + 16 * kHtMaxWN;   // any N tile of the half-transform stays in bounds
   h->n_mtiles = cdiv(nao, 128);
   h->nblk_forced = o.nblk;
   h->ksplit_forced = o.ksplit;
   // split-K partial slots: enough to fill the SMs about three times with one set's tiles
   {
     const int ntiles = h->n_mtiles * (h->n_mtiles + 1) / 2;
-    h->ksplit = o.ksplit ? o.ksplit : cdiv(3 * 148, ntiles);
+    h->ksplit = o.ksplit ? o.ksplit : cdiv(4 * 148, ntiles);
     if (h->ksplit > 64 && !o.ksplit) h->ksplit = 64;
   }
-  // X capacity: the cap, but at least one aux row at full column capacity
+  // X capacity (k-tiled layout [nch][mu_pad][36] per aux row): the cap, but at least one aux row
+  // at full column capacity
   {
     const size_t cap = o.workspace_cap_bytes ? o.workspace_cap_bytes : ((size_t)1 << 30);
-    const size_t one_row = (size_t)nao * h->nocc_pad_cap;
+    const size_t one_row = (size_t)cdiv(h->nocc_pad_cap, kBK) * h->mu_pad * kLdT;
     size_t dbl = cap / sizeof(double);
     if (o.nblk > 0) dbl = (size_t)o.nblk * one_row;
     if (dbl < one_row) dbl = one_row;
@@ -136,7 +139,7 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   const int naux_pad = round_up(naux > 0 ? naux : 1, kJ1Rows);
   const size_t n2 = (size_t)nao * nao;
   bool ok = true;
-  ok = ok && dev_alloc(h, &h->Ct, (size_t)h->nocc_pad_cap * h->nao_k);
+  ok = ok && dev_alloc(h, &h->Ct, (size_t)h->nck * h->ct_rows * kHtLd);
   ok = ok && dev_alloc(h, &h->Dw, (size_t)h->max_nset * h->npair);
   ok = ok && dev_alloc(h, &h->rho_part, (size_t)h->j1_chunks * 8 * naux_pad);
   ok = ok && dev_alloc(h, &h->rho, (size_t)h->max_nset * (naux > 0 ? naux : 1));

@@ -8,7 +8,11 @@
 namespace dfjk {
 
 constexpr int kMaxSets = 32;       // hard upper bound for options.max_nset
-constexpr int kBK = 32;            // k-chunk (doubles) of the DMMA tile pipelines
+constexpr int kBK = 32;            // k-chunk (doubles) of the SYRK tile pipeline
+constexpr int kLdT = kBK + 4;      // 36: row stride of a [rows][32] tile (4 mod 16: conflict-free fragments)
+constexpr int kHtBK = 16;          // k-chunk of the half-transform
+constexpr int kHtLd = kHtBK + 4;   // 20: row stride of [rows][16] tiles (4 mod 16)
+constexpr int kHtMaxWN = 20;       // half-transform N tile = 16*WN columns, WN <= 20
 constexpr int kJ1Rows = 64;        // aux rows per J-pass-1 work item (8 DMMA row groups per warp)
 constexpr int kJ1SubChunk = 2048;  // pairs per warp per J-pass-1 work item
 constexpr int kJ1Warps = 8;
@@ -31,7 +35,9 @@ struct SetInfo {
 struct dfjk_ctx {
   int naux, nao;
   size_t npair;
-  int nao_k;                 // nao rounded up to kBK (k extent of the half-transform)
+  int nck;                   // 16-wide k chunks of the half-transform = ceil(nao/16)
+  int ct_rows;               // rows (padded columns of C') per chunk in the tiled C' buffer
+  int mu_pad;                // nao rounded up to 128 (row extent of the tiled X)
   int device;
   const double* B;           // packed tensor (borrowed or owned)
   double* B_owned;
@@ -43,12 +49,12 @@ struct dfjk_ctx {
   int n_mtiles;              // 128-row tiles along nao
   int j1_chunks, j2_splits;
   // scratch (all allocated at create)
-  double* Ct;                // [nocc_pad_cap][nao_k]     C' transposed, sqrt(occ) folded, zero padded
+  double* Ct;                // [nck][ct_rows][20]  C' transposed and k-tiled, sqrt(occ) folded, zero padded
   double* Dw;                // [max_nset][npair]         packed density, off-diagonal weight 2
   double* rho_part;          // [j1_chunks][8][naux_pad]
   double* rho;               // [max_nset][naux]
   double* Jp_part;           // [j2_splits][max_nset][npair]
-  double* X;                 // [plan_nblk][nao][nocc_pad] half-transformed block
+  double* X;                 // [plan_nblk][nch][mu_pad][36] half-transformed block, k-tiled
   size_t X_doubles;          // capacity of X
   double* Kpart;             // [ksplit][max_nset][nao][nao]
   // staging for dfjk_get_jk_host

@@ -7,132 +7,196 @@
 //          lower-triangle 128x128 tiles, split-K over the aux rows of the block, partials
 //          read-modify-written by exactly one CTA each (no atomics: deterministic).
 //   a9     epilogue        fixed-order sum of the split-K partials, mirrored to both triangles.
-// Both GEMMs run DMMA.8x8x4 (mma.sync m8n8k4 f64) from shared-memory tiles whose row stride is
-// 4 mod 16 doubles, which makes both the [row][k] and the [k][row] fragment reads conflict-free.
+// Both GEMMs are warp-specialised: warpgroups 0-1 (8 warps) only issue LDS + DMMA.8x8x4
+// (mma.sync m8n8k4 f64; FP64 has no tcgen05/TMEM kind), warpgroup 2 produces the shared-memory
+// stages -- bulk async copies (TMA engine, SASS UBLKCP) for the pre-tiled operands C' and X,
+// 8-byte cp.async gathers for the packed triangle -- through a 3-stage full/empty mbarrier ring,
+// with setmaxnreg moving registers from the producers to the consumers.  All tiles have a row
+// stride of 4 mod 16 doubles, which makes both the [row][k] and the [k][row] fragment reads
+// bank-conflict-free.
 #include "common.cuh"
 #include "ctx.h"
+#include "pipeline.cuh"
 
 namespace dfjk {
 
 constexpr int kStages = 3;
-constexpr int kLdT = kBK + 4;        // 36: row stride of a [rows][kBK] tile
-constexpr int kLdTT = 128 + 4;       // 132: row stride of a transposed [kBK][128] tile
-constexpr int kTileDoubles = 128 * kLdT;  // 4608 >= kBK * kLdTT = 4224
+constexpr int kThreads = 384;             // 2 consumer warpgroups + 1 producer warpgroup
+constexpr int kConsumerRegs = 232, kProducerRegs = 40;
 
 // ------------------------------------------------------------------ half-transform
-// CTA: 128 rows (mu) of one aux slice x NT = 8*WN columns; 8 warps stacked along M (16 rows each).
+// CTA: 64 rows (mu) of one aux slice x NT = 16*WN columns (normally ALL columns of C', so the
+// packed tensor passes through the SM once per row block).  Consumers: 4 (M, 16 rows) x 2 (N
+// halves); warps w and w+4 share an SM sub-partition.  k-chunks of 16 (kHtBK).
+//   C' tiled:  Ct[(chunk * ct_rows + n) * 20 + k]                  (written by k_prep_ct)
+//   X tiled:   X[((pl * nch + n/32) * mu_pad + mu) * 36 + n%32]    (read by k_syrk with bulk copies)
+constexpr int kHtATile = 64 * kHtLd;       // 1280 doubles >= 16 * 68 = 1088
+constexpr int kHtLdT = 64 + 4;             // 68: row stride of the transposed [16][64] A tile
+
 template <int WN>
-__global__ void __launch_bounds__(256, 1)
-k_half_transform(const double* __restrict__ Bp, size_t npair, int nao, int nao_k,
-                 const double* __restrict__ Ct, int nocc_pad, double* __restrict__ X, int p_first) {
-  extern __shared__ __align__(16) double smem[];
-  constexpr int NT = 8 * WN;
-  double* sA = smem;                               // kStages x kTileDoubles
-  double* sB = smem + kStages * kTileDoubles;      // kStages x NT*kLdT
-  const int tid = threadIdx.x, w = tid >> 5, l = tid & 31, r = l >> 2, j = l & 3;
-  const int n0 = blockIdx.x * NT, m0 = blockIdx.y * 128, pl = blockIdx.z;
-  const double* BpP = Bp + (size_t)(p_first + pl) * npair;
-  const int nchunks = nao_k / kBK;
+__global__ void __launch_bounds__(kThreads, 1)
+k_half_transform(const double* __restrict__ Bp, size_t npair, int nao, const double* __restrict__ Ct,
+                 int ct_rows, int nocc_pad, double* __restrict__ X, int nch, int mu_pad, int p_first) {
+  extern __shared__ __align__(128) double smem[];
+  constexpr int NT = 16 * WN;
+  constexpr uint32_t kBBytes = NT * kHtLd * 8;
+  double* sA = smem;                               // kStages x kHtATile
+  double* sB = smem + kStages * kHtATile;          // kStages x NT*kHtLd
+  __shared__ __align__(8) unsigned long long bars[2 * kStages];
+  const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kStages]);
+  const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
+  const int n0 = blockIdx.x * NT, m0 = blockIdx.y * 64, pl = blockIdx.z;
+  const int nk4 = (nao + 3) >> 2;                  // k4 steps that carry data
+  const int nchunks = (nk4 + 3) >> 2;
 
-  auto chunk_mode = [&](int c) -> int {  // 0 = stored rows (direct), 1 = transposed, 2 = crossing
-    const int l0 = c * kBK;
-    if (l0 + kBK - 1 <= m0) return 0;
-    if (l0 >= m0 + 127) return 1;
-    return 2;
-  };
-  auto load_chunk = [&](int c, int stage) {
-    const int l0 = c * kBK, mode = chunk_mode(c);
-    const uint32_t a_base = smem_u32(sA + stage * kTileDoubles);
-    if (mode == 1) {
-      const int m = tid & 127, mu = m0 + m;
-#pragma unroll
-      for (int q = 0; q < 16; q++) {
-        const int k = (tid >> 7) + 2 * q, lam = l0 + k;
-        const bool ok = mu < nao && lam < nao;
-        const double* src = BpP + (ok ? tri(lam) + mu : 0);
-        cp_async8(a_base + (uint32_t)(k * kLdTT + m) * 8u, src, ok);
-      }
-    } else {
-      const int k = tid & 31, lam = l0 + k;
-#pragma unroll
-      for (int q = 0; q < 16; q++) {
-        const int m = (tid >> 5) + 8 * q, mu = m0 + m;
-        const bool ok = mu < nao && lam < nao;
-        size_t off = 0;
-        if (ok) off = (lam <= mu) ? tri(mu) + lam : tri(lam) + mu;
-        cp_async8(a_base + (uint32_t)(m * kLdT + k) * 8u, BpP + off, ok);
-      }
+  if (tid == 0) {
+    for (int s = 0; s < kStages; s++) {
+      mbar_init(full0 + 8 * s, 128 + 1);   // 128 cp.async arrivals + the expect_tx arrival
+      mbar_init(empty0 + 8 * s, 8);        // one arrival per consumer warp
     }
-    const uint32_t b_base = smem_u32(sB + stage * NT * kLdT);
-    for (int e = tid; e < NT * (kBK / 2); e += 256) {
-      const int n = e >> 4, k2 = (e & 15) * 2;
-      const bool ok = n0 + n < nocc_pad;
-      const double* src = Ct + (ok ? (size_t)(n0 + n) * nao_k + l0 + k2 : 0);
-      cp_async16(b_base + (uint32_t)(n * kLdT + k2) * 8u, src, ok);
-    }
-  };
+    mbar_fence_init();
+  }
+  __syncthreads();
 
+  if (w >= 8) {
+    // ===================== producer warpgroup =====================
+    reg_dec<kProducerRegs>();
+    const int tp = tid - 256;
+    const double* BpP = Bp + (size_t)(p_first + pl) * npair;
+    const int kd = tp & 15, md = tp >> 4;          // direct / crossing: element (md + 8q, kd)
+    const int mt = tp & 63, kt = tp >> 6;          // transposed:        element (mt, kt + 2q)
+    const bool okt = m0 + mt < nao;
+    const uint32_t sA_u32 = smem_u32(sA), sB_u32 = smem_u32(sB);
+    const uint32_t a_dst_d = (uint32_t)(md * kHtLd + kd) * 8u, a_dst_t = (uint32_t)(kt * kHtLdT + mt) * 8u;
+    for (int c = 0; c < nchunks; c++) {
+      const int stage = c % kStages;
+      const uint32_t fullb = full0 + 8 * stage;
+      mbar_wait(empty0 + 8 * stage, ((c / kStages) & 1) ^ 1);
+      const int l0 = c * kHtBK;
+      if (tp == 0) {
+        mbar_arrive_expect_tx(fullb, kBBytes);
+        bulk_g2s(sB_u32 + (uint32_t)stage * kBBytes, Ct + ((size_t)c * ct_rows + n0) * kHtLd, kBBytes, fullb);
+      }
+      const uint32_t a_base = sA_u32 + (uint32_t)(stage * kHtATile) * 8u;
+      if (l0 + kHtBK - 1 <= m0) {                  // stored rows, all lam <= mu
+#pragma unroll
+        for (int q = 0; q < 8; q++) {
+          const int mu = m0 + md + 8 * q;
+          const bool ok = mu < nao;
+          cp_async8(a_base + a_dst_d + (uint32_t)(q * 8 * kHtLd) * 8u,
+                    BpP + (ok ? (uint32_t)(mu * (mu + 1) / 2 + l0 + kd) : 0u), ok);
+        }
+      } else if (l0 >= m0 + 63) {                  // transpose of the stored tile, all lam >= mu
+#pragma unroll
+        for (int q = 0; q < 8; q++) {
+          const int lam = l0 + kt + 2 * q;
+          const bool ok = okt && lam < nao;
+          cp_async8(a_base + a_dst_t + (uint32_t)(q * 2 * kHtLdT) * 8u,
+                    BpP + (ok ? (uint32_t)(lam * (lam + 1) / 2 + m0 + mt) : 0u), ok);
+        }
+      } else {                                     // crossing the diagonal
+        const int lam = l0 + kd;
+#pragma unroll
+        for (int q = 0; q < 8; q++) {
+          const int mu = m0 + md + 8 * q;
+          const bool ok = mu < nao && lam < nao;
+          uint32_t off = 0;
+          if (ok) off = (lam <= mu) ? (uint32_t)(mu * (mu + 1) / 2 + lam) : (uint32_t)(lam * (lam + 1) / 2 + mu);
+          cp_async8(a_base + a_dst_d + (uint32_t)(q * 8 * kHtLd) * 8u, BpP + off, ok);
+        }
+      }
+      cp_async_mbar_arrive_noinc(fullb);
+    }
+    return;
+  }
+
+  // ===================== consumer warpgroups =====================
+  reg_inc<kConsumerRegs>();
+  const int r = l >> 2, j = l & 3;
+  const int wm = w & 3, wn = w >> 2;
   double acc[2][WN][2];
 #pragma unroll
   for (int t = 0; t < 2; t++)
 #pragma unroll
     for (int u = 0; u < WN; u++) acc[t][u][0] = acc[t][u][1] = 0.0;
 
-  for (int s = 0; s < kStages - 1; s++) {
-    if (s < nchunks) load_chunk(s, s);
-    cp_async_commit();
-  }
   for (int c = 0; c < nchunks; c++) {
-    cp_async_wait<kStages - 2>();
-    __syncthreads();
-    if (c + kStages - 1 < nchunks) load_chunk(c + kStages - 1, (c + kStages - 1) % kStages);
-    cp_async_commit();
     const int stage = c % kStages;
-    const bool tr = chunk_mode(c) == 1;
-    const int sM = tr ? 1 : kLdT, sK = tr ? kLdTT : 1;
-    const double* a_ptr = sA + stage * kTileDoubles + (w * 16 + r) * sM + j * sK;
-    const double* b_ptr = sB + stage * NT * kLdT + r * kLdT + j;
+    const int l0 = c * kHtBK;
+    const bool tr = (l0 >= m0 + 63) && !(l0 + kHtBK - 1 <= m0);
+    const int ksteps = min(4, nk4 - c * 4);
+    mbar_wait(full0 + 8 * stage, (c / kStages) & 1);
+    const double* b_ptr = sB + stage * NT * kHtLd + (wn * 8 * WN + r) * kHtLd + j;
+    if (!tr) {
+      const double* a_ptr = sA + stage * kHtATile + (wm * 16 + r) * kHtLd + j;
 #pragma unroll
-    for (int kk = 0; kk < kBK / 4; kk++) {
-      const double a0 = a_ptr[4 * kk * sK], a1 = a_ptr[8 * sM + 4 * kk * sK];
-      double b[WN];
+      for (int kk = 0; kk < 4; kk++) {
+        if (kk < ksteps) {
+          const double a0 = a_ptr[4 * kk], a1 = a_ptr[8 * kHtLd + 4 * kk];
+          double b[WN];
 #pragma unroll
-      for (int u = 0; u < WN; u++) b[u] = b_ptr[u * 8 * kLdT + 4 * kk];
+          for (int u = 0; u < WN; u++) b[u] = b_ptr[u * 8 * kHtLd + 4 * kk];
 #pragma unroll
-      for (int u = 0; u < WN; u++) {
-        dmma884(acc[0][u][0], acc[0][u][1], a0, b[u]);
-        dmma884(acc[1][u][0], acc[1][u][1], a1, b[u]);
+          for (int u = 0; u < WN; u++) {
+            dmma884(acc[0][u][0], acc[0][u][1], a0, b[u]);
+            dmma884(acc[1][u][0], acc[1][u][1], a1, b[u]);
+          }
+        }
+      }
+    } else {
+      const double* a_ptr = sA + stage * kHtATile + (wm * 16 + r) + j * kHtLdT;
+#pragma unroll
+      for (int kk = 0; kk < 4; kk++) {
+        if (kk < ksteps) {
+          const double a0 = a_ptr[4 * kk * kHtLdT], a1 = a_ptr[8 + 4 * kk * kHtLdT];
+          double b[WN];
+#pragma unroll
+          for (int u = 0; u < WN; u++) b[u] = b_ptr[u * 8 * kHtLd + 4 * kk];
+#pragma unroll
+          for (int u = 0; u < WN; u++) {
+            dmma884(acc[0][u][0], acc[0][u][1], a0, b[u]);
+            dmma884(acc[1][u][0], acc[1][u][1], a1, b[u]);
+          }
+        }
       }
     }
+    __syncwarp();
+    if (l == 0) mbar_arrive(empty0 + 8 * stage);
   }
-  cp_async_wait<0>();
-  // epilogue: lane owns X[mu][n], X[mu][n+1] with mu = m0 + 16w + 8t + r, n = n0 + 8u + 2j
-  double* Xp = X + (size_t)pl * nao * nocc_pad;
+  // epilogue: lane owns X[mu][n], X[mu][n+1] with mu = m0 + 16 wm + 8t + r, n = n0 + 8 (wn WN + u) + 2j
+  double* Xp = X + (size_t)pl * nch * mu_pad * kLdT;
 #pragma unroll
   for (int t = 0; t < 2; t++) {
-    const int mu = m0 + w * 16 + 8 * t + r;
+    const int mu = m0 + wm * 16 + 8 * t + r;
     if (mu >= nao) continue;
 #pragma unroll
     for (int u = 0; u < WN; u++) {
-      const int n = n0 + 8 * u + 2 * j;
+      const int n = n0 + 8 * (wn * WN + u) + 2 * j;
       if (n < nocc_pad)
-        *reinterpret_cast<double2*>(Xp + (size_t)mu * nocc_pad + n) = make_double2(acc[t][u][0], acc[t][u][1]);
+        *reinterpret_cast<double2*>(Xp + ((size_t)(n >> 5) * mu_pad + mu) * kLdT + (n & 31)) =
+            make_double2(acc[t][u][0], acc[t][u][1]);
     }
   }
 }
 
 // ------------------------------------------------------------------ SYRK
 // CTA: one lower-triangle 128x128 tile (ta >= tb) of K_s, one split of the block's aux rows.
-// 8 warps as 2 (M) x 4 (N), warp tile 64x32 = 8x4 MMA tiles.  The reduction runs over chunks
-// (P, 32 columns of set s); both operands are [row][k] tiles of X, the diagonal tile loads one.
-__global__ void __launch_bounds__(256, 1)
-k_syrk(const double* __restrict__ X, int nao, int ldx, int c0, int c1, int nrows_blk, int rows_per_split,
-       int ntiles_m, double* __restrict__ Kpart_s, size_t split_stride, int first) {
-  extern __shared__ __align__(16) double smem[];
+// Consumers: 2 (M) x 4 (N) warps, warp tile 64x32 = 8x4 MMA tiles.  The reduction runs over
+// (aux row, 32-column chunk of X) pairs; a chunk that straddles two sets contributes only the k4
+// steps of this set.  Both operand tiles are contiguous 128x36 blocks of the tiled X, fetched by
+// one elected producer thread with bulk async copies; the diagonal tile fetches one.
+constexpr int kTileDoubles = 128 * kLdT;            // 4608
+constexpr uint32_t kTileBytes = kTileDoubles * 8;   // 36864
+
+__global__ void __launch_bounds__(kThreads, 1)
+k_syrk(const double* __restrict__ X, int nao, int nch, int mu_pad, int c0, int c1, int nrows_blk,
+       int rows_per_split, int ntiles_m, double* __restrict__ Kpart_s, size_t split_stride, int first) {
+  extern __shared__ __align__(128) double smem[];
   double* sA = smem;
   double* sB = smem + kStages * kTileDoubles;
-  const int tid = threadIdx.x, w = tid >> 5, l = tid & 31, r = l >> 2, j = l & 3;
-  const int wm = w >> 2, wn = w & 3;
+  __shared__ __align__(8) unsigned long long bars[2 * kStages];
+  const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kStages]);
+  const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
   // tile index -> (ta, tb), ta >= tb
   const int ntiles = ntiles_m * (ntiles_m + 1) / 2;
   const int t = blockIdx.x % ntiles, g = blockIdx.x / ntiles;
@@ -146,64 +210,88 @@ k_syrk(const double* __restrict__ X, int nao, int ldx, int c0, int c1, int nrows
   int p_end = p_beg + rows_per_split;
   if (p_end > nrows_blk) p_end = nrows_blk;
   const int np = p_end > p_beg ? p_end - p_beg : 0;
-  const int cps = (c1 - c0 + kBK - 1) / kBK;   // chunks per aux row
+  const int ch0 = c0 >> 5, ch1 = (c1 + 31) >> 5;   // X chunks that hold columns of this set
+  const int cps = ch1 - ch0;
   const int nchunks = np * cps;
 
-  auto load_chunk = [&](int c, int stage) {
-    const int P = p_beg + c / cps, i0 = c0 + (c % cps) * kBK;
-    const int klen = min(kBK, c1 - i0);          // multiple of 8
-    const double* Xp = X + (size_t)P * nao * ldx + i0;
-    const uint32_t a_base = smem_u32(sA + stage * kTileDoubles);
-    const uint32_t b_base = smem_u32(sB + stage * kTileDoubles);
-    const int k2 = (tid & 15) * 2;
-    if (k2 < klen) {
-#pragma unroll
-      for (int q = 0; q < 8; q++) {
-        const int m = (tid >> 4) + 16 * q;
-        const bool oka = a0 + m < nao;
-        cp_async16(a_base + (uint32_t)(m * kLdT + k2) * 8u, Xp + (oka ? (size_t)(a0 + m) * ldx + k2 : 0), oka);
-        if (!diag) {
-          const bool okb = b0 + m < nao;
-          cp_async16(b_base + (uint32_t)(m * kLdT + k2) * 8u, Xp + (okb ? (size_t)(b0 + m) * ldx + k2 : 0), okb);
-        }
+  if (tid == 0) {
+    for (int s = 0; s < kStages; s++) {
+      mbar_init(full0 + 8 * s, 1);         // the expect_tx arrival of the elected producer
+      mbar_init(empty0 + 8 * s, 8);        // one arrival per consumer warp
+    }
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  if (w >= 8) {
+    // ===================== producer warpgroup (one elected thread works) =====================
+    reg_dec<kProducerRegs>();
+    if (tid == 256) {
+      const uint32_t sA_u32 = smem_u32(sA), sB_u32 = smem_u32(sB);
+      const size_t chunk_stride = (size_t)mu_pad * kLdT, row_stride = (size_t)nch * chunk_stride;
+      int P = p_beg, ch = ch0;
+      for (int c = 0; c < nchunks; c++) {
+        const int stage = c % kStages;
+        const uint32_t fullb = full0 + 8 * stage;
+        mbar_wait(empty0 + 8 * stage, ((c / kStages) & 1) ^ 1);
+        const double* src = X + (size_t)P * row_stride + (size_t)ch * chunk_stride;
+        mbar_arrive_expect_tx(fullb, diag ? kTileBytes : 2 * kTileBytes);
+        bulk_g2s(sA_u32 + (uint32_t)stage * kTileBytes, src + (size_t)a0 * kLdT, kTileBytes, fullb);
+        if (!diag) bulk_g2s(sB_u32 + (uint32_t)stage * kTileBytes, src + (size_t)b0 * kLdT, kTileBytes, fullb);
+        if (++ch == ch1) { ch = ch0; P++; }
       }
     }
-  };
+    return;
+  }
 
+  // ===================== consumer warpgroups =====================
+  reg_inc<kConsumerRegs>();
+  const int r = l >> 2, j = l & 3;
+  const int wm = w >> 2, wn = w & 3;
   double acc[8][4][2];
 #pragma unroll
   for (int tt = 0; tt < 8; tt++)
 #pragma unroll
     for (int u = 0; u < 4; u++) acc[tt][u][0] = acc[tt][u][1] = 0.0;
 
-  for (int s = 0; s < kStages - 1; s++) {
-    if (s < nchunks) load_chunk(s, s);
-    cp_async_commit();
-  }
+  int ch = ch0;
   for (int c = 0; c < nchunks; c++) {
-    cp_async_wait<kStages - 2>();
-    __syncthreads();
-    if (c + kStages - 1 < nchunks) load_chunk(c + kStages - 1, (c + kStages - 1) % kStages);
-    cp_async_commit();
     const int stage = c % kStages;
-    const int i0 = c0 + (c % cps) * kBK;
-    const int ksteps = min(kBK, c1 - i0) / 4;
+    // k4 steps of this chunk that belong to the set: columns [max(c0, 32 ch), min(c1, 32 ch + 32))
+    const int k_lo = (max(c0, ch * 32) - ch * 32) >> 2, k_hi = (min(c1, ch * 32 + 32) - ch * 32) >> 2;
+    if (++ch == ch1) ch = ch0;
+    mbar_wait(full0 + 8 * stage, (c / kStages) & 1);
     const double* a_ptr = sA + stage * kTileDoubles + (wm * 64 + r) * kLdT + j;
     const double* b_ptr = (diag ? sA : sB) + stage * kTileDoubles + (wn * 32 + r) * kLdT + j;
-#pragma unroll 2
-    for (int kk = 0; kk < ksteps; kk++) {
-      double a[8], b[4];
+    if (k_lo == 0 && k_hi == 8) {
 #pragma unroll
-      for (int tt = 0; tt < 8; tt++) a[tt] = a_ptr[tt * 8 * kLdT + 4 * kk];
+      for (int kk = 0; kk < 8; kk++) {
+        double a[8], b[4];
 #pragma unroll
-      for (int u = 0; u < 4; u++) b[u] = b_ptr[u * 8 * kLdT + 4 * kk];
+        for (int tt = 0; tt < 8; tt++) a[tt] = a_ptr[tt * 8 * kLdT + 4 * kk];
 #pragma unroll
-      for (int tt = 0; tt < 8; tt++)
+        for (int u = 0; u < 4; u++) b[u] = b_ptr[u * 8 * kLdT + 4 * kk];
 #pragma unroll
-        for (int u = 0; u < 4; u++) dmma884(acc[tt][u][0], acc[tt][u][1], a[tt], b[u]);
+        for (int tt = 0; tt < 8; tt++)
+#pragma unroll
+          for (int u = 0; u < 4; u++) dmma884(acc[tt][u][0], acc[tt][u][1], a[tt], b[u]);
+      }
+    } else {
+      for (int kk = k_lo; kk < k_hi; kk++) {
+        double a[8], b[4];
+#pragma unroll
+        for (int tt = 0; tt < 8; tt++) a[tt] = a_ptr[tt * 8 * kLdT + 4 * kk];
+#pragma unroll
+        for (int u = 0; u < 4; u++) b[u] = b_ptr[u * 8 * kLdT + 4 * kk];
+#pragma unroll
+        for (int tt = 0; tt < 8; tt++)
+#pragma unroll
+          for (int u = 0; u < 4; u++) dmma884(acc[tt][u][0], acc[tt][u][1], a[tt], b[u]);
+      }
     }
+    __syncwarp();
+    if (l == 0) mbar_arrive(empty0 + 8 * stage);
   }
-  cp_async_wait<0>();
   // read-modify-write this CTA's private partial tile (full 128x128, also above the diagonal of
   // a diagonal tile; the epilogue reads mu >= nu only)
   double* Kp = Kpart_s + (size_t)g * split_stride;
@@ -256,31 +344,36 @@ __global__ void k_zero(double* p, size_t n) {
 }
 
 // ------------------------------------------------------------------ launchers (step a8)
-static size_t ht_smem_bytes(int wn) { return (size_t)kStages * (kTileDoubles + 8 * wn * kLdT) * sizeof(double); }
+static size_t ht_smem_bytes(int wn) { return (size_t)kStages * (kHtATile + 16 * wn * kHtLd) * sizeof(double); }
 static size_t syrk_smem_bytes() { return (size_t)kStages * 2 * kTileDoubles * sizeof(double); }
 
+struct HtArgs {
+  const double* Bp; size_t npair; int nao; const double* Ct; int ct_rows; int nocc_pad; double* X;
+  int nch; int mu_pad; int p_first;
+};
+
 template <int WN>
-static cudaError_t launch_ht(dim3 grid, cudaStream_t st, const double* Bp, size_t npair, int nao, int nao_k,
-                             const double* Ct, int nocc_pad, double* X, int p_first) {
-  static bool attr_set = false;  // per-process, per-instantiation; the attribute is per-function
+static cudaError_t launch_ht(dim3 grid, cudaStream_t st, const HtArgs& a) {
+  static bool attr_set = false;  // the attribute is per function (per instantiation)
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(k_half_transform<WN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)ht_smem_bytes(WN));
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  k_half_transform<WN><<<grid, 256, ht_smem_bytes(WN), st>>>(Bp, npair, nao, nao_k, Ct, nocc_pad, X, p_first);
+  k_half_transform<WN><<<grid, kThreads, ht_smem_bytes(WN), st>>>(a.Bp, a.npair, a.nao, a.Ct, a.ct_rows, a.nocc_pad,
+                                                                   a.X, a.nch, a.mu_pad, a.p_first);
   return cudaSuccess;
 }
 
-static cudaError_t dispatch_ht(int wn, dim3 grid, cudaStream_t st, const double* Bp, size_t npair, int nao,
-                               int nao_k, const double* Ct, int nocc_pad, double* X, int p_first) {
+static cudaError_t dispatch_ht(int wn, dim3 grid, cudaStream_t st, const HtArgs& a) {
   switch (wn) {
 #define DFJK_HT_CASE(N) \
-  case N: return launch_ht<N>(grid, st, Bp, npair, nao, nao_k, Ct, nocc_pad, X, p_first);
+  case N: return launch_ht<N>(grid, st, a);
     DFJK_HT_CASE(1) DFJK_HT_CASE(2) DFJK_HT_CASE(3) DFJK_HT_CASE(4) DFJK_HT_CASE(5) DFJK_HT_CASE(6)
     DFJK_HT_CASE(7) DFJK_HT_CASE(8) DFJK_HT_CASE(9) DFJK_HT_CASE(10) DFJK_HT_CASE(11) DFJK_HT_CASE(12)
-    DFJK_HT_CASE(13) DFJK_HT_CASE(14) DFJK_HT_CASE(15) DFJK_HT_CASE(16)
+    DFJK_HT_CASE(13) DFJK_HT_CASE(14) DFJK_HT_CASE(15) DFJK_HT_CASE(16) DFJK_HT_CASE(17) DFJK_HT_CASE(18)
+    DFJK_HT_CASE(19) DFJK_HT_CASE(20)
 #undef DFJK_HT_CASE
     default: return cudaErrorInvalidValue;
   }
@@ -304,21 +397,30 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, cudaStream_t st
   if (naux == 0 || ldx == 0) return launches;
 
   // plan: aux block size from the workspace, N tiling of the half-transform, split-K of the SYRK
-  const size_t row_bytes = (size_t)nao * ldx * sizeof(double);
-  long long nblk = (long long)(h->X_doubles * sizeof(double) / row_bytes);
+  const int nch = cdiv(ldx, kBK);
+  const size_t row_doubles = (size_t)nch * h->mu_pad * kLdT;     // tiled X, one aux row
+  long long nblk = (long long)(h->X_doubles / row_doubles);
   if (h->nblk_forced > 0 && nblk > h->nblk_forced) nblk = h->nblk_forced;
   if (nblk > naux) nblk = naux;
   if (nblk > 32768) nblk = 32768;
   if (nblk < 1) nblk = 1;
   const int n8 = ldx / 8;
-  const int ntn = cdiv(n8, 16), wn = cdiv(n8, ntn);
+  const int ntn = cdiv(n8, 2 * kHtMaxWN), wn = cdiv(n8, 2 * ntn);  // N tile = 16*wn columns
+  const int ntm_ht = cdiv(nao, 64);
   const int ntm = h->n_mtiles, ntiles = ntm * (ntm + 1) / 2;
   int ksplit = h->ksplit_forced;
   if (ksplit <= 0) {
-    // fill the 148 SMs (one SYRK CTA each) about three times over with the heaviest set
-    ksplit = cdiv(3 * 148, ntiles);
-    if (ksplit > h->ksplit) ksplit = h->ksplit;
+    // one SYRK CTA per SM: pick the split that fills whole waves of 148 CTAs (about three) best
+    double best = -1.0;
+    ksplit = 1;
+    for (int k = 1; k <= h->ksplit; k++) {
+      const int ctas = ntiles * k, waves = cdiv(ctas, 148);
+      if (waves > 4) break;
+      const double eff = (double)ctas / (148.0 * waves) - 0.01 * (waves < 2) - 0.005 * (waves < 3);
+      if (eff > best) { best = eff; ksplit = k; }
+    }
   }
+  if (ksplit > h->ksplit) ksplit = h->ksplit;
   if (ksplit > nblk) ksplit = (int)nblk;
   if (ksplit < 1) ksplit = 1;
   const size_t split_stride = (size_t)h->max_nset * n2;
@@ -332,16 +434,18 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, cudaStream_t st
   int nblocks = 0;
   for (int p0 = 0; p0 < naux; p0 += (int)nblk, nblocks++) {
     const int nb = (int)(naux - p0 < nblk ? naux - p0 : nblk);
-    dim3 gh(ntn, ntm, nb);
+    dim3 gh(ntn, ntm_ht, nb);
     prof_mark(h, DFJK_PHASE_HALF_TRANSFORM, st);
-    if (dispatch_ht(wn, gh, st, h->B, h->npair, nao, h->nao_k, h->Ct, ldx, h->X, p0) != cudaSuccess) return -1;
+    HtArgs a{h->B, h->npair, nao, h->Ct, h->ct_rows, ldx, h->X, nch, h->mu_pad, p0};
+    if (dispatch_ht(wn, gh, st, a) != cudaSuccess) return -1;
     launches++;
     const int rps = cdiv(nb, ksplit);
     prof_mark(h, DFJK_PHASE_SYRK, st);
     for (int s = 0; s < si.nset; s++) {
       if (si.col0[s + 1] == si.col0[s]) continue;
-      k_syrk<<<ntiles * ksplit, 256, syrk_smem_bytes(), st>>>(h->X, nao, ldx, si.col0[s], si.col0[s + 1], nb, rps,
-                                                            ntm, h->Kpart + n2 * s, split_stride, p0 == 0 ? 1 : 0);
+      k_syrk<<<ntiles * ksplit, kThreads, syrk_smem_bytes(), st>>>(h->X, nao, nch, h->mu_pad, si.col0[s], si.col0[s + 1],
+                                                                 nb, rps, ntm, h->Kpart + n2 * s, split_stride,
+                                                                 p0 == 0 ? 1 : 0);
       launches++;
     }
   }

@@ -1,7 +1,9 @@
 // Step a1, density prep (Eq. 14 needs D; Eq. 16 needs gamma = C n C^T):
 //   Ct[i][lam]  = sqrt(n_i) C[lam][i]   all sets concatenated, each set padded to 8 columns with
-//                                       zeros, lam padded to kBK with zeros (k-contiguous operand
-//                                       of the half-transform);
+//                                       zeros, lam padded to a multiple of 16 with zeros; stored
+//                                       k-tiled as Ct[(lam/16 * ct_rows + i) * 20 + lam%16] so that
+//                                       the half-transform fetches a whole k-chunk of its B operand
+//                                       with one bulk copy, already in the padded smem layout;
 //   Dw_s[pair]  = (2 - delta_{mu nu}) sum_i Ct[i][mu] Ct[i][nu]   packed, off-diagonal weight 2, so
 //                 that the packed dot product with B_P equals the full-square sum of Eq. 14.
 #include "common.cuh"
@@ -11,7 +13,7 @@ namespace dfjk {
 
 __global__ void __launch_bounds__(256)
 k_prep_ct(const __grid_constant__ SetInfo si, const double* __restrict__ C, const double* __restrict__ occ,
-          double* __restrict__ Ct, int nao, int nao_k) {
+          double* __restrict__ Ct, int nao, int nk_pad, int ct_rows) {
   __shared__ double t[32][33];
   const int tx = threadIdx.x, ty = threadIdx.y;
   const int lam0 = blockIdx.x * 32, ip0 = blockIdx.y * 32;
@@ -35,14 +37,15 @@ k_prep_ct(const __grid_constant__ SetInfo si, const double* __restrict__ C, cons
   __syncthreads();
   for (int r = ty; r < 32; r += 8) {
     const int ipw = ip0 + r, lam = lam0 + tx;
-    if (ipw < si.nocc_pad && lam < nao_k) Ct[(size_t)ipw * nao_k + lam] = t[tx][r];
+    if (ipw < si.nocc_pad && lam < nk_pad)
+      Ct[((size_t)(lam >> 4) * ct_rows + ipw) * kHtLd + (lam & 15)] = t[tx][r];
   }
 }
 
 // 64x64 tile of D_s per CTA, 4x4 per thread, plain DFMA (0.4 GFLOP at nao=1200: negligible).
 __global__ void __launch_bounds__(256)
 k_prep_dw(const __grid_constant__ SetInfo si, const double* __restrict__ Ct, double* __restrict__ Dw,
-          int nao, int nao_k, size_t npair) {
+          int nao, int nk_pad, int ct_rows, size_t npair) {
   const int bi = blockIdx.x, bj = blockIdx.y, s = blockIdx.z;
   if (bj > bi) return;
   __shared__ double As[16][64], Bs[16][64];
@@ -57,8 +60,8 @@ k_prep_dw(const __grid_constant__ SetInfo si, const double* __restrict__ Ct, dou
     for (int e = tid; e < 16 * 64; e += 256) {
       const int ii = e >> 6, m = e & 63, i = i0 + ii;
       const int la = bi * 64 + m, lb = bj * 64 + m;
-      As[ii][m] = (i < c1 && la < nao_k) ? Ct[(size_t)i * nao_k + la] : 0.0;
-      Bs[ii][m] = (i < c1 && lb < nao_k) ? Ct[(size_t)i * nao_k + lb] : 0.0;
+      As[ii][m] = (i < c1 && la < nk_pad) ? Ct[((size_t)(la >> 4) * ct_rows + i) * kHtLd + (la & 15)] : 0.0;
+      Bs[ii][m] = (i < c1 && lb < nk_pad) ? Ct[((size_t)(lb >> 4) * ct_rows + i) * kHtLd + (lb & 15)] : 0.0;
     }
     __syncthreads();
 #pragma unroll
@@ -91,8 +94,8 @@ k_prep_dw(const __grid_constant__ SetInfo si, const double* __restrict__ Ct, dou
 int launch_prep_ct(dfjk_ctx* h, const SetInfo& si, const double* C, const double* occ, cudaStream_t st) {
   if (si.nocc_pad == 0) return 0;
   prof_mark(h, DFJK_PHASE_PREP, st);
-  dim3 grid(cdiv(h->nao_k, 32), cdiv(si.nocc_pad, 32)), block(32, 8);
-  k_prep_ct<<<grid, block, 0, st>>>(si, C, occ, h->Ct, h->nao, h->nao_k);
+  dim3 grid(cdiv(h->nck * kHtBK, 32), cdiv(si.nocc_pad, 32)), block(32, 8);
+  k_prep_ct<<<grid, block, 0, st>>>(si, C, occ, h->Ct, h->nao, h->nck * kHtBK, h->ct_rows);
   return 1;
 }
 
@@ -100,7 +103,7 @@ int launch_prep_dw(dfjk_ctx* h, const SetInfo& si, cudaStream_t st) {
   prof_mark(h, DFJK_PHASE_PREP, st);
   const int nb = cdiv(h->nao, 64);
   dim3 grid(nb, nb, si.nset);
-  k_prep_dw<<<grid, 256, 0, st>>>(si, h->Ct, h->Dw, h->nao, h->nao_k, h->npair);
+  k_prep_dw<<<grid, 256, 0, st>>>(si, h->Ct, h->Dw, h->nao, h->nck * kHtBK, h->ct_rows, h->npair);
   return 1;
 }
 
