@@ -100,7 +100,7 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   h->naux = naux; h->nao = nao; h->device = dev;
   h->npair = (size_t)nao * (nao + 1) / 2;
   h->nck = cdiv(nao, kHtBK);
-  h->mu_pad = round_up(nao, 128);
+  h->mu_pad = round_up(nao, 8) + 128;   // any SYRK tile of <= 128 rows stays inside the tiled X
   h->max_nset = o.max_nset ? o.max_nset : 8;
   h->max_nocc_total = o.max_nocc_total ? o.max_nocc_total : nao;
   h->nocc_pad_cap = round_up(h->max_nocc_total + 7 * h->max_nset, 8);
@@ -108,12 +108,8 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   h->n_mtiles = cdiv(nao, 128);
   h->nblk_forced = o.nblk;
   h->ksplit_forced = o.ksplit;
-  // split-K partial slots: enough to fill the SMs about three times with one set's tiles
-  {
-    const int ntiles = h->n_mtiles * (h->n_mtiles + 1) / 2;
-    h->ksplit = o.ksplit ? o.ksplit : cdiv(4 * 148, ntiles);
-    if (h->ksplit > 64 && !o.ksplit) h->ksplit = 64;
-  }
+  // split-K partial slots of the SYRK (each is max_nset x nao x nao doubles)
+  h->ksplit = o.ksplit ? o.ksplit : 16;
   // X capacity (k-tiled layout [nch][mu_pad][36] per aux row): the cap, but at least one aux row
   // at full column capacity
   {

@@ -180,17 +180,81 @@ k_half_transform(const double* __restrict__ Bp, size_t npair, int nao, const dou
 }
 
 // ------------------------------------------------------------------ SYRK
-// CTA: one lower-triangle 128x128 tile (ta >= tb) of K_s, one split of the block's aux rows.
-// Consumers: 2 (M) x 4 (N) warps, warp tile 64x32 = 8x4 MMA tiles.  The reduction runs over
-// (aux row, 32-column chunk of X) pairs; a chunk that straddles two sets contributes only the k4
-// steps of this set.  Both operand tiles are contiguous 128x36 blocks of the tiled X, fetched by
-// one elected producer thread with bulk async copies; the diagonal tile fetches one.
-constexpr int kTileDoubles = 128 * kLdT;            // 4608
-constexpr uint32_t kTileBytes = kTileDoubles * 8;   // 36864
+// CTA: one lower-triangle T x T tile (ta >= tb) of K_s, T = 16*WM in {64,80,96,112,128} chosen per
+// nao to minimise padding, and one split of the block's aux rows.  Consumers: 2 warp rows of
+// WM MMA tiles each, 4 warp columns of ceil(WM/2), ceil(WM/2), floor(WM/2), floor(WM/2) MMA tiles;
+// every SM sub-partition hosts one wide and one narrow warp of the same warp row, so all four
+// issue WM*WM DMMAs per k4 step.  The reduction runs over (aux row, 32-column chunk of X) pairs;
+// a chunk that straddles two sets contributes only the k4 steps of this set.  Both operand tiles
+// are contiguous T x 36 blocks of the tiled X, fetched by one elected producer thread with bulk
+// async copies; the diagonal tile fetches one.
+struct SyrkConsumerArgs {
+  const double* sA; const double* sB; uint32_t full0, empty0;
+  int nchunks, ch0, ch1, c0, c1, tile_doubles, row0, col0, a0, b0, nao, first;
+  double* Kp;
+};
 
+// One consumer warp: rows [row0, row0 + 8 WM), columns [col0, col0 + 8 NC) of the CTA tile.
+template <int WM, int NC>
+__device__ __forceinline__ void syrk_consume(const SyrkConsumerArgs& q, int l) {
+  const int r = l >> 2, j = l & 3;
+  double acc[WM][NC][2];
+#pragma unroll
+  for (int tt = 0; tt < WM; tt++)
+#pragma unroll
+    for (int u = 0; u < NC; u++) acc[tt][u][0] = acc[tt][u][1] = 0.0;
+  int ch = q.ch0;
+  for (int c = 0; c < q.nchunks; c++) {
+    const int stage = c % kStages;
+    // k4 steps of this chunk that belong to the set: columns [max(c0, 32 ch), min(c1, 32 ch + 32))
+    const int k_lo = (max(q.c0, ch * 32) - ch * 32) >> 2, k_hi = (min(q.c1, ch * 32 + 32) - ch * 32) >> 2;
+    if (++ch == q.ch1) ch = q.ch0;
+    mbar_wait(q.full0 + 8 * stage, (c / kStages) & 1);
+    const double* a_ptr = q.sA + stage * q.tile_doubles + (q.row0 + r) * kLdT + j;
+    const double* b_ptr = q.sB + stage * q.tile_doubles + (q.col0 + r) * kLdT + j;
+    auto step = [&](int kk) {
+      double a[WM], b[NC];
+#pragma unroll
+      for (int tt = 0; tt < WM; tt++) a[tt] = a_ptr[tt * 8 * kLdT + 4 * kk];
+#pragma unroll
+      for (int u = 0; u < NC; u++) b[u] = b_ptr[u * 8 * kLdT + 4 * kk];
+#pragma unroll
+      for (int tt = 0; tt < WM; tt++)
+#pragma unroll
+        for (int u = 0; u < NC; u++) dmma884(acc[tt][u][0], acc[tt][u][1], a[tt], b[u]);
+    };
+    if (k_lo == 0 && k_hi == 8) {
+#pragma unroll
+      for (int kk = 0; kk < 8; kk++) step(kk);
+    } else {
+      for (int kk = k_lo; kk < k_hi; kk++) step(kk);
+    }
+    __syncwarp();
+    if (l == 0) mbar_arrive(q.empty0 + 8 * stage);
+  }
+  // read-modify-write this CTA's private partial tile (also above the diagonal of a diagonal
+  // tile; the epilogue reads mu >= nu only)
+#pragma unroll
+  for (int tt = 0; tt < WM; tt++) {
+    const int mu = q.a0 + q.row0 + tt * 8 + r;
+    if (mu >= q.nao) continue;
+#pragma unroll
+    for (int u = 0; u < NC; u++) {
+      const int nu = q.b0 + q.col0 + u * 8 + 2 * j;
+      double* p = q.Kp + (size_t)mu * q.nao + nu;
+      if (nu < q.nao) p[0] = q.first ? acc[tt][u][0] : p[0] + acc[tt][u][0];
+      if (nu + 1 < q.nao) p[1] = q.first ? acc[tt][u][1] : p[1] + acc[tt][u][1];
+    }
+  }
+}
+
+template <int WM>
 __global__ void __launch_bounds__(kThreads, 1)
 k_syrk(const double* __restrict__ X, int nao, int nch, int mu_pad, int c0, int c1, int nrows_blk,
        int rows_per_split, int ntiles_m, double* __restrict__ Kpart_s, size_t split_stride, int first) {
+  constexpr int T = 16 * WM, WNA = (WM + 1) / 2, WNB = WM / 2;
+  constexpr int kTileDoubles = T * kLdT;
+  constexpr uint32_t kTileBytes = kTileDoubles * 8;
   extern __shared__ __align__(128) double smem[];
   double* sA = smem;
   double* sB = smem + kStages * kTileDoubles;
@@ -205,7 +269,7 @@ k_syrk(const double* __restrict__ X, int nao, int nch, int mu_pad, int c0, int c
   while (ta * (ta + 1) / 2 > t) ta--;
   const int tb = t - ta * (ta + 1) / 2;
   const bool diag = ta == tb;
-  const int a0 = ta * 128, b0 = tb * 128;
+  const int a0 = ta * T, b0 = tb * T;
   const int p_beg = g * rows_per_split;
   int p_end = p_beg + rows_per_split;
   if (p_end > nrows_blk) p_end = nrows_blk;
@@ -246,67 +310,14 @@ k_syrk(const double* __restrict__ X, int nao, int nch, int mu_pad, int c0, int c
 
   // ===================== consumer warpgroups =====================
   reg_inc<kConsumerRegs>();
-  const int r = l >> 2, j = l & 3;
-  const int wm = w >> 2, wn = w & 3;
-  double acc[8][4][2];
-#pragma unroll
-  for (int tt = 0; tt < 8; tt++)
-#pragma unroll
-    for (int u = 0; u < 4; u++) acc[tt][u][0] = acc[tt][u][1] = 0.0;
-
-  int ch = ch0;
-  for (int c = 0; c < nchunks; c++) {
-    const int stage = c % kStages;
-    // k4 steps of this chunk that belong to the set: columns [max(c0, 32 ch), min(c1, 32 ch + 32))
-    const int k_lo = (max(c0, ch * 32) - ch * 32) >> 2, k_hi = (min(c1, ch * 32 + 32) - ch * 32) >> 2;
-    if (++ch == ch1) ch = ch0;
-    mbar_wait(full0 + 8 * stage, (c / kStages) & 1);
-    const double* a_ptr = sA + stage * kTileDoubles + (wm * 64 + r) * kLdT + j;
-    const double* b_ptr = (diag ? sA : sB) + stage * kTileDoubles + (wn * 32 + r) * kLdT + j;
-    if (k_lo == 0 && k_hi == 8) {
-#pragma unroll
-      for (int kk = 0; kk < 8; kk++) {
-        double a[8], b[4];
-#pragma unroll
-        for (int tt = 0; tt < 8; tt++) a[tt] = a_ptr[tt * 8 * kLdT + 4 * kk];
-#pragma unroll
-        for (int u = 0; u < 4; u++) b[u] = b_ptr[u * 8 * kLdT + 4 * kk];
-#pragma unroll
-        for (int tt = 0; tt < 8; tt++)
-#pragma unroll
-          for (int u = 0; u < 4; u++) dmma884(acc[tt][u][0], acc[tt][u][1], a[tt], b[u]);
-      }
-    } else {
-      for (int kk = k_lo; kk < k_hi; kk++) {
-        double a[8], b[4];
-#pragma unroll
-        for (int tt = 0; tt < 8; tt++) a[tt] = a_ptr[tt * 8 * kLdT + 4 * kk];
-#pragma unroll
-        for (int u = 0; u < 4; u++) b[u] = b_ptr[u * 8 * kLdT + 4 * kk];
-#pragma unroll
-        for (int tt = 0; tt < 8; tt++)
-#pragma unroll
-          for (int u = 0; u < 4; u++) dmma884(acc[tt][u][0], acc[tt][u][1], a[tt], b[u]);
-      }
-    }
-    __syncwarp();
-    if (l == 0) mbar_arrive(empty0 + 8 * stage);
-  }
-  // read-modify-write this CTA's private partial tile (full 128x128, also above the diagonal of
-  // a diagonal tile; the epilogue reads mu >= nu only)
-  double* Kp = Kpart_s + (size_t)g * split_stride;
-#pragma unroll
-  for (int tt = 0; tt < 8; tt++) {
-    const int mu = a0 + wm * 64 + 8 * tt + r;
-    if (mu >= nao) continue;
-#pragma unroll
-    for (int u = 0; u < 4; u++) {
-      const int nu = b0 + wn * 32 + 8 * u + 2 * j;
-      double* p = Kp + (size_t)mu * nao + nu;
-      if (nu < nao) p[0] = first ? acc[tt][u][0] : p[0] + acc[tt][u][0];
-      if (nu + 1 < nao) p[1] = first ? acc[tt][u][1] : p[1] + acc[tt][u][1];
-    }
-  }
+  const int sp = w & 3;                              // SM sub-partition of this warp
+  const bool wide = (w >> 2) == 0;                   // wide (WNA tiles) or narrow (WNB tiles) warp
+  const int wm = sp & 1;
+  const int col8 = wide ? (sp >> 1) * WNA : 2 * WNA + (sp >> 1) * WNB;   // first MMA tile column
+  SyrkConsumerArgs ca{sA, diag ? sA : sB, full0, empty0, nchunks, ch0, ch1, c0, c1, kTileDoubles,
+                      wm * 8 * WM, col8 * 8, a0, b0, nao, first, Kpart_s + (size_t)g * split_stride};
+  if (wide) syrk_consume<WM, WNA>(ca, l);
+  else syrk_consume<WM, WNB>(ca, l);
 }
 
 // Step a9: K_s[mu][nu] = K_s[nu][mu] = sum_g Kpart[g][s][mu][nu] for mu >= nu, g ascending.
@@ -345,7 +356,7 @@ __global__ void k_zero(double* p, size_t n) {
 
 // ------------------------------------------------------------------ launchers (step a8)
 static size_t ht_smem_bytes(int wn) { return (size_t)kStages * (kHtATile + 16 * wn * kHtLd) * sizeof(double); }
-static size_t syrk_smem_bytes() { return (size_t)kStages * 2 * kTileDoubles * sizeof(double); }
+static size_t syrk_smem_bytes(int wm) { return (size_t)kStages * 2 * (16 * wm * kLdT) * sizeof(double); }
 
 struct HtArgs {
   const double* Bp; size_t npair; int nao; const double* Ct; int ct_rows; int nocc_pad; double* X;
@@ -379,6 +390,37 @@ static cudaError_t dispatch_ht(int wn, dim3 grid, cudaStream_t st, const HtArgs&
   }
 }
 
+struct SyrkArgs {
+  const double* X; int nao, nch, mu_pad, c0, c1, nrows_blk, rows_per_split, ntiles_m; double* Kpart_s;
+  size_t split_stride; int first;
+};
+
+template <int WM>
+static cudaError_t launch_syrk(int grid, cudaStream_t st, const SyrkArgs& a) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(k_syrk<WM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)syrk_smem_bytes(WM));
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  k_syrk<WM><<<grid, kThreads, syrk_smem_bytes(WM), st>>>(a.X, a.nao, a.nch, a.mu_pad, a.c0, a.c1, a.nrows_blk,
+                                                        a.rows_per_split, a.ntiles_m, a.Kpart_s, a.split_stride,
+                                                        a.first);
+  return cudaSuccess;
+}
+
+static cudaError_t dispatch_syrk(int wm, int grid, cudaStream_t st, const SyrkArgs& a) {
+  switch (wm) {
+    case 4: return launch_syrk<4>(grid, st, a);
+    case 5: return launch_syrk<5>(grid, st, a);
+    case 6: return launch_syrk<6>(grid, st, a);
+    case 7: return launch_syrk<7>(grid, st, a);
+    case 8: return launch_syrk<8>(grid, st, a);
+    default: return cudaErrorInvalidValue;
+  }
+}
+
 // Aux-block scheduler: cap the X workspace, pick the split-K factor, enqueue
 // half-transform and SYRK block after block on one stream.  No allocation, no host sync.
 int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, cudaStream_t st) {
@@ -407,16 +449,28 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, cudaStream_t st
   const int n8 = ldx / 8;
   const int ntn = cdiv(n8, 2 * kHtMaxWN), wn = cdiv(n8, 2 * ntn);  // N tile = 16*wn columns
   const int ntm_ht = cdiv(nao, 64);
-  const int ntm = h->n_mtiles, ntiles = ntm * (ntm + 1) / 2;
+  // SYRK tile T = 16*wm_s in {64,...,128}: least executed area ntiles*T^2 (ties -> larger tile)
+  int wm_s = 8;
+  {
+    double best = 1e300;
+    for (int wmc = 8; wmc >= 4; wmc--) {
+      const int T = 16 * wmc, nt = cdiv(nao, T);
+      const double area = 0.5 * nt * (nt + 1) * (double)T * T;
+      if (area < best * 0.995) { best = area; wm_s = wmc; }
+    }
+  }
+  const int ntm = cdiv(nao, 16 * wm_s), ntiles = ntm * (ntm + 1) / 2;
   int ksplit = h->ksplit_forced;
   if (ksplit <= 0) {
-    // one SYRK CTA per SM: pick the split that fills whole waves of 148 CTAs (about three) best
+    // one SYRK CTA per SM; a CTA's work is its rows_per_split aux rows.  Pick the split with the
+    // best modelled efficiency  ntiles*nb / (148 * waves * rows_per_split), fewer splits on ties.
+    const int nb0 = (int)nblk;
     double best = -1.0;
     ksplit = 1;
-    for (int k = 1; k <= h->ksplit; k++) {
-      const int ctas = ntiles * k, waves = cdiv(ctas, 148);
-      if (waves > 4) break;
-      const double eff = (double)ctas / (148.0 * waves) - 0.01 * (waves < 2) - 0.005 * (waves < 3);
+    for (int k = 1; k <= h->ksplit && k <= nb0; k++) {
+      const int rps = cdiv(nb0, k), kk = cdiv(nb0, rps);          // splits that actually get rows
+      const int waves = cdiv(ntiles * kk, 148);
+      const double eff = (double)ntiles * nb0 / (148.0 * waves * rps) - 0.002 * k;
       if (eff > best) { best = eff; ksplit = k; }
     }
   }
@@ -425,12 +479,6 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, cudaStream_t st
   if (ksplit < 1) ksplit = 1;
   const size_t split_stride = (size_t)h->max_nset * n2;
 
-  static bool syrk_attr = false;
-  if (!syrk_attr) {
-    if (cudaFuncSetAttribute(k_syrk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)syrk_smem_bytes()) != cudaSuccess)
-      return -1;
-    syrk_attr = true;
-  }
   int nblocks = 0;
   for (int p0 = 0; p0 < naux; p0 += (int)nblk, nblocks++) {
     const int nb = (int)(naux - p0 < nblk ? naux - p0 : nblk);
@@ -443,9 +491,9 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, cudaStream_t st
     prof_mark(h, DFJK_PHASE_SYRK, st);
     for (int s = 0; s < si.nset; s++) {
       if (si.col0[s + 1] == si.col0[s]) continue;
-      k_syrk<<<ntiles * ksplit, kThreads, syrk_smem_bytes(), st>>>(h->X, nao, nch, h->mu_pad, si.col0[s], si.col0[s + 1],
-                                                                 nb, rps, ntm, h->Kpart + n2 * s, split_stride,
-                                                                 p0 == 0 ? 1 : 0);
+      SyrkArgs sa{h->X, nao, nch, h->mu_pad, si.col0[s], si.col0[s + 1], nb, rps, ntm, h->Kpart + n2 * s,
+                  split_stride, p0 == 0 ? 1 : 0};
+      if (dispatch_syrk(wm_s, ntiles * ksplit, st, sa) != cudaSuccess) return -1;
       launches++;
     }
   }
