@@ -49,6 +49,19 @@ __device__ __forceinline__ double2 ldg_stream2(const double* p) {
   asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
   return v;
 }
+// 256-bit streaming read (sm_100+: SASS LDG.E.256); p must be 32-byte aligned
+struct double4s { double x, y, z, w; };
+__device__ __forceinline__ double4s ldg_stream4(const double* p) {
+  double4s v;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.f64 {%0,%1,%2,%3}, [%4];"
+               : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ double4s ldg_cached4(const double* p) {
+  double4s v;
+  asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));
+  return v;
+}
 __device__ __forceinline__ double ldg_stream1(const double* p) {
   double v;
   asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
