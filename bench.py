@@ -186,6 +186,7 @@ def main():
     ap.add_argument("--no-parity", action="store_true", help="skip the sampled parity check")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--workspace-gib", type=float, default=0.0, help="dfjk_options.workspace_cap_bytes (0 = default)")
     args = ap.parse_args()
     name = args.config
     cfg = dfjk_inputs.CONFIGS[name]
@@ -235,7 +236,7 @@ def main():
     J_host = torch.empty((nset, nao, nao), dtype=torch.float64).pin_memory()
     K_host = torch.empty_like(J_host).pin_memory()
 
-    h = dfjk.DFJK(Bd, nao)
+    h = dfjk.DFJK(Bd, nao, workspace_cap_bytes=int(args.workspace_gib * (1 << 30)))
     stream = torch.cuda.current_stream()
 
     def timed(fn, steps):
@@ -342,7 +343,7 @@ def main():
         torch.cuda.synchronize()
         rs = np.random.default_rng(7)
         samples = [(int(rs.integers(nset)), int(rs.integers(nao)), int(rs.integers(nao))) for _ in range(4)]
-        samples += [(0, 0, 0), (nset - 1, nao - 1, nao - 1), (0, nao - 1, 0), (0, 127, 128)]
+        samples += [(0, 0, 0), (nset - 1, nao - 1, nao - 1), (0, nao - 1, 0), (0, min(127, nao - 1), min(128, nao - 1))]
         t0 = time.perf_counter()
         Jv, Kv = oracle.sample(Bh, nao, C_list, occ_list, samples)
         Jg, Kg = J.cpu().numpy(), K.cpu().numpy()

@@ -113,7 +113,7 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   // X capacity (k-tiled layout [nch][mu_pad][36] per aux row): the cap, but at least one aux row
   // at full column capacity
   {
-    const size_t cap = o.workspace_cap_bytes ? o.workspace_cap_bytes : ((size_t)1 << 30);
+    const size_t cap = o.workspace_cap_bytes ? o.workspace_cap_bytes : ((size_t)4 << 30);
     const size_t one_row = (size_t)cdiv(h->nocc_pad_cap, kBK) * h->mu_pad * kLdT;
     size_t dbl = cap / sizeof(double);
     if (o.nblk > 0) dbl = (size_t)o.nblk * one_row;
