@@ -105,6 +105,43 @@ class ClockSampler:
         return out
 
 
+class Ranks:
+    """One process per GPU, replicas only: the only cross-rank traffic is the
+    barrier around the timed region and the max over ranks of the device time.  backend "nccl" on
+    the GPU box; "gloo" with device=None runs the same logic on CPU (tests/test_multirank_cpu.py)."""
+
+    def __init__(self, backend: str = "nccl", device=None):
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.device = device
+        self.dist = None
+        if self.world > 1:
+            import torch.distributed as dist
+            kw = {"device_id": device} if device is not None else {}
+            dist.init_process_group(backend, **kw)
+            self.dist = dist
+
+    def barrier(self):
+        if self.dist is not None:
+            self.dist.barrier()
+        if self.device is not None:
+            import torch
+            torch.cuda.synchronize()
+
+    def max_over_ranks(self, x: float) -> float:
+        if self.dist is None:
+            return x
+        import torch
+        t = torch.tensor([x], dtype=torch.float64, device=self.device if self.device is not None else "cpu")
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def close(self):
+        if self.dist is not None:
+            self.dist.destroy_process_group()
+            self.dist = None
+
+
 def upload_B(torch, cfg, keep_host: bool):
     """Generate packed B on the host in row chunks (the canonical recipe) and upload it."""
     nao, naux, L, k = cfg["nao"], cfg["naux"], cfg["L"], cfg["k"]
@@ -202,22 +239,8 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    def max_over_ranks(x: float) -> float:
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    ranks = Ranks("nccl", torch.device("cuda", local))
+    barrier, max_over_ranks = ranks.barrier, ranks.max_over_ranks
 
     nao, naux, nocc = cfg["nao"], cfg["naux"], cfg["nocc"]
     nset = len(nocc)
@@ -297,6 +320,8 @@ def main():
     ms_k = max_over_ranks(timed(k_only, nrep))
 
     if not lead:
+        h.close()
+        ranks.close()
         return
     pk = measured_peaks()
     ht_ms, ht_n = phases["half_transform"]
@@ -361,8 +386,7 @@ def main():
                                           "(the oracle's cost is linear in aux rows)"}
     print(json.dumps(line), flush=True)
     h.close()
-    if dist is not None:
-        dist.destroy_process_group()
+    ranks.close()
 
 
 if __name__ == "__main__":
