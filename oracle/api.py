@@ -34,6 +34,10 @@ def _load():
         lib.dfjk_oracle_sample.argtypes = [ct.c_int, ct.c_int, ct.c_int, _ip, _dp, _dp, _dp, ct.c_int,
                                            _ip, _ip, _ip, _dp, _dp]
         lib.dfjk_oracle_sample.restype = ct.c_int
+        lib.dfjk_oracle_ao2mo.argtypes = [ct.c_int] * 5 + [_dp] * 6
+        lib.dfjk_oracle_ao2mo.restype = ct.c_int
+        lib.dfjk_oracle_ao2mo_bruteforce.argtypes = [ct.c_int] * 5 + [_dp] * 4
+        lib.dfjk_oracle_ao2mo_bruteforce.restype = ct.c_int
         _lib = lib
     return _lib
 
@@ -140,3 +144,36 @@ def sample(B_packed: np.ndarray, nao: int, Cs, occs, samples: Sequence[Tuple[int
     if rc != 0:
         raise RuntimeError(f"dfjk_oracle_sample failed with code {rc}")
     return (None if Jv is None else Jv[:n]), (None if Kv is None else Kv[:n])
+
+
+def ao2mo(B_packed: np.ndarray, nao: int, M: np.ndarray, a0: int, nact: int, with_bmo: bool = False):
+    """Eq. 18-21 (oracle/ao2mo_oracle.c): returns (bpa, ppaa, papa[, bmo]) with shapes
+    (naux, nmo, nact), (nmo, nmo, nact, nact), (nmo, nact, nmo, nact)[, (naux, nmo, nmo)]."""
+    B, M = _f64(B_packed), _f64(M)
+    naux, nmo = B.shape[0], M.shape[1]
+    assert M.shape[0] == nao and B.shape[1] == nao * (nao + 1) // 2
+    bpa = np.empty((naux, nmo, nact))
+    ppaa = np.empty((nmo, nmo, nact, nact))
+    papa = np.empty((nmo, nact, nmo, nact))
+    bmo = np.empty((naux, nmo, nmo)) if with_bmo else None
+    z = np.zeros(1)
+    rc = _load().dfjk_oracle_ao2mo(naux, nao, nmo, a0, nact, _d(M if M.size else z), _d(B if B.size else z),
+                                   _d(bmo), _d(bpa if bpa.size else z), _d(ppaa if ppaa.size else z),
+                                   _d(papa if papa.size else z))
+    if rc != 0:
+        raise RuntimeError(f"dfjk_oracle_ao2mo failed with code {rc}")
+    return (bpa, ppaa, papa, bmo) if with_bmo else (bpa, ppaa, papa)
+
+
+def ao2mo_bruteforce(B_packed: np.ndarray, nao: int, M: np.ndarray, a0: int, nact: int):
+    """(ppaa, papa) from the direct 4-index transformation of the Eq. 12 tensor (tiny shapes)."""
+    B, M = _f64(B_packed), _f64(M)
+    nmo = M.shape[1]
+    ppaa = np.empty((nmo, nmo, nact, nact))
+    papa = np.empty((nmo, nact, nmo, nact))
+    z = np.zeros(1)
+    rc = _load().dfjk_oracle_ao2mo_bruteforce(B.shape[0], nao, nmo, a0, nact, _d(M), _d(B if B.size else z),
+                                              _d(ppaa if ppaa.size else z), _d(papa if papa.size else z))
+    if rc != 0:
+        raise RuntimeError(f"dfjk_oracle_ao2mo_bruteforce failed with code {rc}")
+    return ppaa, papa
