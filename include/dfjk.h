@@ -52,6 +52,9 @@ typedef struct {
   int max_nset;               /* capacity for nset; 0 = 8 */
   int copy_B;                 /* 0 = borrow the caller's device pointer (default); 1 = private copy */
   int ksplit;                 /* force the split-K factor of the SYRK; 0 = automatic */
+  int two_pass_j;             /* 0 = when J and K are both requested, rho (Eq. 14) is taken from the
+                                 half-transformed block, rho_P = sum_{mu,i} X^P_{mu i} C'_{mu i}, and B is
+                                 streamed twice instead of three times; 1 = always the two-pass J */
 } dfjk_options;
 
 /*

@@ -1,5 +1,6 @@
 // C ABI of the DF-JK library (include/dfjk.h): handle, validation, planning, enqueue.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -29,7 +30,7 @@ bool dev_alloc(dfjk_ctx* h, T** p, size_t count) {
 }
 
 void free_all(dfjk_ctx* h) {
-  cudaFree(h->B_owned); cudaFree(h->Ct); cudaFree(h->Dw); cudaFree(h->rho_part); cudaFree(h->rho);
+  cudaFree(h->B_owned); cudaFree(h->Ct); cudaFree(h->Dw); cudaFree(h->rho_part); cudaFree(h->rho); cudaFree(h->rho_ht);
   cudaFree(h->Jp_part); cudaFree(h->X); cudaFree(h->Kpart);
   cudaFree(h->C_stage); cudaFree(h->occ_stage); cudaFree(h->J_stage); cudaFree(h->K_stage);
   for (int i = 0; i < h->ev_cap; i++) cudaEventDestroy(h->ev[i]);
@@ -98,6 +99,14 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   if (!h) return DFJK_ERR_ALLOC;
   memset(h, 0, sizeof(*h));
   h->naux = naux; h->nao = nao; h->device = dev;
+  h->num_sms = prop.multiProcessorCount;
+  h->ht_grid = h->num_sms;
+  h->ht_skew = 1;
+  h->two_pass_j = o.two_pass_j;
+  if (const char* e = getenv("DFJK_HT_SKEW")) h->ht_skew = atoi(e) != 0;   // tuning only
+  if (const char* e = getenv("DFJK_SYRK_LEGACY")) h->syrk_legacy = atoi(e) != 0;
+  if (const char* e = getenv("DFJK_SYRK_WM")) h->syrk_wm_forced = atoi(e);
+  if (const char* e = getenv("DFJK_HT_GRID")) { const int g = atoi(e); if (g > 0) h->ht_grid = g; }
   h->npair = (size_t)nao * (nao + 1) / 2;
   h->nck = cdiv(nao, kHtBK);
   h->mu_pad = round_up(nao, 8) + 128;   // any SYRK tile of <= 128 rows stays inside the tiled X
@@ -139,6 +148,9 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   ok = ok && dev_alloc(h, &h->Dw, (size_t)h->max_nset * h->npair);
   ok = ok && dev_alloc(h, &h->rho_part, (size_t)h->j1_chunks * 8 * naux_pad);
   ok = ok && dev_alloc(h, &h->rho, (size_t)h->max_nset * (naux > 0 ? naux : 1));
+  // fused rho: 8 per-warp slots per (aux row, 64-row block, N tile) of the half-transform
+  h->rho_ht_doubles = o.two_pass_j ? 0 : (size_t)(naux > 0 ? naux : 1) * cdiv(nao, 64) * cdiv(h->nocc_pad_cap, 16 * kHtMaxWN) * 8 * h->max_nset;
+  ok = ok && dev_alloc(h, &h->rho_ht, h->rho_ht_doubles);
   ok = ok && dev_alloc(h, &h->Jp_part, (size_t)h->j2_splits * h->max_nset * h->npair);
   ok = ok && dev_alloc(h, &h->X, h->X_doubles);
   ok = ok && dev_alloc(h, &h->Kpart, (size_t)h->ksplit * h->max_nset * n2);
@@ -177,15 +189,18 @@ int dfjk_get_jk(dfjk_handle h, int nset, const int* nocc, const double* C, const
   if (!J_out && !K_out) return DFJK_OK;
   int n = 0, k;
   n += launch_prep_ct(h, si, C, occ, st);
-  if (J_out) {
+  // both outputs: rho falls out of the half-transform, so J needs one stream over B instead of two
+  const bool fuse = J_out && K_out && !h->two_pass_j && h->naux > 0 && si.nocc_pad > 0;
+  if (J_out && !fuse) {
     n += launch_prep_dw(h, si, st);
-    n += launch_j_passes(h, si, J_out, st);
+    n += launch_j_passes(h, si, J_out, false, st);
   }
   if (K_out) {
-    k = launch_k_path(h, si, K_out, st);
+    k = launch_k_path(h, si, K_out, fuse, st);
     if (k < 0) { set_err(h, "k path launch", cudaGetLastError()); return DFJK_ERR_CUDA; }
     n += k;
   }
+  if (fuse) n += launch_j_passes(h, si, J_out, true, st);
   prof_mark(h, -1, st);
   h->last_launches = n;
   cudaError_t e = cudaGetLastError();

@@ -48,11 +48,17 @@ struct dfjk_ctx {
   int plan_nblk, plan_ksplit, plan_nblocks;  // what the last get_jk actually used
   int n_mtiles;              // 128-row tiles along nao
   int j1_chunks, j2_splits;
+  int num_sms;
+  int ht_grid, ht_skew;      // persistent half-transform: CTAs (= SMs), skewed warp pairs on/off
+  int syrk_legacy, syrk_wm_forced;   // tuning only (env): wide/narrow-warp SYRK, forced tile size
+  int two_pass_j;            // option: never fuse J pass 1 into the half-transform
   // scratch (all allocated at create)
   double* Ct;                // [nck][ct_rows][20]  C' transposed and k-tiled, sqrt(occ) folded, zero padded
   double* Dw;                // [max_nset][npair]         packed density, off-diagonal weight 2
   double* rho_part;          // [j1_chunks][8][naux_pad]
   double* rho;               // [max_nset][naux]
+  double* rho_ht;            // [naux][ht slots][nset] per-warp rho partials of the fused half-transform
+  size_t rho_ht_doubles;
   double* Jp_part;           // [j2_splits][max_nset][npair]
   double* X;                 // [plan_nblk][nch][mu_pad][36] half-transformed block, k-tiled
   size_t X_doubles;          // capacity of X
@@ -80,8 +86,8 @@ inline void prof_mark(dfjk_ctx* h, int phase, cudaStream_t st) {
 // Each launcher enqueues on `st` and returns the number of kernels it launched.
 int launch_prep_ct(dfjk_ctx* h, const SetInfo& si, const double* C, const double* occ, cudaStream_t st);
 int launch_prep_dw(dfjk_ctx* h, const SetInfo& si, cudaStream_t st);
-int launch_j_passes(dfjk_ctx* h, const SetInfo& si, double* J_out, cudaStream_t st);
-int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, cudaStream_t st);
+int launch_j_passes(dfjk_ctx* h, const SetInfo& si, double* J_out, bool rho_ready, cudaStream_t st);
+int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, cudaStream_t st);
 int run_dmma_selftest();
 
 }  // namespace dfjk

@@ -312,7 +312,8 @@ static void launch_j2(int ns, dim3 grid, cudaStream_t st, const double* B, size_
   }
 }
 
-int launch_j_passes(dfjk_ctx* h, const SetInfo& si, double* J_out, cudaStream_t st) {
+// rho_ready: rho was already produced by the fused half-transform; only pass 2 and the epilogue run.
+int launch_j_passes(dfjk_ctx* h, const SetInfo& si, double* J_out, bool rho_ready, cudaStream_t st) {
   int launches = 0;
   const int naux = h->naux, nao = h->nao;
   const size_t npair = h->npair;
@@ -322,7 +323,7 @@ int launch_j_passes(dfjk_ctx* h, const SetInfo& si, double* J_out, cudaStream_t 
   const int rows_per_split = round_up(cdiv(naux > 0 ? naux : 1, h->j2_splits), 8);
   for (int s0 = 0; s0 < si.nset; s0 += 8) {  // the MMA N dimension holds 8 sets per pass
     const int ns = si.nset - s0 < 8 ? si.nset - s0 : 8;
-    if (naux > 0) {
+    if (naux > 0 && !rho_ready) {
       prof_mark(h, DFJK_PHASE_J1, st);
       dim3 g1(h->j1_chunks, naux_pad / kJ1Rows);
       if (npair % 4 == 0) k_j1_v4<<<g1, kJ1Warps * 32, 0, st>>>(h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad);

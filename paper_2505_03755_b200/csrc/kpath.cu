@@ -18,6 +18,10 @@
 #include "ctx.h"
 #include "pipeline.cuh"
 
+#include <functional>
+#include <queue>
+#include <vector>
+
 namespace dfjk {
 
 constexpr int kStages = 3;
@@ -33,27 +37,45 @@ constexpr int kConsumerRegs = 232, kProducerRegs = 40;
 constexpr int kHtATile = 64 * kHtLd;       // 1280 doubles >= 16 * 68 = 1088
 constexpr int kHtLdT = 64 + 4;             // 68: row stride of the transposed [16][64] A tile
 
-template <int WN>
+// Launch parameters of the half-transform.  The kernel is persistent: gridDim.x CTAs (one per SM)
+// walk the tiles (aux row, 64-row block, N tile) round-robin, and the mbarrier ring keeps running
+// across tile boundaries, so the producer prefetches the next tile while the consumers write X.
+struct HtParams {
+  const double* Bp; size_t npair; int nao;
+  const double* Ct; int ct_rows; int nocc_pad;
+  double* X; int nch; int mu_pad;       // EPI 0/1: k-tiled X for the SYRK
+  int p_first, nb, ntm, ntn;            // aux rows [p_first, p_first + nb), 64-row blocks, N tiles
+  int skew;                             // 1: the second consumer warpgroup runs half a chunk behind
+  double* rho_ht; int nset; int col0[kMaxSets + 1];   // EPI 1: per-warp partials of rho (step a2 fused)
+  int ldx, xrows;                       // EPI 2: row-major X[(pl * xrows + mu) * ldx + n]
+};
+
+// EPI = 0: X k-tiled for k_syrk.  EPI = 1: the same, plus rho[s][P] = sum_{mu,i in s} X[mu][i] C'[mu][i]
+// (= sum_{mu,lam} B_P[mu][lam] D_s[lam][mu], Eq. 14) as per-warp partials, so that a get_jk call that
+// wants both J and K streams B twice instead of three times.  EPI = 2: X row-major (AO2MO, Eq. 18).
+template <int WN, int EPI>
 __global__ void __launch_bounds__(kThreads, 1)
-k_half_transform(const double* __restrict__ Bp, size_t npair, int nao, const double* __restrict__ Ct,
-                 int ct_rows, int nocc_pad, double* __restrict__ X, int nch, int mu_pad, int p_first) {
+k_half_transform(const __grid_constant__ HtParams q) {
   extern __shared__ __align__(128) double smem[];
   constexpr int NT = 16 * WN;
   constexpr uint32_t kBBytes = NT * kHtLd * 8;
   double* sA = smem;                               // kStages x kHtATile
   double* sB = smem + kStages * kHtATile;          // kStages x NT*kHtLd
-  __shared__ __align__(8) unsigned long long bars[2 * kStages];
+  __shared__ __align__(8) unsigned long long bars[2 * kStages + 1];
   const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kStages]);
+  const uint32_t skewbar = smem_u32(&bars[2 * kStages]);
   const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
-  const int n0 = blockIdx.x * NT, m0 = blockIdx.y * 64, pl = blockIdx.z;
+  const int nao = q.nao;
   const int nk4 = (nao + 3) >> 2;                  // k4 steps that carry data
   const int nchunks = (nk4 + 3) >> 2;
+  const int tiles_per_p = q.ntm * q.ntn, ntiles = q.nb * tiles_per_p;
 
   if (tid == 0) {
     for (int s = 0; s < kStages; s++) {
       mbar_init(full0 + 8 * s, 128 + 1);   // 128 cp.async arrivals + the expect_tx arrival
       mbar_init(empty0 + 8 * s, 8);        // one arrival per consumer warp
     }
+    mbar_init(skewbar, 4);
     mbar_fence_init();
   }
   __syncthreads();
@@ -62,50 +84,55 @@ k_half_transform(const double* __restrict__ Bp, size_t npair, int nao, const dou
     // ===================== producer warpgroup =====================
     reg_dec<kProducerRegs>();
     const int tp = tid - 256;
-    const double* BpP = Bp + (size_t)(p_first + pl) * npair;
     const int kd = tp & 15, md = tp >> 4;          // direct / crossing: element (md + 8q, kd)
     const int mt = tp & 63, kt = tp >> 6;          // transposed:        element (mt, kt + 2q)
-    const bool okt = m0 + mt < nao;
     const uint32_t sA_u32 = smem_u32(sA), sB_u32 = smem_u32(sB);
     const uint32_t a_dst_d = (uint32_t)(md * kHtLd + kd) * 8u, a_dst_t = (uint32_t)(kt * kHtLdT + mt) * 8u;
-    for (int c = 0; c < nchunks; c++) {
-      const int stage = c % kStages;
-      const uint32_t fullb = full0 + 8 * stage;
-      mbar_wait(empty0 + 8 * stage, ((c / kStages) & 1) ^ 1);
-      const int l0 = c * kHtBK;
-      if (tp == 0) {
-        mbar_arrive_expect_tx(fullb, kBBytes);
-        bulk_g2s(sB_u32 + (uint32_t)stage * kBBytes, Ct + ((size_t)c * ct_rows + n0) * kHtLd, kBBytes, fullb);
+    int g = 0;                                     // chunk counter across tiles
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+      const int pl = tile / tiles_per_p, rem = tile - pl * tiles_per_p;
+      const int m0 = (rem / q.ntn) * 64, n0 = (rem % q.ntn) * NT;
+      const double* BpP = q.Bp + (size_t)(q.p_first + pl) * q.npair;
+      const bool okt = m0 + mt < nao;
+      for (int c = 0; c < nchunks; c++, g++) {
+        const int stage = g % kStages;
+        const uint32_t fullb = full0 + 8 * stage;
+        mbar_wait(empty0 + 8 * stage, ((g / kStages) & 1) ^ 1);
+        const int l0 = c * kHtBK;
+        if (tp == 0) {
+          mbar_arrive_expect_tx(fullb, kBBytes);
+          bulk_g2s(sB_u32 + (uint32_t)stage * kBBytes, q.Ct + ((size_t)c * q.ct_rows + n0) * kHtLd, kBBytes, fullb);
+        }
+        const uint32_t a_base = sA_u32 + (uint32_t)(stage * kHtATile) * 8u;
+        if (l0 + kHtBK - 1 <= m0) {                  // stored rows, all lam <= mu
+#pragma unroll
+          for (int qq = 0; qq < 8; qq++) {
+            const int mu = m0 + md + 8 * qq;
+            const bool ok = mu < nao;
+            cp_async8(a_base + a_dst_d + (uint32_t)(qq * 8 * kHtLd) * 8u,
+                      BpP + (ok ? (uint32_t)(mu * (mu + 1) / 2 + l0 + kd) : 0u), ok);
+          }
+        } else if (l0 >= m0 + 63) {                  // transpose of the stored tile, all lam >= mu
+#pragma unroll
+          for (int qq = 0; qq < 8; qq++) {
+            const int lam = l0 + kt + 2 * qq;
+            const bool ok = okt && lam < nao;
+            cp_async8(a_base + a_dst_t + (uint32_t)(qq * 2 * kHtLdT) * 8u,
+                      BpP + (ok ? (uint32_t)(lam * (lam + 1) / 2 + m0 + mt) : 0u), ok);
+          }
+        } else {                                     // crossing the diagonal
+          const int lam = l0 + kd;
+#pragma unroll
+          for (int qq = 0; qq < 8; qq++) {
+            const int mu = m0 + md + 8 * qq;
+            const bool ok = mu < nao && lam < nao;
+            uint32_t off = 0;
+            if (ok) off = (lam <= mu) ? (uint32_t)(mu * (mu + 1) / 2 + lam) : (uint32_t)(lam * (lam + 1) / 2 + mu);
+            cp_async8(a_base + a_dst_d + (uint32_t)(qq * 8 * kHtLd) * 8u, BpP + off, ok);
+          }
+        }
+        cp_async_mbar_arrive_noinc(fullb);
       }
-      const uint32_t a_base = sA_u32 + (uint32_t)(stage * kHtATile) * 8u;
-      if (l0 + kHtBK - 1 <= m0) {                  // stored rows, all lam <= mu
-#pragma unroll
-        for (int q = 0; q < 8; q++) {
-          const int mu = m0 + md + 8 * q;
-          const bool ok = mu < nao;
-          cp_async8(a_base + a_dst_d + (uint32_t)(q * 8 * kHtLd) * 8u,
-                    BpP + (ok ? (uint32_t)(mu * (mu + 1) / 2 + l0 + kd) : 0u), ok);
-        }
-      } else if (l0 >= m0 + 63) {                  // transpose of the stored tile, all lam >= mu
-#pragma unroll
-        for (int q = 0; q < 8; q++) {
-          const int lam = l0 + kt + 2 * q;
-          const bool ok = okt && lam < nao;
-          cp_async8(a_base + a_dst_t + (uint32_t)(q * 2 * kHtLdT) * 8u,
-                    BpP + (ok ? (uint32_t)(lam * (lam + 1) / 2 + m0 + mt) : 0u), ok);
-        }
-      } else {                                     // crossing the diagonal
-        const int lam = l0 + kd;
-#pragma unroll
-        for (int q = 0; q < 8; q++) {
-          const int mu = m0 + md + 8 * q;
-          const bool ok = mu < nao && lam < nao;
-          uint32_t off = 0;
-          if (ok) off = (lam <= mu) ? (uint32_t)(mu * (mu + 1) / 2 + lam) : (uint32_t)(lam * (lam + 1) / 2 + mu);
-          cp_async8(a_base + a_dst_d + (uint32_t)(q * 8 * kHtLd) * 8u, BpP + off, ok);
-        }
-      }
-      cp_async_mbar_arrive_noinc(fullb);
     }
     return;
   }
@@ -115,68 +142,169 @@ k_half_transform(const double* __restrict__ Bp, size_t npair, int nao, const dou
   const int r = l >> 2, j = l & 3;
   const int wm = w & 3, wn = w >> 2;
   double acc[2][WN][2];
-#pragma unroll
-  for (int t = 0; t < 2; t++)
-#pragma unroll
-    for (int u = 0; u < WN; u++) acc[t][u][0] = acc[t][u][1] = 0.0;
+  // warps w and w+4 share an SM sub-partition: the second one starts half a chunk late, so the two
+  // never sit at a chunk boundary (barrier wait + first fragment loads) at the same time
+  if (q.skew && wn == 1) mbar_wait(skewbar, 0);
 
-  for (int c = 0; c < nchunks; c++) {
-    const int stage = c % kStages;
-    const int l0 = c * kHtBK;
-    const bool tr = (l0 >= m0 + 63) && !(l0 + kHtBK - 1 <= m0);
-    const int ksteps = min(4, nk4 - c * 4);
-    mbar_wait(full0 + 8 * stage, (c / kStages) & 1);
-    const double* b_ptr = sB + stage * NT * kHtLd + (wn * 8 * WN + r) * kHtLd + j;
-    if (!tr) {
-      const double* a_ptr = sA + stage * kHtATile + (wm * 16 + r) * kHtLd + j;
+  int g = 0;
+  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const int pl = tile / tiles_per_p, rem = tile - pl * tiles_per_p;
+    const int mb = rem / q.ntn, nt = rem % q.ntn;
+    const int m0 = mb * 64, n0 = nt * NT;
 #pragma unroll
-      for (int kk = 0; kk < 4; kk++) {
-        if (kk < ksteps) {
-          const double a0 = a_ptr[4 * kk], a1 = a_ptr[8 * kHtLd + 4 * kk];
-          double b[WN];
+    for (int t = 0; t < 2; t++)
 #pragma unroll
-          for (int u = 0; u < WN; u++) b[u] = b_ptr[u * 8 * kHtLd + 4 * kk];
+      for (int u = 0; u < WN; u++) acc[t][u][0] = acc[t][u][1] = 0.0;
+
+    for (int c = 0; c < nchunks; c++, g++) {
+      const int stage = g % kStages;
+      const int l0 = c * kHtBK;
+      const bool tr = (l0 >= m0 + 63) && !(l0 + kHtBK - 1 <= m0);
+      const int ksteps = min(4, nk4 - c * 4);
+      mbar_wait(full0 + 8 * stage, (g / kStages) & 1);
+      const double* b_ptr = sB + stage * NT * kHtLd + (wn * 8 * WN + r) * kHtLd + j;
+      if (!tr) {
+        const double* a_ptr = sA + stage * kHtATile + (wm * 16 + r) * kHtLd + j;
 #pragma unroll
-          for (int u = 0; u < WN; u++) {
-            dmma884(acc[0][u][0], acc[0][u][1], a0, b[u]);
-            dmma884(acc[1][u][0], acc[1][u][1], a1, b[u]);
+        for (int kk = 0; kk < 4; kk++) {
+          if (kk < ksteps) {
+            const double a0 = a_ptr[4 * kk], a1 = a_ptr[8 * kHtLd + 4 * kk];
+            double b[WN];
+#pragma unroll
+            for (int u = 0; u < WN; u++) b[u] = b_ptr[u * 8 * kHtLd + 4 * kk];
+#pragma unroll
+            for (int u = 0; u < WN; u++) {
+              dmma884(acc[0][u][0], acc[0][u][1], a0, b[u]);
+              dmma884(acc[1][u][0], acc[1][u][1], a1, b[u]);
+            }
+            // half of the very first chunk done (it is never a transposed one): release the late
+            // warpgroup
+            if (g == 0 && wn == 0 && kk == (ksteps > 1 ? 1 : 0)) {
+              __syncwarp();
+              if (l == 0) mbar_arrive(skewbar);
+            }
           }
+        }
+      } else {
+        const double* a_ptr = sA + stage * kHtATile + (wm * 16 + r) + j * kHtLdT;
+#pragma unroll
+        for (int kk = 0; kk < 4; kk++) {
+          if (kk < ksteps) {
+            const double a0 = a_ptr[4 * kk * kHtLdT], a1 = a_ptr[8 + 4 * kk * kHtLdT];
+            double b[WN];
+#pragma unroll
+            for (int u = 0; u < WN; u++) b[u] = b_ptr[u * 8 * kHtLd + 4 * kk];
+#pragma unroll
+            for (int u = 0; u < WN; u++) {
+              dmma884(acc[0][u][0], acc[0][u][1], a0, b[u]);
+              dmma884(acc[1][u][0], acc[1][u][1], a1, b[u]);
+            }
+          }
+        }
+      }
+      __syncwarp();
+      if (l == 0) mbar_arrive(empty0 + 8 * stage);
+    }
+    // epilogue: lane owns X[mu][n], X[mu][n+1] with mu = m0 + 16 wm + 8t + r, n = n0 + 8 (wn WN + u) + 2j
+    if (EPI == 2) {
+      double* Xp = q.X + (size_t)pl * q.xrows * q.ldx;
+#pragma unroll
+      for (int t = 0; t < 2; t++) {
+        const int mu = m0 + wm * 16 + 8 * t + r;
+        if (mu >= nao) continue;
+#pragma unroll
+        for (int u = 0; u < WN; u++) {
+          const int n = n0 + 8 * (wn * WN + u) + 2 * j;
+          if (n < q.nocc_pad)
+            *reinterpret_cast<double2*>(Xp + (size_t)mu * q.ldx + n) = make_double2(acc[t][u][0], acc[t][u][1]);
         }
       }
     } else {
-      const double* a_ptr = sA + stage * kHtATile + (wm * 16 + r) + j * kHtLdT;
+      double* Xp = q.X + (size_t)pl * q.nch * q.mu_pad * kLdT;
 #pragma unroll
-      for (int kk = 0; kk < 4; kk++) {
-        if (kk < ksteps) {
-          const double a0 = a_ptr[4 * kk * kHtLdT], a1 = a_ptr[8 + 4 * kk * kHtLdT];
-          double b[WN];
+      for (int t = 0; t < 2; t++) {
+        const int mu = m0 + wm * 16 + 8 * t + r;
+        if (mu >= nao) continue;
 #pragma unroll
-          for (int u = 0; u < WN; u++) b[u] = b_ptr[u * 8 * kHtLd + 4 * kk];
-#pragma unroll
-          for (int u = 0; u < WN; u++) {
-            dmma884(acc[0][u][0], acc[0][u][1], a0, b[u]);
-            dmma884(acc[1][u][0], acc[1][u][1], a1, b[u]);
-          }
+        for (int u = 0; u < WN; u++) {
+          const int n = n0 + 8 * (wn * WN + u) + 2 * j;
+          if (n < q.nocc_pad)
+            *reinterpret_cast<double2*>(Xp + ((size_t)(n >> 5) * q.mu_pad + mu) * kLdT + (n & 31)) =
+                make_double2(acc[t][u][0], acc[t][u][1]);
         }
       }
     }
-    __syncwarp();
-    if (l == 0) mbar_arrive(empty0 + 8 * stage);
-  }
-  // epilogue: lane owns X[mu][n], X[mu][n+1] with mu = m0 + 16 wm + 8t + r, n = n0 + 8 (wn WN + u) + 2j
-  double* Xp = X + (size_t)pl * nch * mu_pad * kLdT;
+    if (EPI == 1) {
+      // rho partial of this warp: sum over its 16 rows x 8 WN columns of X .* C', set by set (every
+      // 8-column tile belongs to one set; a warp's tiles of one set are contiguous).  One slot of
+      // nset doubles per (aux row, tile, warp); k_rho_reduce sums the slots in fixed order.
+      const int nslots = tiles_per_p * 8;
+      double* slot = q.rho_ht + ((size_t)(q.p_first + pl) * nslots + (size_t)rem * 8 + w) * q.nset;
+      for (int s = l; s < q.nset; s += 32) slot[s] = 0.0;
+      int myset = -1;
+      if (l < WN) {
+        const int col = n0 + 8 * (wn * WN + l);
+        for (int s = 0; s < q.nset; s++)
+          if (col >= q.col0[s] && col < q.col0[s + 1]) myset = s;
+      }
+      __syncwarp();
+      double cur = 0.0;
+      int cur_s = -1;
+      auto flush = [&]() {
+        double v = cur;
 #pragma unroll
-  for (int t = 0; t < 2; t++) {
-    const int mu = m0 + wm * 16 + 8 * t + r;
-    if (mu >= nao) continue;
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (l == 0) slot[cur_s] = v;
+      };
+      // groups of four column tiles: all 16 C' loads of a group are issued before its FMAs, so the
+      // L2 latency is paid once per group and not once per element
 #pragma unroll
-    for (int u = 0; u < WN; u++) {
-      const int n = n0 + 8 * (wn * WN + u) + 2 * j;
-      if (n < nocc_pad)
-        *reinterpret_cast<double2*>(Xp + ((size_t)(n >> 5) * mu_pad + mu) * kLdT + (n & 31)) =
-            make_double2(acc[t][u][0], acc[t][u][1]);
+      for (int u0 = 0; u0 < WN; u0 += 4) {
+        double cv[4][2][2];
+        int su[4];
+#pragma unroll
+        for (int uu = 0; uu < 4; uu++) {
+          if (u0 + uu >= WN) continue;
+          su[uu] = __shfl_sync(0xffffffffu, myset, u0 + uu);
+          const int n = n0 + 8 * (wn * WN + u0 + uu) + 2 * j;
+#pragma unroll
+          for (int t = 0; t < 2; t++) {
+            const int mu = m0 + wm * 16 + 8 * t + r;
+            const bool ok = su[uu] >= 0 && mu < nao;
+            const double* cp = q.Ct + ((size_t)(ok ? (mu >> 4) : 0) * q.ct_rows + (ok ? n : 0)) * kHtLd + (mu & 15);
+            cv[uu][t][0] = ok ? __ldg(cp) : 0.0;
+            cv[uu][t][1] = ok ? __ldg(cp + kHtLd) : 0.0;
+          }
+        }
+#pragma unroll
+        for (int uu = 0; uu < 4; uu++) {
+          if (u0 + uu >= WN) continue;
+          if (su[uu] != cur_s) {
+            if (cur_s >= 0) flush();
+            cur = 0.0;
+            cur_s = su[uu];
+          }
+#pragma unroll
+          for (int t = 0; t < 2; t++) {
+            cur = fma(acc[t][u0 + uu][0], cv[uu][t][0], cur);
+            cur = fma(acc[t][u0 + uu][1], cv[uu][t][1], cur);
+          }
+        }
+      }
+      if (cur_s >= 0) flush();
     }
   }
+}
+
+// rho[s][P] = sum over the per-warp slots of k_half_transform<., 1>, ascending (fixed order)
+__global__ void k_rho_reduce(const double* __restrict__ rho_ht, int nslots, int nset, int naux,
+                             double* __restrict__ rho) {
+  const int P = blockIdx.x * blockDim.x + threadIdx.x, s = blockIdx.y;
+  if (P >= naux) return;
+  const double* p = rho_ht + (size_t)P * nslots * nset + s;
+  double t = 0.0;
+  for (int k = 0; k < nslots; k++) t += p[(size_t)k * nset];
+  rho[(size_t)s * naux + P] = t;
 }
 
 // ------------------------------------------------------------------ SYRK
@@ -320,6 +448,248 @@ k_syrk(const double* __restrict__ X, int nao, int nch, int mu_pad, int c0, int c
   else syrk_consume<WM, WNB>(ca, l);
 }
 
+// ------------------------------------------------------------------ SYRK, paired-warp version
+// Same CTA tile and producer as k_syrk, for T = 16*WM <= 96.  The T x T tile is cut into 2 x 2
+// blocks of WM x WM MMA tiles, one block per SM sub-partition; the two warps of a sub-partition
+// (w and w+4) both hold the whole block in registers and take alternate k4 steps (an in-CTA
+// split-K), so they are perfectly symmetric: 2 WM fragment loads per WM^2 DMMAs each.  The second
+// warp of each pair starts half a chunk late, so the two never reach a chunk boundary (barrier
+// wait + first fragment loads) together and one of them always has DMMAs to issue.
+// Diagonal tiles (ta == tb) skip what the epilogue never reads: the strictly-upper block is not
+// computed at all -- its sub-partition instead shares the k4 steps of the lower block (4-way) --
+// and the two diagonal blocks compute their lower MMA tiles only: WM(WM+1)/2 DMMAs per k4 step on
+// the critical sub-partition instead of WM^2.
+// At the end the partner warps pass their accumulators through the (drained) pipeline stages and
+// the owner warp adds them in a fixed order before the read-modify-write of the private partial.
+__device__ __forceinline__ void consumer_bar_sync() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+
+struct Syrk2Consumer {
+  const double* sA; const double* sB; uint32_t full0, empty0, skewbar;
+  int nchunks, ch0, ch1, c0, c1, tile_doubles;
+  int row0, col0;          // block origin inside the CTA tile
+  int kidx;                // this warp takes the k4 steps kk = kidx mod KMOD of every chunk
+  bool late;               // second warp of its pair: starts half a chunk late
+};
+
+template <int WM, bool LOWER, int KMOD>
+__device__ __forceinline__ void syrk2_mainloop(const Syrk2Consumer& q, int l, double (&acc)[WM][WM][2]) {
+  const int r = l >> 2, j = l & 3;
+#pragma unroll
+  for (int tt = 0; tt < WM; tt++)
+#pragma unroll
+    for (int u = 0; u < WM; u++) acc[tt][u][0] = acc[tt][u][1] = 0.0;
+  if (q.nchunks == 0) return;
+  if (q.late) mbar_wait(q.skewbar, 0);
+  bool release = !q.late;
+  int ch = q.ch0;
+  for (int c = 0; c < q.nchunks; c++) {
+    const int stage = c % kStages;
+    // k4 steps of this chunk that belong to the set: columns [max(c0, 32 ch), min(c1, 32 ch + 32))
+    const int k_lo = (max(q.c0, ch * 32) - ch * 32) >> 2, k_hi = (min(q.c1, ch * 32 + 32) - ch * 32 + 3) >> 2;
+    if (++ch == q.ch1) ch = q.ch0;
+    mbar_wait(q.full0 + 8 * stage, (c / kStages) & 1);
+    const double* a_ptr = q.sA + stage * q.tile_doubles + (q.row0 + r) * kLdT + j;
+    const double* b_ptr = q.sB + stage * q.tile_doubles + (q.col0 + r) * kLdT + j;
+    auto step = [&](int kk) {
+      double a[WM], b[WM];
+#pragma unroll
+      for (int tt = 0; tt < WM; tt++) a[tt] = a_ptr[tt * 8 * kLdT + 4 * kk];
+#pragma unroll
+      for (int u = 0; u < WM; u++) b[u] = b_ptr[u * 8 * kLdT + 4 * kk];
+#pragma unroll
+      for (int tt = 0; tt < WM; tt++)
+#pragma unroll
+        for (int u = 0; u < WM; u++)
+          if (!LOWER || u <= tt) dmma884(acc[tt][u][0], acc[tt][u][1], a[tt], b[u]);
+    };
+    if (k_lo == 0 && k_hi == 8) {
+#pragma unroll
+      for (int i = 0; i < 8 / KMOD; i++) {
+        step(q.kidx + i * KMOD);
+        if (i == 4 / KMOD - 1 && release) {          // half of the first chunk done
+          release = false;
+          __syncwarp();
+          if (l == 0) mbar_arrive(q.skewbar);
+        }
+      }
+    } else {
+      for (int kk = k_lo + ((q.kidx - k_lo) % KMOD + KMOD) % KMOD; kk < k_hi; kk += KMOD) step(kk);
+    }
+    __syncwarp();
+    if (l == 0) {
+      mbar_arrive(q.empty0 + 8 * stage);
+      if (release) mbar_arrive(q.skewbar);
+    }
+    release = false;
+  }
+}
+
+// accumulators of a partner warp -> shared memory slot / owner adds a slot
+template <int WM, bool LOWER>
+__device__ __forceinline__ void syrk2_put(double* red, int slot, int l, const double (&acc)[WM][WM][2]) {
+  double2* p = reinterpret_cast<double2*>(red) + (size_t)slot * WM * WM * 32 + l;
+#pragma unroll
+  for (int tt = 0; tt < WM; tt++)
+#pragma unroll
+    for (int u = 0; u < WM; u++)
+      if (!LOWER || u <= tt) p[(tt * WM + u) * 32] = make_double2(acc[tt][u][0], acc[tt][u][1]);
+}
+template <int WM, bool LOWER>
+__device__ __forceinline__ void syrk2_add(const double* red, int slot, int l, double (&acc)[WM][WM][2]) {
+  const double2* p = reinterpret_cast<const double2*>(red) + (size_t)slot * WM * WM * 32 + l;
+#pragma unroll
+  for (int tt = 0; tt < WM; tt++)
+#pragma unroll
+    for (int u = 0; u < WM; u++)
+      if (!LOWER || u <= tt) {
+        const double2 v = p[(tt * WM + u) * 32];
+        acc[tt][u][0] += v.x;
+        acc[tt][u][1] += v.y;
+      }
+}
+// read-modify-write of this CTA's private partial tile (entries above the diagonal of a diagonal
+// MMA tile are written too; the epilogue reads mu >= nu only)
+template <int WM, bool LOWER>
+__device__ __forceinline__ void syrk2_store(double* Kp, int nao, int mu0, int nu0, int first, int l,
+                                            const double (&acc)[WM][WM][2]) {
+  const int r = l >> 2, j = l & 3;
+#pragma unroll
+  for (int tt = 0; tt < WM; tt++) {
+    const int mu = mu0 + tt * 8 + r;
+    if (mu >= nao) continue;
+#pragma unroll
+    for (int u = 0; u < WM; u++) {
+      if (LOWER && u > tt) continue;
+      const int nu = nu0 + u * 8 + 2 * j;
+      double* p = Kp + (size_t)mu * nao + nu;
+      if (nu < nao) p[0] = first ? acc[tt][u][0] : p[0] + acc[tt][u][0];
+      if (nu + 1 < nao) p[1] = first ? acc[tt][u][1] : p[1] + acc[tt][u][1];
+    }
+  }
+}
+
+// grid: the n_off * ksplit off-diagonal CTAs first (blockIdx.x = g * n_off + t), then the
+// ntiles_m * ksplit cheaper diagonal ones, which fill the tail of the last wave.
+template <int WM>
+__global__ void __launch_bounds__(kThreads, 1)
+k_syrk2(const double* __restrict__ X, int nao, int nch, int mu_pad, int c0, int c1, int nrows_blk,
+        int rows_per_split, int ntiles_m, int ksplit, double* __restrict__ Kpart_s, size_t split_stride,
+        int first) {
+  constexpr int T = 16 * WM;
+  constexpr int kTileDoubles = T * kLdT;
+  constexpr uint32_t kTileBytes = kTileDoubles * 8;
+  extern __shared__ __align__(128) double smem[];
+  double* sA = smem;
+  double* sB = smem + kStages * kTileDoubles;
+  __shared__ __align__(8) unsigned long long bars[2 * kStages + 1];
+  const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kStages]);
+  const uint32_t skewbar = smem_u32(&bars[2 * kStages]);
+  const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
+  const int n_off = ntiles_m * (ntiles_m - 1) / 2;
+  int ta, tb, g;
+  const bool diag = (int)blockIdx.x >= n_off * ksplit;
+  if (!diag) {
+    const int t = blockIdx.x % n_off;
+    g = blockIdx.x / n_off;
+    ta = (int)((sqrt(8.0 * t + 1.0) + 1.0) * 0.5);          // t = ta(ta-1)/2 + tb, ta > tb
+    while (ta * (ta + 1) / 2 <= t) ta++;
+    while (ta * (ta - 1) / 2 > t) ta--;
+    tb = t - ta * (ta - 1) / 2;
+  } else {
+    const int t = blockIdx.x - n_off * ksplit;
+    ta = tb = t % ntiles_m;
+    g = t / ntiles_m;
+  }
+  const int a0 = ta * T, b0 = tb * T;
+  const int p_beg = g * rows_per_split;
+  int p_end = p_beg + rows_per_split;
+  if (p_end > nrows_blk) p_end = nrows_blk;
+  const int np = p_end > p_beg ? p_end - p_beg : 0;
+  const int ch0 = c0 >> 5, ch1 = (c1 + 31) >> 5;   // X chunks that hold columns of this set
+  const int nchunks = np * (ch1 - ch0);
+
+  if (tid == 0) {
+    for (int s = 0; s < kStages; s++) {
+      mbar_init(full0 + 8 * s, 1);         // the expect_tx arrival of the elected producer
+      mbar_init(empty0 + 8 * s, 8);        // one arrival per consumer warp
+    }
+    mbar_init(skewbar, 4);                 // the four early warps
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  if (w >= 8) {
+    // ===================== producer warpgroup (one elected thread works) =====================
+    reg_dec<kProducerRegs>();
+    if (tid == 256) {
+      const uint32_t sA_u32 = smem_u32(sA), sB_u32 = smem_u32(sB);
+      const size_t chunk_stride = (size_t)mu_pad * kLdT, row_stride = (size_t)nch * chunk_stride;
+      int P = p_beg, ch = ch0;
+      for (int c = 0; c < nchunks; c++) {
+        const int stage = c % kStages;
+        const uint32_t fullb = full0 + 8 * stage;
+        mbar_wait(empty0 + 8 * stage, ((c / kStages) & 1) ^ 1);
+        const double* src = X + (size_t)P * row_stride + (size_t)ch * chunk_stride;
+        mbar_arrive_expect_tx(fullb, diag ? kTileBytes : 2 * kTileBytes);
+        bulk_g2s(sA_u32 + (uint32_t)stage * kTileBytes, src + (size_t)a0 * kLdT, kTileBytes, fullb);
+        if (!diag) bulk_g2s(sB_u32 + (uint32_t)stage * kTileBytes, src + (size_t)b0 * kLdT, kTileBytes, fullb);
+        if (++ch == ch1) { ch = ch0; P++; }
+      }
+    }
+    return;
+  }
+
+  // ===================== consumer warpgroups =====================
+  reg_inc<kConsumerRegs>();
+  const int sp = w & 3, hh = w >> 2;                 // SM sub-partition, first/second warp of the pair
+  double* Kp = Kpart_s + (size_t)g * split_stride;
+  double* red = smem;                                // reused after the main loop
+  Syrk2Consumer q{sA, diag ? sA : sB, full0, empty0, skewbar, nchunks, ch0, ch1, c0, c1, kTileDoubles,
+                  0, 0, 0, hh == 1};
+  if (!diag) {
+    // block (bm, bn) = (sp & 1, sp >> 1); pair split-K 2
+    q.row0 = (sp & 1) * 8 * WM; q.col0 = (sp >> 1) * 8 * WM; q.kidx = hh;
+    double acc[WM][WM][2];
+    syrk2_mainloop<WM, false, 2>(q, l, acc);
+    consumer_bar_sync();
+    if (hh == 1) syrk2_put<WM, false>(red, sp, l, acc);
+    consumer_bar_sync();
+    if (hh == 0) {
+      syrk2_add<WM, false>(red, sp, l, acc);
+      syrk2_store<WM, false>(Kp, nao, a0 + q.row0, b0 + q.col0, first, l, acc);
+    }
+  } else if (sp == 0 || sp == 3) {
+    // diagonal blocks (0,0) and (1,1): lower MMA tiles only, pair split-K 2
+    q.row0 = q.col0 = (sp == 3) * 8 * WM; q.kidx = hh;
+    double acc[WM][WM][2];
+    syrk2_mainloop<WM, true, 2>(q, l, acc);
+    consumer_bar_sync();
+    if (hh == 1) syrk2_put<WM, true>(red, sp, l, acc);
+    consumer_bar_sync();
+    if (hh == 0) {
+      syrk2_add<WM, true>(red, sp, l, acc);
+      syrk2_store<WM, true>(Kp, nao, a0 + q.row0, b0 + q.col0, first, l, acc);
+    }
+  } else {
+    // block (1,0), shared 4-way by the warps of sub-partitions 1 and 2 (the strictly-upper block
+    // (0,1) is not computed): warp (sp, hh) takes the k4 steps kk = (sp - 1) + 2 hh mod 4
+    q.row0 = 8 * WM; q.col0 = 0; q.kidx = (sp - 1) + 2 * hh;
+    double acc[WM][WM][2];
+    syrk2_mainloop<WM, false, 4>(q, l, acc);
+    const bool owner = (sp == 1 && hh == 0);
+    const int slot = (sp == 1) ? 1 : (hh == 0 ? 2 : 4);      // partners: w=5 -> 1, w=2 -> 2, w=6 -> 4
+    consumer_bar_sync();
+    if (!owner) syrk2_put<WM, false>(red, slot, l, acc);
+    consumer_bar_sync();
+    if (owner) {
+      syrk2_add<WM, false>(red, 1, l, acc);
+      syrk2_add<WM, false>(red, 2, l, acc);
+      syrk2_add<WM, false>(red, 4, l, acc);
+      syrk2_store<WM, false>(Kp, nao, a0 + q.row0, b0 + q.col0, first, l, acc);
+    }
+  }
+}
+
 // Step a9: K_s[mu][nu] = K_s[nu][mu] = sum_g Kpart[g][s][mu][nu] for mu >= nu, g ascending.
 __global__ void __launch_bounds__(256)
 k_k_epilogue(const double* __restrict__ Kpart, int nsplit, size_t split_stride, int nao, double* __restrict__ K) {
@@ -358,34 +728,39 @@ __global__ void k_zero(double* p, size_t n) {
 static size_t ht_smem_bytes(int wn) { return (size_t)kStages * (kHtATile + 16 * wn * kHtLd) * sizeof(double); }
 static size_t syrk_smem_bytes(int wm) { return (size_t)kStages * 2 * (16 * wm * kLdT) * sizeof(double); }
 
-struct HtArgs {
-  const double* Bp; size_t npair; int nao; const double* Ct; int ct_rows; int nocc_pad; double* X;
-  int nch; int mu_pad; int p_first;
-};
-
-template <int WN>
-static cudaError_t launch_ht(dim3 grid, cudaStream_t st, const HtArgs& a) {
+template <int WN, int EPI>
+static cudaError_t launch_ht(int grid, cudaStream_t st, const HtParams& a) {
   static bool attr_set = false;  // the attribute is per function (per instantiation)
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_half_transform<WN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t e = cudaFuncSetAttribute(k_half_transform<WN, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)ht_smem_bytes(WN));
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  k_half_transform<WN><<<grid, kThreads, ht_smem_bytes(WN), st>>>(a.Bp, a.npair, a.nao, a.Ct, a.ct_rows, a.nocc_pad,
-                                                                   a.X, a.nch, a.mu_pad, a.p_first);
+  k_half_transform<WN, EPI><<<grid, kThreads, ht_smem_bytes(WN), st>>>(a);
   return cudaSuccess;
 }
 
-static cudaError_t dispatch_ht(int wn, dim3 grid, cudaStream_t st, const HtArgs& a) {
+template <int EPI>
+static cudaError_t dispatch_ht_wn(int wn, int grid, cudaStream_t st, const HtParams& a) {
   switch (wn) {
 #define DFJK_HT_CASE(N) \
-  case N: return launch_ht<N>(grid, st, a);
+  case N: return launch_ht<N, EPI>(grid, st, a);
     DFJK_HT_CASE(1) DFJK_HT_CASE(2) DFJK_HT_CASE(3) DFJK_HT_CASE(4) DFJK_HT_CASE(5) DFJK_HT_CASE(6)
     DFJK_HT_CASE(7) DFJK_HT_CASE(8) DFJK_HT_CASE(9) DFJK_HT_CASE(10) DFJK_HT_CASE(11) DFJK_HT_CASE(12)
     DFJK_HT_CASE(13) DFJK_HT_CASE(14) DFJK_HT_CASE(15) DFJK_HT_CASE(16) DFJK_HT_CASE(17) DFJK_HT_CASE(18)
     DFJK_HT_CASE(19) DFJK_HT_CASE(20)
 #undef DFJK_HT_CASE
+    default: return cudaErrorInvalidValue;
+  }
+}
+
+// epi: 0 = k-tiled X, 1 = k-tiled X + rho partials, 2 = row-major X
+static cudaError_t dispatch_ht(int wn, int epi, int grid, cudaStream_t st, const HtParams& a) {
+  switch (epi) {
+    case 0: return dispatch_ht_wn<0>(wn, grid, st, a);
+    case 1: return dispatch_ht_wn<1>(wn, grid, st, a);
+    case 2: return dispatch_ht_wn<2>(wn, grid, st, a);
     default: return cudaErrorInvalidValue;
   }
 }
@@ -421,9 +796,56 @@ static cudaError_t dispatch_syrk(int wm, int grid, cudaStream_t st, const SyrkAr
   }
 }
 
+template <int WM>
+static cudaError_t launch_syrk2(int ksplit, cudaStream_t st, const SyrkArgs& a) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(k_syrk2<WM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)syrk_smem_bytes(WM));
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  const int grid = a.ntiles_m * (a.ntiles_m + 1) / 2 * ksplit;
+  k_syrk2<WM><<<grid, kThreads, syrk_smem_bytes(WM), st>>>(a.X, a.nao, a.nch, a.mu_pad, a.c0, a.c1, a.nrows_blk,
+                                                         a.rows_per_split, a.ntiles_m, ksplit, a.Kpart_s,
+                                                         a.split_stride, a.first);
+  return cudaSuccess;
+}
+
+static cudaError_t dispatch_syrk2(int wm, int ksplit, cudaStream_t st, const SyrkArgs& a) {
+  switch (wm) {
+    case 4: return launch_syrk2<4>(ksplit, st, a);
+    case 5: return launch_syrk2<5>(ksplit, st, a);
+    case 6: return launch_syrk2<6>(ksplit, st, a);
+    default: return cudaErrorInvalidValue;
+  }
+}
+
+// Modelled SYRK time of one aux block in units of one off-diagonal CTA's aux row: greedy list
+// schedule of the CTAs in launch order (off-diagonal first, then the cheaper diagonal ones) on
+// `sms` SMs, one CTA per SM.
+static double syrk_makespan(int n_off, int n_diag, double diag_cost, int ksplit, int rps, int sms) {
+  const long long total = (long long)(n_off + n_diag) * ksplit;
+  const double work = ((double)n_off + diag_cost * n_diag) * ksplit * rps;
+  if (total > 8192 || total <= sms) return total <= sms ? (double)rps * (n_off ? 1.0 : diag_cost) : work / sms + rps;
+  std::priority_queue<double, std::vector<double>, std::greater<double>> free_at;
+  for (int i = 0; i < sms; i++) free_at.push(0.0);
+  double end = 0.0;
+  for (long long i = 0; i < total; i++) {
+    const double c = (i < (long long)n_off * ksplit ? 1.0 : diag_cost) * rps;
+    const double t = free_at.top() + c;
+    free_at.pop();
+    free_at.push(t);
+    if (t > end) end = t;
+  }
+  return end;
+}
+
 // Aux-block scheduler: cap the X workspace, pick the split-K factor, enqueue
 // half-transform and SYRK block after block on one stream.  No allocation, no host sync.
-int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, cudaStream_t st) {
+// With want_rho the half-transform also produces rho (step a2 fused): the
+// caller then runs J pass 2 only.
+int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, cudaStream_t st) {
   int launches = 0;
   const int nao = h->nao, naux = h->naux;
   const size_t n2 = (size_t)nao * nao;
@@ -449,29 +871,33 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, cudaStream_t st
   const int n8 = ldx / 8;
   const int ntn = cdiv(n8, 2 * kHtMaxWN), wn = cdiv(n8, 2 * ntn);  // N tile = 16*wn columns
   const int ntm_ht = cdiv(nao, 64);
-  // SYRK tile T = 16*wm_s in {64,...,128}: least executed area ntiles*T^2 (ties -> larger tile)
+  // SYRK tile T = 16*wm_s in {64,...,128}: least modelled work (ties -> larger tile).  Tiles up to
+  // 96 run the paired-warp kernel, whose diagonal CTAs cost (WM+1)/(2 WM) of an off-diagonal one.
   int wm_s = 8;
   {
     double best = 1e300;
     for (int wmc = 8; wmc >= 4; wmc--) {
       const int T = 16 * wmc, nt = cdiv(nao, T);
-      const double area = 0.5 * nt * (nt + 1) * (double)T * T;
+      const double dc = wmc <= 6 ? (wmc + 1) / (2.0 * wmc) : 1.0;
+      const double area = (0.5 * nt * (nt - 1) + dc * nt) * (double)T * T * (wmc <= 6 ? 1.0 : 1.03);
       if (area < best * 0.995) { best = area; wm_s = wmc; }
     }
   }
+  if (h->syrk_wm_forced >= 4 && h->syrk_wm_forced <= 8) wm_s = h->syrk_wm_forced;
+  const bool paired = wm_s <= 6 && !h->syrk_legacy;
+  const double diag_cost = paired ? (wm_s + 1) / (2.0 * wm_s) : 1.0;
   const int ntm = cdiv(nao, 16 * wm_s), ntiles = ntm * (ntm + 1) / 2;
   int ksplit = h->ksplit_forced;
   if (ksplit <= 0) {
-    // one SYRK CTA per SM; a CTA's work is its rows_per_split aux rows.  Pick the split with the
-    // best modelled efficiency  ntiles*nb / (148 * waves * rows_per_split), fewer splits on ties.
+    // one SYRK CTA per SM; pick the split with the shortest modelled makespan, fewer splits on ties
     const int nb0 = (int)nblk;
-    double best = -1.0;
+    double best = 1e300;
     ksplit = 1;
     for (int k = 1; k <= h->ksplit && k <= nb0; k++) {
       const int rps = cdiv(nb0, k), kk = cdiv(nb0, rps);          // splits that actually get rows
-      const int waves = cdiv(ntiles * kk, 148);
-      const double eff = (double)ntiles * nb0 / (148.0 * waves * rps) - 0.002 * k;
-      if (eff > best) { best = eff; ksplit = k; }
+      if (kk != k) continue;
+      const double t = syrk_makespan(ntiles - ntm, ntm, diag_cost, k, rps, h->num_sms) * (1.0 + 0.002 * k);
+      if (t < best) { best = t; ksplit = k; }
     }
   }
   if (ksplit > h->ksplit) ksplit = h->ksplit;
@@ -482,18 +908,25 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, cudaStream_t st
   int nblocks = 0;
   for (int p0 = 0; p0 < naux; p0 += (int)nblk, nblocks++) {
     const int nb = (int)(naux - p0 < nblk ? naux - p0 : nblk);
-    dim3 gh(ntn, ntm_ht, nb);
     prof_mark(h, DFJK_PHASE_HALF_TRANSFORM, st);
-    HtArgs a{h->B, h->npair, nao, h->Ct, h->ct_rows, ldx, h->X, nch, h->mu_pad, p0};
-    if (dispatch_ht(wn, gh, st, a) != cudaSuccess) return -1;
+    HtParams a;
+    a.Bp = h->B; a.npair = h->npair; a.nao = nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = ldx;
+    a.X = h->X; a.nch = nch; a.mu_pad = h->mu_pad; a.p_first = p0; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
+    a.skew = h->ht_skew; a.rho_ht = h->rho_ht; a.nset = si.nset; a.ldx = 0; a.xrows = 0;
+    for (int s = 0; s <= si.nset; s++) a.col0[s] = si.col0[s];
+    const long long ht_tiles = (long long)nb * ntm_ht * ntn;
+    const int ht_grid = (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid);
+    if (dispatch_ht(wn, want_rho ? 1 : 0, ht_grid, st, a) != cudaSuccess) return -1;
     launches++;
     const int rps = cdiv(nb, ksplit);
     prof_mark(h, DFJK_PHASE_SYRK, st);
     for (int s = 0; s < si.nset; s++) {
       if (si.col0[s + 1] == si.col0[s]) continue;
-      SyrkArgs sa{h->X, nao, nch, h->mu_pad, si.col0[s], si.col0[s + 1], nb, rps, ntm, h->Kpart + n2 * s,
-                  split_stride, p0 == 0 ? 1 : 0};
-      if (dispatch_syrk(wm_s, ntiles * ksplit, st, sa) != cudaSuccess) return -1;
+      // columns past nocc[s] (padding to the 8-column MMA tile) are zero: stop at the k4 step
+      SyrkArgs sa{h->X, nao, nch, h->mu_pad, si.col0[s], si.col0[s] + round_up(si.nocc[s], 4), nb, rps, ntm,
+                  h->Kpart + n2 * s, split_stride, p0 == 0 ? 1 : 0};
+      const cudaError_t e = paired ? dispatch_syrk2(wm_s, ksplit, st, sa) : dispatch_syrk(wm_s, ntiles * ksplit, st, sa);
+      if (e != cudaSuccess) return -1;
       launches++;
     }
   }
@@ -502,6 +935,12 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, cudaStream_t st
     if (si.col0[s + 1] == si.col0[s]) continue;
     dim3 ge(nb32, nb32, 1), be(32, 8);
     k_k_epilogue<<<ge, be, 0, st>>>(h->Kpart + n2 * s, ksplit, split_stride, nao, K_out + n2 * s);
+    launches++;
+  }
+  if (want_rho) {
+    prof_mark(h, DFJK_PHASE_J1, st);
+    dim3 gr(cdiv(naux, 128), si.nset);
+    k_rho_reduce<<<gr, 128, 0, st>>>(h->rho_ht, ntm_ht * ntn * 8, si.nset, naux, h->rho);
     launches++;
   }
   h->plan_nblk = (int)nblk;
