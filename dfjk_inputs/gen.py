@@ -87,11 +87,14 @@ def _q_of(nao: int, seed: int) -> np.ndarray:
     return q
 
 
-def make_orbitals(name: str):
-    """(C list, occ list) of a named config."""
+def make_orbitals(name: str, all_columns: bool = False):
+    """(C list, occ list) of a named config; with all_columns the whole orthonormal nao x nao
+    matrix Q the columns are taken from (seedC), e.g. as MO coefficients for AO2MO."""
     cfg = CONFIGS[name]
     k, nao, nocc = cfg["k"], cfg["nao"], cfg["nocc"]
     seedC, seedC2, seedO = 2000 + k, 3000 + k, 4000 + k
+    if all_columns:
+        return _q_of(nao, seedC)
     if name == "medium":
         qa, qb = _q_of(nao, seedC), _q_of(nao, seedC2)
         C = [np.ascontiguousarray(qa[:, :nocc[0]]), np.ascontiguousarray(qb[:, :nocc[1]])]

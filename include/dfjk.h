@@ -100,6 +100,29 @@ int dfjk_get_jk(dfjk_handle h, int nset, const int* nocc, const double* C, const
 int dfjk_get_jk_host(dfjk_handle h, int nset, const int* nocc, const double* C, const double* occ,
                      double* J_out, double* K_out, dfjk_stream stream);
 
+/*
+ * dfjk_ao2mo -- the AO2MO kernel of section 2.D.ii (Eq. 18-21) on the same
+ * resident Cholesky vectors, with the index pattern fixed by Eq. 12, g = (m1 m2|m3 m4) = b b:
+ *      X^P[e2][p1]   = sum_{e1} b^P[e1][e2] M[e1][p1]                          Eq. 18
+ *      bmo^P[p1][p2] = sum_{e2} X^P[e2][p1] M[e2][p2]                          Eq. 19
+ *      ppaa[p1][p2][a1][a2] = sum_P bmo^P[p1][p2] bmo^P[a0+a1][a0+a2]          Eq. 20
+ *      papa[p1][a1][p2][a2] = sum_P bmo^P[p1][a0+a1] bmo^P[p2][a0+a2]          Eq. 21
+ *   nmo      number of MO columns, 0 <= nmo <= max_nocc_total (default nao).
+ *   a0,nact  the active orbitals are the MO columns [a0, a0 + nact), a0 + nact <= nmo.
+ *   M        DEVICE, nao x nmo row-major, M[e][p]; columns need not be orthonormal.
+ *   bpa_out  DEVICE, naux x nmo x nact: bpa[P][p][a] = bmo^P[p][a0+a], the block the paper pulls
+ *            back to the host.  Required (it is also the operand of Eq. 21).
+ *   ppaa_out DEVICE, nmo x nmo x nact x nact, or NULL to skip Eq. 20.
+ *   papa_out DEVICE, nmo x nact x nmo x nact, or NULL to skip Eq. 21 (the paper runs it on the CPU).
+ * Same conventions as dfjk_get_jk: enqueue-only on `stream`, no allocation, no host
+ * synchronisation, outputs overwritten, deterministic.  The aux blocks share the X workspace of
+ * the handle (per aux row nao*roundup(nmo,8) + nmo^2 + nact^2 doubles); if the cap
+ * cannot hold one row the call returns DFJK_ERR_INVALID_ARG.  Must not overlap a dfjk_get_jk on
+ * the same handle.
+ */
+int dfjk_ao2mo(dfjk_handle h, int nmo, int a0, int nact, const double* M, double* bpa_out, double* ppaa_out,
+               double* papa_out, dfjk_stream stream);
+
 /* Frees everything the handle owns.  dfjk_destroy(NULL) is a no-op returning DFJK_OK. */
 int dfjk_destroy(dfjk_handle h);
 

@@ -14,7 +14,7 @@ _lib = None
 
 EXPORTS = ["dfjk_create", "dfjk_get_jk", "dfjk_get_jk_host", "dfjk_destroy", "dfjk_strerror",
            "dfjk_last_error", "dfjk_workspace_bytes", "dfjk_get_plan", "dfjk_last_launch_count",
-           "dfjk_selftest_dmma", "dfjk_set_profiling", "dfjk_get_profile"]
+           "dfjk_selftest_dmma", "dfjk_set_profiling", "dfjk_get_profile", "dfjk_ao2mo"]
 
 PHASES = ["prep", "j1", "j2", "j_epilogue", "half_transform", "syrk", "k_epilogue"]
 
@@ -51,6 +51,8 @@ def load_library():
         fn = getattr(lib, name)
         fn.argtypes = [vp, ct.c_int, ip, dp, dp, dp, dp, vp]
         fn.restype = ct.c_int
+    lib.dfjk_ao2mo.argtypes = [vp, ct.c_int, ct.c_int, ct.c_int, dp, dp, dp, dp, vp]
+    lib.dfjk_ao2mo.restype = ct.c_int
     lib.dfjk_destroy.argtypes = [vp]
     lib.dfjk_destroy.restype = ct.c_int
     lib.dfjk_strerror.argtypes = [ct.c_int]
@@ -166,6 +168,28 @@ class DFJK:
                                               ct.c_void_p(st.cuda_stream))
         _check(self._lib, code, self._h)
         return J_host, K_host
+
+    def ao2mo(self, M, a0: int, nact: int, with_ppaa: bool = True, with_papa: bool = True, stream=None):
+        """dfjk_ao2mo (Eq. 18-21): M is a CUDA float64 (nao, nmo) tensor; returns (bpa, ppaa, papa) with
+        shapes (naux, nmo, nact), (nmo, nmo, nact, nact), (nmo, nact, nmo, nact); enqueue-only."""
+        import torch
+        if tuple(M.shape[:1]) != (self.nao,) or M.dim() != 2:
+            raise ValueError(f"M must have shape ({self.nao}, nmo)")
+        M = M.to(device=self._device, dtype=torch.float64).contiguous()
+        nmo = int(M.shape[1])
+        with torch.cuda.device(self._device):
+            st = stream if stream is not None else torch.cuda.current_stream()
+            kw = dict(dtype=torch.float64, device=self._device)
+            bpa = torch.empty((self.naux, nmo, nact), **kw)
+            ppaa = torch.empty((nmo, nmo, nact, nact), **kw) if with_ppaa else None
+            papa = torch.empty((nmo, nact, nmo, nact), **kw) if with_papa else None
+            code = self._lib.dfjk_ao2mo(self._h, nmo, a0, nact, ct.c_void_p(M.data_ptr() if nmo else 0),
+                                        ct.c_void_p(bpa.data_ptr() if bpa.numel() else 0),
+                                        ct.c_void_p(ppaa.data_ptr() if ppaa is not None and ppaa.numel() else 0),
+                                        ct.c_void_p(papa.data_ptr() if papa is not None and papa.numel() else 0),
+                                        ct.c_void_p(st.cuda_stream))
+        _check(self._lib, code, self._h)
+        return bpa, ppaa, papa
 
     def plan(self) -> dict:
         a, b, c = ct.c_int(), ct.c_int(), ct.c_int()

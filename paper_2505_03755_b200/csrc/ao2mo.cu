@@ -1,0 +1,229 @@
+// AO2MO, the paper's second GPU kernel (Eq. 18-21):
+//   Eq. 18  X^P[e2][p1]   = sum_{e1} b^P[e1][e2] M[e1][p1]        the half-transform of the JK path
+//                                                                 (k_half_transform, row-major epilogue)
+//   Eq. 19  bmo^P[p1][p2] = sum_{e2} X^P[e2][p1] M[e2][p2]
+//   Eq. 20  ppaa[p1][p2][a1][a2] = sum_P bmo^P[p1][p2] bmo^P[a0+a1][a0+a2]
+//   Eq. 21  papa[p1][a1][p2][a2] = sum_P bpa[P][p1][a1] bpa[P][p2][a2],   bpa[P][p][a] = bmo^P[p][a0+a]
+// Eq. 19-21 are all of the form C (M x N) (+)= A^T B with both operands stored k-major
+// (A is [K][M], B is [K][N]): one warp-specialised DMMA kernel, k_gemm_tn, serves the three.
+// Aux blocks of N_blk rows bound the workspace (X block + bmo block, "2 N_blk N_emb^2").
+#include "common.cuh"
+#include "ctx.h"
+#include "pipeline.cuh"
+
+namespace dfjk {
+
+constexpr int kGStages = 4;
+constexpr int kGKC = 16;                  // k-chunk of the pipeline (4 k4 steps)
+constexpr int kGThreads = 384;            // 8 consumer warps + 4 producer warps
+
+struct GemmTN {
+  const double* A; const double* B; double* C;
+  int M, N, K;
+  long long lda, ldb, ldc;                // row strides (doubles) of the k-major operands and of C
+  long long sA, sB, sC;                   // batch strides (blockIdx.z)
+  int accumulate;                         // 0: C = A^T B, 1: C += A^T B (one CTA owns each C tile)
+};
+
+// CTA tile (16 WTM) x (32 WTN); consumers 2 (M) x 4 (N), warp tile WTM x WTN MMA tiles.
+// Shared-memory tiles are k-major, [16][TM + 4] and [16][TN + 4]: the row stride is 4 mod 16
+// doubles, so the fragment reads tile[k = l%4][row = l/4] hit 16 distinct banks per half-warp.
+// Producers gather with 8-byte cp.async (any alignment, zero-fill past M, N, K).
+template <int WTM, int WTN>
+__global__ void __launch_bounds__(kGThreads, 1)
+k_gemm_tn(const __grid_constant__ GemmTN g) {
+  constexpr int TM = 16 * WTM, TN = 32 * WTN, LA = TM + 4, LB = TN + 4;
+  constexpr int kStageDoubles = kGKC * (LA + LB);
+  extern __shared__ __align__(128) double smem[];
+  __shared__ __align__(8) unsigned long long bars[2 * kGStages];
+  const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kGStages]);
+  const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
+  const int m0 = blockIdx.x * TM, n0 = blockIdx.y * TN;
+  const double* A = g.A + (size_t)blockIdx.z * g.sA;
+  const double* B = g.B + (size_t)blockIdx.z * g.sB;
+  double* C = g.C + (size_t)blockIdx.z * g.sC;
+  const int nchunks = (g.K + kGKC - 1) / kGKC;
+
+  if (tid == 0) {
+    for (int s = 0; s < kGStages; s++) {
+      mbar_init(full0 + 8 * s, 128);       // one cp.async-completion arrival per producer thread
+      mbar_init(empty0 + 8 * s, 8);        // one arrival per consumer warp
+    }
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  if (w >= 8) {
+    // ===================== producer warpgroup =====================
+    reg_dec<kProducerRegs>();
+    const int tp = tid - 256;
+    for (int c = 0; c < nchunks; c++) {
+      const int stage = c % kGStages;
+      mbar_wait(empty0 + 8 * stage, ((c / kGStages) & 1) ^ 1);
+      const uint32_t sa = smem_u32(smem + stage * kStageDoubles), sb = sa + kGKC * LA * 8;
+      const int k0 = c * kGKC;
+#pragma unroll 4
+      for (int e = tp; e < kGKC * TM; e += 128) {
+        const int k = e / TM, m = e - k * TM;
+        const bool ok = (k0 + k < g.K) && (m0 + m < g.M);
+        cp_async8(sa + (uint32_t)(k * LA + m) * 8u, A + (ok ? (size_t)(k0 + k) * g.lda + m0 + m : 0), ok);
+      }
+#pragma unroll 4
+      for (int e = tp; e < kGKC * TN; e += 128) {
+        const int k = e / TN, n = e - k * TN;
+        const bool ok = (k0 + k < g.K) && (n0 + n < g.N);
+        cp_async8(sb + (uint32_t)(k * LB + n) * 8u, B + (ok ? (size_t)(k0 + k) * g.ldb + n0 + n : 0), ok);
+      }
+      cp_async_mbar_arrive_noinc(full0 + 8 * stage);
+    }
+    return;
+  }
+
+  // ===================== consumer warpgroups =====================
+  reg_inc<kConsumerRegs>();
+  const int r = l >> 2, j = l & 3;
+  const int wm = w & 1, wn = w >> 1;
+  double acc[WTM][WTN][2];
+#pragma unroll
+  for (int t = 0; t < WTM; t++)
+#pragma unroll
+    for (int u = 0; u < WTN; u++) acc[t][u][0] = acc[t][u][1] = 0.0;
+  const int nk4 = (g.K + 3) >> 2;
+  for (int c = 0; c < nchunks; c++) {
+    const int stage = c % kGStages;
+    const int ksteps = min(4, nk4 - c * 4);
+    mbar_wait(full0 + 8 * stage, (c / kGStages) & 1);
+    const double* a_ptr = smem + stage * kStageDoubles + j * LA + wm * 8 * WTM + r;
+    const double* b_ptr = smem + stage * kStageDoubles + kGKC * LA + j * LB + wn * 8 * WTN + r;
+#pragma unroll
+    for (int kk = 0; kk < 4; kk++) {
+      if (kk < ksteps) {
+        double a[WTM], b[WTN];
+#pragma unroll
+        for (int t = 0; t < WTM; t++) a[t] = a_ptr[4 * kk * LA + 8 * t];
+#pragma unroll
+        for (int u = 0; u < WTN; u++) b[u] = b_ptr[4 * kk * LB + 8 * u];
+#pragma unroll
+        for (int t = 0; t < WTM; t++)
+#pragma unroll
+          for (int u = 0; u < WTN; u++) dmma884(acc[t][u][0], acc[t][u][1], a[t], b[u]);
+      }
+    }
+    __syncwarp();
+    if (l == 0) mbar_arrive(empty0 + 8 * stage);
+  }
+  // epilogue: lane owns C[m][n], C[m][n+1], m = m0 + 8 (wm WTM + t) + r, n = n0 + 8 (wn WTN + u) + 2j
+#pragma unroll
+  for (int t = 0; t < WTM; t++) {
+    const int m = m0 + 8 * (wm * WTM + t) + r;
+    if (m >= g.M) continue;
+#pragma unroll
+    for (int u = 0; u < WTN; u++) {
+      const int n = n0 + 8 * (wn * WTN + u) + 2 * j;
+      double* p = C + (size_t)m * g.ldc + n;
+      if (n < g.N) p[0] = g.accumulate ? p[0] + acc[t][u][0] : acc[t][u][0];
+      if (n + 1 < g.N) p[1] = g.accumulate ? p[1] + acc[t][u][1] : acc[t][u][1];
+    }
+  }
+}
+
+__global__ void k_zero_ao(double* p, size_t n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = 0.0;
+}
+
+template <int WTM, int WTN>
+static cudaError_t launch_gemm_tn(const GemmTN& g, int batch, cudaStream_t st) {
+  constexpr int TM = 16 * WTM, TN = 32 * WTN;
+  constexpr size_t smem = (size_t)kGStages * kGKC * (TM + 4 + TN + 4) * sizeof(double);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(k_gemm_tn<WTM, WTN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  if (g.M <= 0 || g.N <= 0 || batch <= 0) return cudaSuccess;
+  dim3 grid(cdiv(g.M, TM), cdiv(g.N, TN), batch);
+  k_gemm_tn<WTM, WTN><<<grid, kGThreads, smem, st>>>(g);
+  return cudaSuccess;
+}
+
+// N tile 128, 64 or 32 columns by the width of the problem
+static cudaError_t gemm_tn(const GemmTN& g, int batch, cudaStream_t st) {
+  if (g.N > 64) return launch_gemm_tn<8, 4>(g, batch, st);
+  if (g.N > 32) return launch_gemm_tn<8, 2>(g, batch, st);
+  return launch_gemm_tn<8, 1>(g, batch, st);
+}
+
+// bpa[P][p][a] = bmo[P][p][a0 + a]  (pulled back by the caller) and
+// baa[P][a1][a2] = bmo[P][a0 + a1][a0 + a2]  (the B operand of Eq. 20)
+__global__ void k_ao2mo_gather(const double* __restrict__ bmo, int nb, int nmo, int a0, int nact,
+                               double* __restrict__ bpa, double* __restrict__ baa) {
+  const int P = blockIdx.y;
+  const double* src = bmo + (size_t)P * nmo * nmo;
+  const int npa = nmo * nact, naa = nact * nact;
+  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < npa + naa; e += gridDim.x * blockDim.x) {
+    if (e < npa) {
+      const int p = e / nact, a = e - p * nact;
+      bpa[(size_t)P * npa + e] = src[(size_t)p * nmo + a0 + a];
+    } else {
+      const int f = e - npa, a1 = f / nact, a2 = f - a1 * nact;
+      baa[(size_t)P * naa + f] = src[(size_t)(a0 + a1) * nmo + a0 + a2];
+    }
+  }
+}
+
+// Eq. 18-21 block after block.  Workspace: the X buffer of the handle holds, per aux row of the
+// block, the half-transformed slice (nao x ldx), bmo (nmo x nmo) and baa (nact x nact).
+int launch_ao2mo(dfjk_ctx* h, int nmo, int a0, int nact, const double* M, double* bpa_out, double* ppaa_out,
+                 double* papa_out, cudaStream_t st) {
+  int launches = 0;
+  const int nao = h->nao, naux = h->naux;
+  const size_t n2 = (size_t)nmo * nmo, npa = (size_t)nmo * nact, naa = (size_t)nact * nact;
+  if (naux == 0 || nmo == 0 || nact == 0) {
+    if (ppaa_out && n2 * naa) { k_zero_ao<<<148, 256, 0, st>>>(ppaa_out, n2 * naa); launches++; }
+    if (papa_out && n2 * naa) { k_zero_ao<<<148, 256, 0, st>>>(papa_out, n2 * naa); launches++; }
+    if (naux == 0 || nmo == 0) return launches;
+  }
+  SetInfo si;
+  si.nset = 1; si.col0[0] = 0; si.nocc[0] = nmo; si.coff[0] = 0; si.ooff[0] = 0;
+  si.col0[1] = si.nocc_pad = round_up(nmo, 8);
+  launches += launch_prep_ct(h, si, M, nullptr, st);          // C' = M (no occupations)
+  const int ldx = si.nocc_pad;
+  const size_t row_doubles = (size_t)nao * ldx + n2 + naa;
+  long long nblk = (long long)(h->X_doubles / row_doubles);
+  if (h->nblk_forced > 0 && nblk > h->nblk_forced) nblk = h->nblk_forced;
+  if (nblk > naux) nblk = naux;
+  if (nblk > 32768) nblk = 32768;
+  if (nblk < 1) return -2;                                    // workspace too small for one aux row
+  double* Xb = h->X;
+  double* bmo = Xb + (size_t)nblk * nao * ldx;
+  double* baa = bmo + (size_t)nblk * n2;
+  for (int p0 = 0; p0 < naux; p0 += (int)nblk) {
+    const int nb = (int)(naux - p0 < nblk ? naux - p0 : nblk);
+    if (launch_half_transform_rowmajor(h, si, p0, nb, Xb, ldx, st) != 0) return -1;      // Eq. 18
+    launches++;
+    GemmTN g19{Xb, M, bmo, nmo, nmo, nao, ldx, nmo, nmo, (long long)nao * ldx, 0, (long long)n2, 0};
+    if (gemm_tn(g19, nb, st) != cudaSuccess) return -1;                                   // Eq. 19
+    launches++;
+    if (nact > 0) {
+      dim3 gg(cdiv((int)(npa + naa), 256) < 64 ? cdiv((int)(npa + naa), 256) : 64, nb);
+      k_ao2mo_gather<<<gg, 256, 0, st>>>(bmo, nb, nmo, a0, nact, bpa_out + (size_t)p0 * npa, baa);
+      launches++;
+      if (ppaa_out) {
+        GemmTN g20{bmo, baa, ppaa_out, (int)n2, (int)naa, nb, (long long)n2, (long long)naa, (long long)naa,
+                   0, 0, 0, p0 > 0 ? 1 : 0};
+        if (gemm_tn(g20, 1, st) != cudaSuccess) return -1;                                // Eq. 20
+        launches++;
+      }
+    }
+  }
+  if (papa_out && nact > 0) {
+    GemmTN g21{bpa_out, bpa_out, papa_out, (int)npa, (int)npa, naux, (long long)npa, (long long)npa,
+               (long long)npa, 0, 0, 0, 0};
+    if (gemm_tn(g21, 1, st) != cudaSuccess) return -1;                                    // Eq. 21
+    launches++;
+  }
+  return launches;
+}
+
+}  // namespace dfjk

@@ -235,6 +235,27 @@ int dfjk_get_jk_host(dfjk_handle h, int nset, const int* nocc, const double* C, 
   return DFJK_OK;
 }
 
+int dfjk_ao2mo(dfjk_handle h, int nmo, int a0, int nact, const double* M, double* bpa_out, double* ppaa_out,
+               double* papa_out, dfjk_stream stream) {
+  if (!h) return DFJK_ERR_INVALID_ARG;
+  if (nmo < 0 || nmo > h->max_nocc_total || round_up(nmo, 8) > h->nocc_pad_cap) return DFJK_ERR_INVALID_ARG;
+  if (nact < 0 || a0 < 0 || a0 + nact > nmo) return DFJK_ERR_INVALID_ARG;
+  if (nmo > 0 && !M) return DFJK_ERR_INVALID_ARG;
+  if (nmo > 0 && nact > 0 && h->naux > 0 && !bpa_out) return DFJK_ERR_INVALID_ARG;
+  if ((long long)nmo * nmo > 2147483647LL || (long long)nmo * nact > 2147483647LL) return DFJK_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  h->last_launches = 0;
+  h->last_error[0] = 0;
+  h->ev_n = 0;
+  const int n = launch_ao2mo(h, nmo, a0, nact, M, bpa_out, ppaa_out, papa_out, st);
+  if (n == -2) { snprintf(h->last_error, sizeof(h->last_error), "workspace cap too small for one aux row of AO2MO"); return DFJK_ERR_INVALID_ARG; }
+  if (n < 0) { set_err(h, "ao2mo launch", cudaGetLastError()); return DFJK_ERR_CUDA; }
+  h->last_launches = n;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { set_err(h, "kernel launch", e); return DFJK_ERR_CUDA; }
+  return DFJK_OK;
+}
+
 int dfjk_destroy(dfjk_handle h) {
   if (!h) return DFJK_OK;
   free_all(h);

@@ -88,6 +88,12 @@ int launch_prep_ct(dfjk_ctx* h, const SetInfo& si, const double* C, const double
 int launch_prep_dw(dfjk_ctx* h, const SetInfo& si, cudaStream_t st);
 int launch_j_passes(dfjk_ctx* h, const SetInfo& si, double* J_out, bool rho_ready, cudaStream_t st);
 int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, cudaStream_t st);
+int launch_half_transform_rowmajor(dfjk_ctx* h, const SetInfo& si, int p_first, int nb, double* X, int ldx,
+                                   cudaStream_t st);
+// AO2MO (Eq. 18-21); returns the number of launches, -1 on a launch failure, -2 if the workspace
+// cannot hold one aux row
+int launch_ao2mo(dfjk_ctx* h, int nmo, int a0, int nact, const double* M, double* bpa_out, double* ppaa_out,
+                 double* papa_out, cudaStream_t st);
 int run_dmma_selftest();
 
 }  // namespace dfjk

@@ -26,7 +26,6 @@ namespace dfjk {
 
 constexpr int kStages = 3;
 constexpr int kThreads = 384;             // 2 consumer warpgroups + 1 producer warpgroup
-constexpr int kConsumerRegs = 232, kProducerRegs = 40;
 
 // ------------------------------------------------------------------ half-transform
 // CTA: 64 rows (mu) of one aux slice x NT = 16*WN columns (normally ALL columns of C', so the
@@ -819,6 +818,23 @@ static cudaError_t dispatch_syrk2(int wm, int ksplit, cudaStream_t st, const Syr
     case 6: return launch_syrk2<6>(ksplit, st, a);
     default: return cudaErrorInvalidValue;
   }
+}
+
+// Eq. 18 for AO2MO: X[pl][mu][n] = sum_lam B_{p_first+pl}[mu][lam] C'[lam][n], row-major with row
+// stride ldx (the same kernel as the JK half-transform, epilogue 2).  Returns 0 on success.
+int launch_half_transform_rowmajor(dfjk_ctx* h, const SetInfo& si, int p_first, int nb, double* X, int ldx,
+                                   cudaStream_t st) {
+  const int n8 = si.nocc_pad / 8;
+  const int ntn = cdiv(n8, 2 * kHtMaxWN), wn = cdiv(n8, 2 * ntn);
+  const int ntm_ht = cdiv(h->nao, 64);
+  HtParams a;
+  a.Bp = h->B; a.npair = h->npair; a.nao = h->nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = si.nocc_pad;
+  a.X = X; a.nch = 0; a.mu_pad = 0; a.p_first = p_first; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
+  a.skew = h->ht_skew; a.rho_ht = nullptr; a.nset = 0; a.ldx = ldx; a.xrows = h->nao;
+  a.col0[0] = 0;
+  const long long ht_tiles = (long long)nb * ntm_ht * ntn;
+  const int ht_grid = (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid);
+  return dispatch_ht(wn, 2, ht_grid, st, a) == cudaSuccess ? 0 : -1;
 }
 
 // Modelled SYRK time of one aux block in units of one off-diagonal CTA's aux row: greedy list

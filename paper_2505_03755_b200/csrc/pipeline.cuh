@@ -5,6 +5,9 @@
 
 namespace dfjk {
 
+// setmaxnreg budgets of the warp-specialised kernels (2 consumer warpgroups + 1 producer warpgroup)
+constexpr int kConsumerRegs = 232, kProducerRegs = 40;
+
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }

@@ -27,7 +27,7 @@ k_prep_ct(const __grid_constant__ SetInfo si, const double* __restrict__ C, cons
     if (il >= si.nocc[s]) s = -1;  // padding column
   }
   double scale = 0.0;
-  if (s >= 0) scale = sqrt(occ[si.ooff[s] + il]);
+  if (s >= 0) scale = occ ? sqrt(occ[si.ooff[s] + il]) : 1.0;   // occ == nullptr: plain coefficients (AO2MO)
   for (int r = ty; r < 32; r += 8) {
     const int lam = lam0 + r;
     double v = 0.0;

@@ -14,7 +14,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def declared_symbols():
     txt = open(os.path.join(ROOT, "include", "dfjk.h")).read()
     txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
-    return sorted(set(re.findall(r"\b(dfjk_[a-z_]+)\s*\(", txt)))
+    return sorted(set(re.findall(r"\b(dfjk_[a-z0-9_]+)\s*\(", txt)))
 
 
 def test_library_loads_and_exports_every_declared_symbol():

@@ -1,0 +1,81 @@
+"""GPU parity of dfjk_ao2mo (Eq. 18-21) against oracle/ao2mo_oracle.c, element by element.
+
+Bar: max|d|/max|.| <= 1e-10 for bpa, ppaa and papa (fp64 sums in a different order; observed ~1e-15).
+"""
+import numpy as np
+import pytest
+
+import dfjk_inputs
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-10
+
+
+def rel(a, b):
+    return float(np.abs(a - b).max() / max(np.abs(b).max(), 1e-300))
+
+
+def run_case(nao, naux, nmo, a0, nact, seed, L=0.0, orth=False, **opts):
+    import torch
+    import oracle
+    import paper_2505_03755_b200 as dfjk
+    inp = dfjk_inputs.make_random(nao, naux, [1], seed, L=L)
+    rng = np.random.default_rng(seed + 7)
+    M = rng.standard_normal((nao, nmo))
+    if orth:
+        M = np.linalg.qr(rng.standard_normal((nao, nao)))[0][:, :nmo].copy()
+    o_bpa, o_ppaa, o_papa = oracle.ao2mo(inp.B_packed, nao, M, a0, nact)
+    B = torch.from_numpy(inp.B_packed).cuda()
+    with dfjk.DFJK(B, nao, **opts) as h:
+        bpa, ppaa, papa = h.ao2mo(torch.from_numpy(M).cuda(), a0, nact)
+        torch.cuda.synchronize()
+        assert h.last_launch_count > 0 or naux == 0 or nmo == 0
+        bpa2, ppaa2, papa2 = h.ao2mo(torch.from_numpy(M).cuda(), a0, nact)     # deterministic
+        torch.cuda.synchronize()
+        assert torch.equal(bpa, bpa2) and torch.equal(ppaa, ppaa2) and torch.equal(papa, papa2)
+    bpa, ppaa, papa = bpa.cpu().numpy(), ppaa.cpu().numpy(), papa.cpu().numpy()
+    if o_bpa.size:
+        assert rel(bpa, o_bpa) <= TOL, rel(bpa, o_bpa)
+        assert rel(ppaa, o_ppaa) <= TOL, rel(ppaa, o_ppaa)
+        assert rel(papa, o_papa) <= TOL, rel(papa, o_papa)
+    return bpa, ppaa, papa
+
+
+@pytest.mark.parametrize("nao,naux,nmo,a0,nact,seed", [
+    (16, 9, 12, 3, 4, 201),         # everything smaller than one tile
+    (67, 45, 50, 11, 5, 202),       # ragged, nmo*nact odd
+    (130, 70, 130, 60, 8, 203),     # nmo = nao, one row past a 128 tile
+    (150, 33, 97, 0, 3, 204),       # active block at the start, odd nmo
+    (96, 20, 40, 34, 6, 205),       # active block at the end (a0 + nact = nmo)
+    (48, 1, 48, 20, 2, 206),        # single aux row
+])
+def test_ragged_shapes(nao, naux, nmo, a0, nact, seed):
+    run_case(nao, naux, nmo, a0, nact, seed, L=max(4.0, nao / 6))
+
+
+@pytest.mark.parametrize("opts", [dict(nblk=1), dict(nblk=7), dict(workspace_cap_bytes=1 << 21)])
+def test_blocking_does_not_change_the_result(opts):
+    run_case(120, 61, 90, 30, 6, 210, L=15.0, **opts)
+
+
+def test_small_config_shape_with_orthonormal_orbitals():
+    """nao=300, naux=1000 (BASELINE.json's `small` B), all 300 MOs, (8 active) -- several tiles and aux blocks"""
+    bpa, ppaa, papa = run_case(300, 1000, 300, 80, 8, 220, L=20.0, orth=True)
+    # permutational symmetry of the CUDA result itself
+    assert rel(ppaa, ppaa.transpose(1, 0, 2, 3)) < 1e-12 and rel(papa, papa.transpose(2, 3, 0, 1)) < 1e-12
+
+
+def test_edges_and_errors():
+    import torch
+    import paper_2505_03755_b200 as dfjk
+    inp = dfjk_inputs.make_random(20, 6, [1], 230)
+    B = torch.from_numpy(inp.B_packed).cuda()
+    M = torch.from_numpy(np.random.default_rng(1).standard_normal((20, 10))).cuda()
+    with dfjk.DFJK(B, 20) as h:
+        bpa, ppaa, papa = h.ao2mo(M, 4, 0)                      # no active orbitals
+        assert bpa.shape == (6, 10, 0) and ppaa.numel() == 0
+        with pytest.raises(dfjk.DFJKError):
+            h.ao2mo(M, 8, 4)                                    # active range past nmo
+        J, K = h.get_jk([M[:, :3].contiguous()], [torch.ones(3, dtype=torch.float64, device="cuda")])
+        torch.cuda.synchronize()                                # the handle still serves get_jk
+        assert torch.isfinite(J).all() and torch.isfinite(K).all()
