@@ -12,7 +12,7 @@ constexpr int kBK = 32;            // k-chunk (doubles) of the SYRK tile pipelin
 constexpr int kLdT = kBK + 4;      // 36: row stride of a [rows][32] tile (4 mod 16: conflict-free fragments)
 constexpr int kHtBK = 16;          // k-chunk of the half-transform
 constexpr int kHtLd = kHtBK + 4;   // 20: row stride of [rows][16] tiles (4 mod 16)
-constexpr int kHtMaxWN = 20;       // half-transform N tile = 16*WN columns, WN <= 20
+constexpr int kHtMaxWN = 22;       // half-transform N tile = 16*WN columns, WN <= 22 (352 columns in one pass)
 constexpr int kJ1Rows = 64;        // aux rows per J-pass-1 work item (8 DMMA row groups per warp)
 constexpr int kJ1SubChunk = 2048;  // pairs per warp per J-pass-1 work item
 constexpr int kJ1Warps = 8;

@@ -748,7 +748,7 @@ static cudaError_t dispatch_ht_wn(int wn, int grid, cudaStream_t st, const HtPar
     DFJK_HT_CASE(1) DFJK_HT_CASE(2) DFJK_HT_CASE(3) DFJK_HT_CASE(4) DFJK_HT_CASE(5) DFJK_HT_CASE(6)
     DFJK_HT_CASE(7) DFJK_HT_CASE(8) DFJK_HT_CASE(9) DFJK_HT_CASE(10) DFJK_HT_CASE(11) DFJK_HT_CASE(12)
     DFJK_HT_CASE(13) DFJK_HT_CASE(14) DFJK_HT_CASE(15) DFJK_HT_CASE(16) DFJK_HT_CASE(17) DFJK_HT_CASE(18)
-    DFJK_HT_CASE(19) DFJK_HT_CASE(20)
+    DFJK_HT_CASE(19) DFJK_HT_CASE(20) DFJK_HT_CASE(21) DFJK_HT_CASE(22)
 #undef DFJK_HT_CASE
     default: return cudaErrorInvalidValue;
   }
