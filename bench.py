@@ -35,6 +35,9 @@ METRIC = "DF get_jk ms at nao=1200/naux=4000; K FP64 TFLOP/s & J HBM GB/s vs pea
 FP64_DMMA_PEAK_TFLOPS = 37.1
 FP64_CUBLAS_TFLOPS = 35.47
 HBM_READ_STREAM_GBS = 7430.0
+# ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum of k_half_transform<19,1> at `large`:
+# 9.90 GB per 1122-aux-row launch (profiles/r01_ncu_large_v2.md)
+HT_DRAM_BYTES_PER_AUX_ROW_LARGE = 9.90e9 / 1122
 
 
 def measured_peaks():
@@ -346,6 +349,7 @@ def main():
         ranks.close()
         return
     pk = measured_peaks()
+    npair_bytes = nao * (nao + 1) // 2 * 8.0
     ht_ms, ht_n = phases["half_transform"]
     sy_ms, sy_n = phases["syrk"]
     ht_tflops = fb["ht"] * args.steps / (ht_ms * 1e-3) * 1e-12 if ht_ms > 0 else 0.0
@@ -367,7 +371,11 @@ def main():
         "gpu_launches": launches,
         "roofline": {"kernel": "k_half_transform", "bound": "tensor", "achieved": ht_tflops,
                      "peak": FP64_DMMA_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ht_tflops / FP64_DMMA_PEAK_TFLOPS,
-                     "traffic": None, "launches": ht_n, "avg_launch_ms": ht_ms / max(ht_n, 1),
+                     "traffic": (HT_DRAM_BYTES_PER_AUX_ROW_LARGE * naux * args.steps / max(ht_n, 1)
+                                 if (nao, sum(nocc)) == (1200, 300) else None),
+                     "traffic_unit": "bytes per launch (ncu dram read + write, profiles/r01_ncu_large_v2.md)",
+                     "algorithmic_bytes_per_launch": (npair_bytes + nao * sum(nocc) * 8.0) * naux * args.steps / max(ht_n, 1),
+                     "launches": ht_n, "avg_launch_ms": ht_ms / max(ht_n, 1),
                      "algorithmic_flops_per_step": fb["ht"],
                      "peak_source": "measured DMMA.8x8x4 issue-rate peak on this pool (profiles/r01_ubench.md); "
                                     "cuBLAS fp64 8192^3 reaches %.2f; MEASURED_PEAKS bf16 %.1f x nominal 45/2250 = %.1f"

@@ -51,6 +51,7 @@ struct dfjk_ctx {
   int num_sms;
   int ht_grid, ht_skew;      // persistent half-transform: CTAs (= SMs), skewed warp pairs on/off
   int syrk_legacy, syrk_wm_forced;   // tuning only (env): wide/narrow-warp SYRK, forced tile size
+  int j1_legacy;             // tuning only (env): DMMA J pass 1 instead of the bulk-copy pipeline
   int two_pass_j;            // option: never fuse J pass 1 into the half-transform
   // scratch (all allocated at create)
   double* Ct;                // [nck][ct_rows][20]  C' transposed and k-tiled, sqrt(occ) folded, zero padded

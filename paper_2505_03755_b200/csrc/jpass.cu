@@ -8,6 +8,7 @@
 // The k index of an MMA is free to permute, so each lane reads 16 contiguous bytes (LDG.128).
 #include "common.cuh"
 #include "ctx.h"
+#include "pipeline.cuh"
 
 namespace dfjk {
 
@@ -187,6 +188,145 @@ k_j1_v4(const double* __restrict__ B, size_t npair, int naux, const double* __re
   }
 }
 
+// Pass 1 as a bulk-copy (TMA engine) pipeline, for npair even (every packed row and every Dw row
+// then starts 16-byte aligned).  CTA = 64 aux rows x kJ1Chunk pairs, walked as 8 row groups of 8
+// rows x 32 chunks of 512 pairs; a stage holds the chunk of the 8 rows (32 KB) and of the NS
+// weighted densities (4 KB each), filled by one elected producer thread with 8 + NS bulk copies,
+// so 100-190 KB per SM are in flight whatever the consumers do.  Consumer warp w owns pairs
+// [64 w, 64 w + 64) of every chunk, a lane two adjacent pairs (one conflict-free LDS.128 per row):
+// 8 x NS accumulators per lane, plain DFMA (the stream needs 3 DFMA/clk/SM per set), reduced by
+// shuffles and a fixed-order sum over the 8 warps once per row group.
+constexpr int kJ1tSC = 512;                       // pairs per stage
+constexpr int kJ1tThreads = 288;                  // 8 consumer warps + 1 producer warp
+__host__ __device__ constexpr int j1t_stages(int ns) { return ns <= 1 ? 6 : ns <= 2 ? 5 : ns <= 4 ? 4 : 3; }
+
+template <int NS>
+__global__ void __launch_bounds__(kJ1tThreads, 1)
+k_j1_tma(const double* __restrict__ B, size_t npair, int naux, const double* __restrict__ Dw,
+         double* __restrict__ part, int naux_pad) {
+  constexpr int STAGES = j1t_stages(NS);
+  constexpr int kStageDoubles = (8 + NS) * kJ1tSC;
+  extern __shared__ __align__(128) double smem[];
+  __shared__ __align__(8) unsigned long long bars[2 * STAGES];
+  __shared__ double red[8][8][NS];
+  const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[STAGES]);
+  const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
+  const int p0 = blockIdx.y * kJ1Rows;
+  const size_t kbeg = (size_t)blockIdx.x * kJ1Chunk;
+  const size_t kend = kbeg + kJ1Chunk < npair ? kbeg + kJ1Chunk : npair;
+  const int nchunk = (int)((kend - kbeg + kJ1tSC - 1) / kJ1tSC);
+  const int ngroups = min(8, (naux - p0 + 7) / 8);
+  const int nstage = ngroups * nchunk;
+  if (tid == 0) {
+    for (int s = 0; s < STAGES; s++) {
+      mbar_init(full0 + 8 * s, 1);
+      mbar_init(empty0 + 8 * s, 8);
+    }
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  if (w == 8) {
+    if (l == 0) {
+      const uint32_t s_u32 = smem_u32(smem);
+      int rg = 0, c = 0;
+      for (int it = 0; it < nstage; it++) {
+        const int stage = it % STAGES;
+        const uint32_t fullb = full0 + 8 * stage;
+        mbar_wait(empty0 + 8 * stage, ((it / STAGES) & 1) ^ 1);
+        const size_t k0 = kbeg + (size_t)c * kJ1tSC;
+        const uint32_t bytes = (uint32_t)((kend - k0 < (size_t)kJ1tSC ? kend - k0 : (size_t)kJ1tSC) * 8);
+        const int nrows = min(8, naux - (p0 + 8 * rg));
+        mbar_arrive_expect_tx(fullb, bytes * (uint32_t)(nrows + NS));
+        const uint32_t dst = s_u32 + (uint32_t)(stage * kStageDoubles) * 8u;
+        for (int g = 0; g < nrows; g++)
+          bulk_g2s(dst + (uint32_t)(g * kJ1tSC) * 8u, B + (size_t)(p0 + 8 * rg + g) * npair + k0, bytes, fullb);
+        for (int s = 0; s < NS; s++)
+          bulk_g2s(dst + (uint32_t)((8 + s) * kJ1tSC) * 8u, Dw + (size_t)s * npair + k0, bytes, fullb);
+        if (++c == nchunk) { c = 0; rg++; }
+      }
+    }
+    return;
+  }
+
+  double acc[8][NS];
+  int it = 0;
+  for (int rg = 0; rg < ngroups; rg++) {
+#pragma unroll
+    for (int g = 0; g < 8; g++)
+#pragma unroll
+      for (int s = 0; s < NS; s++) acc[g][s] = 0.0;
+    const int nrows = min(8, naux - (p0 + 8 * rg));
+    for (int c = 0; c < nchunk; c++, it++) {
+      const int stage = it % STAGES;
+      const size_t k0 = kbeg + (size_t)c * kJ1tSC;
+      const int nvalid = (int)(kend - k0 < (size_t)kJ1tSC ? kend - k0 : (size_t)kJ1tSC);
+      mbar_wait(full0 + 8 * stage, (it / STAGES) & 1);
+      const double* sp = smem + stage * kStageDoubles + w * 64 + 2 * l;
+      if (w * 64 + 2 * l < nvalid) {          // nvalid is even: a lane's two pairs are both in or both out
+        double2 d[NS];
+#pragma unroll
+        for (int s = 0; s < NS; s++) d[s] = *reinterpret_cast<const double2*>(sp + (8 + s) * kJ1tSC);
+#pragma unroll
+        for (int g = 0; g < 8; g++) {
+          if (g < nrows) {
+            const double2 b = *reinterpret_cast<const double2*>(sp + g * kJ1tSC);
+#pragma unroll
+            for (int s = 0; s < NS; s++) acc[g][s] = fma(b.y, d[s].y, fma(b.x, d[s].x, acc[g][s]));
+          }
+        }
+      }
+      __syncwarp();
+      if (l == 0) mbar_arrive(empty0 + 8 * stage);
+    }
+    // row group done: lanes -> warp (xor shuffles), warps -> CTA (fixed order)
+#pragma unroll
+    for (int g = 0; g < 8; g++)
+#pragma unroll
+      for (int s = 0; s < NS; s++) {
+        double v = acc[g][s];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (l == 0) red[w][g][s] = v;
+      }
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+    if (tid < 8 * NS) {
+      const int g = tid / NS, s = tid % NS;
+      double t = 0.0;
+#pragma unroll
+      for (int ww = 0; ww < 8; ww++) t += red[ww][g][s];
+      part[((size_t)blockIdx.x * 8 + s) * naux_pad + p0 + 8 * rg + g] = t;
+    }
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+  }
+}
+
+template <int NS>
+static cudaError_t launch_j1_tma(dim3 grid, cudaStream_t st, const double* B, size_t npair, int naux, const double* Dw,
+                                 double* part, int naux_pad) {
+  constexpr size_t smem = (size_t)j1t_stages(NS) * (8 + NS) * kJ1tSC * sizeof(double);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(k_j1_tma<NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  k_j1_tma<NS><<<grid, kJ1tThreads, smem, st>>>(B, npair, naux, Dw, part, naux_pad);
+  return cudaSuccess;
+}
+
+static cudaError_t dispatch_j1_tma(int ns, dim3 grid, cudaStream_t st, const double* B, size_t npair, int naux,
+                                   const double* Dw, double* part, int naux_pad) {
+  switch (ns) {
+#define DFJK_J1T_CASE(N) \
+  case N: return launch_j1_tma<N>(grid, st, B, npair, naux, Dw, part, naux_pad);
+    DFJK_J1T_CASE(1) DFJK_J1T_CASE(2) DFJK_J1T_CASE(3) DFJK_J1T_CASE(4)
+    DFJK_J1T_CASE(5) DFJK_J1T_CASE(6) DFJK_J1T_CASE(7) DFJK_J1T_CASE(8)
+#undef DFJK_J1T_CASE
+    default: return cudaErrorInvalidValue;
+  }
+}
+
 // rho[s][P] = sum over chunks in ascending order
 __global__ void k_j1_reduce(const double* __restrict__ part, int nchunks, int naux_pad, int naux, int nsetg,
                             double* __restrict__ rho) {
@@ -326,7 +466,8 @@ int launch_j_passes(dfjk_ctx* h, const SetInfo& si, double* J_out, bool rho_read
     if (naux > 0 && !rho_ready) {
       prof_mark(h, DFJK_PHASE_J1, st);
       dim3 g1(h->j1_chunks, naux_pad / kJ1Rows);
-      if (npair % 4 == 0) k_j1_v4<<<g1, kJ1Warps * 32, 0, st>>>(h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad);
+      if (vec && !h->j1_legacy) dispatch_j1_tma(ns, g1, st, h->B, npair, naux, h->Dw + (size_t)s0 * npair, h->rho_part, naux_pad);
+      else if (npair % 4 == 0) k_j1_v4<<<g1, kJ1Warps * 32, 0, st>>>(h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad);
       else if (vec) k_j1<true><<<g1, kJ1Warps * 32, 0, st>>>(h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad);
       else k_j1<false><<<g1, kJ1Warps * 32, 0, st>>>(h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad);
       dim3 gr(cdiv(naux, 128), ns);

@@ -86,6 +86,31 @@ def test_ragged_shapes(torch_cuda, dfjk, nao, naux, nocc, seed):
     check_against_oracle(torch_cuda, dfjk, inp)
 
 
+@pytest.mark.parametrize("nao,naux,nocc,seed", [
+    (5, 3, [2], 121),                      # npair odd: the DMMA fallback of pass 1
+    (8, 13, [3, 2], 122),                  # npair even, 36 pairs: far less than one stage
+    (67, 45, [23, 7], 123),                # npair even, ragged rows (45 = 5 groups of 8 + 5)
+    (181, 70, [9, 8, 8, 1, 40, 3], 124),   # npair = 16471: one full 16384-pair CTA chunk + a ragged one
+    (200, 130, [9, 8, 8, 1, 40, 3, 17, 2], 125),   # eight sets, three row blocks of 64
+    (40, 21, [3, 1, 4, 1, 5, 9, 2, 6, 5, 3, 5], 126),   # eleven sets: two set groups
+])
+def test_j_only_two_pass_path(torch_cuda, dfjk, nao, naux, nocc, seed):
+    """J alone runs the two-pass J (bulk-copy pipeline for pass 1 when npair is even)."""
+    import oracle
+    torch = torch_cuda
+    inp = dfjk_inputs.make_random(nao, naux, nocc, seed, L=max(4.0, nao / 6))
+    Jo, _ = oracle.get_jk_inputs(inp, with_k=False)
+    B, Cs, occs = to_dev(torch, inp)
+    with dfjk.DFJK(B, inp.nao, max_nset=12, max_nocc_total=max(nao, sum(nocc))) as h:
+        J, K = h.get_jk(Cs, occs, with_k=False)
+        torch.cuda.synchronize()
+        assert K is None
+    J = J.cpu().numpy()
+    for s in range(inp.nset):
+        assert rel(J[s], Jo[s]) <= TOL, (s, rel(J[s], Jo[s]))
+        assert np.array_equal(J[s], J[s].T)
+
+
 def test_more_than_eight_sets(torch_cuda, dfjk):
     inp = dfjk_inputs.make_random(40, 21, [3, 1, 4, 1, 5, 9, 2, 6, 5, 3, 5], 109)
     check_against_oracle(torch_cuda, dfjk, inp, max_nset=12, max_nocc_total=44)
