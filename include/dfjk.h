@@ -101,6 +101,19 @@ int dfjk_get_jk_host(dfjk_handle h, int nset, const int* nocc, const double* C, 
                      double* J_out, double* K_out, dfjk_stream stream);
 
 /*
+ * dfjk_get_jk_dm -- the JK call stated with density matrices, Eq. 14-17 exactly as printed
+ * ("the input is a density matrix ..."), for densities that have no
+ * C diag(occ) C^T form with occ >= 0 (differences of densities, transition densities):
+ *      rho_P = sum b^P_{mu nu} D_{mu nu},  J = sum_P rho_P b^P                 Eq. 14-15
+ *      V^P = b^P D (Eq. 16),  K = sum_P V^P b^P (Eq. 17)
+ *   D        DEVICE, nset x nao x nao row-major; every D_s must be symmetric (J uses its symmetric
+ *            part; K = sum_P b^P D b^P is computed on the lower triangle and mirrored).
+ *   J_out, K_out, stream: as in dfjk_get_jk.  1 <= nset <= max_nset; needs max_nocc_total >= nao
+ *            (the default).  Costs 3 naux nao^3 flop per set for K instead of 3 naux nao^2 nocc.
+ */
+int dfjk_get_jk_dm(dfjk_handle h, int nset, const double* D, double* J_out, double* K_out, dfjk_stream stream);
+
+/*
  * dfjk_ao2mo -- the AO2MO kernel of section 2.D.ii (Eq. 18-21) on the same
  * resident Cholesky vectors, with the index pattern fixed by Eq. 12, g = (m1 m2|m3 m4) = b b:
  *      X^P[e2][p1]   = sum_{e1} b^P[e1][e2] M[e1][p1]                          Eq. 18

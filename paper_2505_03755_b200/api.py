@@ -14,7 +14,7 @@ _lib = None
 
 EXPORTS = ["dfjk_create", "dfjk_get_jk", "dfjk_get_jk_host", "dfjk_destroy", "dfjk_strerror",
            "dfjk_last_error", "dfjk_workspace_bytes", "dfjk_get_plan", "dfjk_last_launch_count",
-           "dfjk_selftest_dmma", "dfjk_set_profiling", "dfjk_get_profile", "dfjk_ao2mo"]
+           "dfjk_selftest_dmma", "dfjk_set_profiling", "dfjk_get_profile", "dfjk_ao2mo", "dfjk_get_jk_dm"]
 
 PHASES = ["prep", "j1", "j2", "j_epilogue", "half_transform", "syrk", "k_epilogue"]
 
@@ -51,6 +51,8 @@ def load_library():
         fn = getattr(lib, name)
         fn.argtypes = [vp, ct.c_int, ip, dp, dp, dp, dp, vp]
         fn.restype = ct.c_int
+    lib.dfjk_get_jk_dm.argtypes = [vp, ct.c_int, dp, dp, dp, vp]
+    lib.dfjk_get_jk_dm.restype = ct.c_int
     lib.dfjk_ao2mo.argtypes = [vp, ct.c_int, ct.c_int, ct.c_int, dp, dp, dp, dp, vp]
     lib.dfjk_ao2mo.restype = ct.c_int
     lib.dfjk_destroy.argtypes = [vp]
@@ -168,6 +170,25 @@ class DFJK:
                                               ct.c_void_p(st.cuda_stream))
         _check(self._lib, code, self._h)
         return J_host, K_host
+
+    def get_jk_dm(self, D, with_j: bool = True, with_k: bool = True, out_j=None, out_k=None, stream=None):
+        """dfjk_get_jk_dm: D is a CUDA float64 (nset, nao, nao) tensor of symmetric density matrices
+        (Eq. 14-17 as printed); returns (J, K), enqueue-only."""
+        import torch
+        if D.dim() != 3 or tuple(D.shape[1:]) != (self.nao, self.nao):
+            raise ValueError(f"D must have shape (nset, {self.nao}, {self.nao})")
+        D = D.to(device=self._device, dtype=torch.float64).contiguous()
+        nset = int(D.shape[0])
+        with torch.cuda.device(self._device):
+            st = stream if stream is not None else torch.cuda.current_stream()
+            J = out_j if out_j is not None else (torch.empty_like(D) if with_j else None)
+            K = out_k if out_k is not None else (torch.empty_like(D) if with_k else None)
+            code = self._lib.dfjk_get_jk_dm(self._h, nset, ct.c_void_p(D.data_ptr()),
+                                            ct.c_void_p(J.data_ptr() if J is not None else 0),
+                                            ct.c_void_p(K.data_ptr() if K is not None else 0),
+                                            ct.c_void_p(st.cuda_stream))
+        _check(self._lib, code, self._h)
+        return J, K
 
     def ao2mo(self, M, a0: int, nact: int, with_ppaa: bool = True, with_papa: bool = True, stream=None):
         """dfjk_ao2mo (Eq. 18-21): M is a CUDA float64 (nao, nmo) tensor; returns (bpa, ppaa, papa) with

@@ -236,6 +236,38 @@ int dfjk_get_jk_host(dfjk_handle h, int nset, const int* nocc, const double* C, 
   return DFJK_OK;
 }
 
+int dfjk_get_jk_dm(dfjk_handle h, int nset, const double* D, double* J_out, double* K_out, dfjk_stream stream) {
+  if (!h) return DFJK_ERR_INVALID_ARG;
+  if (nset < 1 || nset > h->max_nset || !D) return DFJK_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  h->last_launches = 0;
+  h->last_error[0] = 0;
+  h->ev_n = 0;
+  if (!J_out && !K_out) return DFJK_OK;
+  int n = 0;
+  if (J_out) {
+    SetInfo si;
+    memset(&si, 0, sizeof(si));
+    si.nset = nset;
+    n += launch_prep_dw_dm(h, nset, D, st);
+    n += launch_j_passes(h, si, J_out, false, st);
+  }
+  if (K_out) {
+    const int k = launch_k_path_dm(h, nset, D, K_out, st);
+    if (k == -2) {
+      snprintf(h->last_error, sizeof(h->last_error), "workspace or column capacity too small for the density-matrix form");
+      return DFJK_ERR_INVALID_ARG;
+    }
+    if (k < 0) { set_err(h, "k path launch", cudaGetLastError()); return DFJK_ERR_CUDA; }
+    n += k;
+  }
+  prof_mark(h, -1, st);
+  h->last_launches = n;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { set_err(h, "kernel launch", e); return DFJK_ERR_CUDA; }
+  return DFJK_OK;
+}
+
 int dfjk_ao2mo(dfjk_handle h, int nmo, int a0, int nact, const double* M, double* bpa_out, double* ppaa_out,
                double* papa_out, dfjk_stream stream) {
   if (!h) return DFJK_ERR_INVALID_ARG;

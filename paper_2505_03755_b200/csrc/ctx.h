@@ -95,6 +95,9 @@ int launch_half_transform_rowmajor(dfjk_ctx* h, const SetInfo& si, int p_first, 
 // cannot hold one aux row
 int launch_ao2mo(dfjk_ctx* h, int nmo, int a0, int nact, const double* M, double* bpa_out, double* ppaa_out,
                  double* papa_out, cudaStream_t st);
+// density-matrix form: packed weighted density from D, and K by Eq. 16-17 as printed
+int launch_prep_dw_dm(dfjk_ctx* h, int nset, const double* D, cudaStream_t st);
+int launch_k_path_dm(dfjk_ctx* h, int nset, const double* D, double* K_out, cudaStream_t st);
 int run_dmma_selftest();
 
 }  // namespace dfjk

@@ -571,9 +571,12 @@ __device__ __forceinline__ void syrk2_store(double* Kp, int nao, int mu0, int nu
 // ntiles_m * ksplit cheaper diagonal ones, which fill the tail of the last wave.
 template <int WM>
 __global__ void __launch_bounds__(kThreads, 1)
-k_syrk2(const double* __restrict__ X, int nao, int nch, int mu_pad, int c0, int c1, int nrows_blk,
-        int rows_per_split, int ntiles_m, int ksplit, double* __restrict__ Kpart_s, size_t split_stride,
-        int first) {
+k_syrk2(const double* __restrict__ X, const double* __restrict__ X2, int nao, int nch, int mu_pad, int c0,
+        int c1, int nrows_blk, int rows_per_split, int ntiles_m, int ksplit, double* __restrict__ Kpart_s,
+        size_t split_stride, int first) {
+  // X2 == nullptr: K += X X^T (SYRK).  Otherwise K += X X2^T for a product known to be symmetric
+  // (density-matrix form, Eq. 16-17: X = B_P D, X2 = B_P): the column operand comes from X2, and
+  // diagonal tiles fetch both operands.
   constexpr int T = 16 * WM;
   constexpr int kTileDoubles = T * kLdT;
   constexpr uint32_t kTileBytes = kTileDoubles * 8;
@@ -599,6 +602,7 @@ k_syrk2(const double* __restrict__ X, int nao, int nch, int mu_pad, int c0, int 
     ta = tb = t % ntiles_m;
     g = t / ntiles_m;
   }
+  const bool one_operand = diag && X2 == nullptr;
   const int a0 = ta * T, b0 = tb * T;
   const int p_beg = g * rows_per_split;
   int p_end = p_beg + rows_per_split;
@@ -628,10 +632,11 @@ k_syrk2(const double* __restrict__ X, int nao, int nch, int mu_pad, int c0, int 
         const int stage = c % kStages;
         const uint32_t fullb = full0 + 8 * stage;
         mbar_wait(empty0 + 8 * stage, ((c / kStages) & 1) ^ 1);
-        const double* src = X + (size_t)P * row_stride + (size_t)ch * chunk_stride;
-        mbar_arrive_expect_tx(fullb, diag ? kTileBytes : 2 * kTileBytes);
-        bulk_g2s(sA_u32 + (uint32_t)stage * kTileBytes, src + (size_t)a0 * kLdT, kTileBytes, fullb);
-        if (!diag) bulk_g2s(sB_u32 + (uint32_t)stage * kTileBytes, src + (size_t)b0 * kLdT, kTileBytes, fullb);
+        const size_t off = (size_t)P * row_stride + (size_t)ch * chunk_stride;
+        mbar_arrive_expect_tx(fullb, one_operand ? kTileBytes : 2 * kTileBytes);
+        bulk_g2s(sA_u32 + (uint32_t)stage * kTileBytes, X + off + (size_t)a0 * kLdT, kTileBytes, fullb);
+        if (!one_operand)
+          bulk_g2s(sB_u32 + (uint32_t)stage * kTileBytes, (X2 ? X2 : X) + off + (size_t)b0 * kLdT, kTileBytes, fullb);
         if (++ch == ch1) { ch = ch0; P++; }
       }
     }
@@ -643,7 +648,7 @@ k_syrk2(const double* __restrict__ X, int nao, int nch, int mu_pad, int c0, int 
   const int sp = w & 3, hh = w >> 2;                 // SM sub-partition, first/second warp of the pair
   double* Kp = Kpart_s + (size_t)g * split_stride;
   double* red = smem;                                // reused after the main loop
-  Syrk2Consumer q{sA, diag ? sA : sB, full0, empty0, skewbar, nchunks, ch0, ch1, c0, c1, kTileDoubles,
+  Syrk2Consumer q{sA, one_operand ? sA : sB, full0, empty0, skewbar, nchunks, ch0, ch1, c0, c1, kTileDoubles,
                   0, 0, 0, hh == 1};
   if (!diag) {
     // block (bm, bn) = (sp & 1, sp >> 1); pair split-K 2
@@ -767,6 +772,7 @@ static cudaError_t dispatch_ht(int wn, int epi, int grid, cudaStream_t st, const
 struct SyrkArgs {
   const double* X; int nao, nch, mu_pad, c0, c1, nrows_blk, rows_per_split, ntiles_m; double* Kpart_s;
   size_t split_stride; int first;
+  const double* X2 = nullptr;   // k_syrk2 only: column operand of the two-operand form
 };
 
 template <int WM>
@@ -805,7 +811,7 @@ static cudaError_t launch_syrk2(int ksplit, cudaStream_t st, const SyrkArgs& a) 
     attr_set = true;
   }
   const int grid = a.ntiles_m * (a.ntiles_m + 1) / 2 * ksplit;
-  k_syrk2<WM><<<grid, kThreads, syrk_smem_bytes(WM), st>>>(a.X, a.nao, a.nch, a.mu_pad, a.c0, a.c1, a.nrows_blk,
+  k_syrk2<WM><<<grid, kThreads, syrk_smem_bytes(WM), st>>>(a.X, a.X2, a.nao, a.nch, a.mu_pad, a.c0, a.c1, a.nrows_blk,
                                                          a.rows_per_split, a.ntiles_m, ksplit, a.Kpart_s,
                                                          a.split_stride, a.first);
   return cudaSuccess;
@@ -962,6 +968,125 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
   h->plan_nblk = (int)nblk;
   h->plan_ksplit = ksplit;
   h->plan_nblocks = nblocks;
+  return launches;
+}
+
+// ------------------------------------------------------------------ density-matrix form (Eq. 16-17 as printed)
+// K = sum_P (B_P D) B_P for a general symmetric D (it need not be positive semidefinite, so no
+// C sqrt(occ) factor exists): Eq. 16 is the half-transform with C' = D (nao columns), Eq. 17 the
+// two-operand form of k_syrk2 against the unpacked slice.
+// The unpacked slice is written in the same k-tiled layout as X ("unpacked to the square-matrix
+// form"): X2[P][sigma/32][nu][sigma%32] = B_P[nu][sigma], zero past nao.
+__global__ void __launch_bounds__(256)
+k_unpack_tiled(const double* __restrict__ Bp, size_t npair, int nao, int p_first, int nch, int mu_pad,
+               double* __restrict__ X2) {
+  const int pl = blockIdx.y, ch = blockIdx.x;
+  const double* BpP = Bp + (size_t)(p_first + pl) * npair;
+  double* dst = X2 + ((size_t)pl * nch + ch) * mu_pad * kLdT;
+  for (int e = threadIdx.x; e < nao * 32; e += 256) {
+    const int nu = e >> 5, k = e & 31, sg = ch * 32 + k;
+    double v = 0.0;
+    if (sg < nao) v = BpP[sg <= nu ? tri(nu) + sg : tri(sg) + nu];
+    dst[(size_t)nu * kLdT + k] = v;
+  }
+}
+
+// Dw[pair] = (2 - delta) (D[mu][nu] + D[nu][mu]) / 2 from a full square density
+__global__ void k_prep_dw_dm(const double* __restrict__ D, int nao, size_t npair, double* __restrict__ Dw) {
+  const int s = blockIdx.y;
+  const double* Ds = D + (size_t)s * nao * nao;
+  for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < (size_t)nao * nao; e += (size_t)gridDim.x * blockDim.x) {
+    const int mu = (int)(e / nao), nu = (int)(e % nao);
+    if (nu <= mu) Dw[(size_t)s * npair + tri(mu) + nu] = (mu == nu) ? Ds[e] : (Ds[e] + Ds[(size_t)nu * nao + mu]);
+  }
+}
+
+int launch_prep_dw_dm(dfjk_ctx* h, int nset, const double* D, cudaStream_t st) {
+  prof_mark(h, DFJK_PHASE_PREP, st);
+  dim3 grid(592, nset);
+  k_prep_dw_dm<<<grid, 256, 0, st>>>(D, h->nao, h->npair, h->Dw);
+  return 1;
+}
+
+int launch_k_path_dm(dfjk_ctx* h, int nset, const double* D, double* K_out, cudaStream_t st) {
+  int launches = 0;
+  const int nao = h->nao, naux = h->naux;
+  const size_t n2 = (size_t)nao * nao;
+  if (naux == 0) {
+    prof_mark(h, DFJK_PHASE_K_EPILOGUE, st);
+    k_zero<<<148, 256, 0, st>>>(K_out, n2 * nset);
+    return 1;
+  }
+  SetInfo si;
+  si.nset = 1; si.col0[0] = 0; si.nocc[0] = nao; si.coff[0] = 0; si.ooff[0] = 0;
+  si.col0[1] = si.nocc_pad = round_up(nao, 8);
+  if (si.nocc_pad > h->nocc_pad_cap) return -2;
+  const int ldx = si.nocc_pad, nch = cdiv(ldx, kBK);
+  const size_t row_doubles = (size_t)nch * h->mu_pad * kLdT;
+  long long nblk = (long long)(h->X_doubles / (2 * row_doubles));     // X = B_P D and the unpacked slice
+  if (h->nblk_forced > 0 && nblk > h->nblk_forced) nblk = h->nblk_forced;
+  if (nblk > naux) nblk = naux;
+  if (nblk > 32768) nblk = 32768;
+  if (nblk < 1) return -2;
+  double* X1 = h->X;
+  double* X2 = h->X + (size_t)nblk * row_doubles;
+  const int n8 = ldx / 8;
+  const int ntn = cdiv(n8, 2 * kHtMaxWN), wn = cdiv(n8, 2 * ntn);
+  const int ntm_ht = cdiv(nao, 64);
+  int wm_s = 6;
+  {
+    double best = 1e300;
+    for (int wmc = 6; wmc >= 4; wmc--) {
+      const int T = 16 * wmc, nt = cdiv(nao, T);
+      const double area = (0.5 * nt * (nt - 1) + (wmc + 1) / (2.0 * wmc) * nt) * (double)T * T;
+      if (area < best * 0.995) { best = area; wm_s = wmc; }
+    }
+  }
+  const double diag_cost = (wm_s + 1) / (2.0 * wm_s);
+  const int ntm = cdiv(nao, 16 * wm_s), ntiles = ntm * (ntm + 1) / 2;
+  int ksplit = h->ksplit_forced;
+  if (ksplit <= 0) {
+    double best = 1e300;
+    ksplit = 1;
+    for (int k = 1; k <= h->ksplit && k <= nblk; k++) {
+      const int rps = cdiv((int)nblk, k);
+      if (cdiv((int)nblk, rps) != k) continue;
+      const double t = syrk_makespan(ntiles - ntm, ntm, diag_cost, k, rps, h->num_sms) * (1.0 + 0.002 * k);
+      if (t < best) { best = t; ksplit = k; }
+    }
+  }
+  if (ksplit > h->ksplit) ksplit = h->ksplit;
+  if (ksplit > nblk) ksplit = (int)nblk;
+  const size_t split_stride = (size_t)h->max_nset * n2;
+  const int nb32 = cdiv(nao, 32);
+  for (int s = 0; s < nset; s++) {
+    SetInfo sj = si;
+    launches += launch_prep_ct(h, sj, D + n2 * s, nullptr, st);         // C' = D_s
+    for (int p0 = 0; p0 < naux; p0 += (int)nblk) {
+      const int nb = (int)(naux - p0 < nblk ? naux - p0 : nblk);
+      prof_mark(h, DFJK_PHASE_HALF_TRANSFORM, st);
+      HtParams a;
+      a.Bp = h->B; a.npair = h->npair; a.nao = nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = ldx;
+      a.X = X1; a.nch = nch; a.mu_pad = h->mu_pad; a.p_first = p0; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
+      a.skew = h->ht_skew; a.rho_ht = nullptr; a.nset = 0; a.ldx = 0; a.xrows = 0; a.col0[0] = 0;
+      const long long ht_tiles = (long long)nb * ntm_ht * ntn;
+      if (dispatch_ht(wn, 0, (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid), st, a) != cudaSuccess) return -1;
+      dim3 gu(nch, nb);
+      k_unpack_tiled<<<gu, 256, 0, st>>>(h->B, h->npair, nao, p0, nch, h->mu_pad, X2);
+      launches += 2;
+      prof_mark(h, DFJK_PHASE_SYRK, st);
+      SyrkArgs sa{X1, nao, nch, h->mu_pad, 0, round_up(nao, 4), nb, cdiv(nb, ksplit), ntm, h->Kpart + n2 * s,
+                  split_stride, p0 == 0 ? 1 : 0, X2};
+      if (dispatch_syrk2(wm_s, ksplit, st, sa) != cudaSuccess) return -1;
+      launches++;
+    }
+    prof_mark(h, DFJK_PHASE_K_EPILOGUE, st);
+    dim3 ge(nb32, nb32, 1), be(32, 8);
+    k_k_epilogue<<<ge, be, 0, st>>>(h->Kpart + n2 * s, ksplit, split_stride, nao, K_out + n2 * s);
+    launches++;
+  }
+  h->plan_nblk = (int)nblk;
+  h->plan_ksplit = ksplit;
   return launches;
 }
 

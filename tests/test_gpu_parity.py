@@ -166,6 +166,37 @@ def test_repeat_calls_are_bitwise_deterministic_and_stream_ordered(torch_cuda, d
         assert torch.equal(J0, J2) and torch.equal(K0, K2)
 
 
+def test_get_jk_is_cuda_graph_capturable(torch_cuda, dfjk):
+    """dfjk_get_jk only enqueues (no allocation, no host sync: PAPER.md:259-261), so a call can be
+    captured into a CUDA graph and replayed on new orbitals -- the many-small-calls regime of the
+    embedded fragments."""
+    import oracle
+    torch = torch_cuda
+    a = dfjk_inputs.make_random(60, 35, [13, 5], 131, L=9.0)
+    b = dfjk_inputs.make_random(60, 35, [13, 5], 132, L=9.0)           # other orbitals, same shapes
+    B = torch.from_numpy(a.B_packed).cuda()
+    C = torch.from_numpy(a.C_concat()).cuda()
+    occ = torch.from_numpy(a.occ_concat()).cuda()
+    J = torch.empty((2, 60, 60), dtype=torch.float64, device="cuda")
+    K = torch.empty_like(J)
+    with dfjk.DFJK(B, 60) as h:
+        h.get_jk_raw(a.nocc, C, occ, out_j=J, out_k=K)                 # warm-up: function attributes set
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            h.get_jk_raw(a.nocc, C, occ, out_j=J, out_k=K)
+        for inp in (b, a):
+            C.copy_(torch.from_numpy(inp.C_concat()))
+            occ.copy_(torch.from_numpy(inp.occ_concat()))
+            J.zero_(); K.zero_()
+            g.replay()
+            torch.cuda.synchronize()
+            Jo, Ko = oracle.get_jk(a.B_packed, 60, inp.C, inp.occ)
+            for s in range(2):
+                assert rel(J[s].cpu().numpy(), Jo[s]) <= TOL and rel(K[s].cpu().numpy(), Ko[s]) <= TOL
+        del g
+
+
 def test_outputs_are_overwritten_not_accumulated(torch_cuda, dfjk):
     torch = torch_cuda
     inp = dfjk_inputs.make_random(33, 12, [7], 113)
