@@ -226,6 +226,9 @@ def main():
     ap.add_argument("--no-parity", action="store_true", help="skip the sampled parity check")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--shard-aux", action="store_true",
+                    help="with --gpus N > 1: shard the aux rows over the ranks and sum-all-reduce J, K (strong scaling) "
+                         "instead of N independent replicas")
     ap.add_argument("--no-ao2mo", action="store_true", help="skip the AO2MO (Eq. 18-21) section")
     ap.add_argument("--workspace-gib", type=float, default=0.0, help="dfjk_options.workspace_cap_bytes (0 = default)")
     args = ap.parse_args()
@@ -253,6 +256,14 @@ def main():
     want_host_B = lead and world == 1 and not (args.no_parity and args.no_cpu_baseline)
     t_gen = time.perf_counter()
     Bd, Bh = upload_B(torch, cfg, keep_host=want_host_B)
+    shard = args.shard_aux and world > 1
+    if shard:
+        from paper_2505_03755_b200.sharded import AuxShardedJK, aux_range
+        lo, hi = aux_range(naux, rank, world)
+        Bd = Bd[lo:hi].clone()                     # this rank's contiguous aux rows
+        torch.cuda.empty_cache()
+        fb = flops_bytes(dict(cfg, naux=hi - lo))  # per-kernel rooflines are per rank
+        args.no_ao2mo = True
     t_gen = time.perf_counter() - t_gen
     C_list, occ_list = dfjk_inputs.make_orbitals(name)
     C_host = torch.from_numpy(np.concatenate([c.ravel() for c in C_list])).pin_memory()
@@ -278,6 +289,9 @@ def main():
         return e0.elapsed_time(e1) / steps
 
     full = lambda: h.get_jk_raw(nocc, C_dev, occ_dev, out_j=J, out_k=K, stream=stream)
+    if shard:
+        local_full = full
+        full = lambda: AuxShardedJK(local_full, None).get_jk()   # partial J, K + one NCCL sum all-reduce each
     j_only = lambda: h.get_jk_raw(nocc, C_dev, occ_dev, with_k=False, out_j=J, stream=stream)
     k_only = lambda: h.get_jk_raw(nocc, C_dev, occ_dev, with_j=False, out_k=K, stream=stream)
     host = lambda: h.get_jk_host(nocc, C_host, occ_host, J_host, K_host, stream=stream)
@@ -357,10 +371,11 @@ def main():
     j1_ms, j2_ms = phases["j1"][0] / args.steps, phases["j2"][0] / args.steps
     line = {
         "metric": METRIC, "value": ms_step, "unit": "ms", "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": False,
+        "scaling": "strong" if shard else "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": name, "nao": nao, "naux": naux, "nset": nset, "nocc": nocc,
-                   "B_packed_GB": fb["b_bytes"] * 1e-9, "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "B_packed_GB": fb["b_bytes"] * 1e-9, "parallelism": ("aux-sharded + all-reduce" if shard else "replicas only") if world > 1 else "1 gpu",
                    "l2": "inputs (packed B) far larger than the 126 MB L2, no flush needed" if fb["b_bytes"] > 1e9
                          else "L2-warm (inputs fit the L2)",
                    "plan": plan, "input_gen_s": round(t_gen, 1)},

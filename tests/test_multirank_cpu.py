@@ -75,3 +75,46 @@ def test_reference_arm_runs_on_rank0_only():
     assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["unit"] == "ms" and d["higher_is_better"] is False
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] == d["value"]
     assert d["e2e"] == {"value": d["value"], "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+
+
+SHARD_WORKER = r"""
+import os, sys
+sys.path.insert(0, sys.argv[1])
+import numpy as np, torch, torch.distributed as dist
+import dfjk_inputs, oracle
+from paper_2505_03755_b200.sharded import AuxShardedJK, aux_range
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+inp = dfjk_inputs.make_random(23, 17, [6, 3], 77, L=5.0)          # 17 aux rows over 2 ranks: 9 + 8
+lo, hi = aux_range(inp.naux, rank, world)
+assert (lo, hi) == ((0, 9) if rank == 0 else (9, 17))
+def local(Cs, occs):                                               # stands in for DFJK.get_jk on B[lo:hi]
+    J, K = oracle.get_jk(inp.B_packed[lo:hi], inp.nao, Cs, occs)
+    return torch.from_numpy(J), torch.from_numpy(K)
+J, K = AuxShardedJK(local).get_jk(inp.C, inp.occ)
+Jo, Ko = oracle.get_jk_inputs(inp)
+assert np.abs(J.numpy() - Jo).max() <= 1e-13 * np.abs(Jo).max()
+assert np.abs(K.numpy() - Ko).max() <= 1e-13 * np.abs(Ko).max()
+Jn, Kn = AuxShardedJK(lambda: (None, torch.from_numpy(oracle.get_jk(inp.B_packed[lo:hi], inp.nao, inp.C, inp.occ)[1]))).get_jk()
+assert Jn is None and np.abs(Kn.numpy() - Ko).max() <= 1e-13 * np.abs(Ko).max()
+dist.destroy_process_group()
+print("rank %d ok" % rank)
+"""
+
+
+def test_aux_range_partitions_the_rows():
+    from paper_2505_03755_b200.sharded import aux_range
+    for naux, world in [(4000, 8), (17, 2), (5, 8), (0, 3), (4001, 4)]:
+        r = [aux_range(naux, k, world) for k in range(world)]
+        assert r[0][0] == 0 and r[-1][1] == naux
+        assert all(a[1] == b[0] for a, b in zip(r, r[1:]))
+        sizes = [b - a for a, b in r]
+        assert max(sizes) - min(sizes) <= 1
+
+
+def test_aux_sharded_partials_sum_to_the_full_result_gloo_world2():
+    """each rank's partial J, K over its aux slice, one sum all-reduce (gloo here, NCCL on GPUs)"""
+    res = _spawn([sys.executable, "-c", SHARD_WORKER, ROOT])
+    for rank, (rc, out, err) in enumerate(res):
+        assert rc == 0, (rank, err[-3000:])
+        assert f"rank {rank} ok" in out
