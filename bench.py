@@ -229,6 +229,7 @@ def main():
     ap.add_argument("--shard-aux", action="store_true",
                     help="with --gpus N > 1: shard the aux rows over the ranks and sum-all-reduce J, K (strong scaling) "
                          "instead of N independent replicas")
+    ap.add_argument("--no-small-calls", action="store_true", help="skip the small-call (CUDA graph) section")
     ap.add_argument("--no-ao2mo", action="store_true", help="skip the AO2MO (Eq. 18-21) section")
     ap.add_argument("--workspace-gib", type=float, default=0.0, help="dfjk_options.workspace_cap_bytes (0 = default)")
     args = ap.parse_args()
@@ -358,6 +359,39 @@ def main():
               "algorithmic_flops": ao_flops, "tflops": ao_flops / (ms_ao * 1e-3) * 1e-12,
               "frac_of_fp64_peak": ao_flops / (ms_ao * 1e-3) * 1e-12 / FP64_DMMA_PEAK_TFLOPS,
               "flops_note": "Eq. 18 + Eq. 19 (full square) + Eq. 20 + Eq. 21 as printed, no symmetry discount"}
+    # ---- the many-small-calls regime of the embedded fragments:
+    # the `small` config called directly and as a replayed CUDA graph (dfjk_get_jk only enqueues)
+    small = None
+    if not args.no_small_calls:
+        sinp = dfjk_inputs.make_config("small")
+        sB = torch.from_numpy(sinp.B_packed).cuda()
+        sC = torch.from_numpy(sinp.C_concat()).cuda()
+        socc = torch.from_numpy(sinp.occ_concat()).cuda()
+        sJ = torch.empty((sinp.nset, sinp.nao, sinp.nao), dtype=torch.float64, device="cuda")
+        sK = torch.empty_like(sJ)
+        hs = dfjk.DFJK(sB, sinp.nao)
+        s_fn = lambda: hs.get_jk_raw(sinp.nocc, sC, socc, out_j=sJ, out_k=sK, stream=stream)
+        for _ in range(3):
+            s_fn()
+        torch.cuda.synchronize()
+        s_launches = hs.last_launch_count
+        ms_direct = max_over_ranks(timed(s_fn, 50))
+        cap = torch.cuda.Stream()
+        cap.wait_stream(stream)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(cap):
+            with torch.cuda.graph(graph, stream=cap):
+                hs.get_jk_raw(sinp.nocc, sC, socc, out_j=sJ, out_k=sK, stream=cap)
+        stream.wait_stream(cap)
+        graph.replay()
+        torch.cuda.synchronize()
+        ms_graph = max_over_ranks(timed(graph.replay, 50))
+        sfb = flops_bytes(dfjk_inputs.CONFIGS["small"])
+        small = {"workload": "small (nao=300, naux=1000, nocc=80), L2-warm", "launches_per_call": s_launches,
+                 "ms_direct": ms_direct, "ms_cuda_graph": ms_graph,
+                 "k_tflops_graph": sfb["k"] / (ms_graph * 1e-3) * 1e-12}
+        del graph
+        hs.close()
     if not lead:
         h.close()
         ranks.close()
@@ -408,6 +442,8 @@ def main():
         "phases_ms_per_step": {p: v[0] / args.steps for p, v in phases.items()},
     }
 
+    if small is not None:
+        line["small_calls"] = small
     if ao is not None:
         line["ao2mo"] = ao
         if Bh is not None and not args.no_parity:

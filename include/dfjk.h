@@ -84,8 +84,9 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
  *   stream   all work is enqueued on this stream.
  * Outputs are overwritten (not accumulated), full squares, both triangles, bitwise symmetric, raw
  * J[D_s], K[D_s] (no factor 1/2, no subtraction: Eq. 13 is the caller's).  The call only
- * enqueues: it never allocates and never synchronises the host.  Results are deterministic
- * (bitwise equal from run to run for equal inputs and options).
+ * enqueues: it never allocates and never synchronises the host (so it may be captured into a
+ * CUDA graph and replayed).  Results are deterministic (bitwise equal from run to run for equal
+ * inputs and options).
  */
 int dfjk_get_jk(dfjk_handle h, int nset, const int* nocc, const double* C, const double* occ,
                 double* J_out, double* K_out, dfjk_stream stream);

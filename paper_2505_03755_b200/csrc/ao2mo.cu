@@ -23,9 +23,15 @@ struct GemmTN {
   long long lda, ldb, ldc;                // row strides (doubles) of the k-major operands and of C
   long long sA, sB, sC;                   // batch strides (blockIdx.z)
   int accumulate;                         // 0: C = A^T B, 1: C += A^T B (one CTA owns each C tile)
+  // grouped M index of A (0 = plain): column m of A lives at (m / a_group) * a_gstride + k * lda +
+  // m % a_group -- the aux rows of a block stacked along M (Eq. 19 for the whole block as ONE
+  // GEMM of nb * nmo rows, so that only the N dimension pays tile padding)
+  int a_group = 0;
+  long long a_gstride = 0;
 };
 
-// CTA tile (16 WTM) x (32 WTN); consumers 2 (M) x 4 (N), warp tile WTM x WTN MMA tiles.
+// CTA tile (16 WTM) x (32 WTN); consumers 2 (M) x 4 (N), warp tile WTM x WTN MMA tiles (WTM = 4 in
+// the product: 64 x up to 352).
 // Shared-memory tiles are k-major, [16][TM + 4] and [16][TN + 4]: the row stride is 4 mod 16
 // doubles, so the fragment reads tile[k = l%4][row = l/4] hit 16 distinct banks per half-warp.
 // Producers gather with 8-byte cp.async (any alignment, zero-fill past M, N, K).
@@ -66,7 +72,15 @@ k_gemm_tn(const __grid_constant__ GemmTN g) {
       for (int e = tp; e < kGKC * TM; e += 128) {
         const int k = e / TM, m = e - k * TM;
         const bool ok = (k0 + k < g.K) && (m0 + m < g.M);
-        cp_async8(sa + (uint32_t)(k * LA + m) * 8u, A + (ok ? (size_t)(k0 + k) * g.lda + m0 + m : 0), ok);
+        size_t off = 0;
+        if (ok) {
+          off = (size_t)(k0 + k) * g.lda + m0 + m;
+          if (g.a_group > 0) {
+            const int grp = (m0 + m) / g.a_group;
+            off = (size_t)grp * g.a_gstride + (size_t)(k0 + k) * g.lda + (m0 + m - grp * g.a_group);
+          }
+        }
+        cp_async8(sa + (uint32_t)(k * LA + m) * 8u, A + off, ok);
       }
 #pragma unroll 4
       for (int e = tp; e < kGKC * TN; e += 128) {
@@ -147,11 +161,19 @@ static cudaError_t launch_gemm_tn(const GemmTN& g, int batch, cudaStream_t st) {
   return cudaSuccess;
 }
 
-// N tile 128, 64 or 32 columns by the width of the problem
+// CTA tile 64 x (32 WTN): the N tile is fitted to the problem (at most 352 columns per tile, the
+// fewest tiles that cover N, then the narrowest WTN that does), so that e.g. N = 340 pays 352.
 static cudaError_t gemm_tn(const GemmTN& g, int batch, cudaStream_t st) {
-  if (g.N > 64) return launch_gemm_tn<8, 4>(g, batch, st);
-  if (g.N > 32) return launch_gemm_tn<8, 2>(g, batch, st);
-  return launch_gemm_tn<8, 1>(g, batch, st);
+  const int n8 = cdiv(g.N > 0 ? g.N : 1, 8);
+  const int ntn = cdiv(n8, 44), wtn = cdiv(n8, 4 * ntn);
+  switch (wtn) {
+#define DFJK_GEMM_CASE(N) \
+  case N: return launch_gemm_tn<4, N>(g, batch, st);
+    DFJK_GEMM_CASE(1) DFJK_GEMM_CASE(2) DFJK_GEMM_CASE(3) DFJK_GEMM_CASE(4) DFJK_GEMM_CASE(5) DFJK_GEMM_CASE(6)
+    DFJK_GEMM_CASE(7) DFJK_GEMM_CASE(8) DFJK_GEMM_CASE(9) DFJK_GEMM_CASE(10) DFJK_GEMM_CASE(11)
+#undef DFJK_GEMM_CASE
+    default: return cudaErrorInvalidValue;
+  }
 }
 
 // bpa[P][p][a] = bmo[P][p][a0 + a]  (pulled back by the caller) and
@@ -194,6 +216,7 @@ int launch_ao2mo(dfjk_ctx* h, int nmo, int a0, int nact, const double* M, double
   if (h->nblk_forced > 0 && nblk > h->nblk_forced) nblk = h->nblk_forced;
   if (nblk > naux) nblk = naux;
   if (nblk > 32768) nblk = 32768;
+  if (nmo > 0 && nblk > (1LL << 30) / nmo) nblk = (1LL << 30) / nmo;   // nb * nmo is an int in Eq. 19
   if (nblk < 1) return -2;                                    // workspace too small for one aux row
   double* Xb = h->X;
   double* bmo = Xb + (size_t)nblk * nao * ldx;
@@ -202,8 +225,9 @@ int launch_ao2mo(dfjk_ctx* h, int nmo, int a0, int nact, const double* M, double
     const int nb = (int)(naux - p0 < nblk ? naux - p0 : nblk);
     if (launch_half_transform_rowmajor(h, si, p0, nb, Xb, ldx, st) != 0) return -1;      // Eq. 18
     launches++;
-    GemmTN g19{Xb, M, bmo, nmo, nmo, nao, ldx, nmo, nmo, (long long)nao * ldx, 0, (long long)n2, 0};
-    if (gemm_tn(g19, nb, st) != cudaSuccess) return -1;                                   // Eq. 19
+    // Eq. 19 for the whole block as one GEMM: rows (P, p1) stacked along M, bmo[P][p1][p2] = C[(P p1)][p2]
+    GemmTN g19{Xb, M, bmo, nb * nmo, nmo, nao, ldx, nmo, nmo, 0, 0, 0, 0, nmo, (long long)nao * ldx};
+    if (gemm_tn(g19, 1, st) != cudaSuccess) return -1;
     launches++;
     if (nact > 0) {
       dim3 gg(cdiv((int)(npa + naa), 256) < 64 ? cdiv((int)(npa + naa), 256) : 64, nb);
