@@ -63,30 +63,50 @@ k_gemm_tn(const __grid_constant__ GemmTN g) {
     // ===================== producer warpgroup =====================
     reg_dec<kProducerRegs>();
     const int tp = tid - 256;
+    // a thread keeps its columns for the whole kernel: one column m of the A tile (k rows tp / TM,
+    // + 128 / TM, ...) and the columns tp, tp + 128, ... of the B tile; only k moves per chunk
+    static_assert(128 % TM == 0 || TM % 128 == 0, "A tile width must divide or be a multiple of 128");
+    constexpr int kAColsPerThread = TM > 128 ? TM / 128 : 1, kAKStep = TM > 128 ? 1 : 128 / TM;
+    constexpr int kBColsPerThread = (TN + 127) / 128;
+    size_t a_off[kAColsPerThread];
+    bool a_ok[kAColsPerThread];
+    const int a_k0 = TM > 128 ? 0 : tp / TM;
+#pragma unroll
+    for (int q = 0; q < kAColsPerThread; q++) {
+      const int m = (TM > 128 ? tp + 128 * q : tp % TM), mg = m0 + m;
+      a_ok[q] = mg < g.M;
+      a_off[q] = mg;
+      if (g.a_group > 0) {
+        const int grp = mg / g.a_group;
+        a_off[q] = (size_t)grp * g.a_gstride + (mg - grp * g.a_group);
+      }
+    }
     for (int c = 0; c < nchunks; c++) {
       const int stage = c % kGStages;
       mbar_wait(empty0 + 8 * stage, ((c / kGStages) & 1) ^ 1);
       const uint32_t sa = smem_u32(smem + stage * kStageDoubles), sb = sa + kGKC * LA * 8;
       const int k0 = c * kGKC;
+#pragma unroll
+      for (int q = 0; q < kAColsPerThread; q++) {
+        const int m = (TM > 128 ? tp + 128 * q : tp % TM);
+#pragma unroll
+        for (int k = a_k0; k < kGKC; k += kAKStep) {
+          const bool ok = a_ok[q] && (k0 + k < g.K);
+          cp_async8(sa + (uint32_t)(k * LA + m) * 8u, A + (ok ? a_off[q] + (size_t)(k0 + k) * g.lda : 0), ok);
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < kBColsPerThread; q++) {
+        const int n = tp + 128 * q;
+        if (n < TN) {
+          const bool okn = n0 + n < g.N;
+          const double* bp = B + (okn ? (size_t)(n0 + n) : 0);
 #pragma unroll 4
-      for (int e = tp; e < kGKC * TM; e += 128) {
-        const int k = e / TM, m = e - k * TM;
-        const bool ok = (k0 + k < g.K) && (m0 + m < g.M);
-        size_t off = 0;
-        if (ok) {
-          off = (size_t)(k0 + k) * g.lda + m0 + m;
-          if (g.a_group > 0) {
-            const int grp = (m0 + m) / g.a_group;
-            off = (size_t)grp * g.a_gstride + (size_t)(k0 + k) * g.lda + (m0 + m - grp * g.a_group);
+          for (int k = 0; k < kGKC; k++) {
+            const bool ok = okn && (k0 + k < g.K);
+            cp_async8(sb + (uint32_t)(k * LB + n) * 8u, bp + (ok ? (size_t)(k0 + k) * g.ldb : 0), ok);
           }
         }
-        cp_async8(sa + (uint32_t)(k * LA + m) * 8u, A + off, ok);
-      }
-#pragma unroll 4
-      for (int e = tp; e < kGKC * TN; e += 128) {
-        const int k = e / TN, n = e - k * TN;
-        const bool ok = (k0 + k < g.K) && (n0 + n < g.N);
-        cp_async8(sb + (uint32_t)(k * LB + n) * 8u, B + (ok ? (size_t)(k0 + k) * g.ldb + n0 + n : 0), ok);
       }
       cp_async_mbar_arrive_noinc(full0 + 8 * stage);
     }

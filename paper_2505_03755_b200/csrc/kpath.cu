@@ -247,6 +247,43 @@ k_half_transform(const __grid_constant__ HtParams q) {
           if (col >= q.col0[s] && col < q.col0[s + 1]) myset = s;
       }
       __syncwarp();
+      // common case: every column tile of this warp belongs to the same set -> straight-line code,
+      // four independent partial sums, one reduction
+      const int set0 = __shfl_sync(0xffffffffu, myset, 0);
+      const bool one_set = set0 >= 0 && __all_sync(0xffffffffu, l >= WN || myset == set0);
+      if (one_set) {
+        double p4[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+        for (int u0 = 0; u0 < WN; u0 += 4) {
+          double cv[4][2][2];
+#pragma unroll
+          for (int uu = 0; uu < 4; uu++) {
+            if (u0 + uu >= WN) continue;
+            const int n = n0 + 8 * (wn * WN + u0 + uu) + 2 * j;
+#pragma unroll
+            for (int t = 0; t < 2; t++) {
+              const int mu = min(m0 + wm * 16 + 8 * t + r, nao - 1);     // rows past nao hold acc = 0
+              const double* cp = q.Ct + ((size_t)(mu >> 4) * q.ct_rows + n) * kHtLd + (mu & 15);
+              cv[uu][t][0] = __ldg(cp);
+              cv[uu][t][1] = __ldg(cp + kHtLd);
+            }
+          }
+#pragma unroll
+          for (int uu = 0; uu < 4; uu++) {
+            if (u0 + uu >= WN) continue;
+#pragma unroll
+            for (int t = 0; t < 2; t++) {
+              p4[2 * t] = fma(acc[t][u0 + uu][0], cv[uu][t][0], p4[2 * t]);
+              p4[2 * t + 1] = fma(acc[t][u0 + uu][1], cv[uu][t][1], p4[2 * t + 1]);
+            }
+          }
+        }
+        double v = (p4[0] + p4[1]) + (p4[2] + p4[3]);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (l == 0) slot[set0] = v;
+        continue;
+      }
       double cur = 0.0;
       int cur_s = -1;
       auto flush = [&]() {
