@@ -101,13 +101,7 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   h->naux = naux; h->nao = nao; h->device = dev;
   h->num_sms = prop.multiProcessorCount;
   h->ht_grid = h->num_sms;
-  h->ht_skew = 1;
   h->two_pass_j = o.two_pass_j;
-  if (const char* e = getenv("DFJK_HT_SKEW")) h->ht_skew = atoi(e) != 0;   // tuning only
-  if (const char* e = getenv("DFJK_J1_LEGACY")) h->j1_legacy = atoi(e) != 0;
-  if (const char* e = getenv("DFJK_SYRK_LEGACY")) h->syrk_legacy = atoi(e) != 0;
-  if (const char* e = getenv("DFJK_SYRK_WM")) h->syrk_wm_forced = atoi(e);
-  if (const char* e = getenv("DFJK_HT_GRID")) { const int g = atoi(e); if (g > 0) h->ht_grid = g; }
   h->npair = (size_t)nao * (nao + 1) / 2;
   h->nck = cdiv(nao, kHtBK);
   h->mu_pad = round_up(nao, 8) + 128;   // any SYRK tile of <= 128 rows stays inside the tiled X

@@ -49,9 +49,7 @@ struct dfjk_ctx {
   int n_mtiles;              // 128-row tiles along nao
   int j1_chunks, j2_splits;
   int num_sms;
-  int ht_grid, ht_skew;      // persistent half-transform: CTAs (= SMs), skewed warp pairs on/off
-  int syrk_legacy, syrk_wm_forced;   // tuning only (env): wide/narrow-warp SYRK, forced tile size
-  int j1_legacy;             // tuning only (env): DMMA J pass 1 instead of the bulk-copy pipeline
+  int ht_grid;               // persistent half-transform: CTAs (= SMs)
   int two_pass_j;            // option: never fuse J pass 1 into the half-transform
   // scratch (all allocated at create)
   double* Ct;                // [nck][ct_rows][20]  C' transposed and k-tiled, sqrt(occ) folded, zero padded

@@ -2,10 +2,10 @@
 //   pass 1  rho[s][P]  = sum_pair B[P][pair] Dw_s[pair]        (one stream over packed B)
 //   pass 2  Jp_s[pair] = sum_P rho[s][P] B[P][pair]            (second stream over packed B)
 //   epilogue: fixed-order sum of the P-split partials and unpack to the full symmetric square.
-// Pass 1 is a (64 aux rows) x (<=8 sets) x (pairs) contraction per warp on DMMA.8x8x4: the
-// row x set accumulators fall out of the MMA fragments, so no per-row shuffle reduction exists,
-// and one Dw fragment is reused against 8 row groups (Dw traffic from L2 = 1/8 of the B stream).
-// The k index of an MMA is free to permute, so each lane reads 16 contiguous bytes (LDG.128).
+// Pass 1 is a bulk-copy (TMA engine) pipeline when npair is even (k_j1_tma); for odd npair, where
+// packed rows are only 8-byte aligned, k_j1 streams with plain loads: a (64 aux rows) x (<=8 sets)
+// x (pairs) contraction per warp on DMMA.8x8x4, whose row x set accumulators fall out of the MMA
+// fragments (no per-row shuffle reduction; one Dw fragment serves 8 row groups).
 #include "common.cuh"
 #include "ctx.h"
 #include "pipeline.cuh"
@@ -86,93 +86,6 @@ k_j1(const double* __restrict__ B, size_t npair, int naux, const double* __restr
     }
   }
   // fixed-order combine of the 8 warps, one partial per CTA
-#pragma unroll
-  for (int g = 0; g < 8; g++) {
-    red[w][8 * g + r][2 * j] = acc[g][0];
-    red[w][8 * g + r][2 * j + 1] = acc[g][1];
-  }
-  __syncthreads();
-  for (int e = threadIdx.x; e < kJ1Rows * 8; e += kJ1Warps * 32) {
-    const int s = e / kJ1Rows, row = e % kJ1Rows;
-    double t = 0.0;
-#pragma unroll
-    for (int ww = 0; ww < kJ1Warps; ww++) t += red[ww][row][s];
-    part[((size_t)blockIdx.x * 8 + s) * naux_pad + p0 + row] = t;
-  }
-}
-
-// Same contraction with 256-bit loads (npair % 4 == 0): lane (r, j) reads 4 consecutive pairs of
-// each of its 8 rows per step, so a warp-wide load covers 8 rows x 128 contiguous bytes (whole
-// L1/L2 lines) and feeds 4 MMAs.  Steps of 16 pairs.
-__global__ void __launch_bounds__(kJ1Warps * 32, 1)
-k_j1_v4(const double* __restrict__ B, size_t npair, int naux, const double* __restrict__ Dw, int nsetg,
-        double* __restrict__ part, int naux_pad) {
-  __shared__ double red[kJ1Warps][kJ1Rows][8];
-  const int w = threadIdx.x >> 5, l = threadIdx.x & 31, r = l >> 2, j = l & 3;
-  const int p0 = blockIdx.y * kJ1Rows;
-  const size_t kbeg = (size_t)blockIdx.x * kJ1Chunk + (size_t)w * kJ1SubChunk;
-  size_t kend = kbeg + kJ1SubChunk;
-  if (kend > npair) kend = npair;
-
-  // row of group g = p0 + 8g + r; rows past naux re-read the lane's first row (or the last row
-  // of B) and land in accumulator rows nobody reads
-  int row0 = p0 + r;
-  if (row0 > naux - 1) row0 = naux - 1;
-  const double* bp = B + (size_t)row0 * npair + 4 * j;
-  const int gmax = (naux - 1 - row0) / 8;          // groups 0..gmax are real rows
-  const size_t s8 = 8 * npair;
-  const bool dw_on = r < nsetg;          // lane's column of the MMA B operand = set index r
-  const double* dwp = Dw + (size_t)(dw_on ? r : 0) * npair + 4 * j;
-
-  double acc[8][2];
-#pragma unroll
-  for (int g = 0; g < 8; g++) acc[g][0] = acc[g][1] = 0.0;
-
-  size_t kk = kbeg;
-  for (; kk + 32 <= kend; kk += 32) {   // two steps per iteration: 16 x 32 B in flight per lane
-    double4s b[2][8], d[2];
-#pragma unroll
-    for (int u = 0; u < 2; u++)
-#pragma unroll
-      for (int g = 0; g < 8; g++) b[u][g] = ldg_stream4(bp + (g <= gmax ? g * s8 : 0) + kk + 16 * u);
-#pragma unroll
-    for (int u = 0; u < 2; u++) {
-      d[u].x = d[u].y = d[u].z = d[u].w = 0.0;
-      if (dw_on) d[u] = ldg_cached4(dwp + kk + 16 * u);
-    }
-#pragma unroll
-    for (int u = 0; u < 2; u++)
-#pragma unroll
-      for (int g = 0; g < 8; g++) {
-        dmma884(acc[g][0], acc[g][1], b[u][g].x, d[u].x);
-        dmma884(acc[g][0], acc[g][1], b[u][g].y, d[u].y);
-        dmma884(acc[g][0], acc[g][1], b[u][g].z, d[u].z);
-        dmma884(acc[g][0], acc[g][1], b[u][g].w, d[u].w);
-      }
-  }
-  for (; kk + 16 <= kend; kk += 16) {
-    double4s b[8], d;
-#pragma unroll
-    for (int g = 0; g < 8; g++) b[g] = ldg_stream4(bp + (g <= gmax ? g * s8 : 0) + kk);
-    d.x = d.y = d.z = d.w = 0.0;
-    if (dw_on) d = ldg_cached4(dwp + kk);
-#pragma unroll
-    for (int g = 0; g < 8; g++) {
-      dmma884(acc[g][0], acc[g][1], b[g].x, d.x);
-      dmma884(acc[g][0], acc[g][1], b[g].y, d.y);
-      dmma884(acc[g][0], acc[g][1], b[g].z, d.z);
-      dmma884(acc[g][0], acc[g][1], b[g].w, d.w);
-    }
-  }
-  for (; kk < kend; kk += 4) {  // guarded tail: one pair per lane per step
-    const bool ok = kk + j < kend;
-    const double d = (dw_on && ok) ? dwp[kk - 3 * j] : 0.0;       // element kk + j of this set
-#pragma unroll
-    for (int g = 0; g < 8; g++) {
-      const double b = ok ? ldg_stream1(bp + (g <= gmax ? g * s8 : 0) + kk - 3 * j) : 0.0;
-      dmma884(acc[g][0], acc[g][1], b, d);
-    }
-  }
 #pragma unroll
   for (int g = 0; g < 8; g++) {
     red[w][8 * g + r][2 * j] = acc[g][0];
@@ -466,9 +379,7 @@ int launch_j_passes(dfjk_ctx* h, const SetInfo& si, double* J_out, bool rho_read
     if (naux > 0 && !rho_ready) {
       prof_mark(h, DFJK_PHASE_J1, st);
       dim3 g1(h->j1_chunks, naux_pad / kJ1Rows);
-      if (vec && !h->j1_legacy) dispatch_j1_tma(ns, g1, st, h->B, npair, naux, h->Dw + (size_t)s0 * npair, h->rho_part, naux_pad);
-      else if (npair % 4 == 0) k_j1_v4<<<g1, kJ1Warps * 32, 0, st>>>(h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad);
-      else if (vec) k_j1<true><<<g1, kJ1Warps * 32, 0, st>>>(h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad);
+      if (vec) dispatch_j1_tma(ns, g1, st, h->B, npair, naux, h->Dw + (size_t)s0 * npair, h->rho_part, naux_pad);
       else k_j1<false><<<g1, kJ1Warps * 32, 0, st>>>(h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad);
       dim3 gr(cdiv(naux, 128), ns);
       k_j1_reduce<<<gr, 128, 0, st>>>(h->rho_part, h->j1_chunks, naux_pad, naux, ns, h->rho + (size_t)s0 * naux);

@@ -44,7 +44,6 @@ struct HtParams {
   const double* Ct; int ct_rows; int nocc_pad;
   double* X; int nch; int mu_pad;       // EPI 0/1: k-tiled X for the SYRK
   int p_first, nb, ntm, ntn;            // aux rows [p_first, p_first + nb), 64-row blocks, N tiles
-  int skew;                             // 1: the second consumer warpgroup runs half a chunk behind
   double* rho_ht; int nset; int col0[kMaxSets + 1];   // EPI 1: per-warp partials of rho (step a2 fused)
   int ldx, xrows;                       // EPI 2: row-major X[(pl * xrows + mu) * ldx + n]
 };
@@ -60,9 +59,8 @@ k_half_transform(const __grid_constant__ HtParams q) {
   constexpr uint32_t kBBytes = NT * kHtLd * 8;
   double* sA = smem;                               // kStages x kHtATile
   double* sB = smem + kStages * kHtATile;          // kStages x NT*kHtLd
-  __shared__ __align__(8) unsigned long long bars[2 * kStages + 1];
+  __shared__ __align__(8) unsigned long long bars[2 * kStages];
   const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kStages]);
-  const uint32_t skewbar = smem_u32(&bars[2 * kStages]);
   const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
   const int nao = q.nao;
   const int nk4 = (nao + 3) >> 2;                  // k4 steps that carry data
@@ -74,7 +72,6 @@ k_half_transform(const __grid_constant__ HtParams q) {
       mbar_init(full0 + 8 * s, 128 + 1);   // 128 cp.async arrivals + the expect_tx arrival
       mbar_init(empty0 + 8 * s, 8);        // one arrival per consumer warp
     }
-    mbar_init(skewbar, 4);
     mbar_fence_init();
   }
   __syncthreads();
@@ -141,9 +138,6 @@ k_half_transform(const __grid_constant__ HtParams q) {
   const int r = l >> 2, j = l & 3;
   const int wm = w & 3, wn = w >> 2;
   double acc[2][WN][2];
-  // warps w and w+4 share an SM sub-partition: the second one starts half a chunk late, so the two
-  // never sit at a chunk boundary (barrier wait + first fragment loads) at the same time
-  if (q.skew && wn == 1) mbar_wait(skewbar, 0);
 
   int g = 0;
   for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
@@ -175,12 +169,6 @@ k_half_transform(const __grid_constant__ HtParams q) {
             for (int u = 0; u < WN; u++) {
               dmma884(acc[0][u][0], acc[0][u][1], a0, b[u]);
               dmma884(acc[1][u][0], acc[1][u][1], a1, b[u]);
-            }
-            // half of the very first chunk done (it is never a transposed one): release the late
-            // warpgroup
-            if (g == 0 && wn == 0 && kk == (ksteps > 1 ? 1 : 0)) {
-              __syncwarp();
-              if (l == 0) mbar_arrive(skewbar);
             }
           }
         }
@@ -829,9 +817,6 @@ static cudaError_t launch_syrk(int grid, cudaStream_t st, const SyrkArgs& a) {
 
 static cudaError_t dispatch_syrk(int wm, int grid, cudaStream_t st, const SyrkArgs& a) {
   switch (wm) {
-    case 4: return launch_syrk<4>(grid, st, a);
-    case 5: return launch_syrk<5>(grid, st, a);
-    case 6: return launch_syrk<6>(grid, st, a);
     case 7: return launch_syrk<7>(grid, st, a);
     case 8: return launch_syrk<8>(grid, st, a);
     default: return cudaErrorInvalidValue;
@@ -873,7 +858,7 @@ int launch_half_transform_rowmajor(dfjk_ctx* h, const SetInfo& si, int p_first, 
   HtParams a;
   a.Bp = h->B; a.npair = h->npair; a.nao = h->nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = si.nocc_pad;
   a.X = X; a.nch = 0; a.mu_pad = 0; a.p_first = p_first; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
-  a.skew = h->ht_skew; a.rho_ht = nullptr; a.nset = 0; a.ldx = ldx; a.xrows = h->nao;
+  a.rho_ht = nullptr; a.nset = 0; a.ldx = ldx; a.xrows = h->nao;
   a.col0[0] = 0;
   const long long ht_tiles = (long long)nb * ntm_ht * ntn;
   const int ht_grid = (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid);
@@ -942,8 +927,7 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
       if (area < best * 0.995) { best = area; wm_s = wmc; }
     }
   }
-  if (h->syrk_wm_forced >= 4 && h->syrk_wm_forced <= 8) wm_s = h->syrk_wm_forced;
-  const bool paired = wm_s <= 6 && !h->syrk_legacy;
+  const bool paired = wm_s <= 6;
   const double diag_cost = paired ? (wm_s + 1) / (2.0 * wm_s) : 1.0;
   const int ntm = cdiv(nao, 16 * wm_s), ntiles = ntm * (ntm + 1) / 2;
   int ksplit = h->ksplit_forced;
@@ -971,7 +955,7 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
     HtParams a;
     a.Bp = h->B; a.npair = h->npair; a.nao = nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = ldx;
     a.X = h->X; a.nch = nch; a.mu_pad = h->mu_pad; a.p_first = p0; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
-    a.skew = h->ht_skew; a.rho_ht = h->rho_ht; a.nset = si.nset; a.ldx = 0; a.xrows = 0;
+    a.rho_ht = h->rho_ht; a.nset = si.nset; a.ldx = 0; a.xrows = 0;
     for (int s = 0; s <= si.nset; s++) a.col0[s] = si.col0[s];
     const long long ht_tiles = (long long)nb * ntm_ht * ntn;
     const int ht_grid = (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid);
@@ -1105,7 +1089,7 @@ int launch_k_path_dm(dfjk_ctx* h, int nset, const double* D, double* K_out, cuda
       HtParams a;
       a.Bp = h->B; a.npair = h->npair; a.nao = nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = ldx;
       a.X = X1; a.nch = nch; a.mu_pad = h->mu_pad; a.p_first = p0; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
-      a.skew = h->ht_skew; a.rho_ht = nullptr; a.nset = 0; a.ldx = 0; a.xrows = 0; a.col0[0] = 0;
+      a.rho_ht = nullptr; a.nset = 0; a.ldx = 0; a.xrows = 0; a.col0[0] = 0;
       const long long ht_tiles = (long long)nb * ntm_ht * ntn;
       if (dispatch_ht(wn, 0, (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid), st, a) != cudaSuccess) return -1;
       dim3 gu(nch, nb);
