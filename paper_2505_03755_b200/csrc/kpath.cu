@@ -45,11 +45,6 @@ struct HtParams {
   double* X; int nch; int mu_pad;       // EPI 0/1: k-tiled X for the SYRK
   int p_first, nb, ntm, ntn;            // aux rows [p_first, p_first + nb), 64-row blocks, N tiles
   double* rho_ht; int nset; int col0[kMaxSets + 1];   // EPI 1: per-warp partials of rho (step a2 fused)
-  // EPI 0/1, aux-packed sets: a set of pk_w[s] = 8 or 16 padded columns does not use the column
-  // chunks; 32 / pk_w[s] consecutive aux rows share one 32-column chunk of its own region at
-  // X + pk_off[s], so that the SYRK of a small set (the rank-8 fragment densities of LASSCF) still
-  // reads fully used chunks
-  int npacked; int pk_w[kMaxSets]; long long pk_off[kMaxSets];
   int ldx, xrows;                       // EPI 2: row-major X[(pl * xrows + mu) * ldx + n]
 };
 
@@ -209,31 +204,6 @@ k_half_transform(const __grid_constant__ HtParams q) {
           const int n = n0 + 8 * (wn * WN + u) + 2 * j;
           if (n < q.nocc_pad)
             *reinterpret_cast<double2*>(Xp + (size_t)mu * q.ldx + n) = make_double2(acc[t][u][0], acc[t][u][1]);
-        }
-      }
-    } else if (q.npacked > 0) {
-      // lane u < WN works out where column tile u of this warp goes (offset of its row 0, column 0)
-      long long toff = -1;
-      if (l < WN) {
-        const int col = n0 + 8 * (wn * WN + l);
-        if (col < q.nocc_pad) {
-          toff = (long long)(((size_t)pl * q.nch + (col >> 5)) * q.mu_pad * kLdT + (col & 31));
-          for (int s = 0; s < q.nset; s++)
-            if (q.pk_w[s] > 0 && col >= q.col0[s] && col < q.col0[s + 1]) {
-              const int G = 32 / q.pk_w[s];
-              toff = q.pk_off[s] + (long long)((size_t)(pl / G) * q.mu_pad * kLdT + (pl % G) * q.pk_w[s] + (col - q.col0[s]));
-            }
-        }
-      }
-#pragma unroll
-      for (int u = 0; u < WN; u++) {
-        const long long off = __shfl_sync(0xffffffffu, toff, u);
-        if (off < 0) continue;
-#pragma unroll
-        for (int t = 0; t < 2; t++) {
-          const int mu = m0 + wm * 16 + 8 * t + r;
-          if (mu < nao)
-            *reinterpret_cast<double2*>(q.X + off + (size_t)mu * kLdT + 2 * j) = make_double2(acc[t][u][0], acc[t][u][1]);
         }
       }
     } else {
@@ -888,54 +858,31 @@ int launch_half_transform_rowmajor(dfjk_ctx* h, const SetInfo& si, int p_first, 
   HtParams a;
   a.Bp = h->B; a.npair = h->npair; a.nao = h->nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = si.nocc_pad;
   a.X = X; a.nch = 0; a.mu_pad = 0; a.p_first = p_first; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
-  a.rho_ht = nullptr; a.nset = 0; a.npacked = 0; a.ldx = ldx; a.xrows = h->nao;
+  a.rho_ht = nullptr; a.nset = 0; a.ldx = ldx; a.xrows = h->nao;
   a.col0[0] = 0;
   const long long ht_tiles = (long long)nb * ntm_ht * ntn;
   const int ht_grid = (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid);
   return dispatch_ht(wn, 2, ht_grid, st, a) == cudaSuccess ? 0 : -1;
 }
 
-// Modelled SYRK time of one aux block: greedy list schedule of the CTAs in launch order (the
-// off-diagonal ones of cost c_off first, then the cheaper diagonal ones of cost c_diag) on `sms`
-// SMs, one CTA per SM.
-static double syrk_makespan(int n_off, int n_diag, double c_off, double c_diag, int ksplit, int sms) {
+// Modelled SYRK time of one aux block in units of one off-diagonal CTA's aux row: greedy list
+// schedule of the CTAs in launch order (off-diagonal first, then the cheaper diagonal ones) on
+// `sms` SMs, one CTA per SM.
+static double syrk_makespan(int n_off, int n_diag, double diag_cost, int ksplit, int rps, int sms) {
   const long long total = (long long)(n_off + n_diag) * ksplit;
-  const double work = ((double)n_off * c_off + (double)n_diag * c_diag) * ksplit;
-  if (total <= sms) return n_off ? c_off : c_diag;
-  if (total > 8192) return work / sms + c_off;
+  const double work = ((double)n_off + diag_cost * n_diag) * ksplit * rps;
+  if (total > 8192 || total <= sms) return total <= sms ? (double)rps * (n_off ? 1.0 : diag_cost) : work / sms + rps;
   std::priority_queue<double, std::vector<double>, std::greater<double>> free_at;
   for (int i = 0; i < sms; i++) free_at.push(0.0);
   double end = 0.0;
   for (long long i = 0; i < total; i++) {
-    const double t = free_at.top() + (i < (long long)n_off * ksplit ? c_off : c_diag);
+    const double c = (i < (long long)n_off * ksplit ? 1.0 : diag_cost) * rps;
+    const double t = free_at.top() + c;
     free_at.pop();
     free_at.push(t);
     if (t > end) end = t;
   }
   return end;
-}
-
-// Split-K factor of one set's SYRK: `nrows` reduction rows per block (aux rows, or groups of
-// aux rows for an aux-packed set), each `chunks_per_row` 32-column chunks long.  A CTA costs its
-// rows plus a fixed overhead (launch, pipeline fill, partial-sum exchange, read-modify-write of
-// its partial tile: ~7 us, i.e. ~14000 cycles against 128 wm^2 DMMA cycles per chunk), which is
-// what keeps the many cheap CTAs of a rank-8 set from being split as finely as a 300-column set.
-static int choose_ksplit(const dfjk_ctx* h, int nrows, double chunks_per_row, int ntiles, int ntm, int wm,
-                         double diag_cost) {
-  int cap = h->ksplit < nrows ? h->ksplit : nrows;
-  if (cap < 1) cap = 1;
-  if (h->ksplit_forced > 0) return h->ksplit_forced < cap ? h->ksplit_forced : cap;
-  const double overhead_rows = 14000.0 / (128.0 * wm * wm * (chunks_per_row > 0.125 ? chunks_per_row : 0.125));
-  double best = 1e300;
-  int ksplit = 1;
-  for (int k = 1; k <= cap; k++) {
-    const int rps = cdiv(nrows, k);
-    if (cdiv(nrows, rps) != k) continue;                         // splits that actually get rows
-    const double t = syrk_makespan(ntiles - ntm, ntm, rps + overhead_rows, diag_cost * rps + overhead_rows, k,
-                                   h->num_sms);
-    if (t < best * 0.999) { best = t; ksplit = k; }              // fewer splits on ties
-  }
-  return ksplit;
 }
 
 // Aux-block scheduler: cap the X workspace, pick the split-K factor, enqueue
@@ -959,46 +906,12 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
 
   // plan: aux block size from the workspace, N tiling of the half-transform, split-K of the SYRK
   const int nch = cdiv(ldx, kBK);
-  const size_t chunk_doubles = (size_t)h->mu_pad * kLdT;
-  const size_t row_doubles = (size_t)nch * chunk_doubles;        // tiled X, one aux row
+  const size_t row_doubles = (size_t)nch * h->mu_pad * kLdT;     // tiled X, one aux row
   long long nblk = (long long)(h->X_doubles / row_doubles);
   if (h->nblk_forced > 0 && nblk > h->nblk_forced) nblk = h->nblk_forced;
   if (nblk > naux) nblk = naux;
   if (nblk > 32768) nblk = 32768;
   if (nblk < 1) nblk = 1;
-  // aux-packed storage for sets of 8 or 16 padded columns (see HtParams): G = 32 / w aux rows per
-  // chunk.  Used when the regions fit next to the column chunks without halving the block.
-  int pk_w[kMaxSets], npacked = 0;
-  long long pk_off[kMaxSets];
-  for (int s = 0; s < si.nset; s++) {
-    const int w = si.col0[s + 1] - si.col0[s];
-    pk_w[s] = (w == 8 || w == 16) ? w : 0;
-    pk_off[s] = -1;
-    npacked += pk_w[s] > 0;
-  }
-  if (npacked > 0) {
-    auto need = [&](long long nb_) {
-      size_t t = (size_t)nb_ * row_doubles;
-      for (int s = 0; s < si.nset; s++)
-        if (pk_w[s]) t += (size_t)cdiv((int)nb_, 32 / pk_w[s]) * chunk_doubles;
-      return t;
-    };
-    long long nb_p = nblk;
-    while (nb_p > 1 && need(nb_p) > h->X_doubles) nb_p -= (nb_p > 64 ? nb_p / 64 : 1);
-    if (nb_p >= 4) nb_p -= nb_p % 4;           // whole groups except in the last block
-    if (need(nb_p) <= h->X_doubles && 2 * nb_p >= nblk) {
-      nblk = nb_p;
-      size_t off = (size_t)nblk * row_doubles;
-      for (int s = 0; s < si.nset; s++)
-        if (pk_w[s]) {
-          pk_off[s] = (long long)off;
-          off += (size_t)cdiv((int)nblk, 32 / pk_w[s]) * chunk_doubles;
-        }
-    } else {
-      npacked = 0;
-      for (int s = 0; s < si.nset; s++) pk_w[s] = 0;
-    }
-  }
   const int n8 = ldx / 8;
   const int ntn = cdiv(n8, 2 * kHtMaxWN), wn = cdiv(n8, 2 * ntn);  // N tile = 16*wn columns
   const int ntm_ht = cdiv(nao, 64);
@@ -1017,16 +930,22 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
   const bool paired = wm_s <= 6;
   const double diag_cost = paired ? (wm_s + 1) / (2.0 * wm_s) : 1.0;
   const int ntm = cdiv(nao, 16 * wm_s), ntiles = ntm * (ntm + 1) / 2;
-  // per set: reduction rows per block and the split-K factor (the same for every block, since the
-  // split-K partials accumulate across blocks)
-  int ks[kMaxSets];
-  for (int s = 0; s < si.nset; s++) {
-    const int w = si.col0[s + 1] - si.col0[s];
-    ks[s] = 1;
-    if (w == 0) continue;
-    if (pk_w[s]) ks[s] = choose_ksplit(h, cdiv((int)nblk, 32 / pk_w[s]), 1.0, ntiles, ntm, wm_s, diag_cost);
-    else ks[s] = choose_ksplit(h, (int)nblk, round_up(si.nocc[s], 4) / 32.0, ntiles, ntm, wm_s, diag_cost);
+  int ksplit = h->ksplit_forced;
+  if (ksplit <= 0) {
+    // one SYRK CTA per SM; pick the split with the shortest modelled makespan, fewer splits on ties
+    const int nb0 = (int)nblk;
+    double best = 1e300;
+    ksplit = 1;
+    for (int k = 1; k <= h->ksplit && k <= nb0; k++) {
+      const int rps = cdiv(nb0, k), kk = cdiv(nb0, rps);          // splits that actually get rows
+      if (kk != k) continue;
+      const double t = syrk_makespan(ntiles - ntm, ntm, diag_cost, k, rps, h->num_sms) * (1.0 + 0.002 * k);
+      if (t < best) { best = t; ksplit = k; }
+    }
   }
+  if (ksplit > h->ksplit) ksplit = h->ksplit;
+  if (ksplit > nblk) ksplit = (int)nblk;
+  if (ksplit < 1) ksplit = 1;
   const size_t split_stride = (size_t)h->max_nset * n2;
 
   int nblocks = 0;
@@ -1038,32 +957,18 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
     a.X = h->X; a.nch = nch; a.mu_pad = h->mu_pad; a.p_first = p0; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
     a.rho_ht = h->rho_ht; a.nset = si.nset; a.ldx = 0; a.xrows = 0;
     for (int s = 0; s <= si.nset; s++) a.col0[s] = si.col0[s];
-    a.npacked = npacked;
-    for (int s = 0; s < si.nset; s++) {
-      a.pk_w[s] = pk_w[s];
-      a.pk_off[s] = pk_off[s];
-      // the last group of a packed set is only partly written when nb is not a multiple of G
-      if (pk_w[s] && nb % (32 / pk_w[s]) != 0) {
-        k_zero<<<32, 256, 0, st>>>(h->X + pk_off[s] + (size_t)(nb / (32 / pk_w[s])) * chunk_doubles, chunk_doubles);
-        launches++;
-      }
-    }
     const long long ht_tiles = (long long)nb * ntm_ht * ntn;
     const int ht_grid = (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid);
     if (dispatch_ht(wn, want_rho ? 1 : 0, ht_grid, st, a) != cudaSuccess) return -1;
     launches++;
+    const int rps = cdiv(nb, ksplit);
     prof_mark(h, DFJK_PHASE_SYRK, st);
     for (int s = 0; s < si.nset; s++) {
       if (si.col0[s + 1] == si.col0[s]) continue;
       // columns past nocc[s] (padding to the 8-column MMA tile) are zero: stop at the k4 step
-      SyrkArgs sa{h->X, nao, nch, h->mu_pad, si.col0[s], si.col0[s] + round_up(si.nocc[s], 4), nb,
-                  cdiv(nb, ks[s]), ntm, h->Kpart + n2 * s, split_stride, p0 == 0 ? 1 : 0};
-      if (pk_w[s]) {                         // aux-packed: one full chunk per group of G aux rows
-        const int G = 32 / pk_w[s];
-        sa.X = h->X + pk_off[s]; sa.nch = 1; sa.c0 = 0; sa.c1 = 32;
-        sa.nrows_blk = cdiv(nb, G); sa.rows_per_split = cdiv(sa.nrows_blk, ks[s]);
-      }
-      const cudaError_t e = paired ? dispatch_syrk2(wm_s, ks[s], st, sa) : dispatch_syrk(wm_s, ntiles * ks[s], st, sa);
+      SyrkArgs sa{h->X, nao, nch, h->mu_pad, si.col0[s], si.col0[s] + round_up(si.nocc[s], 4), nb, rps, ntm,
+                  h->Kpart + n2 * s, split_stride, p0 == 0 ? 1 : 0};
+      const cudaError_t e = paired ? dispatch_syrk2(wm_s, ksplit, st, sa) : dispatch_syrk(wm_s, ntiles * ksplit, st, sa);
       if (e != cudaSuccess) return -1;
       launches++;
     }
@@ -1072,7 +977,7 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
   for (int s = 0; s < si.nset; s++) {
     if (si.col0[s + 1] == si.col0[s]) continue;
     dim3 ge(nb32, nb32, 1), be(32, 8);
-    k_k_epilogue<<<ge, be, 0, st>>>(h->Kpart + n2 * s, ks[s], split_stride, nao, K_out + n2 * s);
+    k_k_epilogue<<<ge, be, 0, st>>>(h->Kpart + n2 * s, ksplit, split_stride, nao, K_out + n2 * s);
     launches++;
   }
   if (want_rho) {
@@ -1082,9 +987,7 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
     launches++;
   }
   h->plan_nblk = (int)nblk;
-  h->plan_ksplit = 1;
-  for (int s = si.nset - 1; s >= 0; s--)
-    if (si.col0[s + 1] > si.col0[s]) h->plan_ksplit = ks[s];    // the first non-empty set's
+  h->plan_ksplit = ksplit;
   h->plan_nblocks = nblocks;
   return launches;
 }
@@ -1162,7 +1065,19 @@ int launch_k_path_dm(dfjk_ctx* h, int nset, const double* D, double* K_out, cuda
   }
   const double diag_cost = (wm_s + 1) / (2.0 * wm_s);
   const int ntm = cdiv(nao, 16 * wm_s), ntiles = ntm * (ntm + 1) / 2;
-  const int ksplit = choose_ksplit(h, (int)nblk, round_up(nao, 4) / 32.0, ntiles, ntm, wm_s, diag_cost);
+  int ksplit = h->ksplit_forced;
+  if (ksplit <= 0) {
+    double best = 1e300;
+    ksplit = 1;
+    for (int k = 1; k <= h->ksplit && k <= nblk; k++) {
+      const int rps = cdiv((int)nblk, k);
+      if (cdiv((int)nblk, rps) != k) continue;
+      const double t = syrk_makespan(ntiles - ntm, ntm, diag_cost, k, rps, h->num_sms) * (1.0 + 0.002 * k);
+      if (t < best) { best = t; ksplit = k; }
+    }
+  }
+  if (ksplit > h->ksplit) ksplit = h->ksplit;
+  if (ksplit > nblk) ksplit = (int)nblk;
   const size_t split_stride = (size_t)h->max_nset * n2;
   const int nb32 = cdiv(nao, 32);
   for (int s = 0; s < nset; s++) {
@@ -1174,7 +1089,7 @@ int launch_k_path_dm(dfjk_ctx* h, int nset, const double* D, double* K_out, cuda
       HtParams a;
       a.Bp = h->B; a.npair = h->npair; a.nao = nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = ldx;
       a.X = X1; a.nch = nch; a.mu_pad = h->mu_pad; a.p_first = p0; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
-      a.rho_ht = nullptr; a.nset = 0; a.npacked = 0; a.ldx = 0; a.xrows = 0; a.col0[0] = 0;
+      a.rho_ht = nullptr; a.nset = 0; a.ldx = 0; a.xrows = 0; a.col0[0] = 0;
       const long long ht_tiles = (long long)nb * ntm_ht * ntn;
       if (dispatch_ht(wn, 0, (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid), st, a) != cudaSuccess) return -1;
       dim3 gu(nch, nb);
