@@ -77,8 +77,9 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
  *            nocc[s] = 0 gives J_s = K_s = 0.
  *   C        DEVICE, blocks [C_0 | C_1 | ...] one after another; block s is row-major
  *            nao x nocc[s].  Columns need not be orthonormal.
- *   occ      DEVICE, concatenated occupations, length sum nocc[s]; must be >= 0
- *            (a negative occupation yields NaN in K_s; J_s is unaffected).
+ *   occ      DEVICE, concatenated occupations, length sum nocc[s]; must be >= 0: the kernels work
+ *            with C' = C sqrt(occ), so a negative occupation yields NaN in J_s and K_s.  Densities
+ *            with negative eigenvalues go through dfjk_get_jk_dm.
  *   J_out    DEVICE, nset x nao x nao, or NULL to skip J.
  *   K_out    DEVICE, nset x nao x nao, or NULL to skip K.
  *   stream   all work is enqueued on this stream.

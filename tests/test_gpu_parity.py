@@ -111,6 +111,59 @@ def test_j_only_two_pass_path(torch_cuda, dfjk, nao, naux, nocc, seed):
         assert np.array_equal(J[s], J[s].T)
 
 
+@pytest.mark.parametrize("nao,naux,nocc,seed,opts", [
+    (1, 2, [1], 141, {}),                                   # a single AO: npair = 1
+    (40, 17, [40], 142, {}),                                # nocc = nao
+    (33, 9, [1] * 16 + [2] * 16, 143, dict(max_nset=32, max_nocc_total=48)),   # 32 sets, the hard maximum
+    (72, 300, [11], 144, dict(workspace_cap_bytes=1)),      # one aux row per block: 300 blocks
+    (260, 12, [130, 129], 145, {}),                         # 259 + 5 padded columns: wide N tile, nao % 8 != 0
+])
+def test_degenerate_and_extreme_shapes(torch_cuda, dfjk, nao, naux, nocc, seed, opts):
+    inp = dfjk_inputs.make_random(nao, naux, nocc, seed, L=max(3.0, nao / 6))
+    check_against_oracle(torch_cuda, dfjk, inp, **opts)
+
+
+def test_no_aux_rows_gives_zeros(torch_cuda, dfjk):
+    torch = torch_cuda
+    B = torch.empty((0, 10 * 11 // 2), dtype=torch.float64, device="cuda")
+    C = torch.ones((10, 3), dtype=torch.float64, device="cuda")
+    with dfjk.DFJK(B, 10) as h:
+        J, K = h.get_jk([C], [torch.ones(3, dtype=torch.float64, device="cuda")],
+                        out_j=torch.full((1, 10, 10), 7.0, dtype=torch.float64, device="cuda"),
+                        out_k=torch.full((1, 10, 10), 7.0, dtype=torch.float64, device="cuda"))
+        torch.cuda.synchronize()
+    assert not J.any() and not K.any()
+
+
+def test_negative_occupation_needs_the_density_matrix_form(torch_cuda, dfjk):
+    """documented in include/dfjk.h: C' = C sqrt(occ) needs occ >= 0 (NaN otherwise); a density with
+    negative eigenvalues goes through dfjk_get_jk_dm"""
+    import oracle
+    torch = torch_cuda
+    inp = dfjk_inputs.make_random(24, 10, [5], 146)
+    inp.occ[0][2] = -0.5
+    B, Cs, occs = to_dev(torch, inp)
+    with dfjk.DFJK(B, 24) as h:
+        J, K = h.get_jk(Cs, occs)
+        torch.cuda.synchronize()
+        assert torch.isnan(K).any() and torch.isnan(J).any()
+        D = (inp.C[0] * inp.occ[0]) @ inp.C[0].T
+        Jd, Kd = h.get_jk_dm(torch.from_numpy(D[None]).cuda())
+        torch.cuda.synchronize()
+    sq = _unpack_np(inp.B_packed, 24)
+    Jo = np.einsum("p,pmn->mn", np.einsum("pmn,mn->p", sq, D), sq)
+    assert rel(Jd[0].cpu().numpy(), Jo) <= TOL
+    assert rel(Kd[0].cpu().numpy(), oracle.get_k_dform(inp.B_packed, 24, D)) <= TOL
+
+
+def _unpack_np(Bp, nao):
+    sq = np.zeros((Bp.shape[0], nao, nao))
+    mu, nu = np.tril_indices(nao)
+    sq[:, mu, nu] = Bp
+    sq[:, nu, mu] = Bp
+    return sq
+
+
 def test_more_than_eight_sets(torch_cuda, dfjk):
     inp = dfjk_inputs.make_random(40, 21, [3, 1, 4, 1, 5, 9, 2, 6, 5, 3, 5], 109)
     check_against_oracle(torch_cuda, dfjk, inp, max_nset=12, max_nocc_total=44)
