@@ -52,6 +52,10 @@ typedef struct {
   int max_nset;               /* capacity for nset; 0 = 8 */
   int copy_B;                 /* 0 = borrow the caller's device pointer (default); 1 = private copy */
   int ksplit;                 /* force the split-K factor of the SYRK; 0 = automatic */
+  int no_retile;              /* 0 = dfjk_create also builds a re-tiled private copy of B for the
+                                 half-transform (1.35x the packed bytes, not counted in
+                                 dfjk_workspace_bytes; silently skipped if the allocation fails);
+                                 1 = never: the half-transform gathers from the packed triangle */
   int two_pass_j;             /* 0 = when J and K are both requested, rho (Eq. 14) is taken from the
                                  half-transformed block, rho_P = sum_{mu,i} X^P_{mu i} C'_{mu i}, and B is
                                  streamed twice instead of three times; 1 = always the two-pass J */

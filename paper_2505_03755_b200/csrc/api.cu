@@ -30,7 +30,7 @@ bool dev_alloc(dfjk_ctx* h, T** p, size_t count) {
 }
 
 void free_all(dfjk_ctx* h) {
-  cudaFree(h->B_owned); cudaFree(h->Ct); cudaFree(h->Dw); cudaFree(h->rho_part); cudaFree(h->rho); cudaFree(h->rho_ht);
+  cudaFree(h->B_owned); cudaFree(h->Bt); cudaFree(h->Ct); cudaFree(h->Dw); cudaFree(h->rho_part); cudaFree(h->rho); cudaFree(h->rho_ht);
   cudaFree(h->Jp_part); cudaFree(h->X); cudaFree(h->Kpart);
   cudaFree(h->C_stage); cudaFree(h->occ_stage); cudaFree(h->J_stage); cudaFree(h->K_stage);
   for (int i = 0; i < h->ev_cap; i++) cudaEventDestroy(h->ev[i]);
@@ -164,6 +164,19 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   }
   if (!ok) { free_all(h); delete h; return DFJK_ERR_ALLOC; }
   h->B = h->B_owned ? h->B_owned : B_packed;
+  // re-tiled copy for the half-transform (1.35x the packed bytes): used if it can be had
+  if (!o.no_retile && naux > 0) {
+    h->bt_pstride = retile_doubles_per_aux_row(nao);
+    cudaError_t e = cudaMalloc((void**)&h->Bt, (size_t)naux * h->bt_pstride * sizeof(double));
+    if (e == cudaSuccess) {
+      e = launch_retile(h->B, h->npair, nao, naux, h->Bt);
+      if (e == cudaSuccess) e = cudaDeviceSynchronize();
+      if (e != cudaSuccess) { set_err(h, "re-tiling B", e); free_all(h); delete h; cudaGetLastError(); return DFJK_ERR_CUDA; }
+    } else {
+      cudaGetLastError();
+      h->Bt = nullptr;                       // not enough memory: gather from the packed triangle instead
+    }
+  }
   *out = h;
   return DFJK_OK;
 }

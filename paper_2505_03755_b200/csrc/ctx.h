@@ -41,6 +41,8 @@ struct dfjk_ctx {
   int device;
   const double* B;           // packed tensor (borrowed or owned)
   double* B_owned;
+  double* Bt;                // optional re-tiled copy of B for the half-transform (HtParams)
+  size_t bt_pstride;
   // options / plan
   int max_nset, max_nocc_total, nocc_pad_cap;
   int nblk, ksplit;          // capacities: aux rows of X at nocc_pad_cap columns; split-K partial slots
@@ -96,6 +98,8 @@ int launch_ao2mo(dfjk_ctx* h, int nmo, int a0, int nact, const double* M, double
 // density-matrix form: packed weighted density from D, and K by Eq. 16-17 as printed
 int launch_prep_dw_dm(dfjk_ctx* h, int nset, const double* D, cudaStream_t st);
 int launch_k_path_dm(dfjk_ctx* h, int nset, const double* D, double* K_out, cudaStream_t st);
+size_t retile_doubles_per_aux_row(int nao);
+cudaError_t launch_retile(const double* Bp, size_t npair, int nao, int naux, double* Bt);
 int run_dmma_selftest();
 
 }  // namespace dfjk

@@ -46,6 +46,11 @@ struct HtParams {
   int p_first, nb, ntm, ntn;            // aux rows [p_first, p_first + nb), 64-row blocks, N tiles
   double* rho_ht; int nset; int col0[kMaxSets + 1];   // EPI 1: per-warp partials of rho (step a2 fused)
   int ldx, xrows;                       // EPI 2: row-major X[(pl * xrows + mu) * ldx + n]
+  // optional re-tiled copy of B (dfjk_create): per aux row the 64 x 16 tiles of the symmetric
+  // slice at and below the diagonal blocks, each stored as the padded [64][20] shared-memory image
+  // (tile (mb, c), c < 4 (mb + 1), at image 2 mb (mb + 1) + c), so that the A operand of every chunk
+  // is one bulk copy (a stored or diagonal tile) or four (the transpose: 16 rows of four images)
+  const double* Bt; size_t bt_pstride;
 };
 
 // EPI = 0: X k-tiled for k_syrk.  EPI = 1: the same, plus rho[s][P] = sum_{mu,i in s} X[mu][i] C'[mu][i]
@@ -69,7 +74,7 @@ k_half_transform(const __grid_constant__ HtParams q) {
 
   if (tid == 0) {
     for (int s = 0; s < kStages; s++) {
-      mbar_init(full0 + 8 * s, 128 + 1);   // 128 cp.async arrivals + the expect_tx arrival
+      mbar_init(full0 + 8 * s, q.Bt ? 1 : 128 + 1);   // the expect_tx arrival (+ 128 cp.async arrivals when gathering)
       mbar_init(empty0 + 8 * s, 8);        // one arrival per consumer warp
     }
     mbar_fence_init();
@@ -80,6 +85,36 @@ k_half_transform(const __grid_constant__ HtParams q) {
     // ===================== producer warpgroup =====================
     reg_dec<kProducerRegs>();
     const int tp = tid - 256;
+    if (q.Bt) {
+      // re-tiled B: one elected thread, bulk copies only
+      if (tp != 0) return;
+      const uint32_t sA_u32 = smem_u32(sA), sB_u32 = smem_u32(sB);
+      constexpr uint32_t kImgBytes = 64 * kHtLd * 8, kPieceBytes = 16 * kHtLd * 8;
+      int g = 0;
+      for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int pl = tile / tiles_per_p, rem = tile - pl * tiles_per_p;
+        const int mb = rem / q.ntn, n0 = (rem % q.ntn) * NT;
+        const double* BtP = q.Bt + (size_t)(q.p_first + pl) * q.bt_pstride;
+        for (int c = 0; c < nchunks; c++, g++) {
+          const int stage = g % kStages;
+          const uint32_t fullb = full0 + 8 * stage;
+          mbar_wait(empty0 + 8 * stage, ((g / kStages) & 1) ^ 1);
+          mbar_arrive_expect_tx(fullb, kBBytes + kImgBytes);
+          bulk_g2s(sB_u32 + (uint32_t)stage * kBBytes, q.Ct + ((size_t)c * q.ct_rows + n0) * kHtLd, kBBytes, fullb);
+          const uint32_t a_base = sA_u32 + (uint32_t)(stage * kHtATile) * 8u;
+          if (c < 4 * (mb + 1)) {                    // stored or diagonal tile: its image as it is
+            bulk_g2s(a_base, BtP + (size_t)(2 * mb * (mb + 1) + c) * (64 * kHtLd), kImgBytes, fullb);
+          } else {                                   // transpose: rows 16 (c % 4) .. + 15 of the images (c / 4, 4 mb + qq)
+            const int mbl = c >> 2;
+            const double* src = BtP + (size_t)(2 * mbl * (mbl + 1) + 4 * mb) * (64 * kHtLd) + (size_t)(c & 3) * 16 * kHtLd;
+#pragma unroll
+            for (int qq = 0; qq < 4; qq++)
+              bulk_g2s(a_base + (uint32_t)qq * kPieceBytes, src + (size_t)qq * (64 * kHtLd), kPieceBytes, fullb);
+          }
+        }
+      }
+      return;
+    }
     const int kd = tp & 15, md = tp >> 4;          // direct / crossing: element (md + 8q, kd)
     const int mt = tp & 63, kt = tp >> 6;          // transposed:        element (mt, kt + 2q)
     const uint32_t sA_u32 = smem_u32(sA), sB_u32 = smem_u32(sB);
@@ -173,11 +208,14 @@ k_half_transform(const __grid_constant__ HtParams q) {
           }
         }
       } else {
-        const double* a_ptr = sA + stage * kHtATile + (wm * 16 + r) + j * kHtLdT;
+        // gathered: one [16 lam][64 mu + 4] tile; re-tiled: four [16 lam][16 mu + 4] pieces, piece wm
+        // holds this warp's 16 rows
+        const int ldt = q.Bt ? kHtLd : kHtLdT;
+        const double* a_ptr = sA + stage * kHtATile + (q.Bt ? wm * 16 * kHtLd + r : wm * 16 + r) + j * ldt;
 #pragma unroll
         for (int kk = 0; kk < 4; kk++) {
           if (kk < ksteps) {
-            const double a0 = a_ptr[4 * kk * kHtLdT], a1 = a_ptr[8 + 4 * kk * kHtLdT];
+            const double a0 = a_ptr[4 * kk * ldt], a1 = a_ptr[8 + 4 * kk * ldt];
             double b[WN];
 #pragma unroll
             for (int u = 0; u < WN; u++) b[u] = b_ptr[u * 8 * kHtLd + 4 * kk];
@@ -318,6 +356,48 @@ k_half_transform(const __grid_constant__ HtParams q) {
       if (cur_s >= 0) flush();
     }
   }
+}
+
+// One-time re-tiling of B for the half-transform (dfjk_create): image (mb, c) of aux row P holds
+// Bsym_P[64 mb + i][16 c + k] for i < 64, k < 16 (zero past nao, zero padding columns 16..19).
+__global__ void __launch_bounds__(256)
+k_retile(const double* __restrict__ Bp, size_t npair, int nao, int ntm, double* __restrict__ Bt, size_t bt_pstride) {
+  const int P = blockIdx.y;
+  const double* BpP = Bp + (size_t)P * npair;
+  double* BtP = Bt + (size_t)P * bt_pstride;
+  const int nimg = 2 * ntm * (ntm + 1);
+  for (int img = blockIdx.x; img < nimg; img += gridDim.x) {
+    int mb = (int)(sqrt(0.5 * img + 0.25) - 0.5);               // img = 2 mb (mb + 1) + c, 0 <= c < 4 (mb + 1)
+    while (2 * (mb + 1) * (mb + 2) <= img) mb++;
+    while (2 * mb * (mb + 1) > img) mb--;
+    const int c = img - 2 * mb * (mb + 1);
+    double* dst = BtP + (size_t)img * (64 * kHtLd);
+    for (int e = threadIdx.x; e < 64 * kHtLd; e += 256) {
+      const int i = e / kHtLd, k = e - i * kHtLd;
+      const int mu = 64 * mb + i, lam = 16 * c + k;
+      double v = 0.0;
+      if (k < kHtBK && mu < nao && lam < nao) v = BpP[lam <= mu ? tri(mu) + lam : tri(lam) + mu];
+      dst[e] = v;
+    }
+  }
+}
+
+size_t retile_doubles_per_aux_row(int nao) {
+  const int ntm = cdiv(nao, 64);
+  return (size_t)2 * ntm * (ntm + 1) * 64 * kHtLd;
+}
+
+cudaError_t launch_retile(const double* Bp, size_t npair, int nao, int naux, double* Bt) {
+  if (naux == 0) return cudaSuccess;
+  const int ntm = cdiv(nao, 64);
+  const int nimg = 2 * ntm * (ntm + 1);
+  for (int p0 = 0; p0 < naux; p0 += 32768) {                   // gridDim.y limit
+    const int nb = naux - p0 < 32768 ? naux - p0 : 32768;
+    dim3 grid(nimg < 64 ? nimg : 64, nb);
+    k_retile<<<grid, 256>>>(Bp + (size_t)p0 * npair, npair, nao, ntm, Bt + (size_t)p0 * retile_doubles_per_aux_row(nao),
+                            retile_doubles_per_aux_row(nao));
+  }
+  return cudaGetLastError();
 }
 
 // rho[s][P] = sum over the per-warp slots of k_half_transform<., 1>, ascending (fixed order)
@@ -856,7 +936,7 @@ int launch_half_transform_rowmajor(dfjk_ctx* h, const SetInfo& si, int p_first, 
   const int ntn = cdiv(n8, 2 * kHtMaxWN), wn = cdiv(n8, 2 * ntn);
   const int ntm_ht = cdiv(h->nao, 64);
   HtParams a;
-  a.Bp = h->B; a.npair = h->npair; a.nao = h->nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = si.nocc_pad;
+  a.Bt = h->Bt; a.bt_pstride = h->bt_pstride; a.Bp = h->B; a.npair = h->npair; a.nao = h->nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = si.nocc_pad;
   a.X = X; a.nch = 0; a.mu_pad = 0; a.p_first = p_first; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
   a.rho_ht = nullptr; a.nset = 0; a.ldx = ldx; a.xrows = h->nao;
   a.col0[0] = 0;
@@ -953,7 +1033,7 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
     const int nb = (int)(naux - p0 < nblk ? naux - p0 : nblk);
     prof_mark(h, DFJK_PHASE_HALF_TRANSFORM, st);
     HtParams a;
-    a.Bp = h->B; a.npair = h->npair; a.nao = nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = ldx;
+    a.Bt = h->Bt; a.bt_pstride = h->bt_pstride; a.Bp = h->B; a.npair = h->npair; a.nao = nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = ldx;
     a.X = h->X; a.nch = nch; a.mu_pad = h->mu_pad; a.p_first = p0; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
     a.rho_ht = h->rho_ht; a.nset = si.nset; a.ldx = 0; a.xrows = 0;
     for (int s = 0; s <= si.nset; s++) a.col0[s] = si.col0[s];
@@ -1087,7 +1167,7 @@ int launch_k_path_dm(dfjk_ctx* h, int nset, const double* D, double* K_out, cuda
       const int nb = (int)(naux - p0 < nblk ? naux - p0 : nblk);
       prof_mark(h, DFJK_PHASE_HALF_TRANSFORM, st);
       HtParams a;
-      a.Bp = h->B; a.npair = h->npair; a.nao = nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = ldx;
+      a.Bt = h->Bt; a.bt_pstride = h->bt_pstride; a.Bp = h->B; a.npair = h->npair; a.nao = nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = ldx;
       a.X = X1; a.nch = nch; a.mu_pad = h->mu_pad; a.p_first = p0; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
       a.rho_ht = nullptr; a.nset = 0; a.ldx = 0; a.xrows = 0; a.col0[0] = 0;
       const long long ht_tiles = (long long)nb * ntm_ht * ntn;

@@ -171,7 +171,7 @@ def test_more_than_eight_sets(torch_cuda, dfjk):
 
 @pytest.mark.parametrize("opts", [dict(nblk=1), dict(nblk=7), dict(nblk=16, ksplit=5), dict(ksplit=1),
                                   dict(workspace_cap_bytes=1 << 20), dict(copy_B=True), dict(two_pass_j=True),
-                                  dict(two_pass_j=True, nblk=5)])
+                                  dict(two_pass_j=True, nblk=5), dict(no_retile=True)])
 def test_blocking_and_split_k_do_not_change_the_result(torch_cuda, dfjk, opts):
     """N_blk and split-K are memory/parallelism knobs, not part of the result."""
     inp = dfjk_inputs.make_random(150, 61, [37, 10], 110, L=20.0)
@@ -200,6 +200,20 @@ def test_j_only_k_only_and_batching(torch_cuda, dfjk):
             torch.cuda.synchronize()
             assert rel(J1[0].cpu().numpy(), J[s].cpu().numpy()) < 1e-13
             assert rel(K1[0].cpu().numpy(), K[s].cpu().numpy()) < 1e-13
+
+
+@pytest.mark.parametrize("nao,naux,nocc,seed", [(67, 21, [23, 7], 151), (257, 33, [64], 152), (300, 40, [80], 153)])
+def test_retiled_and_gathered_half_transform_agree_bitwise(torch_cuda, dfjk, nao, naux, nocc, seed):
+    """the re-tiled copy of B (default) and the gather from the packed triangle feed the same numbers
+    to the same DMMA sequence"""
+    torch = torch_cuda
+    inp = dfjk_inputs.make_random(nao, naux, nocc, seed, L=max(4.0, nao / 6))
+    B, Cs, occs = to_dev(torch, inp)
+    with dfjk.DFJK(B, nao) as h1, dfjk.DFJK(B, nao, no_retile=True) as h2:
+        J1, K1 = h1.get_jk(Cs, occs)
+        J2, K2 = h2.get_jk(Cs, occs)
+        torch.cuda.synchronize()
+        assert torch.equal(J1, J2) and torch.equal(K1, K2)
 
 
 def test_repeat_calls_are_bitwise_deterministic_and_stream_ordered(torch_cuda, dfjk):
