@@ -31,7 +31,7 @@ if ROOT not in sys.path:
 import dfjk_inputs  # noqa: E402
 
 METRIC = "DF get_jk ms at nao=1200/naux=4000; K FP64 TFLOP/s & J HBM GB/s vs peak"
-# measured on this pool (profiles/r01_ubench.md): DMMA.8x8x4 issue-rate peak, burst == sustained
+# measured on this pool (profiles/r01_calib.md): DMMA.8x8x4 issue-rate peak, burst == sustained
 FP64_DMMA_PEAK_TFLOPS = 37.1
 FP64_CUBLAS_TFLOPS = 35.47
 HBM_READ_STREAM_GBS = 7430.0
@@ -426,7 +426,7 @@ def main():
                      "algorithmic_bytes_per_launch": (npair_bytes + nao * sum(nocc) * 8.0) * naux * args.steps / max(ht_n, 1),
                      "launches": ht_n, "avg_launch_ms": ht_ms / max(ht_n, 1),
                      "algorithmic_flops_per_step": fb["ht"],
-                     "peak_source": "measured DMMA.8x8x4 issue-rate peak on this pool (profiles/r01_ubench.md); "
+                     "peak_source": "measured DMMA.8x8x4 issue-rate peak on this pool (profiles/r01_calib.md); "
                                     "cuBLAS fp64 8192^3 reaches %.2f; MEASURED_PEAKS bf16 %.1f x nominal 45/2250 = %.1f"
                                     % (FP64_CUBLAS_TFLOPS, pk["bf16"], pk["bf16"] * 45.0 / 2250.0)},
         "k_path": {"ms": ms_k, "tflops": fb["k"] / (ms_k * 1e-3) * 1e-12,
