@@ -1,15 +1,21 @@
 // Steps a5-a9, the exchange build (Eq. 16-17) on the FP64 tensor pipe:
 //   a5/a6  half-transform  X[P][mu][i] = sum_lam B_P[mu][lam] C'[lam][i]   (k_half_transform)
-//          the A operand is read straight from the packed triangle: chunks below the diagonal
-//          as stored, chunks above it as the transpose of the stored tile (only the shared-memory
-//          read pattern changes), chunks crossing it element by element.
-//   a7     SYRK            K_s[mu>=nu] += sum_{P,i in s} X[P][mu][i] X[P][nu][i]   (k_syrk)
-//          lower-triangle 128x128 tiles, split-K over the aux rows of the block, partials
-//          read-modify-written by exactly one CTA each (no atomics: deterministic).
+//          the A operand comes from the re-tiled copy Bt built once in dfjk_create (k_retile: the
+//          64 x 16 tiles of the symmetric slice as ready shared-memory images, bulk copies only),
+//          or, without it, straight from the packed triangle: chunks below the diagonal as
+//          stored, chunks above it as the transpose of the stored tile (only the shared-memory
+//          read pattern changes), chunks crossing it element by element.  Epilogues: k-tiled X,
+//          k-tiled X + rho partials (step a2 fused), row-major X (AO2MO Eq. 18).
+//   a7     SYRK            K_s[mu>=nu] += sum_{P,i in s} X[P][mu][i] X[P][nu][i]   (k_syrk2, k_syrk)
+//          lower-triangle T x T tiles (T = 64..128), split-K over the aux rows of the block,
+//          partials read-modify-written by exactly one CTA each (no atomics: deterministic);
+//          two-operand form K += X X2^T for the density-matrix form (Eq. 16-17 as printed).
+//   a8     scheduler       launch_k_path / launch_k_path_dm: aux blocks from the workspace cap,
+//          tile size and split-K from a list-schedule model.
 //   a9     epilogue        fixed-order sum of the split-K partials, mirrored to both triangles.
 // Both GEMMs are warp-specialised: warpgroups 0-1 (8 warps) only issue LDS + DMMA.8x8x4
 // (mma.sync m8n8k4 f64; FP64 has no tcgen05/TMEM kind), warpgroup 2 produces the shared-memory
-// stages -- bulk async copies (TMA engine, SASS UBLKCP) for the pre-tiled operands C' and X,
+// stages -- bulk async copies (TMA engine, SASS UBLKCP) for the pre-tiled operands C', Bt and X,
 // 8-byte cp.async gathers for the packed triangle -- through a 3-stage full/empty mbarrier ring,
 // with setmaxnreg moving registers from the producers to the consumers.  All tiles have a row
 // stride of 4 mod 16 doubles, which makes both the [row][k] and the [k][row] fragment reads
