@@ -562,9 +562,7 @@ k_syrk(const double* __restrict__ X, int nao, int nch, int mu_pad, int c0, int c
 // Same CTA tile and producer as k_syrk, for T = 16*WM <= 96.  The T x T tile is cut into 2 x 2
 // blocks of WM x WM MMA tiles, one block per SM sub-partition; the two warps of a sub-partition
 // (w and w+4) both hold the whole block in registers and take alternate k4 steps (an in-CTA
-// split-K), so they are perfectly symmetric: 2 WM fragment loads per WM^2 DMMAs each.  The second
-// warp of each pair starts half a chunk late, so the two never reach a chunk boundary (barrier
-// wait + first fragment loads) together and one of them always has DMMAs to issue.
+// split-K), so they are perfectly symmetric: 2 WM fragment loads per WM^2 DMMAs each.
 // Diagonal tiles (ta == tb) skip what the epilogue never reads: the strictly-upper block is not
 // computed at all -- its sub-partition instead shares the k4 steps of the lower block (4-way) --
 // and the two diagonal blocks compute their lower MMA tiles only: WM(WM+1)/2 DMMAs per k4 step on
@@ -574,11 +572,10 @@ k_syrk(const double* __restrict__ X, int nao, int nch, int mu_pad, int c0, int c
 __device__ __forceinline__ void consumer_bar_sync() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
 
 struct Syrk2Consumer {
-  const double* sA; const double* sB; uint32_t full0, empty0, skewbar;
+  const double* sA; const double* sB; uint32_t full0, empty0;
   int nchunks, ch0, ch1, c0, c1, tile_doubles;
   int row0, col0;          // block origin inside the CTA tile
   int kidx;                // this warp takes the k4 steps kk = kidx mod KMOD of every chunk
-  bool late;               // second warp of its pair: starts half a chunk late
 };
 
 template <int WM, bool LOWER, int KMOD>
@@ -588,9 +585,6 @@ __device__ __forceinline__ void syrk2_mainloop(const Syrk2Consumer& q, int l, do
   for (int tt = 0; tt < WM; tt++)
 #pragma unroll
     for (int u = 0; u < WM; u++) acc[tt][u][0] = acc[tt][u][1] = 0.0;
-  if (q.nchunks == 0) return;
-  if (q.late) mbar_wait(q.skewbar, 0);
-  bool release = !q.late;
   int ch = q.ch0;
   for (int c = 0; c < q.nchunks; c++) {
     const int stage = c % kStages;
@@ -614,23 +608,12 @@ __device__ __forceinline__ void syrk2_mainloop(const Syrk2Consumer& q, int l, do
     };
     if (k_lo == 0 && k_hi == 8) {
 #pragma unroll
-      for (int i = 0; i < 8 / KMOD; i++) {
-        step(q.kidx + i * KMOD);
-        if (i == 4 / KMOD - 1 && release) {          // half of the first chunk done
-          release = false;
-          __syncwarp();
-          if (l == 0) mbar_arrive(q.skewbar);
-        }
-      }
+      for (int i = 0; i < 8 / KMOD; i++) step(q.kidx + i * KMOD);
     } else {
       for (int kk = k_lo + ((q.kidx - k_lo) % KMOD + KMOD) % KMOD; kk < k_hi; kk += KMOD) step(kk);
     }
     __syncwarp();
-    if (l == 0) {
-      mbar_arrive(q.empty0 + 8 * stage);
-      if (release) mbar_arrive(q.skewbar);
-    }
-    release = false;
+    if (l == 0) mbar_arrive(q.empty0 + 8 * stage);
   }
 }
 
@@ -694,9 +677,8 @@ k_syrk2(const double* __restrict__ X, const double* __restrict__ X2, int nao, in
   extern __shared__ __align__(128) double smem[];
   double* sA = smem;
   double* sB = smem + kStages * kTileDoubles;
-  __shared__ __align__(8) unsigned long long bars[2 * kStages + 1];
+  __shared__ __align__(8) unsigned long long bars[2 * kStages];
   const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kStages]);
-  const uint32_t skewbar = smem_u32(&bars[2 * kStages]);
   const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
   const int n_off = ntiles_m * (ntiles_m - 1) / 2;
   int ta, tb, g;
@@ -727,7 +709,6 @@ k_syrk2(const double* __restrict__ X, const double* __restrict__ X2, int nao, in
       mbar_init(full0 + 8 * s, 1);         // the expect_tx arrival of the elected producer
       mbar_init(empty0 + 8 * s, 8);        // one arrival per consumer warp
     }
-    mbar_init(skewbar, 4);                 // the four early warps
     mbar_fence_init();
   }
   __syncthreads();
@@ -759,8 +740,7 @@ k_syrk2(const double* __restrict__ X, const double* __restrict__ X2, int nao, in
   const int sp = w & 3, hh = w >> 2;                 // SM sub-partition, first/second warp of the pair
   double* Kp = Kpart_s + (size_t)g * split_stride;
   double* red = smem;                                // reused after the main loop
-  Syrk2Consumer q{sA, one_operand ? sA : sB, full0, empty0, skewbar, nchunks, ch0, ch1, c0, c1, kTileDoubles,
-                  0, 0, 0, hh == 1};
+  Syrk2Consumer q{sA, one_operand ? sA : sB, full0, empty0, nchunks, ch0, ch1, c0, c1, kTileDoubles, 0, 0, 0};
   if (!diag) {
     // block (bm, bn) = (sp & 1, sp >> 1); pair split-K 2
     q.row0 = (sp & 1) * 8 * WM; q.col0 = (sp >> 1) * 8 * WM; q.kidx = hh;
