@@ -363,35 +363,37 @@ def main():
     # the `small` config called directly and as a replayed CUDA graph (dfjk_get_jk only enqueues)
     small = None
     if not args.no_small_calls:
-        sinp = dfjk_inputs.make_config("small")
-        sB = torch.from_numpy(sinp.B_packed).cuda()
-        sC = torch.from_numpy(sinp.C_concat()).cuda()
-        socc = torch.from_numpy(sinp.occ_concat()).cuda()
-        sJ = torch.empty((sinp.nset, sinp.nao, sinp.nao), dtype=torch.float64, device="cuda")
-        sK = torch.empty_like(sJ)
-        hs = dfjk.DFJK(sB, sinp.nao)
-        s_fn = lambda: hs.get_jk_raw(sinp.nocc, sC, socc, out_j=sJ, out_k=sK, stream=stream)
-        for _ in range(3):
-            s_fn()
-        torch.cuda.synchronize()
-        s_launches = hs.last_launch_count
-        ms_direct = max_over_ranks(timed(s_fn, 50))
-        cap = torch.cuda.Stream()
-        cap.wait_stream(stream)
-        graph = torch.cuda.CUDAGraph()
-        with torch.cuda.stream(cap):
-            with torch.cuda.graph(graph, stream=cap):
-                hs.get_jk_raw(sinp.nocc, sC, socc, out_j=sJ, out_k=sK, stream=cap)
-        stream.wait_stream(cap)
-        graph.replay()
-        torch.cuda.synchronize()
-        ms_graph = max_over_ranks(timed(graph.replay, 50))
-        sfb = flops_bytes(dfjk_inputs.CONFIGS["small"])
-        small = {"workload": "small (nao=300, naux=1000, nocc=80), L2-warm", "launches_per_call": s_launches,
-                 "ms_direct": ms_direct, "ms_cuda_graph": ms_graph,
-                 "k_tflops_graph": sfb["k"] / (ms_graph * 1e-3) * 1e-12}
-        del graph
-        hs.close()
+        small = {}
+        for sname in ("tiny", "small"):
+            sinp = dfjk_inputs.make_config(sname)
+            sB = torch.from_numpy(sinp.B_packed).cuda()
+            sC = torch.from_numpy(sinp.C_concat()).cuda()
+            socc = torch.from_numpy(sinp.occ_concat()).cuda()
+            sJ = torch.empty((sinp.nset, sinp.nao, sinp.nao), dtype=torch.float64, device="cuda")
+            sK = torch.empty_like(sJ)
+            hs = dfjk.DFJK(sB, sinp.nao)
+            s_fn = lambda: hs.get_jk_raw(sinp.nocc, sC, socc, out_j=sJ, out_k=sK, stream=stream)
+            for _ in range(3):
+                s_fn()
+            torch.cuda.synchronize()
+            s_launches = hs.last_launch_count
+            ms_direct = max_over_ranks(timed(s_fn, 100))
+            cap = torch.cuda.Stream()
+            cap.wait_stream(stream)
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.stream(cap):
+                with torch.cuda.graph(graph, stream=cap):
+                    hs.get_jk_raw(sinp.nocc, sC, socc, out_j=sJ, out_k=sK, stream=cap)
+            stream.wait_stream(cap)
+            graph.replay()
+            torch.cuda.synchronize()
+            ms_graph = max_over_ranks(timed(graph.replay, 100))
+            sfb = flops_bytes(dfjk_inputs.CONFIGS[sname])
+            small[sname] = {"nao": sinp.nao, "naux": sinp.naux, "nocc": sinp.nocc, "l2": "L2-warm",
+                            "launches_per_call": s_launches, "ms_direct": ms_direct, "ms_cuda_graph": ms_graph,
+                            "k_tflops_graph": sfb["k"] / (ms_graph * 1e-3) * 1e-12}
+            del graph
+            hs.close()
     if not lead:
         h.close()
         ranks.close()

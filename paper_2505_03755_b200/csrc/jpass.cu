@@ -12,9 +12,8 @@
 
 namespace dfjk {
 
-template <bool VEC>
+// two adjacent pairs of a packed row that is only 8-byte aligned (odd npair)
 __device__ __forceinline__ double2 load_pair(const double* p) {
-  if (VEC) return ldg_stream2(p);
   double2 v;
   v.x = ldg_stream1(p);
   v.y = ldg_stream1(p + 1);
@@ -23,7 +22,6 @@ __device__ __forceinline__ double2 load_pair(const double* p) {
 
 // grid.x = pair chunk (kJ1Chunk pairs), grid.y = block of 64 aux rows; 8 warps, warp w streams
 // pairs [chunk*kJ1Chunk + w*kJ1SubChunk, +kJ1SubChunk) of its 64 rows.
-template <bool VEC>
 __global__ void __launch_bounds__(kJ1Warps * 32, 2)
 k_j1(const double* __restrict__ B, size_t npair, int naux, const double* __restrict__ Dw, int nsetg,
      double* __restrict__ part, int naux_pad) {
@@ -54,13 +52,13 @@ k_j1(const double* __restrict__ B, size_t npair, int naux, const double* __restr
 #pragma unroll
     for (int u = 0; u < 2; u++)
 #pragma unroll
-      for (int g = 0; g < 8; g++) b[u][g] = load_pair<VEC>(rowp[g] + kk + 8 * u);
+      for (int g = 0; g < 8; g++) b[u][g] = load_pair(rowp[g] + kk + 8 * u);
 #pragma unroll
     for (int u = 0; u < 2; u++) {
       d[u] = make_double2(0.0, 0.0);
       if (dw_on) {
-        if (VEC) d[u] = *reinterpret_cast<const double2*>(dwp + kk + 8 * u);
-        else { d[u].x = dwp[kk + 8 * u]; d[u].y = dwp[kk + 8 * u + 1]; }
+        d[u].x = dwp[kk + 8 * u];
+        d[u].y = dwp[kk + 8 * u + 1];
       }
     }
 #pragma unroll
@@ -380,7 +378,7 @@ int launch_j_passes(dfjk_ctx* h, const SetInfo& si, double* J_out, bool rho_read
       prof_mark(h, DFJK_PHASE_J1, st);
       dim3 g1(h->j1_chunks, naux_pad / kJ1Rows);
       if (vec) dispatch_j1_tma(ns, g1, st, h->B, npair, naux, h->Dw + (size_t)s0 * npair, h->rho_part, naux_pad);
-      else k_j1<false><<<g1, kJ1Warps * 32, 0, st>>>(h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad);
+      else k_j1<<<g1, kJ1Warps * 32, 0, st>>>(h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad);
       dim3 gr(cdiv(naux, 128), ns);
       k_j1_reduce<<<gr, 128, 0, st>>>(h->rho_part, h->j1_chunks, naux_pad, naux, ns, h->rho + (size_t)s0 * naux);
       launches += 2;
