@@ -46,7 +46,8 @@ enum {
 /* All fields optional; zero = default.  Pass NULL for all defaults. */
 typedef struct {
   size_t workspace_cap_bytes; /* cap for the half-transformed block X (step a8);
-                                 default 4 GiB.  nblk = floor(cap / bytes of one aux row of X) >= 1 */
+                                 default min(4 GiB, a tenth of the free device memory at
+                                 create).  nblk = floor(cap / bytes of one aux row of X) >= 1 */
   int nblk;                   /* force the aux block size N_blk; 0 = derive from cap */
   int max_nocc_total;         /* capacity for sum_s nocc[s]; 0 = nao */
   int max_nset;               /* capacity for nset; 0 = 8 */

@@ -117,7 +117,15 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   // X capacity (k-tiled layout [nch][mu_pad][36] per aux row): the cap, but at least one aux row
   // at full column capacity
   {
-    const size_t cap = o.workspace_cap_bytes ? o.workspace_cap_bytes : ((size_t)4 << 30);
+    // default: 4 GiB, but no more than a tenth of the memory that is free right now (the "dynamic
+    // N_blk based on available memory" the paper leaves to future work)
+    size_t cap = o.workspace_cap_bytes;
+    if (cap == 0) {
+      cap = (size_t)4 << 30;
+      size_t free_b = 0, total_b = 0;
+      if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && free_b / 10 < cap) cap = free_b / 10;
+      else cudaGetLastError();
+    }
     const size_t one_row = (size_t)cdiv(h->nocc_pad_cap, kBK) * h->mu_pad * kLdT;
     size_t dbl = cap / sizeof(double);
     if (o.nblk > 0) dbl = (size_t)o.nblk * one_row;
