@@ -57,6 +57,10 @@ typedef struct {
                                  half-transform (1.35x the packed bytes, not counted in
                                  dfjk_workspace_bytes; silently skipped if the allocation fails);
                                  1 = never: the half-transform gathers from the packed triangle */
+  int ao2mo_route;            /* dfjk_ao2mo: 0 = the cheaper of the two routes; 1 = Eq. 18-21 in the printed
+                                 order (forms bmo^P per aux block); 2 = "active first" (Eq. 18-19 for the
+                                 active columns only, Eq. 20 contracted over P in the AO basis and then
+                                 transformed; falls back to 1 if its scratch does not fit the workspace) */
   int two_pass_j;             /* 0 = when J and K are both requested, rho (Eq. 14) is taken from the
                                  half-transformed block, rho_P = sum_{mu,i} X^P_{mu i} C'_{mu i}, and B is
                                  streamed twice instead of three times; 1 = always the two-pass J */

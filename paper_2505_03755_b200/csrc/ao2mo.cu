@@ -214,18 +214,13 @@ __global__ void k_ao2mo_gather(const double* __restrict__ bmo, int nb, int nmo, 
   }
 }
 
-// Eq. 18-21 block after block.  Workspace: the X buffer of the handle holds, per aux row of the
-// block, the half-transformed slice (nao x ldx), bmo (nmo x nmo) and baa (nact x nact).
-int launch_ao2mo(dfjk_ctx* h, int nmo, int a0, int nact, const double* M, double* bpa_out, double* ppaa_out,
-                 double* papa_out, cudaStream_t st) {
+// Route 1: Eq. 18-21 as printed, block after block.  Workspace: the X buffer of the handle holds,
+// per aux row of the block, the half-transformed slice (nao x ldx), bmo (nmo x nmo) and baa (nact x nact).
+static int launch_ao2mo_as_printed(dfjk_ctx* h, int nmo, int a0, int nact, const double* M, double* bpa_out,
+                                   double* ppaa_out, double* papa_out, cudaStream_t st) {
   int launches = 0;
   const int nao = h->nao, naux = h->naux;
   const size_t n2 = (size_t)nmo * nmo, npa = (size_t)nmo * nact, naa = (size_t)nact * nact;
-  if (naux == 0 || nmo == 0 || nact == 0) {
-    if (ppaa_out && n2 * naa) { k_zero_ao<<<148, 256, 0, st>>>(ppaa_out, n2 * naa); launches++; }
-    if (papa_out && n2 * naa) { k_zero_ao<<<148, 256, 0, st>>>(papa_out, n2 * naa); launches++; }
-    if (naux == 0 || nmo == 0) return launches;
-  }
   SetInfo si;
   si.nset = 1; si.col0[0] = 0; si.nocc[0] = nmo; si.coff[0] = 0; si.ooff[0] = 0;
   si.col0[1] = si.nocc_pad = round_up(nmo, 8);
@@ -268,6 +263,111 @@ int launch_ao2mo(dfjk_ctx* h, int nmo, int a0, int nact, const double* M, double
     launches++;
   }
   return launches;
+}
+
+// Mact[e][a] = M[e][a0 + a], contiguous
+__global__ void k_copy_cols(const double* __restrict__ M, int nao, int nmo, int a0, int nact, double* __restrict__ dst) {
+  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < nao * nact; e += gridDim.x * blockDim.x) {
+    const int r = e / nact, a = e - r * nact;
+    dst[e] = M[(size_t)r * nmo + a0 + a];
+  }
+}
+
+// Wsq[e1][e2][a] = Wsq[e2][e1][a] = W[tri(e1) + e2][a], e1 >= e2
+__global__ void k_unpack_w(const double* __restrict__ W, int nao, int naa, double* __restrict__ Wsq) {
+  const size_t n = (size_t)nao * nao * naa;
+  for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+    const int a = (int)(e % naa);
+    const size_t ee = e / naa;
+    const int e1 = (int)(ee / nao), e2 = (int)(ee % nao);
+    Wsq[e] = W[(e1 >= e2 ? tri(e1) + e2 : tri(e2) + e1) * naa + a];
+  }
+}
+
+// Route 2, "active first": the same bpa, ppaa, papa without ever forming bmo^P (nmo x nmo per aux
+// row).  Eq. 18-19 are only evaluated for the active columns,
+//      Z^P = b^P M_act (nao x nact),   bpa^P = M^T Z^P,
+// and Eq. 20 is contracted over P in the AO basis first (a Coulomb-like build with the nact^2
+// "densities" baa^P, Eq. 15's pattern), then transformed:
+//      W[e1 e2][a1 a2] = sum_P b^P[e1][e2] bpa^P[a0+a1][a2],
+//      ppaa[p1][p2][a1 a2] = sum_{e1 e2} M[e1][p1] W[e1 e2][a1 a2] M[e2][p2].
+// Work 2 naux nao^2 nact + naux nao^2 nact^2 + small, against 2 naux nao nmo (nao + nmo) for the
+// printed order: 5x less at nmo = 340, nact = 8; the printed order wins for large active spaces.
+static int launch_ao2mo_active_first(dfjk_ctx* h, int nmo, int a0, int nact, const double* M, double* bpa_out,
+                                     double* ppaa_out, double* papa_out, cudaStream_t st) {
+  int launches = 0;
+  const int nao = h->nao, naux = h->naux;
+  const size_t npa = (size_t)nmo * nact, naa = (size_t)nact * nact;
+  const int ldz = round_up(nact, 8);
+  double* Mact = h->X;
+  double* Z = h->X + round_up(nao * nact, 2);
+  long long nbz = (long long)((h->X_doubles - round_up(nao * nact, 2)) / ((size_t)nao * ldz));
+  if (h->nblk_forced > 0 && nbz > h->nblk_forced) nbz = h->nblk_forced;
+  if (nbz > naux) nbz = naux;
+  if (nbz > 32768) nbz = 32768;
+  k_copy_cols<<<64, 256, 0, st>>>(M, nao, nmo, a0, nact, Mact);
+  SetInfo si;
+  si.nset = 1; si.col0[0] = 0; si.nocc[0] = nact; si.coff[0] = 0; si.ooff[0] = 0;
+  si.col0[1] = si.nocc_pad = ldz;
+  launches += 1 + launch_prep_ct(h, si, Mact, nullptr, st);
+  for (int p0 = 0; p0 < naux; p0 += (int)nbz) {
+    const int nb = (int)(naux - p0 < nbz ? naux - p0 : nbz);
+    if (launch_half_transform_rowmajor(h, si, p0, nb, Z, ldz, st) != 0) return -1;        // Z^P = b^P M_act
+    GemmTN gb{M, Z, bpa_out + (size_t)p0 * npa, nmo, nact, nao, nmo, ldz, nact, 0, (long long)nao * ldz,
+              (long long)npa, 0};
+    if (gemm_tn(gb, nb, st) != cudaSuccess) return -1;                                     // bpa^P = M^T Z^P
+    launches += 2;
+  }
+  if (ppaa_out) {
+    double* W = h->X;
+    double* Wsq = W + h->npair * naa;
+    double* T = Wsq + (size_t)nao * nao * naa;
+    GemmTN gw{h->B, bpa_out + (size_t)a0 * nact, W, (int)h->npair, (int)naa, naux, (long long)h->npair,
+              (long long)npa, (long long)naa, 0, 0, 0, 0};
+    if (gemm_tn(gw, 1, st) != cudaSuccess) return -1;                                      // W = sum_P b^P (x) baa^P
+    k_unpack_w<<<1184, 256, 0, st>>>(W, nao, (int)naa, Wsq);
+    GemmTN gt{M, Wsq, T, nmo, (int)(nao * naa), nao, nmo, (long long)(nao * naa), (long long)(nao * naa), 0, 0, 0, 0};
+    if (gemm_tn(gt, 1, st) != cudaSuccess) return -1;                                      // T[p1][e2 a] = M^T W
+    GemmTN gp{M, T, ppaa_out, nmo, (int)naa, nao, nmo, (long long)naa, (long long)naa, 0, (long long)(nao * naa),
+              (long long)(nmo * naa), 0};
+    if (gemm_tn(gp, nmo, st) != cudaSuccess) return -1;                                    // ppaa[p1][p2][a] = T_p1^T M
+    launches += 4;
+  }
+  if (papa_out) {
+    GemmTN g21{bpa_out, bpa_out, papa_out, (int)npa, (int)npa, naux, (long long)npa, (long long)npa,
+               (long long)npa, 0, 0, 0, 0};
+    if (gemm_tn(g21, 1, st) != cudaSuccess) return -1;                                     // Eq. 21
+    launches++;
+  }
+  return launches;
+}
+
+// Picks the cheaper route (h->ao2mo_route forces one: 1 as printed, 2 active first).
+int launch_ao2mo(dfjk_ctx* h, int nmo, int a0, int nact, const double* M, double* bpa_out, double* ppaa_out,
+                 double* papa_out, cudaStream_t st) {
+  int launches = 0;
+  const int nao = h->nao, naux = h->naux;
+  const size_t n2 = (size_t)nmo * nmo, naa = (size_t)nact * nact;
+  if (naux == 0 || nmo == 0 || nact == 0) {
+    if (ppaa_out && n2 * naa) { k_zero_ao<<<148, 256, 0, st>>>(ppaa_out, n2 * naa); launches++; }
+    if (papa_out && n2 * naa) { k_zero_ao<<<148, 256, 0, st>>>(papa_out, n2 * naa); launches++; }
+    if (naux == 0 || nmo == 0) return launches;
+  }
+  const double dn = nao, dm = nmo, da = nact;
+  const double cost_printed = 2.0 * dn * dm * (dn + dm) + 2.0 * dm * dm * da * da;          // per aux row
+  const double cost_active = 2.0 * dn * dn * round_up(nact, 8) + 2.0 * dn * dm * 32.0 + dn * dn * da * da +
+                             2.0 * dn * dm * da * da * (dn + dm) / (naux > 0 ? naux : 1);
+  const size_t need2 = h->npair * naa + (size_t)nao * nao * naa + (size_t)nmo * nao * naa;  // W, Wsq, T
+  const size_t need1 = (size_t)round_up(nao * nact, 2) + (size_t)nao * round_up(nact, 8);   // Mact + one row of Z
+  const bool fits = nact > 0 && need2 <= h->X_doubles && need1 <= h->X_doubles && (double)nao * naa < 2e9 &&
+                    round_up(nact, 8) <= h->nocc_pad_cap;
+  bool active = fits && cost_active < cost_printed;
+  if (h->ao2mo_route == 1) active = false;
+  if (h->ao2mo_route == 2 && fits) active = true;
+  const int n = active ? launch_ao2mo_active_first(h, nmo, a0, nact, M, bpa_out, ppaa_out, papa_out, st)
+                       : launch_ao2mo_as_printed(h, nmo, a0, nact, M, bpa_out, ppaa_out, papa_out, st);
+  h->plan_ao2mo_route = active ? 2 : 1;
+  return n < 0 ? n : n + launches;
 }
 
 }  // namespace dfjk

@@ -84,7 +84,8 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   dfjk_options o;
   memset(&o, 0, sizeof(o));
   if (opt) o = *opt;
-  if (o.nblk < 0 || o.max_nocc_total < 0 || o.max_nset < 0 || o.max_nset > kMaxSets || o.ksplit < 0)
+  if (o.nblk < 0 || o.max_nocc_total < 0 || o.max_nset < 0 || o.max_nset > kMaxSets || o.ksplit < 0 ||
+      o.ao2mo_route < 0 || o.ao2mo_route > 2)
     return DFJK_ERR_INVALID_ARG;
 
   int dev = 0;
@@ -102,6 +103,7 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   h->num_sms = prop.multiProcessorCount;
   h->ht_grid = h->num_sms;
   h->two_pass_j = o.two_pass_j;
+  h->ao2mo_route = o.ao2mo_route;
   h->npair = (size_t)nao * (nao + 1) / 2;
   h->nck = cdiv(nao, kHtBK);
   h->mu_pad = round_up(nao, 8) + 128;   // any SYRK tile of <= 128 rows stays inside the tiled X

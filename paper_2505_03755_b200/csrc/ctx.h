@@ -52,6 +52,8 @@ struct dfjk_ctx {
   int j1_chunks, j2_splits;
   int num_sms;
   int ht_grid;               // persistent half-transform: CTAs (= SMs)
+  int ao2mo_route;           // option: 0 = cheaper route, 1 = Eq. 18-21 as printed, 2 = active first
+  int plan_ao2mo_route;      // what the last dfjk_ao2mo used
   int two_pass_j;            // option: never fuse J pass 1 into the half-transform
   // scratch (all allocated at create)
   double* Ct;                // [nck][ct_rows][20]  C' transposed and k-tiled, sqrt(occ) folded, zero padded

@@ -53,9 +53,19 @@ def test_ragged_shapes(nao, naux, nmo, a0, nact, seed):
     run_case(nao, naux, nmo, a0, nact, seed, L=max(4.0, nao / 6))
 
 
-@pytest.mark.parametrize("opts", [dict(nblk=1), dict(nblk=7), dict(workspace_cap_bytes=1 << 21)])
-def test_blocking_does_not_change_the_result(opts):
+@pytest.mark.parametrize("opts", [dict(nblk=1), dict(nblk=7), dict(workspace_cap_bytes=1 << 21),
+                                  dict(ao2mo_route=1), dict(ao2mo_route=2), dict(ao2mo_route=1, nblk=5),
+                                  dict(ao2mo_route=2, nblk=5)])
+def test_blocking_and_route_do_not_change_the_result(opts):
+    """route 1 = Eq. 18-21 in the printed order, route 2 = active first (never forms bmo)"""
     run_case(120, 61, 90, 30, 6, 210, L=15.0, **opts)
+
+
+@pytest.mark.parametrize("route", [1, 2])
+@pytest.mark.parametrize("nao,naux,nmo,a0,nact,seed", [(67, 45, 50, 11, 5, 241), (130, 70, 130, 60, 8, 242),
+                                                       (150, 33, 97, 0, 3, 243), (48, 1, 48, 20, 2, 244)])
+def test_both_routes_on_ragged_shapes(route, nao, naux, nmo, a0, nact, seed):
+    run_case(nao, naux, nmo, a0, nact, seed, L=max(4.0, nao / 6), ao2mo_route=route)
 
 
 def test_small_config_shape_with_orthonormal_orbitals():
