@@ -351,14 +351,20 @@ def main():
         outs = ao_fn()
         torch.cuda.synchronize()
         ao_launches = h.last_launch_count
+        ao_route = h.last_ao2mo_route
         del outs
         ms_ao = max_over_ranks(timed(lambda: ao_fn() and None, max(2, min(args.steps, 3))))
         ao_flops = (2.0 * naux * nao * nao * nmo + 2.0 * naux * nao * nmo * nmo
                     + 2.0 * naux * nmo * nmo * nact * nact + 2.0 * naux * (nmo * nact) ** 2)
+        ao_exec = (2.0 * naux * nao * nao * nact + 2.0 * naux * nao * nmo * nact + 2.0 * naux * (nao * (nao + 1) // 2) * nact * nact
+                   + 2.0 * nao * nmo * nact * nact * (nao + nmo) + 2.0 * naux * (nmo * nact) ** 2) if ao_route == 2 else ao_flops
         ao = {"ms": ms_ao, "nmo": nmo, "a0": a0, "nact": nact, "launches_per_call": ao_launches,
+              "route": {1: "Eq. 18-21 in the printed order", 2: "active first (bmo never formed)"}.get(ao_route, "?"),
+              "executed_flops": ao_exec, "executed_tflops": ao_exec / (ms_ao * 1e-3) * 1e-12,
               "algorithmic_flops": ao_flops, "tflops": ao_flops / (ms_ao * 1e-3) * 1e-12,
               "frac_of_fp64_peak": ao_flops / (ms_ao * 1e-3) * 1e-12 / FP64_DMMA_PEAK_TFLOPS,
-              "flops_note": "Eq. 18 + Eq. 19 (full square) + Eq. 20 + Eq. 21 as printed, no symmetry discount"}
+              "flops_note": "algorithmic_flops / tflops count Eq. 18 + Eq. 19 (full square) + Eq. 20 + Eq. 21 as printed; "
+                            "executed_* count what the chosen route really computes"}
     # ---- the many-small-calls regime of the embedded fragments:
     # the `small` config called directly and as a replayed CUDA graph (dfjk_get_jk only enqueues)
     small = None

@@ -147,6 +147,10 @@ int dfjk_get_jk_dm(dfjk_handle h, int nset, const double* D, double* J_out, doub
 int dfjk_ao2mo(dfjk_handle h, int nmo, int a0, int nact, const double* M, double* bpa_out, double* ppaa_out,
                double* papa_out, dfjk_stream stream);
 
+/* Route the last dfjk_ao2mo took on this handle: 1 = Eq. 18-21 in the printed order, 2 = active first
+ * (see dfjk_options.ao2mo_route); 0 before the first call. */
+int dfjk_last_ao2mo_route(dfjk_handle h);
+
 /* Frees everything the handle owns.  dfjk_destroy(NULL) is a no-op returning DFJK_OK. */
 int dfjk_destroy(dfjk_handle h);
 

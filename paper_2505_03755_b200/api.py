@@ -14,7 +14,7 @@ _lib = None
 
 EXPORTS = ["dfjk_create", "dfjk_get_jk", "dfjk_get_jk_host", "dfjk_destroy", "dfjk_strerror",
            "dfjk_last_error", "dfjk_workspace_bytes", "dfjk_get_plan", "dfjk_last_launch_count",
-           "dfjk_selftest_dmma", "dfjk_set_profiling", "dfjk_get_profile", "dfjk_ao2mo", "dfjk_get_jk_dm"]
+           "dfjk_selftest_dmma", "dfjk_set_profiling", "dfjk_get_profile", "dfjk_ao2mo", "dfjk_get_jk_dm", "dfjk_last_ao2mo_route"]
 
 PHASES = ["prep", "j1", "j2", "j_epilogue", "half_transform", "syrk", "k_epilogue"]
 
@@ -67,6 +67,8 @@ def load_library():
     lib.dfjk_get_plan.restype = ct.c_int
     lib.dfjk_last_launch_count.argtypes = [vp]
     lib.dfjk_last_launch_count.restype = ct.c_int
+    lib.dfjk_last_ao2mo_route.argtypes = [vp]
+    lib.dfjk_last_ao2mo_route.restype = ct.c_int
     lib.dfjk_set_profiling.argtypes = [vp, ct.c_int]
     lib.dfjk_set_profiling.restype = ct.c_int
     lib.dfjk_get_profile.argtypes = [vp, ct.POINTER(ct.c_double), ip]
@@ -230,6 +232,10 @@ class DFJK:
     @property
     def workspace_bytes(self) -> int:
         return int(self._lib.dfjk_workspace_bytes(self._h))
+
+    @property
+    def last_ao2mo_route(self) -> int:
+        return int(self._lib.dfjk_last_ao2mo_route(self._h))
 
     @property
     def last_launch_count(self) -> int:

@@ -28,6 +28,11 @@ struct GemmTN {
   // GEMM of nb * nmo rows, so that only the N dimension pays tile padding)
   int a_group = 0;
   long long a_gstride = 0;
+  // grouped row index of C (0 = plain): element (m, n) is stored at (m / c_group) * c_gstride +
+  // n * c_nstride + m % c_group -- the transposed per-aux-row blocks bpa[P][p][a] written by a GEMM
+  // whose rows are (P, a) and whose columns are p
+  int c_group = 0;
+  long long c_gstride = 0, c_nstride = 0;
 };
 
 // CTA tile (16 WTM) x (32 WTN); consumers 2 (M) x 4 (N), warp tile WTM x WTN MMA tiles (WTM = 4 in
@@ -154,6 +159,12 @@ k_gemm_tn(const __grid_constant__ GemmTN g) {
 #pragma unroll
     for (int u = 0; u < WTN; u++) {
       const int n = n0 + 8 * (wn * WTN + u) + 2 * j;
+      if (g.c_group > 0) {
+        double* p = C + (size_t)(m / g.c_group) * g.c_gstride + (size_t)n * g.c_nstride + m % g.c_group;
+        if (n < g.N) p[0] = g.accumulate ? p[0] + acc[t][u][0] : acc[t][u][0];
+        if (n + 1 < g.N) p[g.c_nstride] = g.accumulate ? p[g.c_nstride] + acc[t][u][1] : acc[t][u][1];
+        continue;
+      }
       double* p = C + (size_t)m * g.ldc + n;
       if (n < g.N) p[0] = g.accumulate ? p[0] + acc[t][u][0] : acc[t][u][0];
       if (n + 1 < g.N) p[1] = g.accumulate ? p[1] + acc[t][u][1] : acc[t][u][1];
@@ -186,6 +197,9 @@ static cudaError_t launch_gemm_tn(const GemmTN& g, int batch, cudaStream_t st) {
 static cudaError_t gemm_tn(const GemmTN& g, int batch, cudaStream_t st) {
   const int n8 = cdiv(g.N > 0 ? g.N : 1, 8);
   const int ntn = cdiv(n8, 44), wtn = cdiv(n8, 4 * ntn);
+  if (wtn <= 2 && g.M >= 128 * 148) {       // narrow and tall (W of the active-first route): 128-row tiles
+    return wtn == 1 ? launch_gemm_tn<8, 1>(g, batch, st) : launch_gemm_tn<8, 2>(g, batch, st);
+  }
   switch (wtn) {
 #define DFJK_GEMM_CASE(N) \
   case N: return launch_gemm_tn<4, N>(g, batch, st);
@@ -313,9 +327,11 @@ static int launch_ao2mo_active_first(dfjk_ctx* h, int nmo, int a0, int nact, con
   for (int p0 = 0; p0 < naux; p0 += (int)nbz) {
     const int nb = (int)(naux - p0 < nbz ? naux - p0 : nbz);
     if (launch_half_transform_rowmajor(h, si, p0, nb, Z, ldz, st) != 0) return -1;        // Z^P = b^P M_act
-    GemmTN gb{M, Z, bpa_out + (size_t)p0 * npa, nmo, nact, nao, nmo, ldz, nact, 0, (long long)nao * ldz,
-              (long long)npa, 0};
-    if (gemm_tn(gb, nb, st) != cudaSuccess) return -1;                                     // bpa^P = M^T Z^P
+    // bpa^P = M^T Z^P for the whole block as one GEMM with rows (P, a) and columns p:
+    // C[(P a)][p] = sum_mu Z^P[mu][a] M[mu][p], stored transposed into bpa[P][p][a]
+    GemmTN gb{Z, M, bpa_out + (size_t)p0 * npa, nb * nact, nmo, nao, ldz, nmo, 0, 0, 0, 0, 0,
+              nact, (long long)nao * ldz, nact, (long long)npa, nact};
+    if (gemm_tn(gb, 1, st) != cudaSuccess) return -1;
     launches += 2;
   }
   if (ppaa_out) {

@@ -327,6 +327,8 @@ int dfjk_get_plan(dfjk_handle h, int* nblk, int* ksplit, int* nocc_pad_capacity)
 
 int dfjk_last_launch_count(dfjk_handle h) { return h ? h->last_launches : 0; }
 
+int dfjk_last_ao2mo_route(dfjk_handle h) { return h ? h->plan_ao2mo_route : 0; }
+
 int dfjk_set_profiling(dfjk_handle h, int on) {
   if (!h) return DFJK_ERR_INVALID_ARG;
   if (on && !h->ev) {

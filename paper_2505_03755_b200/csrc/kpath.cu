@@ -31,6 +31,13 @@
 namespace dfjk {
 
 constexpr int kStages = 3;
+// Pipeline depth of the half-transform by N tile width: 3 stages of 59 KB at 304 columns; a thin
+// tile (AO2MO's active columns, small sets) is bandwidth-bound and keeps up to 8 stages in flight.
+__host__ __device__ constexpr int ht_stages(int wn) {
+  const int stage_bytes = (64 * kHtLd + 16 * wn * kHtLd) * 8;
+  const int fit = (200 * 1024) / stage_bytes;
+  return fit < 3 ? 3 : (fit > 8 ? 8 : fit);
+}
 constexpr int kThreads = 384;             // 2 consumer warpgroups + 1 producer warpgroup
 
 // ------------------------------------------------------------------ half-transform
@@ -67,11 +74,12 @@ __global__ void __launch_bounds__(kThreads, 1)
 k_half_transform(const __grid_constant__ HtParams q) {
   extern __shared__ __align__(128) double smem[];
   constexpr int NT = 16 * WN;
+  constexpr int kS = ht_stages(WN);               // 3 for the wide tiles, up to 8 for thin ones
   constexpr uint32_t kBBytes = NT * kHtLd * 8;
-  double* sA = smem;                               // kStages x kHtATile
-  double* sB = smem + kStages * kHtATile;          // kStages x NT*kHtLd
-  __shared__ __align__(8) unsigned long long bars[2 * kStages];
-  const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kStages]);
+  double* sA = smem;                               // kS x kHtATile
+  double* sB = smem + kS * kHtATile;          // kS x NT*kHtLd
+  __shared__ __align__(8) unsigned long long bars[2 * kS];
+  const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kS]);
   const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
   const int nao = q.nao;
   const int nk4 = (nao + 3) >> 2;                  // k4 steps that carry data
@@ -79,7 +87,7 @@ k_half_transform(const __grid_constant__ HtParams q) {
   const int tiles_per_p = q.ntm * q.ntn, ntiles = q.nb * tiles_per_p;
 
   if (tid == 0) {
-    for (int s = 0; s < kStages; s++) {
+    for (int s = 0; s < kS; s++) {
       mbar_init(full0 + 8 * s, q.Bt ? 1 : 128 + 1);   // the expect_tx arrival (+ 128 cp.async arrivals when gathering)
       mbar_init(empty0 + 8 * s, 8);        // one arrival per consumer warp
     }
@@ -102,9 +110,9 @@ k_half_transform(const __grid_constant__ HtParams q) {
         const int mb = rem / q.ntn, n0 = (rem % q.ntn) * NT;
         const double* BtP = q.Bt + (size_t)(q.p_first + pl) * q.bt_pstride;
         for (int c = 0; c < nchunks; c++, g++) {
-          const int stage = g % kStages;
+          const int stage = g % kS;
           const uint32_t fullb = full0 + 8 * stage;
-          mbar_wait(empty0 + 8 * stage, ((g / kStages) & 1) ^ 1);
+          mbar_wait(empty0 + 8 * stage, ((g / kS) & 1) ^ 1);
           mbar_arrive_expect_tx(fullb, kBBytes + kImgBytes);
           bulk_g2s(sB_u32 + (uint32_t)stage * kBBytes, q.Ct + ((size_t)c * q.ct_rows + n0) * kHtLd, kBBytes, fullb);
           const uint32_t a_base = sA_u32 + (uint32_t)(stage * kHtATile) * 8u;
@@ -132,9 +140,9 @@ k_half_transform(const __grid_constant__ HtParams q) {
       const double* BpP = q.Bp + (size_t)(q.p_first + pl) * q.npair;
       const bool okt = m0 + mt < nao;
       for (int c = 0; c < nchunks; c++, g++) {
-        const int stage = g % kStages;
+        const int stage = g % kS;
         const uint32_t fullb = full0 + 8 * stage;
-        mbar_wait(empty0 + 8 * stage, ((g / kStages) & 1) ^ 1);
+        mbar_wait(empty0 + 8 * stage, ((g / kS) & 1) ^ 1);
         const int l0 = c * kHtBK;
         if (tp == 0) {
           mbar_arrive_expect_tx(fullb, kBBytes);
@@ -191,11 +199,11 @@ k_half_transform(const __grid_constant__ HtParams q) {
       for (int u = 0; u < WN; u++) acc[t][u][0] = acc[t][u][1] = 0.0;
 
     for (int c = 0; c < nchunks; c++, g++) {
-      const int stage = g % kStages;
+      const int stage = g % kS;
       const int l0 = c * kHtBK;
       const bool tr = (l0 >= m0 + 63) && !(l0 + kHtBK - 1 <= m0);
       const int ksteps = min(4, nk4 - c * 4);
-      mbar_wait(full0 + 8 * stage, (g / kStages) & 1);
+      mbar_wait(full0 + 8 * stage, (g / kS) & 1);
       const double* b_ptr = sB + stage * NT * kHtLd + (wn * 8 * WN + r) * kHtLd + j;
       if (!tr) {
         const double* a_ptr = sA + stage * kHtATile + (wm * 16 + r) * kHtLd + j;
@@ -820,7 +828,7 @@ __global__ void k_zero(double* p, size_t n) {
 }
 
 // ------------------------------------------------------------------ launchers (step a8)
-static size_t ht_smem_bytes(int wn) { return (size_t)kStages * (kHtATile + 16 * wn * kHtLd) * sizeof(double); }
+static size_t ht_smem_bytes(int wn) { return (size_t)ht_stages(wn) * (kHtATile + 16 * wn * kHtLd) * sizeof(double); }
 static size_t syrk_smem_bytes(int wm) { return (size_t)kStages * 2 * (16 * wm * kLdT) * sizeof(double); }
 
 template <int WN, int EPI>
