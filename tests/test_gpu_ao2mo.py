@@ -89,3 +89,23 @@ def test_edges_and_errors():
         J, K = h.get_jk([M[:, :3].contiguous()], [torch.ones(3, dtype=torch.float64, device="cuda")])
         torch.cuda.synchronize()                                # the handle still serves get_jk
         assert torch.isfinite(J).all() and torch.isfinite(K).all()
+
+
+def test_route_follows_the_flop_model():
+    """few active orbitals: active first (route 2); an active space as large as the MO space: the
+    printed order (route 1); both against the oracle"""
+    import torch
+    import oracle
+    import paper_2505_03755_b200 as dfjk
+    inp = dfjk_inputs.make_random(64, 30, [1], 251, L=10.0)
+    M = np.random.default_rng(252).standard_normal((64, 40))
+    B = torch.from_numpy(inp.B_packed).cuda()
+    with dfjk.DFJK(B, 64) as h:
+        assert h.last_ao2mo_route == 0
+        for a0, nact, want in ((10, 3, 2), (0, 40, 1)):
+            bpa, ppaa, papa = h.ao2mo(torch.from_numpy(M).cuda(), a0, nact)
+            torch.cuda.synchronize()
+            assert h.last_ao2mo_route == want
+            o_bpa, o_ppaa, o_papa = oracle.ao2mo(inp.B_packed, 64, M, a0, nact)
+            assert rel(bpa.cpu().numpy(), o_bpa) <= TOL
+            assert rel(ppaa.cpu().numpy(), o_ppaa) <= TOL and rel(papa.cpu().numpy(), o_papa) <= TOL
