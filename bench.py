@@ -225,7 +225,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-parity", action="store_true", help="skip the sampled parity check")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--cpu-seconds", type=float, default=20.0)
     ap.add_argument("--shard-aux", action="store_true",
                     help="with --gpus N > 1: shard the aux rows over the ranks and sum-all-reduce J, K (strong scaling) "
                          "instead of N independent replicas")
