@@ -6,8 +6,8 @@
 //          stored, chunks above it as the transpose of the stored tile (only the shared-memory
 //          read pattern changes), chunks crossing it element by element.  Epilogues: k-tiled X,
 //          k-tiled X + rho partials (step a2 fused), row-major X (AO2MO Eq. 18).
-//   a7     SYRK            K_s[mu>=nu] += sum_{P,i in s} X[P][mu][i] X[P][nu][i]   (k_syrk2, k_syrk)
-//          lower-triangle T x T tiles (T = 64..128), split-K over the aux rows of the block,
+//   a7     SYRK            K_s[mu>=nu] += sum_{P,i in s} X[P][mu][i] X[P][nu][i]   (k_syrk2)
+//          lower-triangle T x T tiles (T = 64..112), split-K over the aux rows of the block,
 //          partials read-modify-written by exactly one CTA each (no atomics: deterministic);
 //          two-operand form K += X X2^T for the density-matrix form (Eq. 16-17 as printed).
 //   a8     scheduler       launch_k_path / launch_k_path_dm: aux blocks from the workspace cap,
@@ -45,7 +45,7 @@ constexpr int kThreads = 384;             // 2 consumer warpgroups + 1 producer 
 // packed tensor passes through the SM once per row block).  Consumers: 4 (M, 16 rows) x 2 (N
 // halves); warps w and w+4 share an SM sub-partition.  k-chunks of 16 (kHtBK).
 //   C' tiled:  Ct[(chunk * ct_rows + n) * 20 + k]                  (written by k_prep_ct)
-//   X tiled:   X[((pl * nch + n/32) * mu_pad + mu) * 36 + n%32]    (read by k_syrk with bulk copies)
+//   X tiled:   X[((pl * nch + n/32) * mu_pad + mu) * 36 + n%32]    (read by k_syrk2 with bulk copies)
 constexpr int kHtATile = 64 * kHtLd;       // 1280 doubles >= 16 * 68 = 1088
 constexpr int kHtLdT = 64 + 4;             // 68: row stride of the transposed [16][64] A tile
 
@@ -66,7 +66,7 @@ struct HtParams {
   const double* Bt; size_t bt_pstride;
 };
 
-// EPI = 0: X k-tiled for k_syrk.  EPI = 1: the same, plus rho[s][P] = sum_{mu,i in s} X[mu][i] C'[mu][i]
+// EPI = 0: X k-tiled for k_syrk2.  EPI = 1: the same, plus rho[s][P] = sum_{mu,i in s} X[mu][i] C'[mu][i]
 // (= sum_{mu,lam} B_P[mu][lam] D_s[lam][mu], Eq. 14) as per-warp partials, so that a get_jk call that
 // wants both J and K streams B twice instead of three times.  EPI = 2: X row-major (AO2MO, Eq. 18).
 template <int WN, int EPI>
@@ -426,148 +426,11 @@ __global__ void k_rho_reduce(const double* __restrict__ rho_ht, int nslots, int 
 }
 
 // ------------------------------------------------------------------ SYRK
-// CTA: one lower-triangle T x T tile (ta >= tb) of K_s, T = 16*WM in {64,80,96,112,128} chosen per
-// nao to minimise padding, and one split of the block's aux rows.  Consumers: 2 warp rows of
-// WM MMA tiles each, 4 warp columns of ceil(WM/2), ceil(WM/2), floor(WM/2), floor(WM/2) MMA tiles;
-// every SM sub-partition hosts one wide and one narrow warp of the same warp row, so all four
-// issue WM*WM DMMAs per k4 step.  The reduction runs over (aux row, 32-column chunk of X) pairs;
-// a chunk that straddles two sets contributes only the k4 steps of this set.  Both operand tiles
-// are contiguous T x 36 blocks of the tiled X, fetched by one elected producer thread with bulk
-// async copies; the diagonal tile fetches one.
-struct SyrkConsumerArgs {
-  const double* sA; const double* sB; uint32_t full0, empty0;
-  int nchunks, ch0, ch1, c0, c1, tile_doubles, row0, col0, a0, b0, nao, first;
-  double* Kp;
-};
-
-// One consumer warp: rows [row0, row0 + 8 WM), columns [col0, col0 + 8 NC) of the CTA tile.
-template <int WM, int NC>
-__device__ __forceinline__ void syrk_consume(const SyrkConsumerArgs& q, int l) {
-  const int r = l >> 2, j = l & 3;
-  double acc[WM][NC][2];
-#pragma unroll
-  for (int tt = 0; tt < WM; tt++)
-#pragma unroll
-    for (int u = 0; u < NC; u++) acc[tt][u][0] = acc[tt][u][1] = 0.0;
-  int ch = q.ch0;
-  for (int c = 0; c < q.nchunks; c++) {
-    const int stage = c % kStages;
-    // k4 steps of this chunk that belong to the set: columns [max(c0, 32 ch), min(c1, 32 ch + 32))
-    const int k_lo = (max(q.c0, ch * 32) - ch * 32) >> 2, k_hi = (min(q.c1, ch * 32 + 32) - ch * 32) >> 2;
-    if (++ch == q.ch1) ch = q.ch0;
-    mbar_wait(q.full0 + 8 * stage, (c / kStages) & 1);
-    const double* a_ptr = q.sA + stage * q.tile_doubles + (q.row0 + r) * kLdT + j;
-    const double* b_ptr = q.sB + stage * q.tile_doubles + (q.col0 + r) * kLdT + j;
-    auto step = [&](int kk) {
-      double a[WM], b[NC];
-#pragma unroll
-      for (int tt = 0; tt < WM; tt++) a[tt] = a_ptr[tt * 8 * kLdT + 4 * kk];
-#pragma unroll
-      for (int u = 0; u < NC; u++) b[u] = b_ptr[u * 8 * kLdT + 4 * kk];
-#pragma unroll
-      for (int tt = 0; tt < WM; tt++)
-#pragma unroll
-        for (int u = 0; u < NC; u++) dmma884(acc[tt][u][0], acc[tt][u][1], a[tt], b[u]);
-    };
-    if (k_lo == 0 && k_hi == 8) {
-#pragma unroll
-      for (int kk = 0; kk < 8; kk++) step(kk);
-    } else {
-      for (int kk = k_lo; kk < k_hi; kk++) step(kk);
-    }
-    __syncwarp();
-    if (l == 0) mbar_arrive(q.empty0 + 8 * stage);
-  }
-  // read-modify-write this CTA's private partial tile (also above the diagonal of a diagonal
-  // tile; the epilogue reads mu >= nu only)
-#pragma unroll
-  for (int tt = 0; tt < WM; tt++) {
-    const int mu = q.a0 + q.row0 + tt * 8 + r;
-    if (mu >= q.nao) continue;
-#pragma unroll
-    for (int u = 0; u < NC; u++) {
-      const int nu = q.b0 + q.col0 + u * 8 + 2 * j;
-      double* p = q.Kp + (size_t)mu * q.nao + nu;
-      if (nu < q.nao) p[0] = q.first ? acc[tt][u][0] : p[0] + acc[tt][u][0];
-      if (nu + 1 < q.nao) p[1] = q.first ? acc[tt][u][1] : p[1] + acc[tt][u][1];
-    }
-  }
-}
-
-template <int WM>
-__global__ void __launch_bounds__(kThreads, 1)
-k_syrk(const double* __restrict__ X, int nao, int nch, int mu_pad, int c0, int c1, int nrows_blk,
-       int rows_per_split, int ntiles_m, double* __restrict__ Kpart_s, size_t split_stride, int first) {
-  constexpr int T = 16 * WM, WNA = (WM + 1) / 2, WNB = WM / 2;
-  constexpr int kTileDoubles = T * kLdT;
-  constexpr uint32_t kTileBytes = kTileDoubles * 8;
-  extern __shared__ __align__(128) double smem[];
-  double* sA = smem;
-  double* sB = smem + kStages * kTileDoubles;
-  __shared__ __align__(8) unsigned long long bars[2 * kStages];
-  const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kStages]);
-  const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
-  // tile index -> (ta, tb), ta >= tb
-  const int ntiles = ntiles_m * (ntiles_m + 1) / 2;
-  const int t = blockIdx.x % ntiles, g = blockIdx.x / ntiles;
-  int ta = (int)((sqrt(8.0 * t + 1.0) - 1.0) * 0.5);
-  while ((ta + 1) * (ta + 2) / 2 <= t) ta++;
-  while (ta * (ta + 1) / 2 > t) ta--;
-  const int tb = t - ta * (ta + 1) / 2;
-  const bool diag = ta == tb;
-  const int a0 = ta * T, b0 = tb * T;
-  const int p_beg = g * rows_per_split;
-  int p_end = p_beg + rows_per_split;
-  if (p_end > nrows_blk) p_end = nrows_blk;
-  const int np = p_end > p_beg ? p_end - p_beg : 0;
-  const int ch0 = c0 >> 5, ch1 = (c1 + 31) >> 5;   // X chunks that hold columns of this set
-  const int cps = ch1 - ch0;
-  const int nchunks = np * cps;
-
-  if (tid == 0) {
-    for (int s = 0; s < kStages; s++) {
-      mbar_init(full0 + 8 * s, 1);         // the expect_tx arrival of the elected producer
-      mbar_init(empty0 + 8 * s, 8);        // one arrival per consumer warp
-    }
-    mbar_fence_init();
-  }
-  __syncthreads();
-
-  if (w >= 8) {
-    // ===================== producer warpgroup (one elected thread works) =====================
-    reg_dec<kProducerRegs>();
-    if (tid == 256) {
-      const uint32_t sA_u32 = smem_u32(sA), sB_u32 = smem_u32(sB);
-      const size_t chunk_stride = (size_t)mu_pad * kLdT, row_stride = (size_t)nch * chunk_stride;
-      int P = p_beg, ch = ch0;
-      for (int c = 0; c < nchunks; c++) {
-        const int stage = c % kStages;
-        const uint32_t fullb = full0 + 8 * stage;
-        mbar_wait(empty0 + 8 * stage, ((c / kStages) & 1) ^ 1);
-        const double* src = X + (size_t)P * row_stride + (size_t)ch * chunk_stride;
-        mbar_arrive_expect_tx(fullb, diag ? kTileBytes : 2 * kTileBytes);
-        bulk_g2s(sA_u32 + (uint32_t)stage * kTileBytes, src + (size_t)a0 * kLdT, kTileBytes, fullb);
-        if (!diag) bulk_g2s(sB_u32 + (uint32_t)stage * kTileBytes, src + (size_t)b0 * kLdT, kTileBytes, fullb);
-        if (++ch == ch1) { ch = ch0; P++; }
-      }
-    }
-    return;
-  }
-
-  // ===================== consumer warpgroups =====================
-  reg_inc<kConsumerRegs>();
-  const int sp = w & 3;                              // SM sub-partition of this warp
-  const bool wide = (w >> 2) == 0;                   // wide (WNA tiles) or narrow (WNB tiles) warp
-  const int wm = sp & 1;
-  const int col8 = wide ? (sp >> 1) * WNA : 2 * WNA + (sp >> 1) * WNB;   // first MMA tile column
-  SyrkConsumerArgs ca{sA, diag ? sA : sB, full0, empty0, nchunks, ch0, ch1, c0, c1, kTileDoubles,
-                      wm * 8 * WM, col8 * 8, a0, b0, nao, first, Kpart_s + (size_t)g * split_stride};
-  if (wide) syrk_consume<WM, WNA>(ca, l);
-  else syrk_consume<WM, WNB>(ca, l);
-}
-
-// ------------------------------------------------------------------ SYRK, paired-warp version
-// Same CTA tile and producer as k_syrk, for T = 16*WM <= 96.  The T x T tile is cut into 2 x 2
+// CTA: one lower-triangle T x T tile (ta >= tb) of K_s, T = 16*WM in {64,80,96,112} chosen per nao
+// by least modelled work, and one split of the block's aux rows.  The reduction runs over (aux
+// row, 32-column chunk of X) pairs; a chunk that straddles two sets contributes only the k4 steps
+// of this set.  Both operand tiles are contiguous T x 36 blocks of the tiled X, fetched by one
+// elected producer thread with bulk async copies.  The T x T tile is cut into 2 x 2
 // blocks of WM x WM MMA tiles, one block per SM sub-partition; the two warps of a sub-partition
 // (w and w+4) both hold the whole block in registers and take alternate k4 steps (an in-CTA
 // split-K), so they are perfectly symmetric: 2 WM fragment loads per WM^2 DMMAs each.
@@ -875,29 +738,6 @@ struct SyrkArgs {
 };
 
 template <int WM>
-static cudaError_t launch_syrk(int grid, cudaStream_t st, const SyrkArgs& a) {
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_syrk<WM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)syrk_smem_bytes(WM));
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
-  k_syrk<WM><<<grid, kThreads, syrk_smem_bytes(WM), st>>>(a.X, a.nao, a.nch, a.mu_pad, a.c0, a.c1, a.nrows_blk,
-                                                        a.rows_per_split, a.ntiles_m, a.Kpart_s, a.split_stride,
-                                                        a.first);
-  return cudaSuccess;
-}
-
-static cudaError_t dispatch_syrk(int wm, int grid, cudaStream_t st, const SyrkArgs& a) {
-  switch (wm) {
-    case 7: return launch_syrk<7>(grid, st, a);
-    case 8: return launch_syrk<8>(grid, st, a);
-    default: return cudaErrorInvalidValue;
-  }
-}
-
-template <int WM>
 static cudaError_t launch_syrk2(int ksplit, cudaStream_t st, const SyrkArgs& a) {
   static bool attr_set = false;
   if (!attr_set) {
@@ -918,6 +758,7 @@ static cudaError_t dispatch_syrk2(int wm, int ksplit, cudaStream_t st, const Syr
     case 4: return launch_syrk2<4>(ksplit, st, a);
     case 5: return launch_syrk2<5>(ksplit, st, a);
     case 6: return launch_syrk2<6>(ksplit, st, a);
+    case 7: return launch_syrk2<7>(ksplit, st, a);
     default: return cudaErrorInvalidValue;
   }
 }
@@ -989,20 +830,18 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
   const int n8 = ldx / 8;
   const int ntn = cdiv(n8, 2 * kHtMaxWN), wn = cdiv(n8, 2 * ntn);  // N tile = 16*wn columns
   const int ntm_ht = cdiv(nao, 64);
-  // SYRK tile T = 16*wm_s in {64,...,128}: least modelled work (ties -> larger tile).  Tiles up to
-  // 96 run the paired-warp kernel, whose diagonal CTAs cost (WM+1)/(2 WM) of an off-diagonal one.
-  int wm_s = 8;
+  // SYRK tile T = 16*wm_s in {64,...,112}: least modelled work (ties -> larger tile); a diagonal
+  // CTA costs (WM+1)/(2 WM) of an off-diagonal one
+  int wm_s = 7;
   {
     double best = 1e300;
-    for (int wmc = 8; wmc >= 4; wmc--) {
+    for (int wmc = 7; wmc >= 4; wmc--) {
       const int T = 16 * wmc, nt = cdiv(nao, T);
-      const double dc = wmc <= 6 ? (wmc + 1) / (2.0 * wmc) : 1.0;
-      const double area = (0.5 * nt * (nt - 1) + dc * nt) * (double)T * T * (wmc <= 6 ? 1.0 : 1.03);
+      const double area = (0.5 * nt * (nt - 1) + (wmc + 1) / (2.0 * wmc) * nt) * (double)T * T;
       if (area < best * 0.995) { best = area; wm_s = wmc; }
     }
   }
-  const bool paired = wm_s <= 6;
-  const double diag_cost = paired ? (wm_s + 1) / (2.0 * wm_s) : 1.0;
+  const double diag_cost = (wm_s + 1) / (2.0 * wm_s);
   const int ntm = cdiv(nao, 16 * wm_s), ntiles = ntm * (ntm + 1) / 2;
   int ksplit = h->ksplit_forced;
   if (ksplit <= 0) {
@@ -1042,8 +881,7 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
       // columns past nocc[s] (padding to the 8-column MMA tile) are zero: stop at the k4 step
       SyrkArgs sa{h->X, nao, nch, h->mu_pad, si.col0[s], si.col0[s] + round_up(si.nocc[s], 4), nb, rps, ntm,
                   h->Kpart + n2 * s, split_stride, p0 == 0 ? 1 : 0};
-      const cudaError_t e = paired ? dispatch_syrk2(wm_s, ksplit, st, sa) : dispatch_syrk(wm_s, ntiles * ksplit, st, sa);
-      if (e != cudaSuccess) return -1;
+      if (dispatch_syrk2(wm_s, ksplit, st, sa) != cudaSuccess) return -1;
       launches++;
     }
   }
@@ -1128,10 +966,10 @@ int launch_k_path_dm(dfjk_ctx* h, int nset, const double* D, double* K_out, cuda
   const int n8 = ldx / 8;
   const int ntn = cdiv(n8, 2 * kHtMaxWN), wn = cdiv(n8, 2 * ntn);
   const int ntm_ht = cdiv(nao, 64);
-  int wm_s = 6;
+  int wm_s = 7;
   {
     double best = 1e300;
-    for (int wmc = 6; wmc >= 4; wmc--) {
+    for (int wmc = 7; wmc >= 4; wmc--) {
       const int T = 16 * wmc, nt = cdiv(nao, T);
       const double area = (0.5 * nt * (nt - 1) + (wmc + 1) / (2.0 * wmc) * nt) * (double)T * T;
       if (area < best * 0.995) { best = area; wm_s = wmc; }

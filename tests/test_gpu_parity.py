@@ -80,6 +80,7 @@ def test_small_config(torch_cuda, dfjk):
     (200, 130, [9, 8, 8, 1, 40, 3, 17, 2], 106),  # eight sets
     (257, 33, [64], 107),        # three m-tiles: direct, crossing and transposed chunks all occur
     (48, 1, [12], 108),          # single aux row
+    (330, 20, [40, 9], 161),     # 3 x 112: the 112 x 112 SYRK tile
 ])
 def test_ragged_shapes(torch_cuda, dfjk, nao, naux, nocc, seed):
     inp = dfjk_inputs.make_random(nao, naux, nocc, seed, L=max(4.0, nao / 6))
