@@ -481,7 +481,13 @@ __device__ __forceinline__ void syrk2_mainloop(const Syrk2Consumer& q, int l, do
 #pragma unroll
       for (int i = 0; i < 8 / KMOD; i++) step(q.kidx + i * KMOD);
     } else {
-      for (int kk = k_lo + ((q.kidx - k_lo) % KMOD + KMOD) % KMOD; kk < k_hi; kk += KMOD) step(kk);
+      // chunk shared with another set (or the ragged last chunk): same unrolled steps, each under a
+      // warp-uniform predicate
+#pragma unroll
+      for (int i = 0; i < 8 / KMOD; i++) {
+        const int kk = q.kidx + i * KMOD;
+        if (kk >= k_lo && kk < k_hi) step(kk);
+      }
     }
     __syncwarp();
     if (l == 0) mbar_arrive(q.empty0 + 8 * stage);
