@@ -115,7 +115,15 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   h->nblk_forced = o.nblk;
   h->ksplit_forced = o.ksplit;
   // split-K partial slots of the SYRK (each is max_nset x nao x nao doubles)
-  h->ksplit = o.ksplit ? o.ksplit : 16;
+  // 16 slots, more for small bases (up to 64 while the slots stay under 1 GB): the finer the split
+  // can be, the closer the SYRK's CTA count gets to a whole number of waves
+  {
+    const double slot_bytes = (double)h->max_nset * nao * nao * sizeof(double);
+    int cap = (int)(1.0e9 / slot_bytes);
+    if (cap < 16) cap = 16;
+    if (cap > 64) cap = 64;
+    h->ksplit = o.ksplit ? o.ksplit : cap;
+  }
   // X capacity (k-tiled layout [nch][mu_pad][36] per aux row): the cap, but at least one aux row
   // at full column capacity
   {

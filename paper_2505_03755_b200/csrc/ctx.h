@@ -48,6 +48,7 @@ struct dfjk_ctx {
   int nblk, ksplit;          // capacities: aux rows of X at nocc_pad_cap columns; split-K partial slots
   int nblk_forced, ksplit_forced;
   int plan_nblk, plan_ksplit, plan_nblocks;  // what the last get_jk actually used
+  int ks_cache_nblk, ks_cache_ntiles, ks_cache_val;   // last answer of the split-K model
   int n_mtiles;              // 128-row tiles along nao
   int j1_chunks, j2_splits;
   int num_sms;

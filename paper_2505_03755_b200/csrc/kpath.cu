@@ -806,6 +806,28 @@ static double syrk_makespan(int n_off, int n_diag, double diag_cost, int ksplit,
   return end;
 }
 
+// Split-K factor of the SYRK for blocks of nblk aux rows: the split with the shortest modelled
+// makespan (one CTA per SM), 0.2 % per split for the extra partial tiles; remembered in the handle
+// because the model costs a few thousand heap operations.
+static int pick_ksplit(dfjk_ctx* h, int nblk, int ntiles, int ntm, double diag_cost) {
+  int ksplit = h->ksplit_forced;
+  if (ksplit <= 0) {
+    if (h->ks_cache_val > 0 && h->ks_cache_nblk == nblk && h->ks_cache_ntiles == ntiles) return h->ks_cache_val;
+    double best = 1e300;
+    ksplit = 1;
+    for (int k = 1; k <= h->ksplit && k <= nblk; k++) {
+      const int rps = cdiv(nblk, k);
+      if (cdiv(nblk, rps) != k) continue;                       // splits that actually get rows
+      const double t = syrk_makespan(ntiles - ntm, ntm, diag_cost, k, rps, h->num_sms) * (1.0 + 0.002 * k);
+      if (t < best) { best = t; ksplit = k; }
+    }
+    h->ks_cache_nblk = nblk; h->ks_cache_ntiles = ntiles; h->ks_cache_val = ksplit;
+  }
+  if (ksplit > h->ksplit) ksplit = h->ksplit;
+  if (ksplit > nblk) ksplit = nblk;
+  return ksplit < 1 ? 1 : ksplit;
+}
+
 // Aux-block scheduler: cap the X workspace, pick the split-K factor, enqueue
 // half-transform and SYRK block after block on one stream.  No allocation, no host sync.
 // With want_rho the half-transform also produces rho (step a2 fused): the
@@ -849,22 +871,7 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
   }
   const double diag_cost = (wm_s + 1) / (2.0 * wm_s);
   const int ntm = cdiv(nao, 16 * wm_s), ntiles = ntm * (ntm + 1) / 2;
-  int ksplit = h->ksplit_forced;
-  if (ksplit <= 0) {
-    // one SYRK CTA per SM; pick the split with the shortest modelled makespan, fewer splits on ties
-    const int nb0 = (int)nblk;
-    double best = 1e300;
-    ksplit = 1;
-    for (int k = 1; k <= h->ksplit && k <= nb0; k++) {
-      const int rps = cdiv(nb0, k), kk = cdiv(nb0, rps);          // splits that actually get rows
-      if (kk != k) continue;
-      const double t = syrk_makespan(ntiles - ntm, ntm, diag_cost, k, rps, h->num_sms) * (1.0 + 0.002 * k);
-      if (t < best) { best = t; ksplit = k; }
-    }
-  }
-  if (ksplit > h->ksplit) ksplit = h->ksplit;
-  if (ksplit > nblk) ksplit = (int)nblk;
-  if (ksplit < 1) ksplit = 1;
+  const int ksplit = pick_ksplit(h, (int)nblk, ntiles, ntm, diag_cost);
   const size_t split_stride = (size_t)h->max_nset * n2;
 
   int nblocks = 0;
@@ -983,19 +990,7 @@ int launch_k_path_dm(dfjk_ctx* h, int nset, const double* D, double* K_out, cuda
   }
   const double diag_cost = (wm_s + 1) / (2.0 * wm_s);
   const int ntm = cdiv(nao, 16 * wm_s), ntiles = ntm * (ntm + 1) / 2;
-  int ksplit = h->ksplit_forced;
-  if (ksplit <= 0) {
-    double best = 1e300;
-    ksplit = 1;
-    for (int k = 1; k <= h->ksplit && k <= nblk; k++) {
-      const int rps = cdiv((int)nblk, k);
-      if (cdiv((int)nblk, rps) != k) continue;
-      const double t = syrk_makespan(ntiles - ntm, ntm, diag_cost, k, rps, h->num_sms) * (1.0 + 0.002 * k);
-      if (t < best) { best = t; ksplit = k; }
-    }
-  }
-  if (ksplit > h->ksplit) ksplit = h->ksplit;
-  if (ksplit > nblk) ksplit = (int)nblk;
+  const int ksplit = pick_ksplit(h, (int)nblk, ntiles, ntm, diag_cost);
   const size_t split_stride = (size_t)h->max_nset * n2;
   const int nb32 = cdiv(nao, 32);
   for (int s = 0; s < nset; s++) {
