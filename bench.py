@@ -230,6 +230,7 @@ def main():
                     help="with --gpus N > 1: shard the aux rows over the ranks and sum-all-reduce J, K (strong scaling) "
                          "instead of N independent replicas")
     ap.add_argument("--no-small-calls", action="store_true", help="skip the small-call (CUDA graph) section")
+    ap.add_argument("--no-dm-form", action="store_true", help="skip the density-matrix-form (Eq. 16-17 as printed) section")
     ap.add_argument("--no-ao2mo", action="store_true", help="skip the AO2MO (Eq. 18-21) section")
     ap.add_argument("--workspace-gib", type=float, default=0.0, help="dfjk_options.workspace_cap_bytes (0 = default)")
     args = ap.parse_args()
@@ -365,6 +366,30 @@ def main():
               "frac_of_fp64_peak": ao_flops / (ms_ao * 1e-3) * 1e-12 / FP64_DMMA_PEAK_TFLOPS,
               "flops_note": "algorithmic_flops / tflops count Eq. 18 + Eq. 19 (full square) + Eq. 20 + Eq. 21 as printed; "
                             "executed_* count what the chosen route really computes"}
+    # ---- the density-matrix form (Eq. 14-17 exactly as printed) on the first set's
+    # density D = C n C^T, checked against the C-form result of the same density
+    dmf = None
+    if not args.no_dm_form and not shard:
+        n0 = nocc[0]
+        C0 = C_dev[: nao * n0].view(nao, n0)
+        D_dev = ((C0 * occ_dev[:n0]) @ C0.T).contiguous()[None]      # input construction only
+        Jd = torch.empty((1, nao, nao), dtype=torch.float64, device="cuda")
+        Kd = torch.empty_like(Jd)
+        dm_fn = lambda: h.get_jk_dm(D_dev, out_j=Jd, out_k=Kd, stream=stream)
+        dm_fn()
+        torch.cuda.synchronize()
+        dm_launches = h.last_launch_count
+        ms_dm = max_over_ranks(timed(dm_fn, 2))
+        full()
+        torch.cuda.synchronize()
+        dm_flops = 2.0 * naux * nao * nao * nao + 1.0 * naux * nao * (nao + 1) * nao
+        dmf = {"ms": ms_dm, "launches_per_call": dm_launches, "algorithmic_flops": dm_flops,
+               "tflops": dm_flops / (ms_dm * 1e-3) * 1e-12,
+               "frac_of_fp64_peak": dm_flops / (ms_dm * 1e-3) * 1e-12 / FP64_DMMA_PEAK_TFLOPS,
+               "max_rel_diff_vs_c_form_J": float((Jd[0] - J[0]).abs().max() / J[0].abs().max()),
+               "max_rel_diff_vs_c_form_K": float((Kd[0] - K[0]).abs().max() / K[0].abs().max()),
+               "flops_note": "Eq. 16 (2 naux nao^3) + Eq. 17 on the lower triangle (naux nao^2 (nao+1))"}
+        del D_dev, Jd, Kd
     # ---- the many-small-calls regime of the embedded fragments:
     # the `small` config called directly and as a replayed CUDA graph (dfjk_get_jk only enqueues)
     small = None
@@ -452,6 +477,8 @@ def main():
 
     if small is not None:
         line["small_calls"] = small
+    if dmf is not None:
+        line["dm_form"] = dmf
     if ao is not None:
         line["ao2mo"] = ao
         if Bh is not None and not args.no_parity:
