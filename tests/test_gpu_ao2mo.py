@@ -109,3 +109,9 @@ def test_route_follows_the_flop_model():
             o_bpa, o_ppaa, o_papa = oracle.ao2mo(inp.B_packed, 64, M, a0, nact)
             assert rel(bpa.cpu().numpy(), o_bpa) <= TOL
             assert rel(ppaa.cpu().numpy(), o_ppaa) <= TOL and rel(papa.cpu().numpy(), o_papa) <= TOL
+
+
+@pytest.mark.parametrize("route", [1, 2])
+def test_more_mo_columns_than_one_n_tile(route):
+    """nmo = 380 > 352: Eq. 18 (route 1) needs two N tiles of the half-transform; k_gemm_tn two N tiles"""
+    run_case(400, 9, 380, 100, 4, 261, L=40.0, ao2mo_route=route)

@@ -39,6 +39,7 @@ def oracle_j_of_dm(Bp, nao, D):
     (130, 40, 1, 303, {}),                        # one row past a 128 boundary, several N passes impossible here
     (150, 33, 3, 304, dict(nblk=7)),              # several aux blocks, three sets
     (200, 21, 1, 305, dict(ksplit=3)),
+    (400, 8, 1, 306, {}),                         # 400 columns: two N passes of the half-transform
 ])
 def test_density_matrix_form(nao, naux, nset, seed, opts):
     import torch
