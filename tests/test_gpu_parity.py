@@ -81,6 +81,7 @@ def test_small_config(torch_cuda, dfjk):
     (257, 33, [64], 107),        # three m-tiles: direct, crossing and transposed chunks all occur
     (48, 1, [12], 108),          # single aux row
     (330, 20, [40, 9], 161),     # 3 x 112: the 112 x 112 SYRK tile
+    (1203, 3, [35, 8], 164),     # large ragged basis: 19 row blocks, the last with 51 rows; 16 x 16 SYRK tiles
     (420, 14, [400], 162),       # 400 columns: two N tiles of the half-transform (fused rho over both)
     (400, 10, [180, 150, 60], 163),   # 392 padded columns in two N tiles, a set straddling them
 ])
