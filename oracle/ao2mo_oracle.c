@@ -166,3 +166,68 @@ int dfjk_oracle_ao2mo_bruteforce(int naux, int nao, int nmo, int a0, int nact, c
   free(g); free(Bsq);
   return DFJK_ORACLE_OK;
 }
+
+/*
+ * Single elements of Eq. 20 and Eq. 21 straight from the definitions, for parity at sizes where
+ * the full outputs (nmo^2 nact^2 entries over naux slices) are too slow to form on the host:
+ *   bmo^P[p][q] = sum_{e1} sum_{e2} M[e1][p] b^P[e1][e2] M[e2][q]                      (Eq. 18-19)
+ *   ppaa_v[t] = sum_P bmo^P[p1][p2] bmo^P[a0+a1][a0+a2]   at (p1,p2,a1,a2) = sample t   (Eq. 20)
+ *   papa_v[t] = sum_P bmo^P[p1][a0+a1] bmo^P[p2][a0+a2]   at (p1,a1,p2,a2) = the same four numbers
+ *               read in papa's index order                                             (Eq. 21)
+ * i.e. sample t = (p1, p2, a1, a2) addresses ppaa[p1][p2][a1][a2] and papa[p1][a1][p2][a2].
+ * The packed triangle is read in place (no unpack), e1 and e2 ascending, then P ascending.
+ * OpenMP splits the aux slices; the per-slice terms are summed afterwards in ascending P.
+ * Pinned against dfjk_oracle_ao2mo at small sizes (tests/test_ao2mo_oracle_pins.py).
+ */
+static double packed_at(const double* BpP, int e1, int e2) {
+  return e1 >= e2 ? BpP[(size_t)e1 * (e1 + 1) / 2 + e2] : BpP[(size_t)e2 * (e2 + 1) / 2 + e1];
+}
+
+static double bmo_at(int nao, int nmo, const double* M, const double* BpP, int p, int q) {
+  double s = 0.0;
+  for (int e1 = 0; e1 < nao; e1++) {
+    double y = 0.0;
+    for (int e2 = 0; e2 < nao; e2++) y += packed_at(BpP, e1, e2) * M[(size_t)e2 * nmo + q];
+    s += M[(size_t)e1 * nmo + p] * y;
+  }
+  return s;
+}
+
+int dfjk_oracle_ao2mo_sample(int naux, int nao, int nmo, int a0, int nact, const double* M, const double* Bp,
+                             int nsample, const int* sp1, const int* sp2, const int* sa1, const int* sa2,
+                             double* ppaa_v, double* papa_v) {
+  if (naux < 0 || nao < 1 || nmo < 1 || nact < 1 || a0 < 0 || a0 + nact > nmo || nsample < 0 || !M || !Bp)
+    return DFJK_ORACLE_ERR_ARG;
+  for (int t = 0; t < nsample; t++)
+    if (sp1[t] < 0 || sp1[t] >= nmo || sp2[t] < 0 || sp2[t] >= nmo || sa1[t] < 0 || sa1[t] >= nact ||
+        sa2[t] < 0 || sa2[t] >= nact)
+      return DFJK_ORACLE_ERR_ARG;
+  const size_t npair = (size_t)nao * (nao + 1) / 2;
+  const size_t nterm = (size_t)(nsample > 0 ? nsample : 1) * (size_t)(naux > 0 ? naux : 1);
+  double* t20 = (double*)malloc(nterm * sizeof(double));
+  double* t21 = (double*)malloc(nterm * sizeof(double));
+  if (!t20 || !t21) {
+    free(t20); free(t21);
+    return DFJK_ORACLE_ERR_ALLOC;
+  }
+#pragma omp parallel for schedule(dynamic)
+  for (int P = 0; P < naux; P++) {
+    const double* BpP = Bp + (size_t)P * npair;
+    for (int t = 0; t < nsample; t++) {
+      const int p1 = sp1[t], p2 = sp2[t], a1 = a0 + sa1[t], a2 = a0 + sa2[t];
+      if (ppaa_v) t20[(size_t)t * naux + P] = bmo_at(nao, nmo, M, BpP, p1, p2) * bmo_at(nao, nmo, M, BpP, a1, a2);
+      if (papa_v) t21[(size_t)t * naux + P] = bmo_at(nao, nmo, M, BpP, p1, a1) * bmo_at(nao, nmo, M, BpP, p2, a2);
+    }
+  }
+  for (int t = 0; t < nsample; t++) {
+    double s20 = 0.0, s21 = 0.0;
+    for (int P = 0; P < naux; P++) {
+      if (ppaa_v) s20 += t20[(size_t)t * naux + P];
+      if (papa_v) s21 += t21[(size_t)t * naux + P];
+    }
+    if (ppaa_v) ppaa_v[t] = s20;
+    if (papa_v) papa_v[t] = s21;
+  }
+  free(t20); free(t21);
+  return DFJK_ORACLE_OK;
+}

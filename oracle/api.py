@@ -38,6 +38,8 @@ def _load():
         lib.dfjk_oracle_ao2mo.restype = ct.c_int
         lib.dfjk_oracle_ao2mo_bruteforce.argtypes = [ct.c_int] * 5 + [_dp] * 4
         lib.dfjk_oracle_ao2mo_bruteforce.restype = ct.c_int
+        lib.dfjk_oracle_ao2mo_sample.argtypes = [ct.c_int] * 5 + [_dp, _dp, ct.c_int] + [_ip] * 4 + [_dp, _dp]
+        lib.dfjk_oracle_ao2mo_sample.restype = ct.c_int
         _lib = lib
     return _lib
 
@@ -177,3 +179,21 @@ def ao2mo_bruteforce(B_packed: np.ndarray, nao: int, M: np.ndarray, a0: int, nac
     if rc != 0:
         raise RuntimeError(f"dfjk_oracle_ao2mo_bruteforce failed with code {rc}")
     return ppaa, papa
+
+
+def ao2mo_sample(B_packed: np.ndarray, nao: int, M: np.ndarray, a0: int, nact: int,
+                 samples: Sequence[Tuple[int, int, int, int]]):
+    """(ppaa[p1][p2][a1][a2], papa[p1][a1][p2][a2]) at the listed (p1, p2, a1, a2), each element from
+    the definitions Eq. 18-21 (plain loops over the packed triangle)."""
+    B, M = _f64(B_packed), _f64(M)
+    nmo = M.shape[1]
+    assert M.shape[0] == nao and B.shape[1] == nao * (nao + 1) // 2
+    sm = np.ascontiguousarray(np.asarray(samples, dtype=np.int32).reshape(-1, 4))
+    cols = [np.ascontiguousarray(sm[:, k]) for k in range(4)]
+    n = sm.shape[0]
+    v20, v21 = np.empty(max(n, 1)), np.empty(max(n, 1))
+    rc = _load().dfjk_oracle_ao2mo_sample(B.shape[0], nao, nmo, a0, nact, _d(M), _d(B if B.size else np.zeros(1)), n,
+                                          _i(cols[0]), _i(cols[1]), _i(cols[2]), _i(cols[3]), _d(v20), _d(v21))
+    if rc != 0:
+        raise RuntimeError(f"dfjk_oracle_ao2mo_sample failed with code {rc}")
+    return v20[:n], v21[:n]

@@ -1,6 +1,6 @@
 """Build and run the calibration microbenchmarks on cuda:0; prints their tables to stdout.
 
-    python -m paper_2505_03755_b200.calib [peaks] [dmma_loop] [pipeline] [matmul]
+    python -m paper_2505_03755_b200.calib [peaks] [matmul]
 """
 from __future__ import annotations
 
@@ -9,7 +9,7 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-PROGRAMS = ["peaks", "dmma_loop", "pipeline"]
+PROGRAMS = ["peaks"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17"]
 
 

@@ -124,3 +124,29 @@ def test_edge_shapes():
     assert not ppaa.any() and not papa.any()
     with pytest.raises(RuntimeError):
         oracle.ao2mo(Bp, 6, M, 4, 2)                                        # active range past nmo
+
+
+def test_element_sampler_against_the_full_oracle_and_the_brute_force():
+    """dfjk_oracle_ao2mo_sample (single elements of Eq. 20-21 from the definitions, used for parity at
+    bench size) against the full oracle at a ragged small size (every element of both outputs), and
+    against the direct 4-index transformation of the Eq. 12 tensor at a tiny size.  A wrong index
+    order between ppaa[p1][p2][a1][a2] and papa[p1][a1][p2][a2] fails: the case is non-symmetric
+    in all four indices (non-orthonormal M, a0 > 0, nact < nmo)."""
+    nao, naux, nmo, a0, nact = 19, 11, 9, 2, 3
+    Bp, M = make(nao, naux, nmo, 91, L=5.0)
+    _, ppaa, papa = oracle.ao2mo(Bp, nao, M, a0, nact)
+    samples = [(p1, p2, a1, a2) for p1 in range(nmo) for p2 in range(nmo) for a1 in range(nact) for a2 in range(nact)]
+    v20, v21 = oracle.ao2mo_sample(Bp, nao, M, a0, nact, samples)
+    assert relerr(v20.reshape(nmo, nmo, nact, nact), ppaa) < 1e-13
+    assert relerr(v21.reshape(nmo, nmo, nact, nact).transpose(0, 2, 1, 3), papa) < 1e-13
+    assert relerr(ppaa, papa.transpose(0, 2, 1, 3)) > 1e-2          # the two outputs really differ
+    nao, naux, nmo, a0, nact = 7, 5, 6, 1, 4
+    Bp, M = make(nao, naux, nmo, 92)
+    b20, b21 = oracle.ao2mo_bruteforce(Bp, nao, M, a0, nact)
+    samples = [(5, 0, 3, 1), (0, 5, 1, 3), (2, 2, 0, 0), (4, 1, 2, 3)]
+    v20, v21 = oracle.ao2mo_sample(Bp, nao, M, a0, nact, samples)
+    for t, (p1, p2, a1, a2) in enumerate(samples):
+        assert abs(v20[t] - b20[p1, p2, a1, a2]) < 1e-12 * np.abs(b20).max()
+        assert abs(v21[t] - b21[p1, a1, p2, a2]) < 1e-12 * np.abs(b21).max()
+    with pytest.raises(RuntimeError):
+        oracle.ao2mo_sample(Bp, nao, M, a0, nact, [(0, 0, nact, 0)])        # active index out of range

@@ -204,11 +204,27 @@ def test_batched_sets_equal_one_at_a_time_and_empty_set():
     assert np.array_equal(Jo, J) and np.array_equal(Ko, K)
 
 
-def test_thread_count_does_not_change_bits(tiny_inputs):
-    """OpenMP splits output rows only, so a sub-range of aux rows sums in the same order."""
-    J, K = oracle.get_jk_inputs(tiny_inputs)
-    J2, K2 = oracle.get_jk_inputs(tiny_inputs)
-    assert np.array_equal(J, J2) and np.array_equal(K, K2)
+def test_thread_count_does_not_change_bits():
+    """OpenMP splits output rows only, so every output element is summed in the same order whatever
+    the thread count: the oracle run with 1 thread and with 4 threads (separate processes, the
+    runtime reads OMP_NUM_THREADS at start-up) gives bit-identical J, K and rho."""
+    import hashlib
+    import subprocess
+    import sys
+    code = ("import sys, hashlib; sys.path.insert(0, %r); import dfjk_inputs, oracle; "
+            "inp = dfjk_inputs.make_random(67, 45, [23, 7], 45, L=9.0); "
+            "J, K, rho = oracle.get_jk_inputs(inp, with_rho=True); "
+            "print(oracle.num_threads(), hashlib.sha256(J.tobytes() + K.tobytes() + rho.tobytes()).hexdigest())"
+            % os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    got = {}
+    for nt in (1, 4):
+        env = dict(os.environ, OMP_NUM_THREADS=str(nt), OMP_DYNAMIC="false")
+        out = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=300)
+        assert out.returncode == 0, out.stderr[-2000:]
+        threads, digest = out.stdout.split()
+        assert int(threads) == nt                              # the runs really differ in thread count
+        got[nt] = digest
+    assert got[1] == got[4]
 
 
 # ---------------------------------------------------------------- library third opinion
