@@ -208,8 +208,8 @@ def run_reference(args, cfg, name):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_full, "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": name, "nao": nao, "naux": naux, "nocc": cfg["nocc"], "sample": sample},
-        "cpu_baseline": {"value": ms_full, "unit": "ms", "cores": oracle.num_threads(), "kind": "oracle",
-                         "sample": sample},
+        "cpu_baseline": {"value": ms_full, "unit": "ms", "cores": oracle.num_threads(),
+                         "kind": f"oracle, extrapolated from {R} of {naux} aux rows", "sample": sample},
         "e2e": {"value": ms_full, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -307,18 +307,21 @@ def main():
     phases = {p: [0.0, 0] for p in dfjk.api.PHASES}
     launches = 0
     clocks = ClockSampler(local)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    marks = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     barrier()
-    e0.record(stream)
-    for _ in range(args.steps):
+    marks[0].record(stream)
+    for i in range(args.steps):
         full()
+        marks[i + 1].record(stream)
         launches += h.last_launch_count
         for p, (ms, n) in h.profile().items():     # waits for this step's last event only
             phases[p][0] += ms
             phases[p][1] += n
-    e1.record(stream)
     barrier()
-    ms_step = max_over_ranks(e0.elapsed_time(e1) / args.steps)
+    ms_step = max_over_ranks(marks[0].elapsed_time(marks[-1]) / args.steps)     # mean over exactly K steps
+    per_step = [marks[i].elapsed_time(marks[i + 1]) for i in range(args.steps)]
+    ms_median = max_over_ranks(float(np.median(per_step)))
+    ms_best = max_over_ranks(float(min(per_step)))
     clk = clocks.stop()
     h.set_profiling(False)
     plan = h.plan()
@@ -338,6 +341,19 @@ def main():
     j_only(); k_only()
     ms_j = max_over_ranks(timed(j_only, nrep))
     ms_k = max_over_ranks(timed(k_only, nrep))
+    h.set_profiling(True)                       # phases of the two-pass J (the fused call has no pass 1)
+    j_only()
+    jprof = h.profile()
+    h.set_profiling(False)
+    j1_only_ms, j2_only_ms = jprof["j1"][0], jprof["j2"][0]
+    # ---- signed occupations (differences of densities): the same call with every
+    # third occupation negated must cost what the unsigned call costs
+    occ_signed = occ_dev.clone()
+    occ_signed[::3] *= -1.0
+    signed = lambda: h.get_jk_raw(nocc, C_dev, occ_signed, out_j=J, out_k=K, stream=stream)
+    signed()
+    ms_signed = max_over_ranks(timed(signed, nrep))
+    ms_unsigned = max_over_ranks(timed(full, nrep)) if not shard else ms_step
 
     # ---- AO2MO (Eq. 18-21) on the same resident B: an embedding-sized MO set
     ao = None
@@ -362,10 +378,11 @@ def main():
         ao = {"ms": ms_ao, "nmo": nmo, "a0": a0, "nact": nact, "launches_per_call": ao_launches,
               "route": {1: "Eq. 18-21 in the printed order", 2: "active first (bmo never formed)"}.get(ao_route, "?"),
               "executed_flops": ao_exec, "executed_tflops": ao_exec / (ms_ao * 1e-3) * 1e-12,
-              "algorithmic_flops": ao_flops, "tflops": ao_flops / (ms_ao * 1e-3) * 1e-12,
-              "frac_of_fp64_peak": ao_flops / (ms_ao * 1e-3) * 1e-12 / FP64_DMMA_PEAK_TFLOPS,
-              "flops_note": "algorithmic_flops / tflops count Eq. 18 + Eq. 19 (full square) + Eq. 20 + Eq. 21 as printed; "
-                            "executed_* count what the chosen route really computes"}
+              "frac_of_fp64_peak": ao_exec / (ms_ao * 1e-3) * 1e-12 / FP64_DMMA_PEAK_TFLOPS,
+              "algorithmic_flops_as_printed": ao_flops,
+              "flops_note": "executed_* (and the fraction) count what the chosen route really computes; "
+                            "algorithmic_flops_as_printed counts Eq. 18 + Eq. 19 (full square) + Eq. 20 + Eq. 21 in the "
+                            "printed order, which the active-first route avoids"}
     # ---- the density-matrix form (Eq. 14-17 exactly as printed) on the first set's
     # density D = C n C^T, checked against the C-form result of the same density
     dmf = None
@@ -435,10 +452,10 @@ def main():
     sy_ms, sy_n = phases["syrk"]
     ht_tflops = fb["ht"] * args.steps / (ht_ms * 1e-3) * 1e-12 if ht_ms > 0 else 0.0
     sy_tflops = fb["syrk"] * args.steps / (sy_ms * 1e-3) * 1e-12 if sy_ms > 0 else 0.0
-    j1_ms, j2_ms = phases["j1"][0] / args.steps, phases["j2"][0] / args.steps
     line = {
         "metric": METRIC, "value": ms_step, "unit": "ms", "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": False,
+        "warmup": args.warmup, "ms_per_step": ms_step, "ms_per_step_median": ms_median, "ms_per_step_best": ms_best,
+        "higher_is_better": False,
         "scaling": "strong" if shard else "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": name, "nao": nao, "naux": naux, "nset": nset, "nocc": nocc,
@@ -469,9 +486,12 @@ def main():
         "j_pass": {"ms": ms_j, "gbs": fb["j_bytes"] / (ms_j * 1e-3) * 1e-9,
                    "frac_of_measured_hbm": fb["j_bytes"] / (ms_j * 1e-3) * 1e-9 / pk["hbm_gbs"],
                    "frac_of_8TBs": fb["j_bytes"] / (ms_j * 1e-3) * 1e-9 / 8000.0,
-                   "pass1_gbs": fb["b_bytes"] / (j1_ms * 1e-3) * 1e-9 if j1_ms > 0 else None,
-                   "pass2_gbs": fb["b_bytes"] / (j2_ms * 1e-3) * 1e-9 if j2_ms > 0 else None,
+                   "pass1_gbs": fb["b_bytes"] / (j1_only_ms * 1e-3) * 1e-9 if j1_only_ms > 0 else None,
+                   "pass2_gbs": fb["b_bytes"] / (j2_only_ms * 1e-3) * 1e-9 if j2_only_ms > 0 else None,
+                   "pass_note": "per-pass GB/s from the event profile of one J-only (two-pass) call",
                    "algorithmic_bytes": fb["j_bytes"], "hbm_peak_source": pk["source"]},
+        "signed_occ": {"ms": ms_signed, "ms_unsigned": ms_unsigned, "ratio": ms_signed / ms_unsigned,
+                       "note": "same call with every third occupation negated (C' = C sqrt|occ|, sign-bit flip in the SYRK)"},
         "phases_ms_per_step": {p: v[0] / args.steps for p, v in phases.items()},
     }
 
@@ -483,14 +503,22 @@ def main():
         line["ao2mo"] = ao
         if Bh is not None and not args.no_parity:
             import oracle
-            bpa, _, _ = h.ao2mo(M_dev, ao["a0"], ao["nact"], with_ppaa=False, with_papa=False, stream=stream)
+            bpa, ppaa, papa = h.ao2mo(M_dev, ao["a0"], ao["nact"], stream=stream)
             torch.cuda.synchronize()
             rows = [0, naux - 1]
             o_bpa, _, _ = oracle.ao2mo(Bh[rows], nao, M_host, ao["a0"], ao["nact"])
             g_bpa = bpa[rows].cpu().numpy()
-            ao["parity"] = {"kind": "oracle.ao2mo bpa of aux rows 0 and naux-1 (Eq. 18-19), every element",
-                            "max_rel_err": float(np.abs(g_bpa - o_bpa).max() / np.abs(o_bpa).max()), "tolerance": 1e-10}
-            del bpa
+            nm, na = ao["nmo"], ao["nact"]
+            smp = [(0, 0, 0, 0), (nm - 1, nm // 2, na - 1, 0), (nm // 3, nm - 1, na // 2, na - 1), (ao["a0"], 1, 1, 1)]
+            v20, v21 = oracle.ao2mo_sample(Bh, nao, M_host, ao["a0"], na, smp)
+            s20, s21 = float(ppaa.abs().max()), float(papa.abs().max())
+            e20 = max(abs(float(ppaa[p1, p2, a1, a2]) - v20[t]) / s20 for t, (p1, p2, a1, a2) in enumerate(smp))
+            e21 = max(abs(float(papa[p1, a1, p2, a2]) - v21[t]) / s21 for t, (p1, p2, a1, a2) in enumerate(smp))
+            ao["parity"] = {"kind": "oracle.ao2mo bpa of aux rows 0 and naux-1 (Eq. 18-19), every element; "
+                                    "oracle.ao2mo_sample on %d elements of ppaa and papa (Eq. 20-21)" % len(smp),
+                            "max_rel_err": float(np.abs(g_bpa - o_bpa).max() / np.abs(o_bpa).max()),
+                            "max_rel_err_ppaa": float(e20), "max_rel_err_papa": float(e21), "tolerance": 1e-10}
+            del bpa, ppaa, papa
     if Bh is not None and not args.no_parity:
         import oracle
         torch.cuda.synchronize()
@@ -509,7 +537,7 @@ def main():
         import oracle
         secs, R = oracle_sample_time(cfg, C_list, occ_list, Bh, args.cpu_seconds)
         line["cpu_baseline"] = {"value": secs * 1e3 * naux / R, "unit": "ms", "cores": oracle.num_threads(),
-                                "kind": "oracle",
+                                "kind": f"oracle, extrapolated from {R} of {naux} aux rows",
                                 "sample": f"first {R} of {naux} aux rows in {secs:.1f} s, scaled by {naux}/{R} "
                                           "(the oracle's cost is linear in aux rows)"}
     print(json.dumps(line), flush=True)

@@ -69,26 +69,33 @@ typedef struct {
 /*
  * dfjk_create -- bind a resident packed tensor and allocate every scratch buffer (step a0).
  *   naux, nao   sizes, naux >= 0, nao >= 1.
- *   B_packed    DEVICE pointer, naux * nao(nao+1)/2 doubles, 16-byte aligned.  Aux index P slowest,
- *               then the row-major lower triangle: B[P][mu(mu+1)/2 + nu], mu >= nu.
+ *   B_packed    DEVICE pointer, naux * nao(nao+1)/2 doubles, 8-byte aligned; 16-byte alignment (what
+ *               cudaMalloc and row slices of an even-npair tensor give) lets the J passes use bulk
+ *               copies and 128-bit loads, otherwise they fall back to scalar loads.  Aux index P
+ *               slowest, then the row-major lower triangle: B[P][mu(mu+1)/2 + nu], mu >= nu
+ *               (PAPER.md:152).  A contiguous range of aux rows of a larger tensor is a valid B: J and
+ *               K are sums over P, so handles on disjoint row ranges return partial results that add
+ *               up to the full ones (the aux-sharded mode).
  *               Borrowed unless opt->copy_B: it must stay valid and unchanged until dfjk_destroy.
  *   opt         options or NULL.
  *   out         receives the handle.
- * Allocates on the CURRENT device; may synchronise.  Returns DFJK_OK or an error code (then
- * *out = NULL).
+ * Allocates on the CURRENT device; may synchronise.  Every later call on the handle must be made
+ * with that device current (DFJK_ERR_INVALID_ARG otherwise); handles on different devices of one
+ * process are independent.  Returns DFJK_OK or an error code (then *out = NULL).
  */
 int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* opt, dfjk_handle* out);
 
 /*
  * dfjk_get_jk -- J and K of nset densities D_s = C_s diag(occ_s) C_s^T (steps a1-a9).
- *   nset     number of sets, 1 <= nset <= max_nset.
+ *   nset     number of sets, 1 <= nset <= max_nset (<= 32).  The J passes hold 8 sets per pass: more
+ *            than 8 sets stream B once per pass for every group of 8.
  *   nocc     HOST array, length nset; 0 <= nocc[s] <= nao, sum <= max_nocc_total.
  *            nocc[s] = 0 gives J_s = K_s = 0.
  *   C        DEVICE, blocks [C_0 | C_1 | ...] one after another; block s is row-major
  *            nao x nocc[s].  Columns need not be orthonormal.
- *   occ      DEVICE, concatenated occupations, length sum nocc[s]; must be >= 0: the kernels work
- *            with C' = C sqrt(occ), so a negative occupation yields NaN in J_s and K_s.  Densities
- *            with negative eigenvalues go through dfjk_get_jk_dm.
+ *   occ      DEVICE, concatenated occupations, length sum nocc[s]; any sign (differences of
+ *            densities): the kernels work with C' = C sqrt(|occ|) and carry
+ *            sign(occ) as a sign-bit flip, D = C' diag(sign occ) C'^T exactly, at the same cost.
  *   J_out    DEVICE, nset x nao x nao, or NULL to skip J.
  *   K_out    DEVICE, nset x nao x nao, or NULL to skip K.
  *   stream   all work is enqueued on this stream.
@@ -163,9 +170,11 @@ const char* dfjk_last_error(dfjk_handle h);
 /* Bytes of device scratch the handle owns (excluding a private copy of B). */
 size_t dfjk_workspace_bytes(dfjk_handle h);
 
-/* Plan of the last/next call, for tests and the bench: aux block size, number of aux blocks,
- * SYRK split-K factor, padded column count of X.  Any pointer may be NULL. */
-int dfjk_get_plan(dfjk_handle h, int* nblk, int* ksplit, int* nocc_pad_capacity);
+/* Plan of the last/next call, for tests and the bench: aux block size, SYRK split-K factor, padded
+ * column capacity of X, and whether the half-transform reads the re-tiled private copy of B
+ * (1) or gathers from the packed triangle (0: option no_retile, or the copy did not fit the
+ * device memory at create).  Any pointer may be NULL. */
+int dfjk_get_plan(dfjk_handle h, int* nblk, int* ksplit, int* nocc_pad_capacity, int* retiled);
 
 /* Number of kernel launches dfjk_get_jk enqueued in its last call on this handle. */
 int dfjk_last_launch_count(dfjk_handle h);
@@ -174,8 +183,9 @@ int dfjk_last_launch_count(dfjk_handle h);
  * Optional per-phase profile with CUDA events recorded on the launching stream (the paper used
  * wall-clock timers per stage and Nsight timelines).  Off by default.
  * dfjk_set_profiling(h, 1) makes every later dfjk_get_jk record an event at each phase boundary
- * (a few microseconds each).  dfjk_get_profile synchronises on the last event of the last call and
- * returns, per phase, the summed milliseconds and the number of kernel-launch groups.
+ * (a few microseconds each; the event pool grows with the number of aux blocks).
+ * dfjk_get_profile synchronises on the last event of the last call and returns, per phase, the
+ * summed milliseconds and the number of kernel-launch groups.
  */
 enum {
   DFJK_PHASE_PREP = 0,           /* a1: C' and packed weighted density */

@@ -63,7 +63,7 @@ def load_library():
     lib.dfjk_last_error.restype = ct.c_char_p
     lib.dfjk_workspace_bytes.argtypes = [vp]
     lib.dfjk_workspace_bytes.restype = ct.c_size_t
-    lib.dfjk_get_plan.argtypes = [vp, ip, ip, ip]
+    lib.dfjk_get_plan.argtypes = [vp, ip, ip, ip, ip]
     lib.dfjk_get_plan.restype = ct.c_int
     lib.dfjk_last_launch_count.argtypes = [vp]
     lib.dfjk_last_launch_count.restype = ct.c_int
@@ -138,9 +138,12 @@ class DFJK:
                out_j=None, out_k=None, stream=None):
         """J, K (nset, nao, nao) of D_s = C_s diag(occ_s) C_s^T; enqueue-only on `stream`."""
         import torch
-        nset = len(Cs)
-        nocc, C, occ = self._concat(Cs, occs, self.nao, self._device, torch)
-        return self.get_jk_raw(nocc, C, occ, with_j, with_k, out_j, out_k, stream)
+        with torch.cuda.device(self._device):
+            st = stream if stream is not None else torch.cuda.current_stream()
+            # the concatenated temporaries are produced, consumed and released on `st`
+            with torch.cuda.stream(st):
+                nocc, C, occ = self._concat(Cs, occs, self.nao, self._device, torch)
+                return self.get_jk_raw(nocc, C, occ, with_j, with_k, out_j, out_k, st)
 
     def get_jk_raw(self, nocc: List[int], C, occ, with_j=True, with_k=True, out_j=None, out_k=None, stream=None):
         """Same, with C/occ already concatenated on the device (no torch ops in the call path)."""
@@ -179,16 +182,17 @@ class DFJK:
         import torch
         if D.dim() != 3 or tuple(D.shape[1:]) != (self.nao, self.nao):
             raise ValueError(f"D must have shape (nset, {self.nao}, {self.nao})")
-        D = D.to(device=self._device, dtype=torch.float64).contiguous()
         nset = int(D.shape[0])
         with torch.cuda.device(self._device):
             st = stream if stream is not None else torch.cuda.current_stream()
-            J = out_j if out_j is not None else (torch.empty_like(D) if with_j else None)
-            K = out_k if out_k is not None else (torch.empty_like(D) if with_k else None)
-            code = self._lib.dfjk_get_jk_dm(self._h, nset, ct.c_void_p(D.data_ptr()),
-                                            ct.c_void_p(J.data_ptr() if J is not None else 0),
-                                            ct.c_void_p(K.data_ptr() if K is not None else 0),
-                                            ct.c_void_p(st.cuda_stream))
+            with torch.cuda.stream(st):            # a converted copy of D lives and dies on `st`
+                D = D.to(device=self._device, dtype=torch.float64).contiguous()
+                J = out_j if out_j is not None else (torch.empty_like(D) if with_j else None)
+                K = out_k if out_k is not None else (torch.empty_like(D) if with_k else None)
+                code = self._lib.dfjk_get_jk_dm(self._h, nset, ct.c_void_p(D.data_ptr()),
+                                                ct.c_void_p(J.data_ptr() if J is not None else 0),
+                                                ct.c_void_p(K.data_ptr() if K is not None else 0),
+                                                ct.c_void_p(st.cuda_stream))
         _check(self._lib, code, self._h)
         return J, K
 
@@ -198,26 +202,27 @@ class DFJK:
         import torch
         if tuple(M.shape[:1]) != (self.nao,) or M.dim() != 2:
             raise ValueError(f"M must have shape ({self.nao}, nmo)")
-        M = M.to(device=self._device, dtype=torch.float64).contiguous()
         nmo = int(M.shape[1])
         with torch.cuda.device(self._device):
             st = stream if stream is not None else torch.cuda.current_stream()
-            kw = dict(dtype=torch.float64, device=self._device)
-            bpa = torch.empty((self.naux, nmo, nact), **kw)
-            ppaa = torch.empty((nmo, nmo, nact, nact), **kw) if with_ppaa else None
-            papa = torch.empty((nmo, nact, nmo, nact), **kw) if with_papa else None
-            code = self._lib.dfjk_ao2mo(self._h, nmo, a0, nact, ct.c_void_p(M.data_ptr() if nmo else 0),
-                                        ct.c_void_p(bpa.data_ptr() if bpa.numel() else 0),
-                                        ct.c_void_p(ppaa.data_ptr() if ppaa is not None and ppaa.numel() else 0),
-                                        ct.c_void_p(papa.data_ptr() if papa is not None and papa.numel() else 0),
-                                        ct.c_void_p(st.cuda_stream))
+            with torch.cuda.stream(st):            # a converted copy of M lives and dies on `st`
+                M = M.to(device=self._device, dtype=torch.float64).contiguous()
+                kw = dict(dtype=torch.float64, device=self._device)
+                bpa = torch.empty((self.naux, nmo, nact), **kw)
+                ppaa = torch.empty((nmo, nmo, nact, nact), **kw) if with_ppaa else None
+                papa = torch.empty((nmo, nact, nmo, nact), **kw) if with_papa else None
+                code = self._lib.dfjk_ao2mo(self._h, nmo, a0, nact, ct.c_void_p(M.data_ptr() if nmo else 0),
+                                            ct.c_void_p(bpa.data_ptr() if bpa.numel() else 0),
+                                            ct.c_void_p(ppaa.data_ptr() if ppaa is not None and ppaa.numel() else 0),
+                                            ct.c_void_p(papa.data_ptr() if papa is not None and papa.numel() else 0),
+                                            ct.c_void_p(st.cuda_stream))
         _check(self._lib, code, self._h)
         return bpa, ppaa, papa
 
     def plan(self) -> dict:
-        a, b, c = ct.c_int(), ct.c_int(), ct.c_int()
-        _check(self._lib, self._lib.dfjk_get_plan(self._h, ct.byref(a), ct.byref(b), ct.byref(c)))
-        return dict(nblk=a.value, ksplit=b.value, nocc_pad_capacity=c.value)
+        a, b, c, d = ct.c_int(), ct.c_int(), ct.c_int(), ct.c_int()
+        _check(self._lib, self._lib.dfjk_get_plan(self._h, ct.byref(a), ct.byref(b), ct.byref(c), ct.byref(d)))
+        return dict(nblk=a.value, ksplit=b.value, nocc_pad_capacity=c.value, retiled=d.value)
 
     def set_profiling(self, on: bool) -> None:
         _check(self._lib, self._lib.dfjk_set_profiling(self._h, int(on)), self._h)

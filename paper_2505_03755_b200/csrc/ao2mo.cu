@@ -177,15 +177,12 @@ __global__ void k_zero_ao(double* p, size_t n) {
 }
 
 template <int WTM, int WTN>
-static cudaError_t launch_gemm_tn(const GemmTN& g, int batch, cudaStream_t st) {
+static cudaError_t launch_gemm_tn(int device, const GemmTN& g, int batch, cudaStream_t st) {
   constexpr int TM = 16 * WTM, TN = 32 * WTN;
   constexpr size_t smem = (size_t)kGStages * kGKC * (TM + 4 + TN + 4) * sizeof(double);
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_gemm_tn<WTM, WTN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  static std::atomic<unsigned long long> attr_done{0};
+  cudaError_t e = ensure_dyn_smem(k_gemm_tn<WTM, WTN>, smem, device, attr_done);
+  if (e != cudaSuccess) return e;
   if (g.M <= 0 || g.N <= 0 || batch <= 0) return cudaSuccess;
   dim3 grid(cdiv(g.M, TM), cdiv(g.N, TN), batch);
   k_gemm_tn<WTM, WTN><<<grid, kGThreads, smem, st>>>(g);
@@ -194,15 +191,15 @@ static cudaError_t launch_gemm_tn(const GemmTN& g, int batch, cudaStream_t st) {
 
 // CTA tile 64 x (32 WTN): the N tile is fitted to the problem (at most 352 columns per tile, the
 // fewest tiles that cover N, then the narrowest WTN that does), so that e.g. N = 340 pays 352.
-static cudaError_t gemm_tn(const GemmTN& g, int batch, cudaStream_t st) {
+static cudaError_t gemm_tn(int device, const GemmTN& g, int batch, cudaStream_t st) {
   const int n8 = cdiv(g.N > 0 ? g.N : 1, 8);
   const int ntn = cdiv(n8, 44), wtn = cdiv(n8, 4 * ntn);
   if (wtn <= 2 && g.M >= 128 * 148) {       // narrow and tall (W of the active-first route): 128-row tiles
-    return wtn == 1 ? launch_gemm_tn<8, 1>(g, batch, st) : launch_gemm_tn<8, 2>(g, batch, st);
+    return wtn == 1 ? launch_gemm_tn<8, 1>(device, g, batch, st) : launch_gemm_tn<8, 2>(device, g, batch, st);
   }
   switch (wtn) {
 #define DFJK_GEMM_CASE(N) \
-  case N: return launch_gemm_tn<4, N>(g, batch, st);
+  case N: return launch_gemm_tn<4, N>(device, g, batch, st);
     DFJK_GEMM_CASE(1) DFJK_GEMM_CASE(2) DFJK_GEMM_CASE(3) DFJK_GEMM_CASE(4) DFJK_GEMM_CASE(5) DFJK_GEMM_CASE(6)
     DFJK_GEMM_CASE(7) DFJK_GEMM_CASE(8) DFJK_GEMM_CASE(9) DFJK_GEMM_CASE(10) DFJK_GEMM_CASE(11)
 #undef DFJK_GEMM_CASE
@@ -256,7 +253,7 @@ static int launch_ao2mo_as_printed(dfjk_ctx* h, int nmo, int a0, int nact, const
     launches++;
     // Eq. 19 for the whole block as one GEMM: rows (P, p1) stacked along M, bmo[P][p1][p2] = C[(P p1)][p2]
     GemmTN g19{Xb, M, bmo, nb * nmo, nmo, nao, ldx, nmo, nmo, 0, 0, 0, 0, nmo, (long long)nao * ldx};
-    if (gemm_tn(g19, 1, st) != cudaSuccess) return -1;
+    if (gemm_tn(h->device, g19, 1, st) != cudaSuccess) return -1;
     launches++;
     if (nact > 0) {
       dim3 gg(cdiv((int)(npa + naa), 256) < 64 ? cdiv((int)(npa + naa), 256) : 64, nb);
@@ -265,7 +262,7 @@ static int launch_ao2mo_as_printed(dfjk_ctx* h, int nmo, int a0, int nact, const
       if (ppaa_out) {
         GemmTN g20{bmo, baa, ppaa_out, (int)n2, (int)naa, nb, (long long)n2, (long long)naa, (long long)naa,
                    0, 0, 0, p0 > 0 ? 1 : 0};
-        if (gemm_tn(g20, 1, st) != cudaSuccess) return -1;                                // Eq. 20
+        if (gemm_tn(h->device, g20, 1, st) != cudaSuccess) return -1;                                // Eq. 20
         launches++;
       }
     }
@@ -273,7 +270,7 @@ static int launch_ao2mo_as_printed(dfjk_ctx* h, int nmo, int a0, int nact, const
   if (papa_out && nact > 0) {
     GemmTN g21{bpa_out, bpa_out, papa_out, (int)npa, (int)npa, naux, (long long)npa, (long long)npa,
                (long long)npa, 0, 0, 0, 0};
-    if (gemm_tn(g21, 1, st) != cudaSuccess) return -1;                                    // Eq. 21
+    if (gemm_tn(h->device, g21, 1, st) != cudaSuccess) return -1;                                    // Eq. 21
     launches++;
   }
   return launches;
@@ -331,7 +328,7 @@ static int launch_ao2mo_active_first(dfjk_ctx* h, int nmo, int a0, int nact, con
     // C[(P a)][p] = sum_mu Z^P[mu][a] M[mu][p], stored transposed into bpa[P][p][a]
     GemmTN gb{Z, M, bpa_out + (size_t)p0 * npa, nb * nact, nmo, nao, ldz, nmo, 0, 0, 0, 0, 0,
               nact, (long long)nao * ldz, nact, (long long)npa, nact};
-    if (gemm_tn(gb, 1, st) != cudaSuccess) return -1;
+    if (gemm_tn(h->device, gb, 1, st) != cudaSuccess) return -1;
     launches += 2;
   }
   if (ppaa_out) {
@@ -340,19 +337,19 @@ static int launch_ao2mo_active_first(dfjk_ctx* h, int nmo, int a0, int nact, con
     double* T = Wsq + (size_t)nao * nao * naa;
     GemmTN gw{h->B, bpa_out + (size_t)a0 * nact, W, (int)h->npair, (int)naa, naux, (long long)h->npair,
               (long long)npa, (long long)naa, 0, 0, 0, 0};
-    if (gemm_tn(gw, 1, st) != cudaSuccess) return -1;                                      // W = sum_P b^P (x) baa^P
+    if (gemm_tn(h->device, gw, 1, st) != cudaSuccess) return -1;                                      // W = sum_P b^P (x) baa^P
     k_unpack_w<<<1184, 256, 0, st>>>(W, nao, (int)naa, Wsq);
     GemmTN gt{M, Wsq, T, nmo, (int)(nao * naa), nao, nmo, (long long)(nao * naa), (long long)(nao * naa), 0, 0, 0, 0};
-    if (gemm_tn(gt, 1, st) != cudaSuccess) return -1;                                      // T[p1][e2 a] = M^T W
+    if (gemm_tn(h->device, gt, 1, st) != cudaSuccess) return -1;                                      // T[p1][e2 a] = M^T W
     GemmTN gp{M, T, ppaa_out, nmo, (int)naa, nao, nmo, (long long)naa, (long long)naa, 0, (long long)(nao * naa),
               (long long)(nmo * naa), 0};
-    if (gemm_tn(gp, nmo, st) != cudaSuccess) return -1;                                    // ppaa[p1][p2][a] = T_p1^T M
+    if (gemm_tn(h->device, gp, nmo, st) != cudaSuccess) return -1;                                    // ppaa[p1][p2][a] = T_p1^T M
     launches += 4;
   }
   if (papa_out) {
     GemmTN g21{bpa_out, bpa_out, papa_out, (int)npa, (int)npa, naux, (long long)npa, (long long)npa,
                (long long)npa, 0, 0, 0, 0};
-    if (gemm_tn(g21, 1, st) != cudaSuccess) return -1;                                     // Eq. 21
+    if (gemm_tn(h->device, g21, 1, st) != cudaSuccess) return -1;                                     // Eq. 21
     launches++;
   }
   return launches;

@@ -30,7 +30,7 @@ bool dev_alloc(dfjk_ctx* h, T** p, size_t count) {
 }
 
 void free_all(dfjk_ctx* h) {
-  cudaFree(h->B_owned); cudaFree(h->Bt); cudaFree(h->Ct); cudaFree(h->Dw); cudaFree(h->rho_part); cudaFree(h->rho); cudaFree(h->rho_ht);
+  cudaFree(h->B_owned); cudaFree(h->Bt); cudaFree(h->Ct); cudaFree(h->sgnbits); cudaFree(h->Dw); cudaFree(h->rho_part); cudaFree(h->rho); cudaFree(h->rho_ht);
   cudaFree(h->Jp_part); cudaFree(h->X); cudaFree(h->Kpart);
   cudaFree(h->C_stage); cudaFree(h->occ_stage); cudaFree(h->J_stage); cudaFree(h->K_stage);
   for (int i = 0; i < h->ev_cap; i++) cudaEventDestroy(h->ev[i]);
@@ -60,7 +60,39 @@ int build_setinfo(const dfjk_ctx* h, int nset, const int* nocc, SetInfo* si) {
   return DFJK_OK;
 }
 
+// Every entry point that touches the device runs on the handle's device: the scratch, the
+// function attributes and the caller's stream all belong to it.
+bool on_handle_device(dfjk_ctx* h) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return false; }
+  if (dev != h->device) {
+    snprintf(h->last_error, sizeof(h->last_error), "current device %d is not the handle's device %d", dev, h->device);
+    return false;
+  }
+  return true;
+}
+
 }  // namespace
+
+namespace dfjk {
+// doubles the event pool of the phase profile; false if no more events can be had
+bool prof_grow(dfjk_ctx* h) {
+  const int cap = h->ev_cap > 0 ? 2 * h->ev_cap : 1024;
+  cudaEvent_t* ev = new (std::nothrow) cudaEvent_t[cap];
+  int* ph = new (std::nothrow) int[cap];
+  if (!ev || !ph) { delete[] ev; delete[] ph; return false; }
+  for (int i = 0; i < h->ev_cap; i++) { ev[i] = h->ev[i]; ph[i] = h->ev_phase[i]; }
+  int n = h->ev_cap;
+  for (; n < cap; n++)
+    if (cudaEventCreate(&ev[n]) != cudaSuccess) { cudaGetLastError(); break; }
+  delete[] h->ev;
+  delete[] h->ev_phase;
+  h->ev = ev; h->ev_phase = ph;
+  const bool grew = n > h->ev_cap;
+  h->ev_cap = n;
+  return grew;
+}
+}  // namespace dfjk
 
 extern "C" {
 
@@ -80,7 +112,7 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   *out = nullptr;
   if (naux < 0 || nao < 1 || nao > 32768) return DFJK_ERR_INVALID_ARG;
   if (naux > 0 && !B_packed) return DFJK_ERR_INVALID_ARG;
-  if (((uintptr_t)B_packed & 15u) != 0) return DFJK_ERR_INVALID_ARG;
+  if (((uintptr_t)B_packed & 7u) != 0) return DFJK_ERR_INVALID_ARG;
   dfjk_options o;
   memset(&o, 0, sizeof(o));
   if (opt) o = *opt;
@@ -158,6 +190,8 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   const size_t n2 = (size_t)nao * nao;
   bool ok = true;
   ok = ok && dev_alloc(h, &h->Ct, (size_t)h->nck * h->ct_rows * kHtLd);
+  ok = ok && dev_alloc(h, &h->sgnbits, (size_t)h->ct_rows / 32 + 2);
+  if (ok && cudaMemset(h->sgnbits, 0, ((size_t)h->ct_rows / 32 + 2) * sizeof(unsigned int)) != cudaSuccess) { cudaGetLastError(); ok = false; }
   ok = ok && dev_alloc(h, &h->Dw, (size_t)h->max_nset * h->npair);
   ok = ok && dev_alloc(h, &h->rho_part, (size_t)h->j1_chunks * 8 * naux_pad);
   ok = ok && dev_alloc(h, &h->rho, (size_t)h->max_nset * (naux > 0 ? naux : 1));
@@ -182,6 +216,7 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   }
   if (!ok) { free_all(h); delete h; return DFJK_ERR_ALLOC; }
   h->B = h->B_owned ? h->B_owned : B_packed;
+  h->b_aligned16 = ((uintptr_t)h->B & 15u) == 0;
   // re-tiled copy for the half-transform (1.35x the packed bytes): used if it can be had
   if (!o.no_retile && naux > 0) {
     h->bt_pstride = retile_doubles_per_aux_row(nao);
@@ -212,6 +247,7 @@ int dfjk_get_jk(dfjk_handle h, int nset, const int* nocc, const double* C, const
   h->last_launches = 0;
   h->last_error[0] = 0;
   h->ev_n = 0;
+  if (!on_handle_device(h)) return DFJK_ERR_INVALID_ARG;
   if (!J_out && !K_out) return DFJK_OK;
   int n = 0, k;
   n += launch_prep_ct(h, si, C, occ, st);
@@ -219,14 +255,20 @@ int dfjk_get_jk(dfjk_handle h, int nset, const int* nocc, const double* C, const
   const bool fuse = J_out && K_out && !h->two_pass_j && h->naux > 0 && si.nocc_pad > 0;
   if (J_out && !fuse) {
     n += launch_prep_dw(h, si, st);
-    n += launch_j_passes(h, si, J_out, false, st);
+    k = launch_j_passes(h, si, J_out, false, st);
+    if (k < 0) { set_err(h, "j pass launch", cudaGetLastError()); return DFJK_ERR_CUDA; }
+    n += k;
   }
   if (K_out) {
     k = launch_k_path(h, si, K_out, fuse, st);
     if (k < 0) { set_err(h, "k path launch", cudaGetLastError()); return DFJK_ERR_CUDA; }
     n += k;
   }
-  if (fuse) n += launch_j_passes(h, si, J_out, true, st);
+  if (fuse) {
+    k = launch_j_passes(h, si, J_out, true, st);
+    if (k < 0) { set_err(h, "j pass launch", cudaGetLastError()); return DFJK_ERR_CUDA; }
+    n += k;
+  }
   prof_mark(h, -1, st);
   h->last_launches = n;
   cudaError_t e = cudaGetLastError();
@@ -243,6 +285,7 @@ int dfjk_get_jk_host(dfjk_handle h, int nset, const int* nocc, const double* C, 
   size_t ntot = 0;
   for (int s = 0; s < nset; s++) ntot += (size_t)nocc[s];
   if (ntot > 0 && (!C || !occ)) return DFJK_ERR_INVALID_ARG;
+  if (!on_handle_device(h)) return DFJK_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   cudaError_t e = cudaSuccess;
   if (ntot > 0) {
@@ -268,6 +311,7 @@ int dfjk_get_jk_dm(dfjk_handle h, int nset, const double* D, double* J_out, doub
   h->last_launches = 0;
   h->last_error[0] = 0;
   h->ev_n = 0;
+  if (!on_handle_device(h)) return DFJK_ERR_INVALID_ARG;
   if (!J_out && !K_out) return DFJK_OK;
   int n = 0;
   if (J_out) {
@@ -275,7 +319,9 @@ int dfjk_get_jk_dm(dfjk_handle h, int nset, const double* D, double* J_out, doub
     memset(&si, 0, sizeof(si));
     si.nset = nset;
     n += launch_prep_dw_dm(h, nset, D, st);
-    n += launch_j_passes(h, si, J_out, false, st);
+    const int kj = launch_j_passes(h, si, J_out, false, st);
+    if (kj < 0) { set_err(h, "j pass launch", cudaGetLastError()); return DFJK_ERR_CUDA; }
+    n += kj;
   }
   if (K_out) {
     const int k = launch_k_path_dm(h, nset, D, K_out, st);
@@ -305,6 +351,7 @@ int dfjk_ao2mo(dfjk_handle h, int nmo, int a0, int nact, const double* M, double
   h->last_launches = 0;
   h->last_error[0] = 0;
   h->ev_n = 0;
+  if (!on_handle_device(h)) return DFJK_ERR_INVALID_ARG;
   const int n = launch_ao2mo(h, nmo, a0, nact, M, bpa_out, ppaa_out, papa_out, st);
   if (n == -2) { snprintf(h->last_error, sizeof(h->last_error), "workspace cap too small for one aux row of AO2MO"); return DFJK_ERR_INVALID_ARG; }
   if (n < 0) { set_err(h, "ao2mo launch", cudaGetLastError()); return DFJK_ERR_CUDA; }
@@ -325,11 +372,12 @@ const char* dfjk_last_error(dfjk_handle h) { return h ? h->last_error : ""; }
 
 size_t dfjk_workspace_bytes(dfjk_handle h) { return h ? h->workspace_bytes : 0; }
 
-int dfjk_get_plan(dfjk_handle h, int* nblk, int* ksplit, int* nocc_pad_capacity) {
+int dfjk_get_plan(dfjk_handle h, int* nblk, int* ksplit, int* nocc_pad_capacity, int* retiled) {
   if (!h) return DFJK_ERR_INVALID_ARG;
   if (nblk) *nblk = h->plan_nblk ? h->plan_nblk : h->nblk;
   if (ksplit) *ksplit = h->plan_ksplit ? h->plan_ksplit : h->ksplit;
   if (nocc_pad_capacity) *nocc_pad_capacity = h->nocc_pad_cap;
+  if (retiled) *retiled = h->Bt ? 1 : 0;
   return DFJK_OK;
 }
 
@@ -339,16 +387,7 @@ int dfjk_last_ao2mo_route(dfjk_handle h) { return h ? h->plan_ao2mo_route : 0; }
 
 int dfjk_set_profiling(dfjk_handle h, int on) {
   if (!h) return DFJK_ERR_INVALID_ARG;
-  if (on && !h->ev) {
-    const int cap = 8192;
-    h->ev = new (std::nothrow) cudaEvent_t[cap];
-    h->ev_phase = new (std::nothrow) int[cap];
-    if (!h->ev || !h->ev_phase) return DFJK_ERR_ALLOC;
-    for (int i = 0; i < cap; i++) {
-      if (cudaEventCreate(&h->ev[i]) != cudaSuccess) { cudaGetLastError(); return DFJK_ERR_CUDA; }
-      h->ev_cap = i + 1;
-    }
-  }
+  if (on && !h->ev && !prof_grow(h)) return DFJK_ERR_ALLOC;
   h->profiling = on ? 1 : 0;
   h->ev_n = 0;
   return DFJK_OK;

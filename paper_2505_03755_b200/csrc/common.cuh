@@ -24,6 +24,11 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
                : "d"(a), "d"(b));
 }
 
+// x with its sign bit flipped when m = 0x80000000 (m = 0: unchanged); an integer op on the high word
+__device__ __forceinline__ double flip_sign(double x, unsigned int m) {
+  return __hiloint2double(__double2hiint(x) ^ (int)m, __double2loint(x));
+}
+
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return (uint32_t)__cvta_generic_to_shared(p);
 }

@@ -3,6 +3,8 @@
 #include <cuda_runtime.h>
 #include <stddef.h>
 
+#include <atomic>
+
 #include "../../include/dfjk.h"
 
 namespace dfjk {
@@ -40,6 +42,7 @@ struct dfjk_ctx {
   int mu_pad;                // nao rounded up to 128 (row extent of the tiled X)
   int device;
   const double* B;           // packed tensor (borrowed or owned)
+  int b_aligned16;           // B is 16-byte aligned (8-byte aligned tensors take the scalar-load J paths)
   double* B_owned;
   double* Bt;                // optional re-tiled copy of B for the half-transform (HtParams)
   size_t bt_pstride;
@@ -58,6 +61,7 @@ struct dfjk_ctx {
   int two_pass_j;            // option: never fuse J pass 1 into the half-transform
   // scratch (all allocated at create)
   double* Ct;                // [nck][ct_rows][20]  C' transposed and k-tiled, sqrt(occ) folded, zero padded
+  unsigned int* sgnbits;     // [nocc_pad_cap / 32 + 1]   bit c%32 of word c/32 = 1 iff padded column c has occ < 0
   double* Dw;                // [max_nset][npair]         packed density, off-diagonal weight 2
   double* rho_part;          // [j1_chunks][8][naux_pad]
   double* rho;               // [max_nset][naux]
@@ -80,11 +84,26 @@ struct dfjk_ctx {
 
 namespace dfjk {
 
-// Phase marker of the event profile: the phase lasts until the next marker on the stream.
+// Phase marker of the event profile: the phase lasts until the next marker on the stream.  The
+// event pool grows on demand (host-side only; profiling is never on during a graph capture).
+bool prof_grow(dfjk_ctx* h);
 inline void prof_mark(dfjk_ctx* h, int phase, cudaStream_t st) {
-  if (!h->profiling || h->ev_n >= h->ev_cap) return;
+  if (!h->profiling) return;
+  if (h->ev_n >= h->ev_cap && !prof_grow(h)) return;
   cudaEventRecord(h->ev[h->ev_n], st);
   h->ev_phase[h->ev_n++] = phase;
+}
+
+// Opt-in to more than 48 KB of dynamic shared memory.  The attribute is per function AND per
+// device, so every launcher keeps one bit per device (a second handle on another GPU of the same
+// process sets it again); setting it twice is harmless, which makes the race between threads benign.
+template <typename F>
+inline cudaError_t ensure_dyn_smem(F* func, size_t bytes, int device, std::atomic<unsigned long long>& done) {
+  const unsigned long long bit = device >= 0 && device < 64 ? 1ull << device : 0ull;
+  if (bit && (done.load(std::memory_order_acquire) & bit)) return cudaSuccess;
+  cudaError_t e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+  if (e == cudaSuccess && bit) done.fetch_or(bit, std::memory_order_release);
+  return e;
 }
 
 // Each launcher enqueues on `st` and returns the number of kernels it launched.

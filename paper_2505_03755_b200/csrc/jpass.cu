@@ -213,24 +213,21 @@ k_j1_tma(const double* __restrict__ B, size_t npair, int naux, const double* __r
 }
 
 template <int NS>
-static cudaError_t launch_j1_tma(dim3 grid, cudaStream_t st, const double* B, size_t npair, int naux, const double* Dw,
-                                 double* part, int naux_pad) {
+static cudaError_t launch_j1_tma(int device, dim3 grid, cudaStream_t st, const double* B, size_t npair, int naux,
+                                 const double* Dw, double* part, int naux_pad) {
   constexpr size_t smem = (size_t)j1t_stages(NS) * (8 + NS) * kJ1tSC * sizeof(double);
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_j1_tma<NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  static std::atomic<unsigned long long> attr_done{0};
+  cudaError_t e = ensure_dyn_smem(k_j1_tma<NS>, smem, device, attr_done);
+  if (e != cudaSuccess) return e;
   k_j1_tma<NS><<<grid, kJ1tThreads, smem, st>>>(B, npair, naux, Dw, part, naux_pad);
   return cudaSuccess;
 }
 
-static cudaError_t dispatch_j1_tma(int ns, dim3 grid, cudaStream_t st, const double* B, size_t npair, int naux,
-                                   const double* Dw, double* part, int naux_pad) {
+static cudaError_t dispatch_j1_tma(int device, int ns, dim3 grid, cudaStream_t st, const double* B, size_t npair,
+                                   int naux, const double* Dw, double* part, int naux_pad) {
   switch (ns) {
 #define DFJK_J1T_CASE(N) \
-  case N: return launch_j1_tma<N>(grid, st, B, npair, naux, Dw, part, naux_pad);
+  case N: return launch_j1_tma<N>(device, grid, st, B, npair, naux, Dw, part, naux_pad);
     DFJK_J1T_CASE(1) DFJK_J1T_CASE(2) DFJK_J1T_CASE(3) DFJK_J1T_CASE(4)
     DFJK_J1T_CASE(5) DFJK_J1T_CASE(6) DFJK_J1T_CASE(7) DFJK_J1T_CASE(8)
 #undef DFJK_J1T_CASE
@@ -349,8 +346,8 @@ k_j_epilogue(const double* __restrict__ part, int nsplit, size_t split_stride, s
 }
 
 template <bool VEC>
-static void launch_j2(int ns, dim3 grid, cudaStream_t st, const double* B, size_t npair, int naux,
-                      const double* rho, double* part, size_t split_stride, int rows_per_split) {
+static cudaError_t launch_j2(int ns, dim3 grid, cudaStream_t st, const double* B, size_t npair, int naux,
+                             const double* rho, double* part, size_t split_stride, int rows_per_split) {
   switch (ns) {
 #define DFJK_J2_CASE(N)                                                                               \
   case N:                                                                                             \
@@ -359,34 +356,42 @@ static void launch_j2(int ns, dim3 grid, cudaStream_t st, const double* B, size_
     DFJK_J2_CASE(1) DFJK_J2_CASE(2) DFJK_J2_CASE(3) DFJK_J2_CASE(4)
     DFJK_J2_CASE(5) DFJK_J2_CASE(6) DFJK_J2_CASE(7) DFJK_J2_CASE(8)
 #undef DFJK_J2_CASE
-    default: break;
+    default: return cudaErrorInvalidValue;
   }
+  return cudaSuccess;
 }
 
 // rho_ready: rho was already produced by the fused half-transform; only pass 2 and the epilogue run.
+// More than 8 sets are processed in groups of 8 (the accumulators of one pass), each group
+// streaming B once per pass.  Returns the number of launches, -1 on a launch failure.
 int launch_j_passes(dfjk_ctx* h, const SetInfo& si, double* J_out, bool rho_ready, cudaStream_t st) {
   int launches = 0;
   const int naux = h->naux, nao = h->nao;
   const size_t npair = h->npair;
-  const bool vec = (npair % 2 == 0);
+  const bool vec = (npair % 2 == 0) && h->b_aligned16;   // 16-byte aligned packed rows: 128-bit loads, bulk copies
   const int naux_pad = round_up(naux > 0 ? naux : 1, kJ1Rows);
   const size_t split_stride = (size_t)h->max_nset * npair;
   const int rows_per_split = round_up(cdiv(naux > 0 ? naux : 1, h->j2_splits), 8);
-  for (int s0 = 0; s0 < si.nset; s0 += 8) {  // the MMA N dimension holds 8 sets per pass
+  for (int s0 = 0; s0 < si.nset; s0 += 8) {
     const int ns = si.nset - s0 < 8 ? si.nset - s0 : 8;
     if (naux > 0 && !rho_ready) {
       prof_mark(h, DFJK_PHASE_J1, st);
       dim3 g1(h->j1_chunks, naux_pad / kJ1Rows);
-      if (vec) dispatch_j1_tma(ns, g1, st, h->B, npair, naux, h->Dw + (size_t)s0 * npair, h->rho_part, naux_pad);
-      else k_j1<<<g1, kJ1Warps * 32, 0, st>>>(h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad);
+      if (vec) {
+        if (dispatch_j1_tma(h->device, ns, g1, st, h->B, npair, naux, h->Dw + (size_t)s0 * npair, h->rho_part, naux_pad) != cudaSuccess)
+          return -1;
+      } else {
+        k_j1<<<g1, kJ1Warps * 32, 0, st>>>(h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad);
+      }
       dim3 gr(cdiv(naux, 128), ns);
       k_j1_reduce<<<gr, 128, 0, st>>>(h->rho_part, h->j1_chunks, naux_pad, naux, ns, h->rho + (size_t)s0 * naux);
       launches += 2;
     }
     prof_mark(h, DFJK_PHASE_J2, st);
     dim3 g2((unsigned)((npair + 2 * kJ2Threads - 1) / (2 * kJ2Threads)), h->j2_splits);
-    if (vec) launch_j2<true>(ns, g2, st, h->B, npair, naux, h->rho + (size_t)s0 * naux, h->Jp_part + (size_t)s0 * npair, split_stride, rows_per_split);
-    else launch_j2<false>(ns, g2, st, h->B, npair, naux, h->rho + (size_t)s0 * naux, h->Jp_part + (size_t)s0 * npair, split_stride, rows_per_split);
+    cudaError_t e2 = vec ? launch_j2<true>(ns, g2, st, h->B, npair, naux, h->rho + (size_t)s0 * naux, h->Jp_part + (size_t)s0 * npair, split_stride, rows_per_split)
+                         : launch_j2<false>(ns, g2, st, h->B, npair, naux, h->rho + (size_t)s0 * naux, h->Jp_part + (size_t)s0 * npair, split_stride, rows_per_split);
+    if (e2 != cudaSuccess) return -1;
     launches += 1;
   }
   prof_mark(h, DFJK_PHASE_J_EPILOGUE, st);

@@ -58,6 +58,7 @@ struct HtParams {
   double* X; int nch; int mu_pad;       // EPI 0/1: k-tiled X for the SYRK
   int p_first, nb, ntm, ntn;            // aux rows [p_first, p_first + nb), 64-row blocks, N tiles
   double* rho_ht; int nset; int col0[kMaxSets + 1];   // EPI 1: per-warp partials of rho (step a2 fused)
+  const unsigned int* sgnbits;          // EPI 1: sign bits of the occupations (k_prep_ct)
   int ldx, xrows;                       // EPI 2: row-major X[(pl * xrows + mu) * ldx + n]
   // optional re-tiled copy of B (dfjk_create): per aux row the 64 x 16 tiles of the symmetric
   // slice at and below the diagonal blocks, each stored as the padded [64][20] shared-memory image
@@ -307,6 +308,15 @@ k_half_transform(const __grid_constant__ HtParams q) {
               cv[uu][t][0] = __ldg(cp);
               cv[uu][t][1] = __ldg(cp + kHtLd);
             }
+            // rho = sum X' C' sign(occ): flip the sign bit of C' for columns with a negative occupation
+            const unsigned int sw = __ldg(q.sgnbits + (n >> 5)) >> (n & 31);
+            if (sw & 3u) {
+#pragma unroll
+              for (int t = 0; t < 2; t++) {
+                cv[uu][t][0] = flip_sign(cv[uu][t][0], (sw & 1u) << 31);
+                cv[uu][t][1] = flip_sign(cv[uu][t][1], (sw & 2u) << 30);
+              }
+            }
           }
 #pragma unroll
           for (int uu = 0; uu < 4; uu++) {
@@ -350,6 +360,14 @@ k_half_transform(const __grid_constant__ HtParams q) {
             const double* cp = q.Ct + ((size_t)(ok ? (mu >> 4) : 0) * q.ct_rows + (ok ? n : 0)) * kHtLd + (mu & 15);
             cv[uu][t][0] = ok ? __ldg(cp) : 0.0;
             cv[uu][t][1] = ok ? __ldg(cp + kHtLd) : 0.0;
+          }
+          if (su[uu] >= 0) {
+            const unsigned int sw = __ldg(q.sgnbits + (n >> 5)) >> (n & 31);
+#pragma unroll
+            for (int t = 0; t < 2; t++) {
+              cv[uu][t][0] = flip_sign(cv[uu][t][0], (sw & 1u) << 31);
+              cv[uu][t][1] = flip_sign(cv[uu][t][1], (sw & 2u) << 30);
+            }
           }
         }
 #pragma unroll
@@ -447,6 +465,7 @@ struct Syrk2Consumer {
   int nchunks, ch0, ch1, c0, c1, tile_doubles;
   int row0, col0;          // block origin inside the CTA tile
   int kidx;                // this warp takes the k4 steps kk = kidx mod KMOD of every chunk
+  const unsigned int* sgn; // sign bits of the occupations per 32-column chunk (nullptr: all positive)
 };
 
 template <int WM, bool LOWER, int KMOD>
@@ -461,6 +480,9 @@ __device__ __forceinline__ void syrk2_mainloop(const Syrk2Consumer& q, int l, do
     const int stage = c % kStages;
     // k4 steps of this chunk that belong to the set: columns [max(c0, 32 ch), min(c1, 32 ch + 32))
     const int k_lo = (max(q.c0, ch * 32) - ch * 32) >> 2, k_hi = (min(q.c1, ch * 32 + 32) - ch * 32 + 3) >> 2;
+    // K = sum_i sign(occ_i) X'_i X'_i^T: columns with a negative occupation flip the sign bit of the
+    // column-operand fragment (an integer op; the word is warp-uniform and zero in the common case)
+    const unsigned int sw = q.sgn ? __ldg(q.sgn + ch) : 0u;
     if (++ch == q.ch1) ch = q.ch0;
     mbar_wait(q.full0 + 8 * stage, (c / kStages) & 1);
     const double* a_ptr = q.sA + stage * q.tile_doubles + (q.row0 + r) * kLdT + j;
@@ -471,6 +493,11 @@ __device__ __forceinline__ void syrk2_mainloop(const Syrk2Consumer& q, int l, do
       for (int tt = 0; tt < WM; tt++) a[tt] = a_ptr[tt * 8 * kLdT + 4 * kk];
 #pragma unroll
       for (int u = 0; u < WM; u++) b[u] = b_ptr[u * 8 * kLdT + 4 * kk];
+      if (sw) {
+        const unsigned int m = ((sw >> (4 * kk + j)) & 1u) << 31;
+#pragma unroll
+        for (int u = 0; u < WM; u++) b[u] = flip_sign(b[u], m);
+      }
 #pragma unroll
       for (int tt = 0; tt < WM; tt++)
 #pragma unroll
@@ -542,9 +569,9 @@ __device__ __forceinline__ void syrk2_store(double* Kp, int nao, int mu0, int nu
 // ntiles_m * ksplit cheaper diagonal ones, which fill the tail of the last wave.
 template <int WM>
 __global__ void __launch_bounds__(kThreads, 1)
-k_syrk2(const double* __restrict__ X, const double* __restrict__ X2, int nao, int nch, int mu_pad, int c0,
-        int c1, int nrows_blk, int rows_per_split, int ntiles_m, int ksplit, double* __restrict__ Kpart_s,
-        size_t split_stride, int first) {
+k_syrk2(const double* __restrict__ X, const double* __restrict__ X2, const unsigned int* __restrict__ sgn, int nao,
+        int nch, int mu_pad, int c0, int c1, int nrows_blk, int rows_per_split, int ntiles_m, int ksplit,
+        double* __restrict__ Kpart_s, size_t split_stride, int first) {
   // X2 == nullptr: K += X X^T (SYRK).  Otherwise K += X X2^T for a product known to be symmetric
   // (density-matrix form, Eq. 16-17: X = B_P D, X2 = B_P): the column operand comes from X2, and
   // diagonal tiles fetch both operands.
@@ -617,7 +644,7 @@ k_syrk2(const double* __restrict__ X, const double* __restrict__ X2, int nao, in
   const int sp = w & 3, hh = w >> 2;                 // SM sub-partition, first/second warp of the pair
   double* Kp = Kpart_s + (size_t)g * split_stride;
   double* red = smem;                                // reused after the main loop
-  Syrk2Consumer q{sA, one_operand ? sA : sB, full0, empty0, nchunks, ch0, ch1, c0, c1, kTileDoubles, 0, 0, 0};
+  Syrk2Consumer q{sA, one_operand ? sA : sB, full0, empty0, nchunks, ch0, ch1, c0, c1, kTileDoubles, 0, 0, 0, sgn};
   if (!diag) {
     // block (bm, bn) = (sp & 1, sp >> 1); pair split-K 2
     q.row0 = (sp & 1) * 8 * WM; q.col0 = (sp >> 1) * 8 * WM; q.kidx = hh;
@@ -701,23 +728,19 @@ static size_t ht_smem_bytes(int wn) { return (size_t)ht_stages(wn) * (kHtATile +
 static size_t syrk_smem_bytes(int wm) { return (size_t)kStages * 2 * (16 * wm * kLdT) * sizeof(double); }
 
 template <int WN, int EPI>
-static cudaError_t launch_ht(int grid, cudaStream_t st, const HtParams& a) {
-  static bool attr_set = false;  // the attribute is per function (per instantiation)
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_half_transform<WN, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)ht_smem_bytes(WN));
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+static cudaError_t launch_ht(int device, int grid, cudaStream_t st, const HtParams& a) {
+  static std::atomic<unsigned long long> attr_done{0};   // per instantiation, one bit per device
+  cudaError_t e = ensure_dyn_smem(k_half_transform<WN, EPI>, ht_smem_bytes(WN), device, attr_done);
+  if (e != cudaSuccess) return e;
   k_half_transform<WN, EPI><<<grid, kThreads, ht_smem_bytes(WN), st>>>(a);
   return cudaSuccess;
 }
 
 template <int EPI>
-static cudaError_t dispatch_ht_wn(int wn, int grid, cudaStream_t st, const HtParams& a) {
+static cudaError_t dispatch_ht_wn(int device, int wn, int grid, cudaStream_t st, const HtParams& a) {
   switch (wn) {
 #define DFJK_HT_CASE(N) \
-  case N: return launch_ht<N, EPI>(grid, st, a);
+  case N: return launch_ht<N, EPI>(device, grid, st, a);
     DFJK_HT_CASE(1) DFJK_HT_CASE(2) DFJK_HT_CASE(3) DFJK_HT_CASE(4) DFJK_HT_CASE(5) DFJK_HT_CASE(6)
     DFJK_HT_CASE(7) DFJK_HT_CASE(8) DFJK_HT_CASE(9) DFJK_HT_CASE(10) DFJK_HT_CASE(11) DFJK_HT_CASE(12)
     DFJK_HT_CASE(13) DFJK_HT_CASE(14) DFJK_HT_CASE(15) DFJK_HT_CASE(16) DFJK_HT_CASE(17) DFJK_HT_CASE(18)
@@ -728,11 +751,11 @@ static cudaError_t dispatch_ht_wn(int wn, int grid, cudaStream_t st, const HtPar
 }
 
 // epi: 0 = k-tiled X, 1 = k-tiled X + rho partials, 2 = row-major X
-static cudaError_t dispatch_ht(int wn, int epi, int grid, cudaStream_t st, const HtParams& a) {
+static cudaError_t dispatch_ht(int device, int wn, int epi, int grid, cudaStream_t st, const HtParams& a) {
   switch (epi) {
-    case 0: return dispatch_ht_wn<0>(wn, grid, st, a);
-    case 1: return dispatch_ht_wn<1>(wn, grid, st, a);
-    case 2: return dispatch_ht_wn<2>(wn, grid, st, a);
+    case 0: return dispatch_ht_wn<0>(device, wn, grid, st, a);
+    case 1: return dispatch_ht_wn<1>(device, wn, grid, st, a);
+    case 2: return dispatch_ht_wn<2>(device, wn, grid, st, a);
     default: return cudaErrorInvalidValue;
   }
 }
@@ -741,30 +764,27 @@ struct SyrkArgs {
   const double* X; int nao, nch, mu_pad, c0, c1, nrows_blk, rows_per_split, ntiles_m; double* Kpart_s;
   size_t split_stride; int first;
   const double* X2 = nullptr;   // k_syrk2 only: column operand of the two-operand form
+  const unsigned int* sgn = nullptr;   // sign bits of the occupations (C-form), nullptr for the two-operand form
 };
 
 template <int WM>
-static cudaError_t launch_syrk2(int ksplit, cudaStream_t st, const SyrkArgs& a) {
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_syrk2<WM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)syrk_smem_bytes(WM));
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+static cudaError_t launch_syrk2(int device, int ksplit, cudaStream_t st, const SyrkArgs& a) {
+  static std::atomic<unsigned long long> attr_done{0};
+  cudaError_t e = ensure_dyn_smem(k_syrk2<WM>, syrk_smem_bytes(WM), device, attr_done);
+  if (e != cudaSuccess) return e;
   const int grid = a.ntiles_m * (a.ntiles_m + 1) / 2 * ksplit;
-  k_syrk2<WM><<<grid, kThreads, syrk_smem_bytes(WM), st>>>(a.X, a.X2, a.nao, a.nch, a.mu_pad, a.c0, a.c1, a.nrows_blk,
+  k_syrk2<WM><<<grid, kThreads, syrk_smem_bytes(WM), st>>>(a.X, a.X2, a.sgn, a.nao, a.nch, a.mu_pad, a.c0, a.c1, a.nrows_blk,
                                                          a.rows_per_split, a.ntiles_m, ksplit, a.Kpart_s,
                                                          a.split_stride, a.first);
   return cudaSuccess;
 }
 
-static cudaError_t dispatch_syrk2(int wm, int ksplit, cudaStream_t st, const SyrkArgs& a) {
+static cudaError_t dispatch_syrk2(int device, int wm, int ksplit, cudaStream_t st, const SyrkArgs& a) {
   switch (wm) {
-    case 4: return launch_syrk2<4>(ksplit, st, a);
-    case 5: return launch_syrk2<5>(ksplit, st, a);
-    case 6: return launch_syrk2<6>(ksplit, st, a);
-    case 7: return launch_syrk2<7>(ksplit, st, a);
+    case 4: return launch_syrk2<4>(device, ksplit, st, a);
+    case 5: return launch_syrk2<5>(device, ksplit, st, a);
+    case 6: return launch_syrk2<6>(device, ksplit, st, a);
+    case 7: return launch_syrk2<7>(device, ksplit, st, a);
     default: return cudaErrorInvalidValue;
   }
 }
@@ -779,11 +799,11 @@ int launch_half_transform_rowmajor(dfjk_ctx* h, const SetInfo& si, int p_first, 
   HtParams a;
   a.Bt = h->Bt; a.bt_pstride = h->bt_pstride; a.Bp = h->B; a.npair = h->npair; a.nao = h->nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = si.nocc_pad;
   a.X = X; a.nch = 0; a.mu_pad = 0; a.p_first = p_first; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
-  a.rho_ht = nullptr; a.nset = 0; a.ldx = ldx; a.xrows = h->nao;
+  a.rho_ht = nullptr; a.nset = 0; a.ldx = ldx; a.xrows = h->nao; a.sgnbits = nullptr;
   a.col0[0] = 0;
   const long long ht_tiles = (long long)nb * ntm_ht * ntn;
   const int ht_grid = (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid);
-  return dispatch_ht(wn, 2, ht_grid, st, a) == cudaSuccess ? 0 : -1;
+  return dispatch_ht(h->device, wn, 2, ht_grid, st, a) == cudaSuccess ? 0 : -1;
 }
 
 // Modelled SYRK time of one aux block in units of one off-diagonal CTA's aux row: greedy list
@@ -881,11 +901,11 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
     HtParams a;
     a.Bt = h->Bt; a.bt_pstride = h->bt_pstride; a.Bp = h->B; a.npair = h->npair; a.nao = nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = ldx;
     a.X = h->X; a.nch = nch; a.mu_pad = h->mu_pad; a.p_first = p0; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
-    a.rho_ht = h->rho_ht; a.nset = si.nset; a.ldx = 0; a.xrows = 0;
+    a.rho_ht = h->rho_ht; a.nset = si.nset; a.ldx = 0; a.xrows = 0; a.sgnbits = h->sgnbits;
     for (int s = 0; s <= si.nset; s++) a.col0[s] = si.col0[s];
     const long long ht_tiles = (long long)nb * ntm_ht * ntn;
     const int ht_grid = (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid);
-    if (dispatch_ht(wn, want_rho ? 1 : 0, ht_grid, st, a) != cudaSuccess) return -1;
+    if (dispatch_ht(h->device, wn, want_rho ? 1 : 0, ht_grid, st, a) != cudaSuccess) return -1;
     launches++;
     const int rps = cdiv(nb, ksplit);
     prof_mark(h, DFJK_PHASE_SYRK, st);
@@ -894,7 +914,8 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
       // columns past nocc[s] (padding to the 8-column MMA tile) are zero: stop at the k4 step
       SyrkArgs sa{h->X, nao, nch, h->mu_pad, si.col0[s], si.col0[s] + round_up(si.nocc[s], 4), nb, rps, ntm,
                   h->Kpart + n2 * s, split_stride, p0 == 0 ? 1 : 0};
-      if (dispatch_syrk2(wm_s, ksplit, st, sa) != cudaSuccess) return -1;
+      sa.sgn = h->sgnbits;
+      if (dispatch_syrk2(h->device, wm_s, ksplit, st, sa) != cudaSuccess) return -1;
       launches++;
     }
   }
@@ -1002,16 +1023,16 @@ int launch_k_path_dm(dfjk_ctx* h, int nset, const double* D, double* K_out, cuda
       HtParams a;
       a.Bt = h->Bt; a.bt_pstride = h->bt_pstride; a.Bp = h->B; a.npair = h->npair; a.nao = nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = ldx;
       a.X = X1; a.nch = nch; a.mu_pad = h->mu_pad; a.p_first = p0; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
-      a.rho_ht = nullptr; a.nset = 0; a.ldx = 0; a.xrows = 0; a.col0[0] = 0;
+      a.rho_ht = nullptr; a.nset = 0; a.ldx = 0; a.xrows = 0; a.col0[0] = 0; a.sgnbits = nullptr;
       const long long ht_tiles = (long long)nb * ntm_ht * ntn;
-      if (dispatch_ht(wn, 0, (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid), st, a) != cudaSuccess) return -1;
+      if (dispatch_ht(h->device, wn, 0, (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid), st, a) != cudaSuccess) return -1;
       dim3 gu(nch, nb);
       k_unpack_tiled<<<gu, 256, 0, st>>>(h->B, h->npair, nao, p0, nch, h->mu_pad, X2);
       launches += 2;
       prof_mark(h, DFJK_PHASE_SYRK, st);
       SyrkArgs sa{X1, nao, nch, h->mu_pad, 0, round_up(nao, 4), nb, cdiv(nb, ksplit), ntm, h->Kpart + n2 * s,
                   split_stride, p0 == 0 ? 1 : 0, X2};
-      if (dispatch_syrk2(wm_s, ksplit, st, sa) != cudaSuccess) return -1;
+      if (dispatch_syrk2(h->device, wm_s, ksplit, st, sa) != cudaSuccess) return -1;
       launches++;
     }
     prof_mark(h, DFJK_PHASE_K_EPILOGUE, st);

@@ -1,11 +1,14 @@
 // Step a1, density prep (Eq. 14 needs D; Eq. 16 needs gamma = C n C^T):
-//   Ct[i][lam]  = sqrt(n_i) C[lam][i]   all sets concatenated, each set padded to 8 columns with
+//   Ct[i][lam]  = sqrt(|n_i|) C[lam][i] all sets concatenated, each set padded to 8 columns with
 //                                       zeros, lam padded to a multiple of 16 with zeros; stored
 //                                       k-tiled as Ct[(lam/16 * ct_rows + i) * 20 + lam%16] so that
 //                                       the half-transform fetches a whole k-chunk of its B operand
 //                                       with one bulk copy, already in the padded smem layout;
-//   Dw_s[pair]  = (2 - delta_{mu nu}) sum_i Ct[i][mu] Ct[i][nu]   packed, off-diagonal weight 2, so
-//                 that the packed dot product with B_P equals the full-square sum of Eq. 14.
+//   sgnbits     bit i%32 of word i/32 is set iff n_i < 0: D = C' diag(sign n) C'^T exactly, so signed
+//               occupations (differences of densities) cost what unsigned ones do;
+//               the SYRK, the fused rho and Dw apply the sign as a flip of the fp64 sign bit;
+//   Dw_s[pair]  = (2 - delta_{mu nu}) sum_i sign(n_i) Ct[i][mu] Ct[i][nu]   packed, off-diagonal
+//                 weight 2, so that the packed dot product with B_P equals the full-square sum of Eq. 14.
 #include "common.cuh"
 #include "ctx.h"
 
@@ -13,7 +16,7 @@ namespace dfjk {
 
 __global__ void __launch_bounds__(256)
 k_prep_ct(const __grid_constant__ SetInfo si, const double* __restrict__ C, const double* __restrict__ occ,
-          double* __restrict__ Ct, int nao, int nk_pad, int ct_rows) {
+          double* __restrict__ Ct, unsigned int* __restrict__ sgnbits, int nao, int nk_pad, int ct_rows) {
   __shared__ double t[32][33];
   const int tx = threadIdx.x, ty = threadIdx.y;
   const int lam0 = blockIdx.x * 32, ip0 = blockIdx.y * 32;
@@ -27,7 +30,16 @@ k_prep_ct(const __grid_constant__ SetInfo si, const double* __restrict__ C, cons
     if (il >= si.nocc[s]) s = -1;  // padding column
   }
   double scale = 0.0;
-  if (s >= 0) scale = occ ? sqrt(occ[si.ooff[s] + il]) : 1.0;   // occ == nullptr: plain coefficients (AO2MO)
+  bool neg = false;
+  if (s >= 0) {
+    const double n = occ ? occ[si.ooff[s] + il] : 1.0;          // occ == nullptr: plain coefficients (AO2MO)
+    scale = sqrt(fabs(n));
+    neg = n < 0.0;
+  }
+  if (blockIdx.x == 0 && ty == 0) {                             // this block's 32 padded columns = one sign word
+    const unsigned int word = __ballot_sync(0xffffffffu, neg);
+    if (tx == 0) sgnbits[blockIdx.y] = word;
+  }
   for (int r = ty; r < 32; r += 8) {
     const int lam = lam0 + r;
     double v = 0.0;
@@ -44,8 +56,8 @@ k_prep_ct(const __grid_constant__ SetInfo si, const double* __restrict__ C, cons
 
 // 64x64 tile of D_s per CTA, 4x4 per thread, plain DFMA (0.4 GFLOP at nao=1200: negligible).
 __global__ void __launch_bounds__(256)
-k_prep_dw(const __grid_constant__ SetInfo si, const double* __restrict__ Ct, double* __restrict__ Dw,
-          int nao, int nk_pad, int ct_rows, size_t npair) {
+k_prep_dw(const __grid_constant__ SetInfo si, const double* __restrict__ Ct, const unsigned int* __restrict__ sgnbits,
+          double* __restrict__ Dw, int nao, int nk_pad, int ct_rows, size_t npair) {
   const int bi = blockIdx.x, bj = blockIdx.y, s = blockIdx.z;
   if (bj > bi) return;
   __shared__ double As[16][64], Bs[16][64];
@@ -61,7 +73,9 @@ k_prep_dw(const __grid_constant__ SetInfo si, const double* __restrict__ Ct, dou
       const int ii = e >> 6, m = e & 63, i = i0 + ii;
       const int la = bi * 64 + m, lb = bj * 64 + m;
       As[ii][m] = (i < c1 && la < nk_pad) ? Ct[((size_t)(la >> 4) * ct_rows + i) * kHtLd + (la & 15)] : 0.0;
-      Bs[ii][m] = (i < c1 && lb < nk_pad) ? Ct[((size_t)(lb >> 4) * ct_rows + i) * kHtLd + (lb & 15)] : 0.0;
+      double bv = (i < c1 && lb < nk_pad) ? Ct[((size_t)(lb >> 4) * ct_rows + i) * kHtLd + (lb & 15)] : 0.0;
+      if (i < c1 && ((sgnbits[i >> 5] >> (i & 31)) & 1u)) bv = -bv;
+      Bs[ii][m] = bv;
     }
     __syncthreads();
 #pragma unroll
@@ -95,7 +109,7 @@ int launch_prep_ct(dfjk_ctx* h, const SetInfo& si, const double* C, const double
   if (si.nocc_pad == 0) return 0;
   prof_mark(h, DFJK_PHASE_PREP, st);
   dim3 grid(cdiv(h->nck * kHtBK, 32), cdiv(si.nocc_pad, 32)), block(32, 8);
-  k_prep_ct<<<grid, block, 0, st>>>(si, C, occ, h->Ct, h->nao, h->nck * kHtBK, h->ct_rows);
+  k_prep_ct<<<grid, block, 0, st>>>(si, C, occ, h->Ct, h->sgnbits, h->nao, h->nck * kHtBK, h->ct_rows);
   return 1;
 }
 
@@ -103,7 +117,7 @@ int launch_prep_dw(dfjk_ctx* h, const SetInfo& si, cudaStream_t st) {
   prof_mark(h, DFJK_PHASE_PREP, st);
   const int nb = cdiv(h->nao, 64);
   dim3 grid(nb, nb, si.nset);
-  k_prep_dw<<<grid, 256, 0, st>>>(si, h->Ct, h->Dw, h->nao, h->nck * kHtBK, h->ct_rows, h->npair);
+  k_prep_dw<<<grid, 256, 0, st>>>(si, h->Ct, h->sgnbits, h->Dw, h->nao, h->nck * kHtBK, h->ct_rows, h->npair);
   return 1;
 }
 

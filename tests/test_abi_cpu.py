@@ -39,7 +39,7 @@ def test_calls_that_need_no_device():
     h = ct.c_void_p()
     assert lib.dfjk_create(4, 0, None, None, ct.byref(h)) == 1        # nao < 1
     assert lib.dfjk_create(-1, 4, None, None, ct.byref(h)) == 1       # naux < 0
-    assert lib.dfjk_create(4, 4, ct.c_void_p(8), None, ct.byref(h)) == 1   # misaligned B
+    assert lib.dfjk_create(4, 4, ct.c_void_p(12), None, ct.byref(h)) == 1  # B not 8-byte aligned
     assert lib.dfjk_create(4, 4, None, None, None) == 1               # no out pointer
     arr = (ct.c_int * 1)(1)
     assert lib.dfjk_get_jk(None, 1, arr, None, None, None, None, None) == 1

@@ -1,9 +1,11 @@
 """Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (default options).
 
-medium: every element against the full oracle.  large / lasscf: the oracle would need ~2 minutes of
-16 host cores each, so sampled outputs are computed one by one from the definitions
-(oracle.sample) plus properties that hold at any size (bitwise symmetry, Tr(D J) = sum rho^2 >= 0 is
-implied by the sampled J; linearity across the lasscf sets is covered at small size).
+All five configs are compared with the full oracle on EVERY element (R7: per set,
+max|dJ|/max|J| and max|dK|/max|K| over all nao^2 entries <= 1e-10); tiny and small live in
+test_gpu_parity.py, medium / large / lasscf here.  The oracle needs about two minutes of the GPU
+box's 16 host cores for each of the two nao=1200 configs (plus a minute to draw the 23 GB tensor).
+AO2MO (Eq. 18-21) at the bench's size is compared on sampled elements that the oracle computes one
+by one from the definitions (oracle.ao2mo_sample) and on whole aux rows of bpa.
 """
 import numpy as np
 import pytest
@@ -14,10 +16,11 @@ pytestmark = pytest.mark.gpu
 TOL = 1e-10
 
 
-def _gpu_jk(inp):
+def _gpu_jk(inp, B=None):
     import torch
     import paper_2505_03755_b200 as dfjk
-    B = torch.from_numpy(inp.B_packed).cuda()
+    if B is None:
+        B = torch.from_numpy(inp.B_packed).cuda()
     Cs = [torch.from_numpy(c).cuda() for c in inp.C]
     occs = [torch.from_numpy(o).cuda() for o in inp.occ]
     with dfjk.DFJK(B, inp.nao) as h:
@@ -30,34 +33,62 @@ def _gpu_jk(inp):
     return out
 
 
-def test_medium_config_every_element():
-    import oracle
-    inp = dfjk_inputs.make_config("medium")
-    J, K, plan = _gpu_jk(inp)
-    Jo, Ko = oracle.get_jk_inputs(inp)
+def _assert_every_element(inp, J, K, Jo, Ko, plan):
     for s in range(inp.nset):
         ej = np.abs(J[s] - Jo[s]).max() / np.abs(Jo[s]).max()
         ek = np.abs(K[s] - Ko[s]).max() / np.abs(Ko[s]).max()
-        assert ej <= TOL and ek <= TOL, (s, ej, ek, plan)
-        assert np.array_equal(J[s], J[s].T) and np.array_equal(K[s], K[s].T)
+        print(f"{inp.name} set {s}: max|dJ|/max|J| = {ej:.2e}, max|dK|/max|K| = {ek:.2e} over all "
+              f"{inp.nao}^2 entries, plan {plan}")
+        assert ej <= TOL and ek <= TOL, (inp.name, s, ej, ek, plan)
+        assert np.isfinite(J[s]).all() and np.isfinite(K[s]).all()
+        assert np.array_equal(J[s], J[s].T) and np.array_equal(K[s], K[s].T)    # bitwise symmetric
 
 
-@pytest.mark.parametrize("name", ["large", "lasscf"])
-def test_full_size_sampled(name):
+@pytest.mark.parametrize("name", ["medium", "large", "lasscf"])
+def test_config_every_element(name):
     import oracle
     inp = dfjk_inputs.make_config(name)
     J, K, plan = _gpu_jk(inp)
-    nao, nset = inp.nao, inp.nset
-    rs = np.random.default_rng(11)
-    samples = [(int(rs.integers(nset)), int(rs.integers(nao)), int(rs.integers(nao))) for _ in range(6)]
-    samples += [(0, 0, 0), (nset - 1, nao - 1, nao - 1), (0, nao - 1, 0), (nset - 1, 63, 64), (0, 80, 79),
-                (nset - 1, 1199, 1120)]
-    Jv, Kv = oracle.sample(inp.B_packed, nao, inp.C, inp.occ, samples)
-    for t, (s, mu, nu) in enumerate(samples):
-        assert abs(J[s, mu, nu] - Jv[t]) <= TOL * np.abs(J[s]).max(), (name, samples[t], plan)
-        assert abs(K[s, mu, nu] - Kv[t]) <= TOL * np.abs(K[s]).max(), (name, samples[t], plan)
-    for s in range(nset):
-        assert np.isfinite(J[s]).all() and np.isfinite(K[s]).all()
-        assert np.array_equal(J[s], J[s].T) and np.array_equal(K[s], K[s].T)
-        # K is positive semidefinite for occ >= 0: its diagonal is non-negative
-        assert (np.diagonal(K[s]) >= 0).all()
+    Jo, Ko = oracle.get_jk_inputs(inp)
+    _assert_every_element(inp, J, K, Jo, Ko, plan)
+    if name != "medium":
+        # the launch configuration the bench times: several aux blocks, split-K, the re-tiled copy
+        assert plan["nblk"] < inp.naux and plan["ksplit"] > 1 and plan["retiled"] == 1, plan
+
+
+def test_ao2mo_at_bench_size_sampled():
+    """nao = 1200, nmo = 340, nact = 8 (the bench's AO2MO call, active-first route) on the first 400
+    aux rows of the `large` tensor: ppaa / papa at sampled (p1, p2, a1, a2) against the oracle's
+    element sampler, bpa of two whole aux rows against the full oracle (Eq. 18-19)."""
+    import oracle
+    import torch
+    import paper_2505_03755_b200 as dfjk
+    naux = 400
+    inp = dfjk_inputs.make_config("large", aux_rows=naux)
+    nao, nmo, nact = inp.nao, 340, 8
+    a0 = nmo - nact
+    M = np.ascontiguousarray(dfjk_inputs.make_orbitals("large", all_columns=True)[:, :nmo])
+    B = torch.from_numpy(inp.B_packed).cuda()
+    with dfjk.DFJK(B, nao) as h:
+        bpa, ppaa, papa = h.ao2mo(torch.from_numpy(M).cuda(), a0, nact)
+        torch.cuda.synchronize()
+        assert h.last_ao2mo_route == 2
+    bpa, ppaa, papa = bpa.cpu().numpy(), ppaa.cpu().numpy(), papa.cpu().numpy()
+    rs = np.random.default_rng(17)
+    samples = [(int(rs.integers(nmo)), int(rs.integers(nmo)), int(rs.integers(nact)), int(rs.integers(nact)))
+               for _ in range(8)]
+    samples += [(0, 0, 0, 0), (nmo - 1, nmo - 1, nact - 1, nact - 1), (nmo - 1, 0, 0, nact - 1), (a0 + 3, a0 + 5, 5, 3),
+                (63, 64, 1, 2), (128, 127, 7, 0)]
+    v20, v21 = oracle.ao2mo_sample(inp.B_packed, nao, M, a0, nact, samples)
+    s20, s21 = np.abs(ppaa).max(), np.abs(papa).max()
+    for t, (p1, p2, a1, a2) in enumerate(samples):
+        assert abs(ppaa[p1, p2, a1, a2] - v20[t]) <= TOL * s20, (samples[t], ppaa[p1, p2, a1, a2], v20[t])
+        assert abs(papa[p1, a1, p2, a2] - v21[t]) <= TOL * s21, (samples[t], papa[p1, a1, p2, a2], v21[t])
+    rows = [0, naux - 1]
+    o_bpa, _, _ = oracle.ao2mo(inp.B_packed[rows], nao, M, a0, nact)
+    assert np.abs(bpa[rows] - o_bpa).max() <= TOL * np.abs(o_bpa).max()
+    # properties that hold at any size: (p1 p2|a1 a2) is symmetric in p1 <-> p2 and in a1 <-> a2,
+    # (p1 a1|p2 a2) under the pair exchange (p1 a1) <-> (p2 a2)
+    assert np.abs(ppaa - ppaa.transpose(1, 0, 2, 3)).max() <= 1e-12 * s20
+    assert np.abs(ppaa - ppaa.transpose(0, 1, 3, 2)).max() <= 1e-12 * s20
+    assert np.abs(papa - papa.transpose(2, 3, 0, 1)).max() <= 1e-12 * s21

@@ -139,33 +139,68 @@ def test_no_aux_rows_gives_zeros(torch_cuda, dfjk):
     assert not J.any() and not K.any()
 
 
-def test_negative_occupation_needs_the_density_matrix_form(torch_cuda, dfjk):
-    """documented in include/dfjk.h: C' = C sqrt(occ) needs occ >= 0 (NaN otherwise); a density with
-    negative eigenvalues goes through dfjk_get_jk_dm"""
+@pytest.mark.parametrize("nao,naux,nocc,seed,opts", [
+    (24, 10, [5], 146, {}),                                  # one negative column
+    (67, 45, [23, 7], 147, {}),                              # two sets sharing a 32-column chunk, mixed signs
+    (150, 61, [37, 10, 3], 148, dict(two_pass_j=True)),      # Eq. 14 through the signed packed density
+    (150, 61, [37, 10, 3], 148, dict(nblk=7, ksplit=3)),     # several aux blocks and splits
+    (330, 20, [40, 9], 149, {}),                             # 112 x 112 SYRK tiles
+    (420, 14, [400], 150, {}),                               # two N tiles of the half-transform
+    (200, 33, [9, 8, 8, 1, 40, 3, 17, 2], 155, {}),          # eight sets
+])
+def test_signed_occupations_at_c_form_cost(torch_cuda, dfjk, nao, naux, nocc, seed, opts):
+    """occupations of any sign (differences of densities) through dfjk_get_jk: the
+    kernels use C' = C sqrt(|occ|) and flip a sign bit, D = C' diag(sign occ) C'^T exactly.  The
+    oracle takes the occupations as they are (no sqrt folding)."""
     import oracle
     torch = torch_cuda
-    inp = dfjk_inputs.make_random(24, 10, [5], 146)
-    inp.occ[0][2] = -0.5
+    inp = dfjk_inputs.make_random(nao, naux, nocc, seed, L=max(4.0, nao / 6))
+    rs = np.random.default_rng(seed + 1000)
+    for o in inp.occ:                                        # about half of the columns negative, one exact zero
+        o *= rs.choice([-1.0, 1.0], size=o.shape)
+        if o.size > 2:
+            o[1] = 0.0
+    assert any((o < 0).any() for o in inp.occ)
+    Jo, Ko = oracle.get_jk_inputs(inp)
     B, Cs, occs = to_dev(torch, inp)
-    with dfjk.DFJK(B, 24) as h:
+    with dfjk.DFJK(B, inp.nao, **opts) as h:
         J, K = h.get_jk(Cs, occs)
+        Jonly, _ = h.get_jk(Cs, occs, with_k=False)          # two-pass J on the signed packed density
+        _, Konly = h.get_jk(Cs, occs, with_j=False)
         torch.cuda.synchronize()
-        assert torch.isnan(K).any() and torch.isnan(J).any()
-        D = (inp.C[0] * inp.occ[0]) @ inp.C[0].T
-        Jd, Kd = h.get_jk_dm(torch.from_numpy(D[None]).cuda())
-        torch.cuda.synchronize()
-    sq = _unpack_np(inp.B_packed, 24)
-    Jo = np.einsum("p,pmn->mn", np.einsum("pmn,mn->p", sq, D), sq)
-    assert rel(Jd[0].cpu().numpy(), Jo) <= TOL
-    assert rel(Kd[0].cpu().numpy(), oracle.get_k_dform(inp.B_packed, 24, D)) <= TOL
+        assert torch.equal(K, Konly)
+    J, K, Jonly = J.cpu().numpy(), K.cpu().numpy(), Jonly.cpu().numpy()
+    for s in range(inp.nset):
+        assert rel(J[s], Jo[s]) <= TOL and rel(K[s], Ko[s]) <= TOL and rel(Jonly[s], Jo[s]) <= TOL, (s, opts)
+        assert np.array_equal(J[s], J[s].T) and np.array_equal(K[s], K[s].T)
+    # the indefinite density also goes through the density-matrix form: same numbers
+    D = np.stack([(c * o) @ c.T for c, o in zip(inp.C, inp.occ)])
+    if sum(nocc) <= 60:
+        with dfjk.DFJK(B, inp.nao) as h:
+            Jd, Kd = h.get_jk_dm(torch.from_numpy(D).cuda())
+            torch.cuda.synchronize()
+        assert rel(Jd.cpu().numpy(), Jo) <= TOL and rel(Kd.cpu().numpy(), Ko) <= TOL
 
 
-def _unpack_np(Bp, nao):
-    sq = np.zeros((Bp.shape[0], nao, nao))
-    mu, nu = np.tril_indices(nao)
-    sq[:, mu, nu] = Bp
-    sq[:, nu, mu] = Bp
-    return sq
+def test_sign_of_occupations_does_not_leak_between_calls(torch_cuda, dfjk):
+    """the sign bits are rewritten by every call: a signed call followed by an unsigned one (and an
+    AO2MO call, which has no occupations) gives the unsigned answers bit for bit"""
+    torch = torch_cuda
+    inp = dfjk_inputs.make_random(90, 31, [20, 11], 156, L=15.0)
+    B, Cs, occs = to_dev(torch, inp)
+    with dfjk.DFJK(B, inp.nao) as h:
+        J0, K0 = h.get_jk(Cs, occs)
+        M = torch.from_numpy(np.random.default_rng(5).standard_normal((90, 31))).cuda()
+        ref = [t.clone() for t in h.ao2mo(M, 20, 6)]
+        h.get_jk(Cs, [-o for o in occs])
+        J1, K1 = h.get_jk(Cs, occs)
+        got = h.ao2mo(M, 20, 6)
+        torch.cuda.synchronize()
+        assert torch.equal(J0, J1) and torch.equal(K0, K1)
+        assert all(torch.equal(a, b) for a, b in zip(ref, got))
+        Jn, Kn = h.get_jk(Cs, [-o for o in occs])           # J and K are linear in D: D -> -D
+        torch.cuda.synchronize()
+        assert torch.equal(Jn, -J0) and torch.equal(Kn, -K0)
 
 
 def test_more_than_eight_sets(torch_cuda, dfjk):
