@@ -64,6 +64,14 @@ typedef struct {
   int two_pass_j;             /* 0 = when J and K are both requested, rho (Eq. 14) is taken from the
                                  half-transformed block, rho_P = sum_{mu,i} X^P_{mu i} C'_{mu i}, and B is
                                  streamed twice instead of three times; 1 = always the two-pass J */
+  int k_emulation_slices;     /* 0 = K on the native FP64 tensor instruction (default).  3..6 = opt-in FP64
+                                 emulation of the SYRK (Eq. 17) on the int8 tensor cores (the paper's
+                                 reduced-precision outlook): X is split into that many signed
+                                 7-bit slices against a power-of-two scale per AO row and group of aux rows,
+                                 the slice products are exact in int32, the recombination is fp64.  Error
+                                 bound per element: (S+2) 2^(-7S) sum over groups of
+                                 (terms) 2^(e_mu + e_nu); 6 slices keep max|dK|/max|K| <= 1e-10 */
+  int k_emulation_group;      /* aux rows sharing one scale per AO row in the emulated SYRK; 0 = 16, <= 64 */
 } dfjk_options;
 
 /*

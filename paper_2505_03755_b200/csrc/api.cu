@@ -119,6 +119,8 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   if (o.nblk < 0 || o.max_nocc_total < 0 || o.max_nset < 0 || o.max_nset > kMaxSets || o.ksplit < 0 ||
       o.ao2mo_route < 0 || o.ao2mo_route > 2)
     return DFJK_ERR_INVALID_ARG;
+  if (o.k_emulation_slices != 0 && (o.k_emulation_slices < 3 || o.k_emulation_slices > 6)) return DFJK_ERR_INVALID_ARG;
+  if (o.k_emulation_group < 0 || o.k_emulation_group > 64) return DFJK_ERR_INVALID_ARG;
 
   int dev = 0;
   cudaDeviceProp prop;
@@ -135,6 +137,8 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   h->num_sms = prop.multiProcessorCount;
   h->ht_grid = h->num_sms;
   h->two_pass_j = o.two_pass_j;
+  h->k_emu_slices = o.k_emulation_slices;
+  h->k_emu_pgroup = o.k_emulation_group ? o.k_emulation_group : 16;
   h->ao2mo_route = o.ao2mo_route;
   h->npair = (size_t)nao * (nao + 1) / 2;
   h->nck = cdiv(nao, kHtBK);
@@ -168,7 +172,9 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
       if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && free_b / 10 < cap) cap = free_b / 10;
       else cudaGetLastError();
     }
-    const size_t one_row = (size_t)cdiv(h->nocc_pad_cap, kBK) * h->mu_pad * kLdT;
+    size_t one_row = (size_t)cdiv(h->nocc_pad_cap, kBK) * h->mu_pad * kLdT;
+    if (h->k_emu_slices > 0)    // the emulated SYRK keeps the int8 slices of the block beside the fp64 block
+      one_row += emu_bytes_per_aux_row(nao, cdiv(h->nocc_pad_cap, kBK) + 1, h->k_emu_slices, h->k_emu_pgroup) / sizeof(double) + 1024;
     size_t dbl = cap / sizeof(double);
     if (o.nblk > 0) dbl = (size_t)o.nblk * one_row;
     if (dbl < one_row) dbl = one_row;
@@ -261,6 +267,10 @@ int dfjk_get_jk(dfjk_handle h, int nset, const int* nocc, const double* C, const
   }
   if (K_out) {
     k = launch_k_path(h, si, K_out, fuse, st);
+    if (k == -2) {
+      snprintf(h->last_error, sizeof(h->last_error), "workspace cap too small for one aux row of the emulated K path");
+      return DFJK_ERR_INVALID_ARG;
+    }
     if (k < 0) { set_err(h, "k path launch", cudaGetLastError()); return DFJK_ERR_CUDA; }
     n += k;
   }

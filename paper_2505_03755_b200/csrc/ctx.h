@@ -59,6 +59,8 @@ struct dfjk_ctx {
   int ao2mo_route;           // option: 0 = cheaper route, 1 = Eq. 18-21 as printed, 2 = active first
   int plan_ao2mo_route;      // what the last dfjk_ao2mo used
   int two_pass_j;            // option: never fuse J pass 1 into the half-transform
+  int k_emu_slices;          // option: 0 = native fp64 SYRK (DMMA); 3..6 = FP64 emulated on the int8 tensor cores with that many 7-bit slices
+  int k_emu_pgroup;          // aux rows that share one power-of-two scale per AO row in the emulated SYRK
   // scratch (all allocated at create)
   double* Ct;                // [nck][ct_rows][20]  C' transposed and k-tiled, sqrt(occ) folded, zero padded
   unsigned int* sgnbits;     // [nocc_pad_cap / 32 + 1]   bit c%32 of word c/32 = 1 iff padded column c has occ < 0
@@ -120,6 +122,12 @@ int launch_ao2mo(dfjk_ctx* h, int nmo, int a0, int nact, const double* M, double
 // density-matrix form: packed weighted density from D, and K by Eq. 16-17 as printed
 int launch_prep_dw_dm(dfjk_ctx* h, int nset, const double* D, cudaStream_t st);
 int launch_k_path_dm(dfjk_ctx* h, int nset, const double* D, double* K_out, cudaStream_t st);
+// FP64-emulated SYRK on the int8 tensor cores (emu.cu)
+int emu_mu_q(int nao);
+size_t emu_bytes_per_aux_row(int nao, int nchs_max, int S, int pgroup);
+int emu_pick_ksplit(int nao, int ngroups, int max_split, int sms);
+int launch_emu_syrk_set(dfjk_ctx* h, const double* X, int nch, int c0, int c1, int nb, signed char* Xq, double* scale,
+                        double* Kpart_s, size_t split_stride, int ksplit, int first, cudaStream_t st);
 size_t retile_doubles_per_aux_row(int nao);
 cudaError_t launch_retile(const double* Bp, size_t npair, int nao, int naux, double* Bt);
 int run_dmma_selftest();

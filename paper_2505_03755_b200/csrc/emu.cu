@@ -1,0 +1,384 @@
+// Opt-in FP64-emulated exchange build on the low-precision tensor cores (the
+// paper's reduced-precision outlook, "error arising from such ... must be quantified"):
+//   K_s[mu>=nu] = sum_{P,i} X[P][mu][i] X[P][nu][i]      (Eq. 17)
+// with X split into S signed 7-bit integer slices against a shared power-of-two scale per
+// (row mu, group of `pgroup` aux rows):
+//   X[P][mu][i] = 2^e(pg,mu) * sum_{s<S} q_s[P][mu][i] 2^(-6-7s) + r,  |q_s| <= 64,  |r| <= 2^(e-6-7(S-1)) / 2
+// (an Ozaki-style error-free splitting).  The slice products q_s q_t are EXACT on the int8 tensor
+// cores: tcgen05.mma kind::i8 (SASS UTCIMMA), int32 accumulators in TMEM, operands staged in shared
+// memory by bulk async copies (UBLKCP) in the K-major no-swizzle core-matrix layout.  All pairs with
+// the same s + t share one TMEM accumulator (their scale 2^(-12-7(s+t)) is common); pairs with
+// s + t >= S are dropped (below the splitting remainder).  After every group of aux rows the
+// accumulators are read back (tcgen05.ld, SASS LDTM), recombined in fp64 and scaled by
+// 2^(e_mu + e_nu) into fp64 register accumulators.  Error bound per output element:
+//   |dK[mu][nu]| <= (S + 2) 2^(-7S) sum_pg n_pg 2^(e(pg,mu) + e(pg,nu)),  n_pg = terms of group pg,
+// which the tests evaluate from the measured result (<= 1e-10 of max|K| needs S = 6 in the worst
+// case; the measured error at S = 5 is already below it because the dropped terms do not add up
+// coherently).  The native fp64 DMMA path stays the default; this path is selected by
+// dfjk_options.k_emulation_slices.
+#include "common.cuh"
+#include "ctx.h"
+#include "pipeline.cuh"
+
+namespace dfjk {
+
+constexpr int kEmuMinS = 3, kEmuMaxS = 6;   // S * 80 accumulator columns must fit the 512 TMEM columns
+constexpr int kEmuTM = 128;          // tile rows   = UMMA M (one TMEM lane per row)
+constexpr int kEmuTN = 80;           // tile columns = UMMA N; S accumulator groups x 80 columns <= 512 TMEM columns for S <= 6
+constexpr int kEmuStages = 4;
+constexpr int kEmuThreads = 192;     // warp 0: bulk-copy producer, warp 1: MMA issuer, warps 2-5: epilogue (TMEM lane quarters 2,3,0,1)
+
+// ------------------------------------------------------------------ tcgen05 / TMEM wrappers
+__device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+// D[tmem] (+)= A[smem] * B[smem]^T, int8 x int8 -> int32, issued by one thread for the CTA
+__device__ __forceinline__ void umma_i8(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "setp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n"
+      "}\n" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// mbarrier arrive once every tcgen05.mma issued so far by this thread has completed
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// 8 consecutive 32-bit columns of this thread's TMEM lane
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, int (&v)[8]) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+               : "r"(taddr)
+               : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// Shared-memory matrix descriptor, K-major, no swizzle: 8 rows x 16 bytes form one contiguous
+// 128-byte core matrix; `lbo` = byte distance between the two core matrices along K (the 32 int8 of
+// one MMA), `sbo` = byte distance between consecutive 8-row groups.  Descriptor version 1 (sm_100).
+__device__ __forceinline__ uint64_t umma_desc_kmajor(uint32_t smem_addr, uint32_t lbo, uint32_t sbo) {
+  return (uint64_t)((smem_addr >> 4) & 0x3FFFu) | ((uint64_t)((lbo >> 4) & 0x3FFFu) << 16) |
+         ((uint64_t)((sbo >> 4) & 0x3FFFu) << 32) | (1ull << 46);
+}
+// Instruction descriptor of kind::i8: D = s32, A = B = signed int8, both K-major, M x N
+__host__ __device__ constexpr uint32_t umma_idesc_i8(int m, int n) {
+  return (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
+}
+
+// ------------------------------------------------------------------ slicing
+// Layout of the sliced block (all int8): image (kb, s) holds rows [0, mu_q) x the 32 columns of
+// k-block kb = pl * nchs + (ch - ch0) of slice s as 8-row groups of two 128-byte core matrices,
+//   byte ((kb * S + s) * (mu_q / 8) + mu / 8) * 256 + (k / 16) * 128 + (mu % 8) * 16 + k % 16,
+// so the rows [r0, r0 + R) of an image (r0, R multiples of 8) are one contiguous run of R * 32
+// bytes, i.e. one bulk copy, and land in shared memory as the operand image of one MMA (lbo = 128,
+// sbo = 256).  scale[pg][mu] = 2^e(pg, mu) as a double (0 for an all-zero row group).
+struct EmuSliceParams {
+  const double* X; int nch, mu_pad;     // k-tiled X of the half-transform: [pl][nch][mu_pad][36]
+  int nao, mu_q, c0, c1, ch0, nchs;     // set columns [c0, c1) = chunks [ch0, ch0 + nchs)
+  int nb, pgroup, S;                    // aux rows of the block, rows per scale group, slices
+  signed char* Xq; double* scale;       // outputs
+  const unsigned int* sgn; int sel;     // sign bits of the occupations; this pass keeps the columns whose bit == sel
+};
+
+// true if any column of [c0, c1) has its sign bit set (a negative occupation)
+__device__ __forceinline__ bool emu_any_negative(const unsigned int* sgn, int c0, int c1) {
+  unsigned int any = 0;
+  for (int w = c0 >> 5; w <= (c1 - 1) >> 5; w++) {
+    unsigned int m = 0xffffffffu;
+    if (w == (c0 >> 5)) m &= 0xffffffffu << (c0 & 31);
+    if (w == ((c1 - 1) >> 5) && (c1 & 31)) m &= 0xffffffffu >> (32 - (c1 & 31));
+    any |= __ldg(sgn + w) & m;
+  }
+  return any != 0;
+}
+
+// grid (mu_q / 8, ceil(nb / pgroup)); 256 threads = 8 rows x 32 columns of one k-block at a time.
+// Pass 1: the row maxima over the group (its second read of X comes from L2); pass 2: the slices.
+__global__ void __launch_bounds__(256)
+k_emu_slice(const __grid_constant__ EmuSliceParams q) {
+  const int tid = threadIdx.x, r = tid >> 5, c = tid & 31;
+  const int mu8 = blockIdx.x, pg = blockIdx.y, mu = mu8 * 8 + r;
+  const int p_beg = pg * q.pgroup, p_end = min(q.nb, p_beg + q.pgroup);
+  const bool row_ok = mu < q.nao;
+  if (q.sel && !emu_any_negative(q.sgn, q.c0, q.c1)) return;   // the pass of the negative occupations has nothing to do
+  double vmax = 0.0;
+  if (row_ok)
+    for (int pl = p_beg; pl < p_end; pl++)
+      for (int ch = 0; ch < q.nchs; ch++) {
+        const int col = (q.ch0 + ch) * 32 + c;
+        if (col >= q.c0 && col < q.c1)
+          vmax = fmax(vmax, fabs(q.X[(((size_t)pl * q.nch + q.ch0 + ch) * q.mu_pad + mu) * kLdT + c]));
+      }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) vmax = fmax(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
+  // |x| < 2^e for every x of the group: e = exponent of vmax + 1
+  int e = 0;
+  double sc = 0.0, inv = 0.0;
+  if (vmax > 0.0) {
+    e = ilogb(vmax) + 1;
+    sc = scalbn(1.0, e);
+    inv = scalbn(1.0, 6 - e);            // y * 2^6 with y = x 2^-e in (-1, 1)
+  }
+  if (c == 0) q.scale[(size_t)pg * q.mu_q + mu] = sc;
+  const size_t img_stride = (size_t)(q.mu_q / 8) * 256;
+  for (int pl = p_beg; pl < p_end; pl++)
+    for (int ch = 0; ch < q.nchs; ch++) {
+      const int col = (q.ch0 + ch) * 32 + c;
+      double y = 0.0;
+      if (row_ok && col >= q.c0 && col < q.c1 && (int)((__ldg(q.sgn + (col >> 5)) >> (col & 31)) & 1u) == q.sel)
+        y = q.X[(((size_t)pl * q.nch + q.ch0 + ch) * q.mu_pad + mu) * kLdT + c] * inv;
+      signed char* dst = q.Xq + ((size_t)(pl * q.nchs + ch) * q.S) * img_stride + (size_t)mu8 * 256 + (c >> 4) * 128 + r * 16 + (c & 15);
+      for (int s = 0; s < q.S; s++) {
+        const double d = rint(y);          // |d| <= 64; the remainder is exact in fp64
+        y = (y - d) * 128.0;
+        // four adjacent columns -> one 32-bit store
+        const int b = (int)d & 0xff;
+        int w = b | (__shfl_down_sync(0xffffffffu, b, 1) << 8);
+        w |= __shfl_down_sync(0xffffffffu, w, 2) << 16;
+        if ((c & 3) == 0) *reinterpret_cast<int*>(dst + (size_t)s * img_stride) = w;
+      }
+    }
+}
+
+// ------------------------------------------------------------------ emulated SYRK
+struct EmuSyrkParams {
+  const signed char* Xq; const double* scale;
+  int nao, mu_q, nchs, nb, pgroup;
+  int ntr, ntiles, ksplit, groups_per_split;   // row tiles, lower tiles, aux splits, scale groups per split
+  double* Kpart_s; size_t split_stride; int first;
+  const unsigned int* sgn; int c0, c1, negate;  // negate: the pass of the negative occupations, K -= X X^T
+};
+
+// lower tile t -> (row tile i, column tile j): row tile i covers rows [128 i, 128 i + 128) and needs the
+// column tiles j with 80 j <= min(128 i + 127, nao - 1)
+__device__ __forceinline__ void emu_tile_of(int t, int nao, int& ti, int& tj) {
+  int i = 0;
+  for (;; i++) {
+    const int last = min(kEmuTM * i + kEmuTM - 1, nao - 1);
+    const int cnt = last / kEmuTN + 1;
+    if (t < cnt) break;
+    t -= cnt;
+  }
+  ti = i; tj = t;
+}
+
+// CTA = one lower tile (128 x 80) of K_s x one split of the block's scale groups.
+//   warp 0 (one thread): producer, per k-block S A-images (128 rows, 4 KB) + S B-images (80 rows, 2.5 KB)
+//   warp 1 (one thread): issues S(S+1)/2 UMMAs per k-block, accumulator group s + t at TMEM column 80 (s + t)
+//   warps 2-5: after every scale group read the S accumulators of their 32 TMEM lanes, recombine in
+//              fp64 (Horner in 2^-7), scale by 2^(e_mu + e_nu - 12) and add to 80 fp64 registers per row
+template <int S>
+__global__ void __launch_bounds__(kEmuThreads, 1)
+k_emu_syrk(const __grid_constant__ EmuSyrkParams q) {
+  constexpr uint32_t kABytes = kEmuTM * 32, kBBytes = kEmuTN * 32, kStageBytes = S * (kABytes + kBBytes);
+  constexpr uint32_t kTmemCols = 512;
+  static_assert(S * kEmuTN <= 512, "accumulator groups exceed the tensor memory");
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  __shared__ __align__(8) unsigned long long bars[2 * kEmuStages + 2];
+  __shared__ uint32_t tmem_base_s;
+  const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kEmuStages]);
+  const uint32_t tfull = smem_u32(&bars[2 * kEmuStages]), tempty = smem_u32(&bars[2 * kEmuStages + 1]);
+  const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
+  if (q.negate && !emu_any_negative(q.sgn, q.c0, q.c1)) return;   // uniform: no negative occupation in this set
+  const int g = blockIdx.x / q.ntiles;
+  int ti, tj;
+  emu_tile_of(blockIdx.x % q.ntiles, q.nao, ti, tj);
+  const int a0 = ti * kEmuTM, b0 = tj * kEmuTN;
+  const int ngroups_blk = (q.nb + q.pgroup - 1) / q.pgroup;
+  const int pg_beg = g * q.groups_per_split, pg_end = min(ngroups_blk, pg_beg + q.groups_per_split);
+
+  if (tid == 0) {
+    for (int s = 0; s < kEmuStages; s++) {
+      mbar_init(full0 + 8 * s, 1);
+      mbar_init(empty0 + 8 * s, 1);       // one tcgen05.commit per stage
+    }
+    mbar_init(tfull, 1);
+    mbar_init(tempty, 4);                  // one arrival per epilogue warp
+    mbar_fence_init();
+  }
+  if (w == 1) tmem_alloc(smem_u32(&tmem_base_s), kTmemCols);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_base_s;
+  const uint32_t smem0 = smem_u32(smem_raw);
+
+  if (w == 0) {
+    // ===================== producer =====================
+    if (l == 0) {
+      const size_t img_stride = (size_t)(q.mu_q / 8) * 256;
+      int it = 0;
+      for (int pg = pg_beg; pg < pg_end; pg++) {
+        const int p_end = min(q.nb, (pg + 1) * q.pgroup);
+        for (int pl = pg * q.pgroup; pl < p_end; pl++)
+          for (int ch = 0; ch < q.nchs; ch++, it++) {
+            const int stage = it % kEmuStages;
+            mbar_wait(empty0 + 8 * stage, ((it / kEmuStages) & 1) ^ 1);
+            const uint32_t fullb = full0 + 8 * stage;
+            mbar_arrive_expect_tx(fullb, kStageBytes);
+            const signed char* src = q.Xq + (size_t)(pl * q.nchs + ch) * S * img_stride;
+            const uint32_t dst = smem0 + (uint32_t)stage * kStageBytes;
+#pragma unroll
+            for (int s = 0; s < S; s++) {
+              bulk_g2s(dst + s * kABytes, src + (size_t)s * img_stride + (size_t)a0 * 32, kABytes, fullb);
+              bulk_g2s(dst + S * kABytes + s * kBBytes, src + (size_t)s * img_stride + (size_t)b0 * 32, kBBytes, fullb);
+            }
+          }
+      }
+    }
+  } else if (w == 1) {
+    // ===================== MMA issuer =====================
+    if (l == 0) {
+      constexpr uint32_t idesc = umma_idesc_i8(kEmuTM, kEmuTN);
+      int it = 0, period = 0;
+      for (int pg = pg_beg; pg < pg_end; pg++, period++) {
+        const int p_end = min(q.nb, (pg + 1) * q.pgroup);
+        const int nkb = (p_end - pg * q.pgroup) * q.nchs;
+        if (period > 0) {                       // the epilogue has drained the previous group's accumulators
+          mbar_wait(tempty, (period - 1) & 1);
+          tc_fence_after();
+        }
+        for (int kb = 0; kb < nkb; kb++, it++) {
+          const int stage = it % kEmuStages;
+          mbar_wait(full0 + 8 * stage, (it / kEmuStages) & 1);
+          tc_fence_after();
+          const uint32_t sa = smem0 + (uint32_t)stage * kStageBytes, sb = sa + S * kABytes;
+#pragma unroll
+          for (int s = 0; s < S; s++)
+#pragma unroll
+            for (int t = 0; t < S - s; t++)
+              umma_i8(tmem_base + (uint32_t)((s + t) * kEmuTN), umma_desc_kmajor(sa + s * kABytes, 128, 256),
+                      umma_desc_kmajor(sb + t * kBBytes, 128, 256), idesc, (kb > 0 || s > 0) ? 1u : 0u);
+          umma_commit(empty0 + 8 * stage);      // frees the stage when these MMAs have read it
+        }
+        umma_commit(tfull);                     // accumulators of this scale group complete
+      }
+    }
+  } else {
+    // ===================== epilogue warps =====================
+    const int quarter = w & 3;                  // TMEM lanes [32 quarter, 32 quarter + 32)
+    const int row = a0 + 32 * quarter + l;
+    const uint32_t lane_addr = tmem_base + ((uint32_t)(32 * quarter) << 16);
+    double acc[kEmuTN];
+#pragma unroll
+    for (int c = 0; c < kEmuTN; c++) acc[c] = 0.0;
+    int period = 0;
+    for (int pg = pg_beg; pg < pg_end; pg++, period++) {
+      const double* sc = q.scale + (size_t)pg * q.mu_q;
+      const double rs = sc[row] * (1.0 / 4096.0);         // 2^(e_mu - 12)
+      mbar_wait(tfull, period & 1);
+      tc_fence_after();
+#pragma unroll
+      for (int c0 = 0; c0 < kEmuTN; c0 += 8) {
+        double t[8];
+        int v[8];
+        tmem_ld8(lane_addr + (uint32_t)((S - 1) * kEmuTN + c0), v);
+        tmem_ld_wait();
+#pragma unroll
+        for (int i = 0; i < 8; i++) t[i] = (double)v[i];
+#pragma unroll
+        for (int gq = S - 2; gq >= 0; gq--) {
+          tmem_ld8(lane_addr + (uint32_t)(gq * kEmuTN + c0), v);
+          tmem_ld_wait();
+#pragma unroll
+          for (int i = 0; i < 8; i++) t[i] = fma(t[i], 1.0 / 128.0, (double)v[i]);
+        }
+#pragma unroll
+        for (int i = 0; i < 8; i++) acc[c0 + i] = fma(t[i], rs * __ldg(sc + b0 + c0 + i), acc[c0 + i]);
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (l == 0) mbar_arrive(tempty);
+    }
+    // read-modify-write of this CTA's private partial tile, lower triangle only
+    if (row < q.nao) {
+      double* Kp = q.Kpart_s + (size_t)g * q.split_stride + (size_t)row * q.nao;
+#pragma unroll
+      for (int c = 0; c < kEmuTN; c++) {
+        const int nu = b0 + c;
+        if (nu <= row) Kp[nu] = q.first ? acc[c] : (q.negate ? Kp[nu] - acc[c] : Kp[nu] + acc[c]);
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (w == 1) tmem_dealloc(tmem_base, kTmemCols);
+}
+
+// ------------------------------------------------------------------ launchers
+int emu_mu_q(int nao) { return round_up(nao, 8) + kEmuTM; }   // any 128-row tile that starts below nao stays inside an image
+
+// workspace bytes per aux row of a block: int8 images of the widest set + this row's share of the scales
+size_t emu_bytes_per_aux_row(int nao, int nchs_max, int S, int pgroup) {
+  const size_t mu_q = (size_t)emu_mu_q(nao);
+  return (size_t)nchs_max * S * mu_q * 32 + (mu_q * sizeof(double) + pgroup - 1) / pgroup + 64;
+}
+
+static int emu_ntiles(int nao) {
+  int n = 0;
+  for (int i = 0; i * kEmuTM < nao; i++) n += min(kEmuTM * i + kEmuTM - 1, nao - 1) / kEmuTN + 1;
+  return n;
+}
+
+template <int S>
+static cudaError_t launch_emu_syrk_s(int device, int grid, cudaStream_t st, const EmuSyrkParams& p) {
+  constexpr size_t smem = (size_t)kEmuStages * S * (kEmuTM + kEmuTN) * 32;
+  static std::atomic<unsigned long long> attr_done{0};
+  cudaError_t e = ensure_dyn_smem(k_emu_syrk<S>, smem, device, attr_done);
+  if (e != cudaSuccess) return e;
+  k_emu_syrk<S><<<grid, kEmuThreads, smem, st>>>(p);
+  return cudaSuccess;
+}
+
+// split factor of the emulated SYRK: fewest (waves x scale groups per CTA)
+int emu_pick_ksplit(int nao, int ngroups, int max_split, int sms) {
+  const int ntiles = emu_ntiles(nao);
+  long long best = -1;
+  int bk = 1;
+  for (int k = 1; k <= max_split && k <= ngroups; k++) {
+    const int gps = cdiv(ngroups, k);
+    if (cdiv(ngroups, gps) != k) continue;
+    const long long cost = (long long)cdiv(ntiles * k, sms) * gps * 1000 + k;
+    if (best < 0 || cost < best) { best = cost; bk = k; }
+  }
+  return bk;
+}
+
+// One set of one aux block: slice the columns [c0, c1) of the k-tiled X block, then accumulate the
+// lower tiles of K_s on the int8 tensor cores.  Returns the number of launches, -1 on failure.
+int launch_emu_syrk_set(dfjk_ctx* h, const double* X, int nch, int c0, int c1, int nb, signed char* Xq, double* scale,
+                        double* Kpart_s, size_t split_stride, int ksplit, int first, cudaStream_t st) {
+  const int S = h->k_emu_slices, pgroup = h->k_emu_pgroup, nao = h->nao, mu_q = emu_mu_q(nao);
+  const int ch0 = c0 >> 5, nchs = ((c1 + 31) >> 5) - ch0;
+  const int ngroups = cdiv(nb, pgroup);
+  // pass 0: the columns with occ >= 0, K += X X^T; pass 1: those with occ < 0, K -= X X^T (both kernels
+  // return at once when the set has no negative occupation: the host cannot know, occ lives on the device)
+  for (int pass = 0; pass < 2; pass++) {
+    EmuSliceParams sp{X, nch, h->mu_pad, nao, mu_q, c0, c1, ch0, nchs, nb, pgroup, S, Xq, scale, h->sgnbits, pass};
+    dim3 gs(mu_q / 8, ngroups);
+    k_emu_slice<<<gs, 256, 0, st>>>(sp);
+    EmuSyrkParams p{Xq, scale, nao, mu_q, nchs, nb, pgroup, cdiv(nao, kEmuTM), emu_ntiles(nao), ksplit, cdiv(ngroups, ksplit),
+                    Kpart_s, split_stride, pass == 0 ? first : 0, h->sgnbits, c0, c1, pass};
+    const int grid = p.ntiles * ksplit;
+    cudaError_t e = cudaErrorInvalidValue;
+    switch (S) {
+      case 3: e = launch_emu_syrk_s<3>(h->device, grid, st, p); break;
+      case 4: e = launch_emu_syrk_s<4>(h->device, grid, st, p); break;
+      case 5: e = launch_emu_syrk_s<5>(h->device, grid, st, p); break;
+      case 6: e = launch_emu_syrk_s<6>(h->device, grid, st, p); break;
+      default: break;
+    }
+    if (e != cudaSuccess) return -1;
+  }
+  return 4;
+}
+
+}  // namespace dfjk

@@ -870,11 +870,19 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
   // plan: aux block size from the workspace, N tiling of the half-transform, split-K of the SYRK
   const int nch = cdiv(ldx, kBK);
   const size_t row_doubles = (size_t)nch * h->mu_pad * kLdT;     // tiled X, one aux row
-  long long nblk = (long long)(h->X_doubles / row_doubles);
+  // opt-in FP64 emulation of the SYRK on the int8 tensor cores: the block also holds the sliced X
+  const bool emu = h->k_emu_slices > 0;
+  int emu_nchs = 0;
+  for (int s = 0; s < si.nset; s++) {
+    const int c0 = si.col0[s], c1 = c0 + si.nocc[s];
+    if (c1 > c0 && ((c1 + 31) >> 5) - (c0 >> 5) > emu_nchs) emu_nchs = ((c1 + 31) >> 5) - (c0 >> 5);
+  }
+  const size_t emu_row_bytes = emu ? emu_bytes_per_aux_row(nao, emu_nchs, h->k_emu_slices, h->k_emu_pgroup) : 0;
+  long long nblk = (long long)((h->X_doubles * sizeof(double) - (emu ? 4096 : 0)) / (row_doubles * sizeof(double) + emu_row_bytes));
   if (h->nblk_forced > 0 && nblk > h->nblk_forced) nblk = h->nblk_forced;
   if (nblk > naux) nblk = naux;
   if (nblk > 32768) nblk = 32768;
-  if (nblk < 1) nblk = 1;
+  if (nblk < 1) { if (emu) return -2; nblk = 1; }
   const int n8 = ldx / 8;
   const int ntn = cdiv(n8, 2 * kHtMaxWN), wn = cdiv(n8, 2 * ntn);  // N tile = 16*wn columns
   const int ntm_ht = cdiv(nao, 64);
@@ -891,8 +899,20 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
   }
   const double diag_cost = (wm_s + 1) / (2.0 * wm_s);
   const int ntm = cdiv(nao, 16 * wm_s), ntiles = ntm * (ntm + 1) / 2;
-  const int ksplit = pick_ksplit(h, (int)nblk, ntiles, ntm, diag_cost);
+  const int ksplit = emu ? emu_pick_ksplit(nao, cdiv((int)nblk, h->k_emu_pgroup), h->ksplit, h->num_sms)
+                         : pick_ksplit(h, (int)nblk, ntiles, ntm, diag_cost);
   const size_t split_stride = (size_t)h->max_nset * n2;
+  // emulated SYRK: int8 slices and scales behind the fp64 block
+  signed char* emu_xq = nullptr;
+  double* emu_scale = nullptr;
+  if (emu) {
+    uintptr_t a = (uintptr_t)(h->X + (size_t)nblk * row_doubles);
+    a = (a + 255) & ~(uintptr_t)255;
+    emu_xq = (signed char*)a;
+    a += (size_t)nblk * emu_nchs * h->k_emu_slices * (size_t)emu_mu_q(nao) * 32;
+    a = (a + 255) & ~(uintptr_t)255;
+    emu_scale = (double*)a;
+  }
 
   int nblocks = 0;
   for (int p0 = 0; p0 < naux; p0 += (int)nblk, nblocks++) {
@@ -911,6 +931,13 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
     prof_mark(h, DFJK_PHASE_SYRK, st);
     for (int s = 0; s < si.nset; s++) {
       if (si.col0[s + 1] == si.col0[s]) continue;
+      if (emu) {
+        const int k = launch_emu_syrk_set(h, h->X, nch, si.col0[s], si.col0[s] + si.nocc[s], nb, emu_xq, emu_scale,
+                                          h->Kpart + n2 * s, split_stride, ksplit, p0 == 0 ? 1 : 0, st);
+        if (k < 0) return -1;
+        launches += k;
+        continue;
+      }
       // columns past nocc[s] (padding to the 8-column MMA tile) are zero: stop at the k4 step
       SyrkArgs sa{h->X, nao, nch, h->mu_pad, si.col0[s], si.col0[s] + round_up(si.nocc[s], 4), nb, rps, ntm,
                   h->Kpart + n2 * s, split_stride, p0 == 0 ? 1 : 0};
