@@ -72,6 +72,12 @@ typedef struct {
                                  bound per element: (S+2) 2^(-7S) sum over groups of
                                  (terms) 2^(e_mu + e_nu); 6 slices keep max|dK|/max|K| <= 1e-10 */
   int k_emulation_group;      /* aux rows sharing one scale per AO row in the emulated SYRK; 0 = 16, <= 64 */
+  int ht_emulation_slices;    /* 0 = half-transform (Eq. 16 / 18) on the native FP64 tensor instruction (default).
+                                 3..6 = opt-in emulation on the int8 tensor cores: dfjk_create builds int8 slice
+                                 images of the unpacked tensor (S x 1.07 naux nao^2 bytes, one power-of-two scale
+                                 per row of every slice b^P; replaces the re-tiled copy), C' is sliced per call
+                                 (one scale per column).  Error per element of X: <= (S+2) 2^(-7S) nao 2^(e_row +
+                                 e_col).  With this option rho always comes from the two-pass J */
 } dfjk_options;
 
 /*

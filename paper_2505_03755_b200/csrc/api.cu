@@ -32,6 +32,7 @@ bool dev_alloc(dfjk_ctx* h, T** p, size_t count) {
 void free_all(dfjk_ctx* h) {
   cudaFree(h->B_owned); cudaFree(h->Bt); cudaFree(h->Ct); cudaFree(h->sgnbits); cudaFree(h->Dw); cudaFree(h->rho_part); cudaFree(h->rho); cudaFree(h->rho_ht);
   cudaFree(h->Jp_part); cudaFree(h->X); cudaFree(h->Kpart);
+  cudaFree(h->Bq); cudaFree(h->bscale); cudaFree(h->Ctq); cudaFree(h->cscale);
   cudaFree(h->C_stage); cudaFree(h->occ_stage); cudaFree(h->J_stage); cudaFree(h->K_stage);
   for (int i = 0; i < h->ev_cap; i++) cudaEventDestroy(h->ev[i]);
   delete[] h->ev;
@@ -121,6 +122,7 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
     return DFJK_ERR_INVALID_ARG;
   if (o.k_emulation_slices != 0 && (o.k_emulation_slices < 3 || o.k_emulation_slices > 6)) return DFJK_ERR_INVALID_ARG;
   if (o.k_emulation_group < 0 || o.k_emulation_group > 64) return DFJK_ERR_INVALID_ARG;
+  if (o.ht_emulation_slices != 0 && (o.ht_emulation_slices < 3 || o.ht_emulation_slices > 6)) return DFJK_ERR_INVALID_ARG;
 
   int dev = 0;
   cudaDeviceProp prop;
@@ -139,6 +141,7 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   h->two_pass_j = o.two_pass_j;
   h->k_emu_slices = o.k_emulation_slices;
   h->k_emu_pgroup = o.k_emulation_group ? o.k_emulation_group : 16;
+  h->ht_emu_slices = o.ht_emulation_slices;
   h->ao2mo_route = o.ao2mo_route;
   h->npair = (size_t)nao * (nao + 1) / 2;
   h->nck = cdiv(nao, kHtBK);
@@ -223,8 +226,24 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   if (!ok) { free_all(h); delete h; return DFJK_ERR_ALLOC; }
   h->B = h->B_owned ? h->B_owned : B_packed;
   h->b_aligned16 = ((uintptr_t)h->B & 15u) == 0;
+  // emulated half-transform: int8 slice images of the unpacked tensor (S x 1.07 naux nao^2 bytes), built once;
+  // it replaces the re-tiled fp64 copy
+  if (h->ht_emu_slices > 0) {
+    size_t ws = h->workspace_bytes;
+    bool ok2 = dev_alloc(h, &h->Bq, emu_bq_bytes(naux > 0 ? naux : 1, nao, h->ht_emu_slices));
+    h->workspace_bytes = ws;
+    ok2 = ok2 && dev_alloc(h, &h->bscale, (size_t)(naux > 0 ? naux : 1) * emu_mu_q(nao));
+    ok2 = ok2 && dev_alloc(h, &h->Ctq, emu_ctq_bytes(nao, h->nocc_pad_cap, h->ht_emu_slices));
+    ok2 = ok2 && dev_alloc(h, &h->cscale, (size_t)emu_i_q(h->nocc_pad_cap));
+    if (!ok2) { free_all(h); delete h; return DFJK_ERR_ALLOC; }
+    if (naux > 0) {
+      cudaError_t e = launch_emu_slice_b(h);
+      if (e == cudaSuccess) e = cudaDeviceSynchronize();
+      if (e != cudaSuccess) { free_all(h); delete h; cudaGetLastError(); return DFJK_ERR_CUDA; }
+    }
+  }
   // re-tiled copy for the half-transform (1.35x the packed bytes): used if it can be had
-  if (!o.no_retile && naux > 0) {
+  if (!o.no_retile && naux > 0 && h->ht_emu_slices == 0) {
     h->bt_pstride = retile_doubles_per_aux_row(nao);
     cudaError_t e = cudaMalloc((void**)&h->Bt, (size_t)naux * h->bt_pstride * sizeof(double));
     if (e == cudaSuccess) {
@@ -258,7 +277,7 @@ int dfjk_get_jk(dfjk_handle h, int nset, const int* nocc, const double* C, const
   int n = 0, k;
   n += launch_prep_ct(h, si, C, occ, st);
   // both outputs: rho falls out of the half-transform, so J needs one stream over B instead of two
-  const bool fuse = J_out && K_out && !h->two_pass_j && h->naux > 0 && si.nocc_pad > 0;
+  const bool fuse = J_out && K_out && !h->two_pass_j && h->naux > 0 && si.nocc_pad > 0 && h->ht_emu_slices == 0;
   if (J_out && !fuse) {
     n += launch_prep_dw(h, si, st);
     k = launch_j_passes(h, si, J_out, false, st);

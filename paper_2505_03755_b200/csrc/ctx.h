@@ -61,6 +61,11 @@ struct dfjk_ctx {
   int two_pass_j;            // option: never fuse J pass 1 into the half-transform
   int k_emu_slices;          // option: 0 = native fp64 SYRK (DMMA); 3..6 = FP64 emulated on the int8 tensor cores with that many 7-bit slices
   int k_emu_pgroup;          // aux rows that share one power-of-two scale per AO row in the emulated SYRK
+  int ht_emu_slices;         // option: 0 = native fp64 half-transform; 3..6 = emulated on the int8 tensor cores
+  signed char* Bq;           // emulated half-transform: int8 slice images of the unpacked B (built at create)
+  double* bscale;            // [naux][mu_q] power-of-two scale of every row of every slice B_P
+  signed char* Ctq;          // int8 slice images of C'^T (per call)
+  double* cscale;            // [i_q] scale of every column of C'
   // scratch (all allocated at create)
   double* Ct;                // [nck][ct_rows][20]  C' transposed and k-tiled, sqrt(occ) folded, zero padded
   unsigned int* sgnbits;     // [nocc_pad_cap / 32 + 1]   bit c%32 of word c/32 = 1 iff padded column c has occ < 0
@@ -128,6 +133,12 @@ size_t emu_bytes_per_aux_row(int nao, int nchs_max, int S, int pgroup);
 int emu_pick_ksplit(int nao, int ngroups, int max_split, int sms);
 int launch_emu_syrk_set(dfjk_ctx* h, const double* X, int nch, int c0, int c1, int nb, signed char* Xq, double* scale,
                         double* Kpart_s, size_t split_stride, int ksplit, int first, cudaStream_t st);
+size_t emu_bq_bytes(int naux, int nao, int S);
+size_t emu_ctq_bytes(int nao, int nocc_pad_cap, int S);
+int emu_i_q(int nocc_pad);
+cudaError_t launch_emu_slice_b(dfjk_ctx* h);
+int launch_emu_slice_ct(dfjk_ctx* h, int nocc_pad, cudaStream_t st);
+int launch_emu_ht(dfjk_ctx* h, int nocc_pad, int p_first, int nb, double* X, int nch, cudaStream_t st);
 size_t retile_doubles_per_aux_row(int nao);
 cudaError_t launch_retile(const double* Bp, size_t npair, int nao, int naux, double* Bt);
 int run_dmma_selftest();

@@ -313,8 +313,221 @@ k_emu_syrk(const __grid_constant__ EmuSyrkParams q) {
   if (w == 1) tmem_dealloc(tmem_base, kTmemCols);
 }
 
+// ------------------------------------------------------------------ emulated half-transform
+//   X[P][mu][i] = sum_lam B_P[mu][lam] C'[lam][i]      (Eq. 16 / Eq. 18)
+// A operand: int8 slices of the unpacked symmetric slice B_P with one power-of-two scale per (P, mu)
+// (built ONCE in dfjk_create: B is resident and never changes); B operand: slices of
+// C'^T with one scale per column i (per call, 3 MB).  Same image format as above with k = lam.
+
+// the S slices of y (|y| < 64) for column c of an 8-row x 32-column k-block, four columns per store
+__device__ __forceinline__ void emu_emit_slices(double y, signed char* dst, size_t img_stride, int S, int c) {
+  for (int s = 0; s < S; s++) {
+    const double d = rint(y);
+    y = (y - d) * 128.0;
+    const int b = (int)d & 0xff;
+    int w = b | (__shfl_down_sync(0xffffffffu, b, 1) << 8);
+    w |= __shfl_down_sync(0xffffffffu, w, 2) << 16;
+    if ((c & 3) == 0) *reinterpret_cast<int*>(dst + (size_t)s * img_stride) = w;
+  }
+}
+
+// grid (mu_q / 8, aux rows of this launch); Bq image (P, kb, s) at ((P nkb + kb) S + s) * (mu_q / 8) * 256
+__global__ void __launch_bounds__(256)
+k_emu_slice_b(const double* __restrict__ Bp, size_t npair, int nao, int mu_q, int nkb, int S, int p_first,
+              signed char* __restrict__ Bq, double* __restrict__ bscale) {
+  const int tid = threadIdx.x, r = tid >> 5, c = tid & 31;
+  const int mu8 = blockIdx.x, P = p_first + blockIdx.y, mu = mu8 * 8 + r;
+  const double* BpP = Bp + (size_t)P * npair;
+  const bool row_ok = mu < nao;
+  double vmax = 0.0;
+  if (row_ok)
+    for (int lam = c; lam < nao; lam += 32) vmax = fmax(vmax, fabs(BpP[lam <= mu ? tri(mu) + lam : tri(lam) + mu]));
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) vmax = fmax(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
+  double sc = 0.0, inv = 0.0;
+  if (vmax > 0.0) {
+    const int e = ilogb(vmax) + 1;
+    sc = scalbn(1.0, e);
+    inv = scalbn(1.0, 6 - e);
+  }
+  if (c == 0) bscale[(size_t)P * mu_q + mu] = sc;
+  const size_t img_stride = (size_t)(mu_q / 8) * 256;
+  for (int kb = 0; kb < nkb; kb++) {
+    const int lam = kb * 32 + c;
+    double y = 0.0;
+    if (row_ok && lam < nao) y = BpP[lam <= mu ? tri(mu) + lam : tri(lam) + mu] * inv;
+    signed char* dst = Bq + ((size_t)((size_t)P * nkb + kb) * S) * img_stride + (size_t)mu8 * 256 + (c >> 4) * 128 + r * 16 + (c & 15);
+    emu_emit_slices(y, dst, img_stride, S, c);
+  }
+}
+
+// grid (i_q / 8); Ctq image (kb, s) at (kb S + s) * (i_q / 8) * 256; cscale[i] = 2^e of column i of C'
+__global__ void __launch_bounds__(256)
+k_emu_slice_ct(const double* __restrict__ Ct, int ct_rows, int nocc_pad, int nao, int i_q, int nkb, int S,
+               signed char* __restrict__ Ctq, double* __restrict__ cscale) {
+  const int tid = threadIdx.x, r = tid >> 5, c = tid & 31;
+  const int i8 = blockIdx.x, i = i8 * 8 + r;
+  const bool row_ok = i < nocc_pad;
+  double vmax = 0.0;
+  if (row_ok)
+    for (int lam = c; lam < nao; lam += 32) vmax = fmax(vmax, fabs(Ct[((size_t)(lam >> 4) * ct_rows + i) * kHtLd + (lam & 15)]));
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) vmax = fmax(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
+  double sc = 0.0, inv = 0.0;
+  if (vmax > 0.0) {
+    const int e = ilogb(vmax) + 1;
+    sc = scalbn(1.0, e);
+    inv = scalbn(1.0, 6 - e);
+  }
+  if (c == 0) cscale[i] = sc;
+  const size_t img_stride = (size_t)(i_q / 8) * 256;
+  for (int kb = 0; kb < nkb; kb++) {
+    const int lam = kb * 32 + c;
+    double y = 0.0;
+    if (row_ok && lam < nao) y = Ct[((size_t)(lam >> 4) * ct_rows + i) * kHtLd + (lam & 15)] * inv;
+    signed char* dst = Ctq + ((size_t)kb * S) * img_stride + (size_t)i8 * 256 + (c >> 4) * 128 + r * 16 + (c & 15);
+    emu_emit_slices(y, dst, img_stride, S, c);
+  }
+}
+
+struct EmuHtParams {
+  const signed char* Bq; const double* bscale;     // [P][kb][s] images over mu_q rows; [P][mu_q]
+  const signed char* Ctq; const double* cscale;    // [kb][s] images over i_q rows; [i_q]
+  double* X; int nch, mu_pad, nocc_pad;            // k-tiled X of the SYRK: [pl][nch][mu_pad][36]
+  int nao, mu_q, i_q, nkb;
+  int p_first, nb, ntm, ntn;                       // aux rows [p_first, p_first + nb), 128-row tiles, 80-column tiles
+};
+
+// Persistent: gridDim.x CTAs walk the tiles (aux row, 128-row tile, 80-column tile); the N tiles of
+// one (aux row, row tile) run side by side on neighbouring SMs, so the A images come from HBM once.
+// Roles as in k_emu_syrk; the accumulators are drained once per tile (K = nao), the epilogue frees
+// the tensor memory before it scales and stores, so the next tile's MMAs overlap the X stores.
+template <int S>
+__global__ void __launch_bounds__(kEmuThreads, 1)
+k_emu_ht(const __grid_constant__ EmuHtParams q) {
+  constexpr uint32_t kABytes = kEmuTM * 32, kBBytes = kEmuTN * 32, kStageBytes = S * (kABytes + kBBytes);
+  constexpr uint32_t kTmemCols = 512;
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  __shared__ __align__(8) unsigned long long bars[2 * kEmuStages + 2];
+  __shared__ uint32_t tmem_base_s;
+  const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kEmuStages]);
+  const uint32_t tfull = smem_u32(&bars[2 * kEmuStages]), tempty = smem_u32(&bars[2 * kEmuStages + 1]);
+  const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
+  const int tiles_per_p = q.ntm * q.ntn, ntiles = q.nb * tiles_per_p;
+  if (tid == 0) {
+    for (int s = 0; s < kEmuStages; s++) {
+      mbar_init(full0 + 8 * s, 1);
+      mbar_init(empty0 + 8 * s, 1);
+    }
+    mbar_init(tfull, 1);
+    mbar_init(tempty, 4);
+    mbar_fence_init();
+  }
+  if (w == 1) tmem_alloc(smem_u32(&tmem_base_s), kTmemCols);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_base_s;
+  const uint32_t smem0 = smem_u32(smem_raw);
+
+  if (w == 0) {
+    if (l == 0) {
+      const size_t a_img = (size_t)(q.mu_q / 8) * 256, b_img = (size_t)(q.i_q / 8) * 256;
+      int it = 0;
+      for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int pl = tile / tiles_per_p, rem = tile - pl * tiles_per_p;
+        const int a0 = (rem / q.ntn) * kEmuTM, n0 = (rem % q.ntn) * kEmuTN;
+        const signed char* srcA = q.Bq + (size_t)(q.p_first + pl) * q.nkb * S * a_img + (size_t)a0 * 32;
+        const signed char* srcB = q.Ctq + (size_t)n0 * 32;
+        for (int kb = 0; kb < q.nkb; kb++, it++) {
+          const int stage = it % kEmuStages;
+          mbar_wait(empty0 + 8 * stage, ((it / kEmuStages) & 1) ^ 1);
+          const uint32_t fullb = full0 + 8 * stage;
+          mbar_arrive_expect_tx(fullb, kStageBytes);
+          const uint32_t dst = smem0 + (uint32_t)stage * kStageBytes;
+#pragma unroll
+          for (int s = 0; s < S; s++) {
+            bulk_g2s(dst + s * kABytes, srcA + ((size_t)kb * S + s) * a_img, kABytes, fullb);
+            bulk_g2s(dst + S * kABytes + s * kBBytes, srcB + ((size_t)kb * S + s) * b_img, kBBytes, fullb);
+          }
+        }
+      }
+    }
+  } else if (w == 1) {
+    if (l == 0) {
+      constexpr uint32_t idesc = umma_idesc_i8(kEmuTM, kEmuTN);
+      int it = 0, nt = 0;
+      for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, nt++) {
+        if (nt > 0) {
+          mbar_wait(tempty, (nt - 1) & 1);
+          tc_fence_after();
+        }
+        for (int kb = 0; kb < q.nkb; kb++, it++) {
+          const int stage = it % kEmuStages;
+          mbar_wait(full0 + 8 * stage, (it / kEmuStages) & 1);
+          tc_fence_after();
+          const uint32_t sa = smem0 + (uint32_t)stage * kStageBytes, sb = sa + S * kABytes;
+#pragma unroll
+          for (int s = 0; s < S; s++)
+#pragma unroll
+            for (int t = 0; t < S - s; t++)
+              umma_i8(tmem_base + (uint32_t)((s + t) * kEmuTN), umma_desc_kmajor(sa + s * kABytes, 128, 256),
+                      umma_desc_kmajor(sb + t * kBBytes, 128, 256), idesc, (kb > 0 || s > 0) ? 1u : 0u);
+          umma_commit(empty0 + 8 * stage);
+        }
+        umma_commit(tfull);
+      }
+    }
+  } else {
+    const int quarter = w & 3;
+    const uint32_t lane_addr = tmem_base + ((uint32_t)(32 * quarter) << 16);
+    int nt = 0;
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, nt++) {
+      const int pl = tile / tiles_per_p, rem = tile - pl * tiles_per_p;
+      const int a0 = (rem / q.ntn) * kEmuTM, n0 = (rem % q.ntn) * kEmuTN;
+      const int mu = a0 + 32 * quarter + l;
+      double t[kEmuTN];
+      mbar_wait(tfull, nt & 1);
+      tc_fence_after();
+#pragma unroll
+      for (int c0 = 0; c0 < kEmuTN; c0 += 8) {
+        int v[8];
+        tmem_ld8(lane_addr + (uint32_t)((S - 1) * kEmuTN + c0), v);
+        tmem_ld_wait();
+#pragma unroll
+        for (int i = 0; i < 8; i++) t[c0 + i] = (double)v[i];
+#pragma unroll
+        for (int gq = S - 2; gq >= 0; gq--) {
+          tmem_ld8(lane_addr + (uint32_t)(gq * kEmuTN + c0), v);
+          tmem_ld_wait();
+#pragma unroll
+          for (int i = 0; i < 8; i++) t[c0 + i] = fma(t[c0 + i], 1.0 / 128.0, (double)v[i]);
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (l == 0) mbar_arrive(tempty);          // the next tile's MMAs may start while this one is stored
+      if (mu < q.nao) {
+        const double rs = q.bscale[(size_t)(q.p_first + pl) * q.mu_q + mu] * (1.0 / 4096.0);
+        double* Xp = q.X + (size_t)pl * q.nch * q.mu_pad * kLdT;
+#pragma unroll
+        for (int c0 = 0; c0 < kEmuTN; c0 += 2) {
+          const int n = n0 + c0;
+          if (n < q.nocc_pad)
+            *reinterpret_cast<double2*>(Xp + ((size_t)(n >> 5) * q.mu_pad + mu) * kLdT + (n & 31)) =
+                make_double2(t[c0] * (rs * __ldg(q.cscale + n)), t[c0 + 1] * (rs * __ldg(q.cscale + n + 1)));
+        }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (w == 1) tmem_dealloc(tmem_base, kTmemCols);
+}
+
 // ------------------------------------------------------------------ launchers
-int emu_mu_q(int nao) { return round_up(nao, 8) + kEmuTM; }   // any 128-row tile that starts below nao stays inside an image
+// rows of an image: every 128-row tile and every 80-row tile that starts below nao stays inside
+int emu_mu_q(int nao) { return max(round_up(nao, kEmuTM), round_up(nao, kEmuTN)); }
 
 // workspace bytes per aux row of a block: int8 images of the widest set + this row's share of the scales
 size_t emu_bytes_per_aux_row(int nao, int nchs_max, int S, int pgroup) {
@@ -350,6 +563,58 @@ int emu_pick_ksplit(int nao, int ngroups, int max_split, int sms) {
     if (best < 0 || cost < best) { best = cost; bk = k; }
   }
   return bk;
+}
+
+template <int S>
+static cudaError_t launch_emu_ht_s(int device, int grid, cudaStream_t st, const EmuHtParams& p) {
+  constexpr size_t smem = (size_t)kEmuStages * S * (kEmuTM + kEmuTN) * 32;
+  static std::atomic<unsigned long long> attr_done{0};
+  cudaError_t e = ensure_dyn_smem(k_emu_ht<S>, smem, device, attr_done);
+  if (e != cudaSuccess) return e;
+  k_emu_ht<S><<<grid, kEmuThreads, smem, st>>>(p);
+  return cudaSuccess;
+}
+
+int emu_nkb(int nao) { return cdiv(nao, 32); }
+int emu_i_q(int nocc_pad) { return round_up(nocc_pad > 0 ? nocc_pad : 1, kEmuTN); }
+size_t emu_bq_bytes(int naux, int nao, int S) { return (size_t)naux * emu_nkb(nao) * S * (size_t)emu_mu_q(nao) * 32; }
+size_t emu_ctq_bytes(int nao, int nocc_pad_cap, int S) { return (size_t)emu_nkb(nao) * S * (size_t)emu_i_q(nocc_pad_cap) * 32; }
+
+// dfjk_create: the int8 slices of the resident tensor, once
+cudaError_t launch_emu_slice_b(dfjk_ctx* h) {
+  const int mu_q = emu_mu_q(h->nao), nkb = emu_nkb(h->nao);
+  for (int p0 = 0; p0 < h->naux; p0 += 16384) {
+    const int nb = h->naux - p0 < 16384 ? h->naux - p0 : 16384;
+    dim3 grid(mu_q / 8, nb);
+    k_emu_slice_b<<<grid, 256>>>(h->B, h->npair, h->nao, mu_q, nkb, h->ht_emu_slices, p0, h->Bq, h->bscale);
+  }
+  return cudaGetLastError();
+}
+
+// per call: the slices of C'^T (after k_prep_ct)
+int launch_emu_slice_ct(dfjk_ctx* h, int nocc_pad, cudaStream_t st) {
+  const int i_q = emu_i_q(nocc_pad);
+  k_emu_slice_ct<<<i_q / 8, 256, 0, st>>>(h->Ct, h->ct_rows, nocc_pad, h->nao, i_q, emu_nkb(h->nao), h->ht_emu_slices, h->Ctq,
+                                        h->cscale);
+  return 1;
+}
+
+// the half-transform of the aux rows [p_first, p_first + nb) on the int8 tensor cores, X k-tiled
+int launch_emu_ht(dfjk_ctx* h, int nocc_pad, int p_first, int nb, double* X, int nch, cudaStream_t st) {
+  const int nao = h->nao, i_q = emu_i_q(nocc_pad);
+  EmuHtParams p{h->Bq, h->bscale, h->Ctq, h->cscale, X, nch, h->mu_pad, nocc_pad, nao, emu_mu_q(nao), i_q, emu_nkb(nao),
+                p_first, nb, cdiv(nao, kEmuTM), i_q / kEmuTN};
+  const long long ntiles = (long long)nb * p.ntm * p.ntn;
+  const int grid = (int)(ntiles < h->num_sms ? ntiles : h->num_sms);
+  cudaError_t e = cudaErrorInvalidValue;
+  switch (h->ht_emu_slices) {
+    case 3: e = launch_emu_ht_s<3>(h->device, grid, st, p); break;
+    case 4: e = launch_emu_ht_s<4>(h->device, grid, st, p); break;
+    case 5: e = launch_emu_ht_s<5>(h->device, grid, st, p); break;
+    case 6: e = launch_emu_ht_s<6>(h->device, grid, st, p); break;
+    default: break;
+  }
+  return e == cudaSuccess ? 1 : -1;
 }
 
 // One set of one aux block: slice the columns [c0, c1) of the k-tiled X block, then accumulate the

@@ -914,6 +914,12 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
     emu_scale = (double*)a;
   }
 
+  const bool emu_ht = h->ht_emu_slices > 0;
+  if (emu_ht) {
+    prof_mark(h, DFJK_PHASE_PREP, st);
+    launches += launch_emu_slice_ct(h, ldx, st);
+  }
+
   int nblocks = 0;
   for (int p0 = 0; p0 < naux; p0 += (int)nblk, nblocks++) {
     const int nb = (int)(naux - p0 < nblk ? naux - p0 : nblk);
@@ -925,7 +931,11 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
     for (int s = 0; s <= si.nset; s++) a.col0[s] = si.col0[s];
     const long long ht_tiles = (long long)nb * ntm_ht * ntn;
     const int ht_grid = (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid);
-    if (dispatch_ht(h->device, wn, want_rho ? 1 : 0, ht_grid, st, a) != cudaSuccess) return -1;
+    if (emu_ht) {
+      if (launch_emu_ht(h, ldx, p0, nb, h->X, nch, st) < 0) return -1;
+    } else if (dispatch_ht(h->device, wn, want_rho ? 1 : 0, ht_grid, st, a) != cudaSuccess) {
+      return -1;
+    }
     launches++;
     const int rps = cdiv(nb, ksplit);
     prof_mark(h, DFJK_PHASE_SYRK, st);

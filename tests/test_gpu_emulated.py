@@ -131,3 +131,42 @@ def test_emulation_option_range():
     for bad in (1, 2, 7):
         with pytest.raises(dfjk.DFJKError):
             dfjk.DFJK(B, 4, k_emulation_slices=bad)
+
+
+@pytest.mark.parametrize("nao,naux,nocc,seed,opts", [
+    (48, 160, [12], 411, {}),
+    (67, 45, [23, 7], 412, {}),                                      # ragged: 3 k-blocks of lam, the last with 3 columns
+    (150, 61, [37, 10], 413, dict(nblk=20)),
+    (330, 35, [40, 9, 60], 414, {}),                                 # 128 padded columns: two 80-column tiles
+    (260, 12, [130, 129], 415, {}),                                  # 264 padded columns: four N tiles
+])
+def test_emulated_half_transform(nao, naux, nocc, seed, opts):
+    """Eq. 16 on the int8 tensor cores (ht_emulation_slices), alone and together with the emulated
+    SYRK; J (two-pass in this mode) is untouched by the emulation."""
+    import oracle
+    import torch
+    import paper_2505_03755_b200 as dfjk
+    inp = dfjk_inputs.make_random(nao, naux, nocc, seed, L=max(4.0, nao / 6))
+    inp.occ[0][0] = -0.3                                             # a signed occupation rides along
+    Jo, Ko = oracle.get_jk_inputs(inp)
+    B = torch.from_numpy(inp.B_packed).cuda()
+    Cs = [torch.from_numpy(c).cuda() for c in inp.C]
+    occs = [torch.from_numpy(o).cuda() for o in inp.occ]
+    out = []
+    for ht, ks in ((6, 0), (6, 6), (5, 5), (4, 0)):
+        with dfjk.DFJK(B, nao, ht_emulation_slices=ht, k_emulation_slices=ks, **opts) as h:
+            J, K = h.get_jk(Cs, occs)
+            _, Konly = h.get_jk(Cs, occs, with_j=False)
+            torch.cuda.synchronize()
+            assert h.plan()["retiled"] == 0 and torch.equal(K, Konly)
+        J, K = J.cpu().numpy(), K.cpu().numpy()
+        ej = max(rel(J[s], Jo[s]) for s in range(inp.nset))
+        ek = max(rel(K[s], Ko[s]) for s in range(inp.nset))
+        out.append(f"ht={ht} syrk={ks}: {ek:.1e}")
+        assert ej <= TOL
+        assert all(np.array_equal(K[s], K[s].T) for s in range(inp.nset))
+        if ht == 6:
+            assert ek <= TOL, (ht, ks, ek)
+        if ht == 4:
+            assert ek <= 1e-5
+    print(f"emulated half-transform nao={nao} naux={naux} nocc={nocc}: " + ", ".join(out))
