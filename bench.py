@@ -230,6 +230,7 @@ def main():
                     help="with --gpus N > 1: shard the aux rows over the ranks and sum-all-reduce J, K (strong scaling) "
                          "instead of N independent replicas")
     ap.add_argument("--no-small-calls", action="store_true", help="skip the small-call (CUDA graph) section")
+    ap.add_argument("--no-emulated", action="store_true", help="skip the opt-in FP64-emulated K path (int8 tensor cores) section")
     ap.add_argument("--no-dm-form", action="store_true", help="skip the density-matrix-form (Eq. 16-17 as printed) section")
     ap.add_argument("--no-ao2mo", action="store_true", help="skip the AO2MO (Eq. 18-21) section")
     ap.add_argument("--workspace-gib", type=float, default=0.0, help="dfjk_options.workspace_cap_bytes (0 = default)")
@@ -409,6 +410,39 @@ def main():
         del D_dev, Jd, Kd
     # ---- the many-small-calls regime of the embedded fragments:
     # the `small` config called directly and as a replayed CUDA graph (dfjk_get_jk only enqueues)
+    # ---- opt-in FP64 emulation of the K path on the int8 tensor cores:
+    # the same call on a second handle, error of K against the native fp64 result over every element
+    emulated = None
+    if not args.no_emulated and not shard:
+        full()
+        torch.cuda.synchronize()
+        K_native = K.clone()
+        emulated = []
+        for ht_s, k_s in ((6, 6), (5, 5)):
+            he = dfjk.DFJK(Bd, nao, ht_emulation_slices=ht_s, k_emulation_slices=k_s,
+                           workspace_cap_bytes=int(args.workspace_gib * (1 << 30)))
+            Je, Ke = torch.empty_like(J), torch.empty_like(K)
+            e_full = lambda: he.get_jk_raw(nocc, C_dev, occ_dev, out_j=Je, out_k=Ke, stream=stream)
+            e_konly = lambda: he.get_jk_raw(nocc, C_dev, occ_dev, with_j=False, out_k=Ke, stream=stream)
+            for _ in range(2):
+                e_full()
+            ms_e = max_over_ranks(timed(e_full, nrep))
+            ms_ek = max_over_ranks(timed(e_konly, nrep))
+            he.set_profiling(True)
+            e_full()
+            ep = he.profile()
+            he.set_profiling(False)
+            errs = [float((Ke[s_] - K_native[s_]).abs().max() / K_native[s_].abs().max()) for s_ in range(nset)]
+            emulated.append({"ht_slices": ht_s, "syrk_slices": k_s, "ms": ms_e, "k_path_ms": ms_ek,
+                             "half_transform_ms": ep["half_transform"][0], "syrk_ms": ep["syrk"][0],
+                             "launches_per_call": he.last_launch_count, "plan": he.plan(),
+                             "equivalent_fp64_tflops": fb["k"] / (ms_ek * 1e-3) * 1e-12,
+                             "max_rel_err_K_vs_native_every_element": max(errs),
+                             "kernels": "tcgen05.mma kind::i8 (UTCIMMA), TMEM int32 accumulators, bulk-copied core-matrix images"})
+            he.close()
+            del Je, Ke
+        del K_native
+        torch.cuda.empty_cache()
     small = None
     if not args.no_small_calls:
         small = {}
@@ -495,6 +529,8 @@ def main():
         "phases_ms_per_step": {p: v[0] / args.steps for p, v in phases.items()},
     }
 
+    if emulated is not None:
+        line["k_emulated"] = emulated
     if small is not None:
         line["small_calls"] = small
     if dmf is not None:

@@ -39,8 +39,13 @@ struct GemmTN {
 // the product: 64 x up to 352).
 // Shared-memory tiles are k-major, [16][TM + 4] and [16][TN + 4]: the row stride is 4 mod 16
 // doubles, so the fragment reads tile[k = l%4][row = l/4] hit 16 distinct banks per half-warp.
-// Producers gather with 8-byte cp.async (any alignment, zero-fill past M, N, K).
-template <int WTM, int WTN>
+// Producers: BULK = true -- both operands are plain k-major matrices whose rows start 16-byte aligned
+// (even leading dimensions and tile origins, K a multiple of 4): every k row of a tile is one
+// contiguous run, fetched by a bulk async copy (TMA engine, UBLKCP); sixteen lanes of one producer
+// warp issue the 32 row copies of a stage, completion is counted in bytes.  Columns past M or N are
+// never stored, so tails need no zero fill.  BULK = false -- 8-byte cp.async gathers (any alignment,
+// grouped A rows, zero-fill past M, N, K).
+template <int WTM, int WTN, bool BULK>
 __global__ void __launch_bounds__(kGThreads, 1)
 k_gemm_tn(const __grid_constant__ GemmTN g) {
   constexpr int TM = 16 * WTM, TN = 32 * WTN, LA = TM + 4, LB = TN + 4;
@@ -57,7 +62,7 @@ k_gemm_tn(const __grid_constant__ GemmTN g) {
 
   if (tid == 0) {
     for (int s = 0; s < kGStages; s++) {
-      mbar_init(full0 + 8 * s, 128);       // one cp.async-completion arrival per producer thread
+      mbar_init(full0 + 8 * s, BULK ? 1 : 128);   // the expect_tx arrival / one cp.async-completion arrival per producer thread
       mbar_init(empty0 + 8 * s, 8);        // one arrival per consumer warp
     }
     mbar_fence_init();
@@ -68,6 +73,27 @@ k_gemm_tn(const __grid_constant__ GemmTN g) {
     // ===================== producer warpgroup =====================
     reg_dec<kProducerRegs>();
     const int tp = tid - 256;
+    if (BULK) {
+      if (tp >= kGKC) return;               // lane k of the first producer warp owns k row k of every stage
+      const int mrows = min(TM, g.M - m0), ncols = min(TN, g.N - n0);
+      const uint32_t a_bytes = (uint32_t)mrows * 8u, b_bytes = (uint32_t)ncols * 8u;
+      const double* Ak = A + (size_t)m0 + (size_t)tp * g.lda;
+      const double* Bk = B + (size_t)n0 + (size_t)tp * g.ldb;
+      for (int c = 0; c < nchunks; c++) {
+        const int stage = c % kGStages;
+        const uint32_t fullb = full0 + 8 * stage;
+        mbar_wait(empty0 + 8 * stage, ((c / kGStages) & 1) ^ 1);
+        const int krows = min(kGKC, g.K - c * kGKC);             // a multiple of 4
+        if (tp == 0) mbar_arrive_expect_tx(fullb, (uint32_t)krows * (a_bytes + b_bytes));
+        __syncwarp(0x0000ffffu);                                  // the barrier is armed before any byte lands
+        if (tp < krows) {
+          const uint32_t sa = smem_u32(smem + stage * kStageDoubles), sb = sa + kGKC * LA * 8;
+          bulk_g2s(sa + (uint32_t)(tp * LA) * 8u, Ak + (size_t)c * kGKC * g.lda, a_bytes, fullb);
+          bulk_g2s(sb + (uint32_t)(tp * LB) * 8u, Bk + (size_t)c * kGKC * g.ldb, b_bytes, fullb);
+        }
+      }
+      return;
+    }
     // a thread keeps its columns for the whole kernel: one column m of the A tile (k rows tp / TM,
     // + 128 / TM, ...) and the columns tp, tp + 128, ... of the B tile; only k moves per chunk
     static_assert(128 % TM == 0 || TM % 128 == 0, "A tile width must divide or be a multiple of 128");
@@ -176,17 +202,30 @@ __global__ void k_zero_ao(double* p, size_t n) {
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = 0.0;
 }
 
-template <int WTM, int WTN>
-static cudaError_t launch_gemm_tn(int device, const GemmTN& g, int batch, cudaStream_t st) {
+template <int WTM, int WTN, bool BULK>
+static cudaError_t launch_gemm_tn_b(int device, const GemmTN& g, int batch, cudaStream_t st) {
   constexpr int TM = 16 * WTM, TN = 32 * WTN;
   constexpr size_t smem = (size_t)kGStages * kGKC * (TM + 4 + TN + 4) * sizeof(double);
   static std::atomic<unsigned long long> attr_done{0};
-  cudaError_t e = ensure_dyn_smem(k_gemm_tn<WTM, WTN>, smem, device, attr_done);
+  cudaError_t e = ensure_dyn_smem(k_gemm_tn<WTM, WTN, BULK>, smem, device, attr_done);
   if (e != cudaSuccess) return e;
   if (g.M <= 0 || g.N <= 0 || batch <= 0) return cudaSuccess;
   dim3 grid(cdiv(g.M, TM), cdiv(g.N, TN), batch);
-  k_gemm_tn<WTM, WTN><<<grid, kGThreads, smem, st>>>(g);
+  k_gemm_tn<WTM, WTN, BULK><<<grid, kGThreads, smem, st>>>(g);
   return cudaSuccess;
+}
+
+// bulk copies need 16-byte aligned k rows of both operands for every tile and batch, and whole k4 steps
+static bool gemm_tn_bulk_ok(const GemmTN& g) {
+  auto even = [](long long v) { return (v & 1) == 0; };
+  return g.a_group == 0 && ((uintptr_t)g.A & 15u) == 0 && ((uintptr_t)g.B & 15u) == 0 && even(g.lda) && even(g.ldb) &&
+         even(g.sA) && even(g.sB) && even(g.M) && even(g.N) && (g.K & 3) == 0;
+}
+
+template <int WTM, int WTN>
+static cudaError_t launch_gemm_tn(int device, const GemmTN& g, int batch, cudaStream_t st) {
+  return gemm_tn_bulk_ok(g) ? launch_gemm_tn_b<WTM, WTN, true>(device, g, batch, st)
+                            : launch_gemm_tn_b<WTM, WTN, false>(device, g, batch, st);
 }
 
 // CTA tile 64 x (32 WTN): the N tile is fitted to the problem (at most 352 columns per tile, the

@@ -148,6 +148,26 @@ k_emu_slice(const __grid_constant__ EmuSliceParams q) {
     }
 }
 
+// All slice pairs (s, t), s + t < S, of one k-block.  The B images t = 0, 1, ... lie one after another
+// in shared memory (80 rows = ten 8-row groups each) and the accumulator of pair (s, t) sits at TMEM
+// column 80 (s + t), so for a fixed s up to three pairs are ONE MMA of N = 80, 160 or 240 columns
+// against the same A image: 9 instructions instead of 21 at S = 6, and the A image is read from
+// shared memory 9 times instead of 21 (operand reads, not math, bound the N = 80 instruction).
+template <int S>
+__device__ __forceinline__ void emu_issue_pairs(uint32_t tmem_base, uint32_t sa, uint32_t sb, bool accumulate_first) {
+  constexpr uint32_t kABytes = kEmuTM * 32, kBBytes = kEmuTN * 32;
+#pragma unroll
+  for (int s = 0; s < S; s++) {
+    const uint64_t a_desc = umma_desc_kmajor(sa + s * kABytes, 128, 256);
+#pragma unroll
+    for (int t0 = 0; t0 < S - s; t0 += 3) {
+      const int cnt = (S - s - t0) < 3 ? (S - s - t0) : 3;
+      umma_i8(tmem_base + (uint32_t)((s + t0) * kEmuTN), a_desc, umma_desc_kmajor(sb + t0 * kBBytes, 128, 256),
+              umma_idesc_i8(kEmuTM, kEmuTN * cnt), (accumulate_first || s > 0) ? 1u : 0u);
+    }
+  }
+}
+
 // ------------------------------------------------------------------ emulated SYRK
 struct EmuSyrkParams {
   const signed char* Xq; const double* scale;
@@ -237,7 +257,6 @@ k_emu_syrk(const __grid_constant__ EmuSyrkParams q) {
   } else if (w == 1) {
     // ===================== MMA issuer =====================
     if (l == 0) {
-      constexpr uint32_t idesc = umma_idesc_i8(kEmuTM, kEmuTN);
       int it = 0, period = 0;
       for (int pg = pg_beg; pg < pg_end; pg++, period++) {
         const int p_end = min(q.nb, (pg + 1) * q.pgroup);
@@ -251,12 +270,7 @@ k_emu_syrk(const __grid_constant__ EmuSyrkParams q) {
           mbar_wait(full0 + 8 * stage, (it / kEmuStages) & 1);
           tc_fence_after();
           const uint32_t sa = smem0 + (uint32_t)stage * kStageBytes, sb = sa + S * kABytes;
-#pragma unroll
-          for (int s = 0; s < S; s++)
-#pragma unroll
-            for (int t = 0; t < S - s; t++)
-              umma_i8(tmem_base + (uint32_t)((s + t) * kEmuTN), umma_desc_kmajor(sa + s * kABytes, 128, 256),
-                      umma_desc_kmajor(sb + t * kBBytes, 128, 256), idesc, (kb > 0 || s > 0) ? 1u : 0u);
+          emu_issue_pairs<S>(tmem_base, sa, sb, kb > 0);
           umma_commit(empty0 + 8 * stage);      // frees the stage when these MMAs have read it
         }
         umma_commit(tfull);                     // accumulators of this scale group complete
@@ -455,7 +469,6 @@ k_emu_ht(const __grid_constant__ EmuHtParams q) {
     }
   } else if (w == 1) {
     if (l == 0) {
-      constexpr uint32_t idesc = umma_idesc_i8(kEmuTM, kEmuTN);
       int it = 0, nt = 0;
       for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, nt++) {
         if (nt > 0) {
@@ -467,12 +480,7 @@ k_emu_ht(const __grid_constant__ EmuHtParams q) {
           mbar_wait(full0 + 8 * stage, (it / kEmuStages) & 1);
           tc_fence_after();
           const uint32_t sa = smem0 + (uint32_t)stage * kStageBytes, sb = sa + S * kABytes;
-#pragma unroll
-          for (int s = 0; s < S; s++)
-#pragma unroll
-            for (int t = 0; t < S - s; t++)
-              umma_i8(tmem_base + (uint32_t)((s + t) * kEmuTN), umma_desc_kmajor(sa + s * kABytes, 128, 256),
-                      umma_desc_kmajor(sb + t * kBBytes, 128, 256), idesc, (kb > 0 || s > 0) ? 1u : 0u);
+          emu_issue_pairs<S>(tmem_base, sa, sb, kb > 0);
           umma_commit(empty0 + 8 * stage);
         }
         umma_commit(tfull);
