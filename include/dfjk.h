@@ -78,6 +78,10 @@ typedef struct {
                                  per row of every slice b^P; replaces the re-tiled copy), C' is sliced per call
                                  (one scale per column).  Error per element of X: <= (S+2) 2^(-7S) nao 2^(e_row +
                                  e_col).  With this option rho always comes from the two-pass J */
+  int no_symm_thin;           /* 0 = a half-transform with at most 8 columns (the active columns of dfjk_ao2mo's
+                                 "active first" route) streams the packed triangle once and uses every stored
+                                 element for both Z[mu] and Z[lam] (needs a 16-byte aligned B and nao <= 1280);
+                                 1 = always the tiled half-transform */
 } dfjk_options;
 
 /*

@@ -359,10 +359,17 @@ static int launch_ao2mo_active_first(dfjk_ctx* h, int nmo, int a0, int nact, con
   SetInfo si;
   si.nset = 1; si.col0[0] = 0; si.nocc[0] = nact; si.coff[0] = 0; si.ooff[0] = 0;
   si.col0[1] = si.nocc_pad = ldz;
-  launches += 1 + launch_prep_ct(h, si, Mact, nullptr, st);
+  // at most 8 active columns: one pass over the packed triangle, every stored element used twice (symm.cu)
+  const bool thin = symm_thin_ok(h, nact) && ldz == 8;
+  launches += 1;
+  if (!thin) launches += launch_prep_ct(h, si, Mact, nullptr, st);
   for (int p0 = 0; p0 < naux; p0 += (int)nbz) {
     const int nb = (int)(naux - p0 < nbz ? naux - p0 : nbz);
-    if (launch_half_transform_rowmajor(h, si, p0, nb, Z, ldz, st) != 0) return -1;        // Z^P = b^P M_act
+    if (thin) {
+      if (launch_symm_thin(h, Mact, nact, nact, p0, nb, Z, ldz, st) != 0) return -1;       // Z^P = b^P M_act
+    } else if (launch_half_transform_rowmajor(h, si, p0, nb, Z, ldz, st) != 0) {
+      return -1;
+    }
     // bpa^P = M^T Z^P for the whole block as one GEMM with rows (P, a) and columns p:
     // C[(P a)][p] = sum_mu Z^P[mu][a] M[mu][p], stored transposed into bpa[P][p][a]
     GemmTN gb{Z, M, bpa_out + (size_t)p0 * npa, nb * nact, nmo, nao, ldz, nmo, 0, 0, 0, 0, 0,

@@ -142,6 +142,7 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   h->k_emu_slices = o.k_emulation_slices;
   h->k_emu_pgroup = o.k_emulation_group ? o.k_emulation_group : 16;
   h->ht_emu_slices = o.ht_emulation_slices;
+  h->no_symm_thin = o.no_symm_thin;
   h->ao2mo_route = o.ao2mo_route;
   h->npair = (size_t)nao * (nao + 1) / 2;
   h->nck = cdiv(nao, kHtBK);

@@ -115,3 +115,51 @@ def test_route_follows_the_flop_model():
 def test_more_mo_columns_than_one_n_tile(route):
     """nmo = 380 > 352: Eq. 18 (route 1) needs two N tiles of the half-transform; k_gemm_tn two N tiles"""
     run_case(400, 9, 380, 100, 4, 261, L=40.0, ao2mo_route=route)
+
+
+# ---- the one-pass symmetric thin half-transform (symm.cu) behind the active-first route, nact <= 8
+@pytest.mark.parametrize("nao,naux,nmo,a0,nact,seed", [
+    (5, 3, 5, 1, 2, 301),           # smaller than one row group; naux * npair odd (plain-load tail of the last row)
+    (33, 7, 20, 4, 8, 302),         # one row past a super-group of 32 rows; npair odd: odd aux rows start 8-byte aligned
+    (129, 5, 60, 10, 7, 303),       # one column past a 128-column chunk, nao % 4 == 1
+    (130, 4, 64, 0, 1, 304),        # nao % 4 == 2, a single active column
+    (263, 6, 100, 50, 8, 305),      # three chunks, ragged last row group, nao % 4 == 3
+    (520, 3, 48, 40, 8, 306),       # five chunks: every warp owns several column blocks
+])
+def test_symm_thin_shapes(nao, naux, nmo, a0, nact, seed):
+    """route 2 with at most 8 active columns streams the packed triangle once (k_symm_thin); every shape
+    is also run with the tiled half-transform (no_symm_thin) and both must match the oracle"""
+    a = run_case(nao, naux, nmo, a0, nact, seed, L=max(4.0, nao / 6), ao2mo_route=2)
+    b = run_case(nao, naux, nmo, a0, nact, seed, L=max(4.0, nao / 6), ao2mo_route=2, no_symm_thin=True)
+    for x, y in zip(a, b):
+        assert rel(x, y) <= 1e-12
+
+
+def test_symm_thin_large_basis_every_block():
+    """nao = 1203 (ragged, 10 chunks, all 20 register-resident column blocks per warp), white-noise B so
+    that a wrong block anywhere shows; more aux rows than SMs so the persistent loop wraps"""
+    run_case(1203, 150, 24, 8, 8, 307, L=0.0, ao2mo_route=2)
+
+
+def test_symm_thin_falls_back_past_its_basis_limit():
+    """nao = 1300 > 1280: the tiled half-transform serves route 2"""
+    run_case(1300, 3, 16, 4, 4, 308, L=100.0, ao2mo_route=2)
+
+
+def test_symm_thin_unaligned_tensor_falls_back():
+    """a row slice of an odd-npair tensor is only 8-byte aligned: the tiled path must be taken"""
+    import torch
+    import oracle
+    import paper_2505_03755_b200 as dfjk
+    nao, naux = 33, 9                                           # npair = 561, odd
+    inp = dfjk_inputs.make_random(nao, naux, [1], 309, L=8.0)
+    M = np.random.default_rng(310).standard_normal((nao, 12))
+    Bfull = torch.from_numpy(inp.B_packed).cuda()
+    Bs = Bfull[1:]                                              # data_ptr = base + 561 * 8
+    assert Bs.data_ptr() % 16 == 8
+    with dfjk.DFJK(Bs, nao, ao2mo_route=2) as h:
+        bpa, ppaa, papa = h.ao2mo(torch.from_numpy(M).cuda(), 2, 6)
+        torch.cuda.synchronize()
+    o_bpa, o_ppaa, o_papa = oracle.ao2mo(inp.B_packed[1:], nao, M, 2, 6)
+    assert rel(bpa.cpu().numpy(), o_bpa) <= TOL and rel(ppaa.cpu().numpy(), o_ppaa) <= TOL
+    assert rel(papa.cpu().numpy(), o_papa) <= TOL
