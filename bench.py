@@ -372,12 +372,22 @@ def main():
         ao_route = h.last_ao2mo_route
         del outs
         ms_ao = max_over_ranks(timed(lambda: ao_fn() and None, max(2, min(args.steps, 3))))
+        h.set_profiling(True)                       # Eq. 18 (the thin half-transform of the active-first route) alone
+        ao_fn()
+        aprof = h.profile()
+        h.set_profiling(False)
+        ht_ao_ms = aprof["half_transform"][0]
+        ht_ao_bytes = naux * (nao * (nao + 1) // 2 * 8.0 + nao * 8 * 8.0)
         ao_flops = (2.0 * naux * nao * nao * nmo + 2.0 * naux * nao * nmo * nmo
                     + 2.0 * naux * nmo * nmo * nact * nact + 2.0 * naux * (nmo * nact) ** 2)
         ao_exec = (2.0 * naux * nao * nao * nact + 2.0 * naux * nao * nmo * nact + 2.0 * naux * (nao * (nao + 1) // 2) * nact * nact
                    + 2.0 * nao * nmo * nact * nact * (nao + nmo) + 2.0 * naux * (nmo * nact) ** 2) if ao_route == 2 else ao_flops
         ao = {"ms": ms_ao, "nmo": nmo, "a0": a0, "nact": nact, "launches_per_call": ao_launches,
               "route": {1: "Eq. 18-21 in the printed order", 2: "active first (bmo never formed)"}.get(ao_route, "?"),
+              "eq18_ms": ht_ao_ms, "contractions_ms": aprof["syrk"][0],
+              "eq18_gbs": (ht_ao_bytes / (ht_ao_ms * 1e-3) * 1e-9) if (ao_route == 2 and nact <= 8 and ht_ao_ms > 0) else None,
+              "eq18_note": "active-first route with <= 8 active columns: one pass over the packed triangle (k_symm_thin), "
+                           "algorithmic bytes = packed B once + Z; HBM-bound",
               "executed_flops": ao_exec, "executed_tflops": ao_exec / (ms_ao * 1e-3) * 1e-12,
               "frac_of_fp64_peak": ao_exec / (ms_ao * 1e-3) * 1e-12 / FP64_DMMA_PEAK_TFLOPS,
               "algorithmic_flops_as_printed": ao_flops,

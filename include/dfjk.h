@@ -71,7 +71,9 @@ typedef struct {
                                  the slice products are exact in int32, the recombination is fp64.  Error
                                  bound per element: (S+2) 2^(-7S) sum over groups of
                                  (terms) 2^(e_mu + e_nu); 6 slices keep max|dK|/max|K| <= 1e-10 */
-  int k_emulation_group;      /* aux rows sharing one scale per AO row in the emulated SYRK; 0 = 16, <= 64 */
+  int k_emulation_group;      /* aux rows sharing one scale per AO row in the emulated SYRK; 0 = 16, <= 64.  The int32
+                                 accumulators bound group x (columns of the widest set, rounded up to 32) x slices
+                                 below 2^19 = 524288; dfjk_get_jk returns DFJK_ERR_INVALID_ARG past that */
   int ht_emulation_slices;    /* 0 = half-transform (Eq. 16 / 18) on the native FP64 tensor instruction (default).
                                  3..6 = opt-in emulation on the int8 tensor cores: dfjk_create builds int8 slice
                                  images of the unpacked tensor (S x 1.07 naux nao^2 bytes, one power-of-two scale
@@ -203,7 +205,8 @@ int dfjk_last_launch_count(dfjk_handle h);
  * dfjk_set_profiling(h, 1) makes every later dfjk_get_jk record an event at each phase boundary
  * (a few microseconds each; the event pool grows with the number of aux blocks).
  * dfjk_get_profile synchronises on the last event of the last call and returns, per phase, the
- * summed milliseconds and the number of kernel-launch groups.
+ * summed milliseconds and the number of kernel-launch groups.  dfjk_ao2mo records too: HALF_TRANSFORM =
+ * the Eq. 18 launches, SYRK = the contractions of Eq. 19-21, PREP = everything else.
  */
 enum {
   DFJK_PHASE_PREP = 0,           /* a1: C' and packed weighted density */

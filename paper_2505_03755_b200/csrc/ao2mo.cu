@@ -274,6 +274,7 @@ static int launch_ao2mo_as_printed(dfjk_ctx* h, int nmo, int a0, int nact, const
   SetInfo si;
   si.nset = 1; si.col0[0] = 0; si.nocc[0] = nmo; si.coff[0] = 0; si.ooff[0] = 0;
   si.col0[1] = si.nocc_pad = round_up(nmo, 8);
+  prof_mark(h, DFJK_PHASE_PREP, st);
   launches += launch_prep_ct(h, si, M, nullptr, st);          // C' = M (no occupations)
   const int ldx = si.nocc_pad;
   const size_t row_doubles = (size_t)nao * ldx + n2 + naa;
@@ -288,8 +289,10 @@ static int launch_ao2mo_as_printed(dfjk_ctx* h, int nmo, int a0, int nact, const
   double* baa = bmo + (size_t)nblk * n2;
   for (int p0 = 0; p0 < naux; p0 += (int)nblk) {
     const int nb = (int)(naux - p0 < nblk ? naux - p0 : nblk);
+    prof_mark(h, DFJK_PHASE_HALF_TRANSFORM, st);
     if (launch_half_transform_rowmajor(h, si, p0, nb, Xb, ldx, st) != 0) return -1;      // Eq. 18
     launches++;
+    prof_mark(h, DFJK_PHASE_SYRK, st);
     // Eq. 19 for the whole block as one GEMM: rows (P, p1) stacked along M, bmo[P][p1][p2] = C[(P p1)][p2]
     GemmTN g19{Xb, M, bmo, nb * nmo, nmo, nao, ldx, nmo, nmo, 0, 0, 0, 0, nmo, (long long)nao * ldx};
     if (gemm_tn(h->device, g19, 1, st) != cudaSuccess) return -1;
@@ -307,6 +310,7 @@ static int launch_ao2mo_as_printed(dfjk_ctx* h, int nmo, int a0, int nact, const
     }
   }
   if (papa_out && nact > 0) {
+    prof_mark(h, DFJK_PHASE_SYRK, st);
     GemmTN g21{bpa_out, bpa_out, papa_out, (int)npa, (int)npa, naux, (long long)npa, (long long)npa,
                (long long)npa, 0, 0, 0, 0};
     if (gemm_tn(h->device, g21, 1, st) != cudaSuccess) return -1;                                    // Eq. 21
@@ -355,6 +359,7 @@ static int launch_ao2mo_active_first(dfjk_ctx* h, int nmo, int a0, int nact, con
   if (h->nblk_forced > 0 && nbz > h->nblk_forced) nbz = h->nblk_forced;
   if (nbz > naux) nbz = naux;
   if (nbz > 32768) nbz = 32768;
+  prof_mark(h, DFJK_PHASE_PREP, st);
   k_copy_cols<<<64, 256, 0, st>>>(M, nao, nmo, a0, nact, Mact);
   SetInfo si;
   si.nset = 1; si.col0[0] = 0; si.nocc[0] = nact; si.coff[0] = 0; si.ooff[0] = 0;
@@ -365,11 +370,13 @@ static int launch_ao2mo_active_first(dfjk_ctx* h, int nmo, int a0, int nact, con
   if (!thin) launches += launch_prep_ct(h, si, Mact, nullptr, st);
   for (int p0 = 0; p0 < naux; p0 += (int)nbz) {
     const int nb = (int)(naux - p0 < nbz ? naux - p0 : nbz);
+    prof_mark(h, DFJK_PHASE_HALF_TRANSFORM, st);
     if (thin) {
       if (launch_symm_thin(h, Mact, nact, nact, p0, nb, Z, ldz, st) != 0) return -1;       // Z^P = b^P M_act
     } else if (launch_half_transform_rowmajor(h, si, p0, nb, Z, ldz, st) != 0) {
       return -1;
     }
+    prof_mark(h, DFJK_PHASE_SYRK, st);
     // bpa^P = M^T Z^P for the whole block as one GEMM with rows (P, a) and columns p:
     // C[(P a)][p] = sum_mu Z^P[mu][a] M[mu][p], stored transposed into bpa[P][p][a]
     GemmTN gb{Z, M, bpa_out + (size_t)p0 * npa, nb * nact, nmo, nao, ldz, nmo, 0, 0, 0, 0, 0,
@@ -377,6 +384,7 @@ static int launch_ao2mo_active_first(dfjk_ctx* h, int nmo, int a0, int nact, con
     if (gemm_tn(h->device, gb, 1, st) != cudaSuccess) return -1;
     launches += 2;
   }
+  prof_mark(h, DFJK_PHASE_SYRK, st);
   if (ppaa_out) {
     double* W = h->X;
     double* Wsq = W + h->npair * naa;
@@ -426,6 +434,7 @@ int launch_ao2mo(dfjk_ctx* h, int nmo, int a0, int nact, const double* M, double
   const int n = active ? launch_ao2mo_active_first(h, nmo, a0, nact, M, bpa_out, ppaa_out, papa_out, st)
                        : launch_ao2mo_as_printed(h, nmo, a0, nact, M, bpa_out, ppaa_out, papa_out, st);
   h->plan_ao2mo_route = active ? 2 : 1;
+  prof_mark(h, -1, st);
   return n < 0 ? n : n + launches;
 }
 

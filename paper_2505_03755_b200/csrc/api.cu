@@ -288,7 +288,7 @@ int dfjk_get_jk(dfjk_handle h, int nset, const int* nocc, const double* C, const
   if (K_out) {
     k = launch_k_path(h, si, K_out, fuse, st);
     if (k == -2) {
-      snprintf(h->last_error, sizeof(h->last_error), "workspace cap too small for one aux row of the emulated K path");
+      snprintf(h->last_error, sizeof(h->last_error), "workspace cap too small for one aux row of the emulated K path (or k_emulation_group x columns of a set >= 87381: int32 accumulators)");
       return DFJK_ERR_INVALID_ARG;
     }
     if (k < 0) { set_err(h, "k path launch", cudaGetLastError()); return DFJK_ERR_CUDA; }

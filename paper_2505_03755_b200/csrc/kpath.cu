@@ -877,6 +877,9 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
     const int c0 = si.col0[s], c1 = c0 + si.nocc[s];
     if (c1 > c0 && ((c1 + 31) >> 5) - (c0 >> 5) > emu_nchs) emu_nchs = ((c1 + 31) >> 5) - (c0 >> 5);
   }
+  // the int32 accumulators of one scale group take pgroup * columns products of at most 64 * 64, S of them
+  // per accumulator: the group must stay below 2^31
+  if (emu && (double)h->k_emu_pgroup * 32.0 * emu_nchs * 4096.0 * h->k_emu_slices >= 2147483648.0) return -2;
   const size_t emu_row_bytes = emu ? emu_bytes_per_aux_row(nao, emu_nchs, h->k_emu_slices, h->k_emu_pgroup) : 0;
   long long nblk = (long long)((h->X_doubles * sizeof(double) - (emu ? 4096 : 0)) / (row_doubles * sizeof(double) + emu_row_bytes));
   if (h->nblk_forced > 0 && nblk > h->nblk_forced) nblk = h->nblk_forced;

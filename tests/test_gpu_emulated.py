@@ -104,21 +104,24 @@ def test_emulated_k_with_signed_occupations():
         assert rel(J[s].cpu().numpy(), Jo[s]) <= TOL and rel(K[s].cpu().numpy(), Ko[s]) <= TOL
 
 
-def test_emulated_k_small_config_every_element():
+@pytest.mark.parametrize("name", ["tiny", "small"])
+def test_emulated_configs_every_element(name):
+    """BASELINE.json's two small configs (medium / large / lasscf: test_gpu_full_size.py): SYRK alone and
+    half-transform + SYRK on the int8 tensor cores against the oracle, every element"""
     import oracle
     import torch
     import paper_2505_03755_b200 as dfjk
-    inp = dfjk_inputs.make_config("small")
+    inp = dfjk_inputs.make_config(name)
     Jo, Ko = oracle.get_jk_inputs(inp)
     B = torch.from_numpy(inp.B_packed).cuda()
     Cs = [torch.from_numpy(c).cuda() for c in inp.C]
     occs = [torch.from_numpy(o).cuda() for o in inp.occ]
-    for S in (5, 6):
-        with dfjk.DFJK(B, inp.nao, k_emulation_slices=S) as h:
+    for ht, S in ((0, 5), (0, 6), (5, 5), (6, 6)):
+        with dfjk.DFJK(B, inp.nao, k_emulation_slices=S, ht_emulation_slices=ht) as h:
             J, K = h.get_jk(Cs, occs)
             torch.cuda.synchronize()
         e = rel(K[0].cpu().numpy(), Ko[0])
-        print(f"emulated K, small config, S={S}: max|dK|/max|K| = {e:.2e}")
+        print(f"emulated K, {name} config, half-transform slices {ht}, SYRK slices {S}: max|dK|/max|K| = {e:.2e}")
         assert rel(J[0].cpu().numpy(), Jo[0]) <= TOL
         if S == 6:
             assert e <= TOL

@@ -16,19 +16,17 @@ pytestmark = pytest.mark.gpu
 TOL = 1e-10
 
 
-def _gpu_jk(inp, B=None):
+def _gpu_jk(inp, B, **opts):
     import torch
     import paper_2505_03755_b200 as dfjk
-    if B is None:
-        B = torch.from_numpy(inp.B_packed).cuda()
     Cs = [torch.from_numpy(c).cuda() for c in inp.C]
     occs = [torch.from_numpy(o).cuda() for o in inp.occ]
-    with dfjk.DFJK(B, inp.nao) as h:
+    with dfjk.DFJK(B, inp.nao, **opts) as h:
         J, K = h.get_jk(Cs, occs)
         torch.cuda.synchronize()
         plan = h.plan()
     out = J.cpu().numpy(), K.cpu().numpy(), plan
-    del B, J, K
+    del J, K
     torch.cuda.empty_cache()
     return out
 
@@ -46,14 +44,32 @@ def _assert_every_element(inp, J, K, Jo, Ko, plan):
 
 @pytest.mark.parametrize("name", ["medium", "large", "lasscf"])
 def test_config_every_element(name):
+    """native fp64 path at the default options, then the opt-in FP64-emulated K path (int8 tensor
+    cores) on the same resident tensor against the same oracle result"""
     import oracle
+    import torch
     inp = dfjk_inputs.make_config(name)
-    J, K, plan = _gpu_jk(inp)
+    B = torch.from_numpy(inp.B_packed).cuda()
+    J, K, plan = _gpu_jk(inp, B)
     Jo, Ko = oracle.get_jk_inputs(inp)
     _assert_every_element(inp, J, K, Jo, Ko, plan)
     if name != "medium":
         # the launch configuration the bench times: several aux blocks, split-K, the re-tiled copy
         assert plan["nblk"] < inp.naux and plan["ksplit"] > 1 and plan["retiled"] == 1, plan
+    for S in (6, 5):
+        Je, Ke, plan_e = _gpu_jk(inp, B, ht_emulation_slices=S, k_emulation_slices=S)
+        errs = [np.abs(Ke[s] - Ko[s]).max() / np.abs(Ko[s]).max() for s in range(inp.nset)]
+        ej = max(np.abs(Je[s] - Jo[s]).max() / np.abs(Jo[s]).max() for s in range(inp.nset))
+        print(f"{inp.name} emulated K (half-transform and SYRK on the int8 tensor cores, {S} slices): "
+              f"max|dK|/max|K| = {max(errs):.2e} over all entries of all sets, J {ej:.2e}, plan {plan_e}")
+        assert ej <= TOL                                         # J is never emulated
+        assert all(np.array_equal(Ke[s], Ke[s].T) for s in range(inp.nset))
+        if S == 6:
+            assert max(errs) <= TOL, (name, errs)                # the stated slice count for 1e-10
+        else:
+            assert max(errs) <= 1e-8, (name, errs)
+    del B
+    torch.cuda.empty_cache()
 
 
 def test_ao2mo_at_bench_size_sampled():
