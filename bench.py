@@ -486,6 +486,17 @@ def main():
                             "k_tflops_graph": sfb["k"] / (ms_graph * 1e-3) * 1e-12}
             del graph
             hs.close()
+            if s_launches == 1:
+                # the single-launch path (csrc/small.cu) served this call: the tiled kernels for comparison
+                ht_ = dfjk.DFJK(sB, sinp.nao, no_small_path=True)
+                t_fn = lambda: ht_.get_jk_raw(sinp.nocc, sC, socc, out_j=sJ, out_k=sK, stream=stream)
+                for _ in range(3):
+                    t_fn()
+                torch.cuda.synchronize()
+                small[sname]["path"] = "single launch (small.cu)"
+                small[sname]["tiled_kernels_launches_per_call"] = ht_.last_launch_count
+                small[sname]["tiled_kernels_ms_direct"] = max_over_ranks(timed(t_fn, 100))
+                ht_.close()
     if not lead:
         h.close()
         ranks.close()

@@ -29,7 +29,7 @@ class dfjk_options(ct.Structure):
     _fields_ = [("workspace_cap_bytes", ct.c_size_t), ("nblk", ct.c_int), ("max_nocc_total", ct.c_int),
                 ("max_nset", ct.c_int), ("copy_B", ct.c_int), ("ksplit", ct.c_int), ("no_retile", ct.c_int), ("ao2mo_route", ct.c_int), ("two_pass_j", ct.c_int),
                 ("k_emulation_slices", ct.c_int), ("k_emulation_group", ct.c_int), ("ht_emulation_slices", ct.c_int),
-                ("no_symm_thin", ct.c_int)]
+                ("no_symm_thin", ct.c_int), ("no_small_path", ct.c_int)]
 
 
 def lib_path() -> str:
@@ -103,7 +103,7 @@ class DFJK:
                  max_nocc_total: int = 0, max_nset: int = 0, copy_B: bool = False, ksplit: int = 0,
                  two_pass_j: bool = False, no_retile: bool = False, ao2mo_route: int = 0,
                  k_emulation_slices: int = 0, k_emulation_group: int = 0, ht_emulation_slices: int = 0,
-                 no_symm_thin: bool = False):
+                 no_symm_thin: bool = False, no_small_path: bool = False):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("dfjk needs a CUDA device (sm_100); there is no CPU fallback")
@@ -117,7 +117,7 @@ class DFJK:
         self._B = None if copy_B else B_packed      # borrowed: keep it alive
         self._device = B_packed.device
         opt = dfjk_options(workspace_cap_bytes, nblk, max_nocc_total, max_nset, int(copy_B), ksplit, int(no_retile), int(ao2mo_route), int(two_pass_j),
-                           int(k_emulation_slices), int(k_emulation_group), int(ht_emulation_slices), int(no_symm_thin))
+                           int(k_emulation_slices), int(k_emulation_group), int(ht_emulation_slices), int(no_symm_thin), int(no_small_path))
         h = ct.c_void_p()
         with torch.cuda.device(self._device):
             code = self._lib.dfjk_create(self.naux, self.nao, ct.c_void_p(B_packed.data_ptr() if self.naux else 0),

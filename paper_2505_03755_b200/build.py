@@ -14,7 +14,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
-SOURCES = ["api.cu", "prep.cu", "jpass.cu", "kpath.cu", "ao2mo.cu", "emu.cu", "symm.cu"]
+SOURCES = ["api.cu", "prep.cu", "jpass.cu", "kpath.cu", "ao2mo.cu", "emu.cu", "symm.cu", "small.cu"]
 HEADERS = ["common.cuh", "ctx.h", "pipeline.cuh", os.path.join("..", "..", "include", "dfjk.h")]
 LIB = os.path.join(HERE, "libdfjk.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

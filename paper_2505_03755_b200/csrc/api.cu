@@ -32,7 +32,7 @@ bool dev_alloc(dfjk_ctx* h, T** p, size_t count) {
 void free_all(dfjk_ctx* h) {
   cudaFree(h->B_owned); cudaFree(h->Bt); cudaFree(h->Ct); cudaFree(h->sgnbits); cudaFree(h->Dw); cudaFree(h->rho_part); cudaFree(h->rho); cudaFree(h->rho_ht);
   cudaFree(h->Jp_part); cudaFree(h->X); cudaFree(h->Kpart);
-  cudaFree(h->Bq); cudaFree(h->bscale); cudaFree(h->Ctq); cudaFree(h->cscale);
+  cudaFree(h->ticket); cudaFree(h->Bq); cudaFree(h->bscale); cudaFree(h->Ctq); cudaFree(h->cscale);
   cudaFree(h->C_stage); cudaFree(h->occ_stage); cudaFree(h->J_stage); cudaFree(h->K_stage);
   for (int i = 0; i < h->ev_cap; i++) cudaEventDestroy(h->ev[i]);
   delete[] h->ev;
@@ -143,6 +143,7 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   h->k_emu_pgroup = o.k_emulation_group ? o.k_emulation_group : 16;
   h->ht_emu_slices = o.ht_emulation_slices;
   h->no_symm_thin = o.no_symm_thin;
+  h->no_small_path = o.no_small_path;
   h->ao2mo_route = o.ao2mo_route;
   h->npair = (size_t)nao * (nao + 1) / 2;
   h->nck = cdiv(nao, kHtBK);
@@ -202,6 +203,8 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
   ok = ok && dev_alloc(h, &h->Ct, (size_t)h->nck * h->ct_rows * kHtLd);
   ok = ok && dev_alloc(h, &h->sgnbits, (size_t)h->ct_rows / 32 + 2);
   if (ok && cudaMemset(h->sgnbits, 0, ((size_t)h->ct_rows / 32 + 2) * sizeof(unsigned int)) != cudaSuccess) { cudaGetLastError(); ok = false; }
+  ok = ok && dev_alloc(h, &h->ticket, (size_t)2);
+  if (ok && cudaMemset(h->ticket, 0, 2 * sizeof(unsigned int)) != cudaSuccess) { cudaGetLastError(); ok = false; }
   ok = ok && dev_alloc(h, &h->Dw, (size_t)h->max_nset * h->npair);
   ok = ok && dev_alloc(h, &h->rho_part, (size_t)h->j1_chunks * 8 * naux_pad);
   ok = ok && dev_alloc(h, &h->rho, (size_t)h->max_nset * (naux > 0 ? naux : 1));
@@ -276,6 +279,16 @@ int dfjk_get_jk(dfjk_handle h, int nset, const int* nocc, const double* C, const
   if (!on_handle_device(h)) return DFJK_ERR_INVALID_ARG;
   if (!J_out && !K_out) return DFJK_OK;
   int n = 0, k;
+  // embedding-sized call: one launch does steps a1-a9 (small.cu)
+  if (const int ctas = small_path_ctas(h, si)) {
+    if (launch_small_fused(h, si, ctas, C, occ, J_out, K_out, st) < 0) { set_err(h, "small path launch", cudaGetLastError()); return DFJK_ERR_CUDA; }
+    prof_mark(h, -1, st);
+    h->last_launches = 1;
+    h->plan_nblk = h->naux; h->plan_ksplit = ctas; h->plan_nblocks = 1;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { set_err(h, "kernel launch", e); return DFJK_ERR_CUDA; }
+    return DFJK_OK;
+  }
   n += launch_prep_ct(h, si, C, occ, st);
   // both outputs: rho falls out of the half-transform, so J needs one stream over B instead of two
   const bool fuse = J_out && K_out && !h->two_pass_j && h->naux > 0 && si.nocc_pad > 0 && h->ht_emu_slices == 0;

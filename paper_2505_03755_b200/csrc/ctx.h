@@ -63,6 +63,8 @@ struct dfjk_ctx {
   int k_emu_pgroup;          // aux rows that share one power-of-two scale per AO row in the emulated SYRK
   int ht_emu_slices;         // option: 0 = native fp64 half-transform; 3..6 = emulated on the int8 tensor cores
   int no_symm_thin;          // option: never use the one-pass symmetric thin half-transform (symm.cu)
+  int no_small_path;         // option: never use the single-launch path for embedding-sized calls (small.cu)
+  unsigned int* ticket;      // arrival counter of the single-launch path (zero between calls)
   signed char* Bq;           // emulated half-transform: int8 slice images of the unpacked B (built at create)
   double* bscale;            // [naux][mu_q] power-of-two scale of every row of every slice B_P
   signed char* Ctq;          // int8 slice images of C'^T (per call)
@@ -140,6 +142,10 @@ int emu_i_q(int nocc_pad);
 cudaError_t launch_emu_slice_b(dfjk_ctx* h);
 int launch_emu_slice_ct(dfjk_ctx* h, int nocc_pad, cudaStream_t st);
 int launch_emu_ht(dfjk_ctx* h, int nocc_pad, int p_first, int nb, double* X, int nch, cudaStream_t st);
+// single-launch path for embedding-sized calls (small.cu): CTAs it would use (0 = not eligible); launch
+int small_path_ctas(const dfjk_ctx* h, const SetInfo& si);
+int launch_small_fused(dfjk_ctx* h, const SetInfo& si, int ctas, const double* C, const double* occ, double* J_out,
+                       double* K_out, cudaStream_t st);
 // one-pass symmetric thin half-transform on the packed triangle (symm.cu): <= 8 columns, row-major Z
 bool symm_thin_ok(const dfjk_ctx* h, int ncols);
 int launch_symm_thin(dfjk_ctx* h, const double* M, int ldm, int ncols, int p_first, int nb, double* X, int ldx,

@@ -1,0 +1,235 @@
+// Single-launch path for embedding-sized calls ("N_emb is
+// independent of the system size", "called thousands of times"): when the whole call is
+// a few MFLOP, the seven dependent launches of the tiled path (prep, half-transform, SYRK, rho
+// reduce, J pass 2, two epilogues) cost more than the arithmetic.  Here ONE kernel does steps a1-a9:
+//   phase 1, per CTA, for its aux rows P (round-robin, one or two each):
+//     b^P unpacked into shared memory, X = b^P C' (Eq. 16), rho_s = <X_s, C'_s sign> (Eq. 14,
+//     DESIGN.md R16), K partial += X_s sign X_s^T (Eq. 17, lower triangle), J partial += rho_s b^P (Eq. 15),
+//     both partials private to the CTA (no atomics on data);
+//   grid barrier (the kernel is launched cooperatively: all CTAs are resident);
+//   phase 2, all CTAs: every output element is the sum of the partials in CTA order, written to both
+//     triangles of J and K (deterministic: the assignment of aux rows to CTAs is fixed).
+// Plain DFMA on purpose: this regime is latency-bound, not throughput-bound (tiny config: 13 MFLOP).
+// Chosen by dfjk_get_jk when nao <= 96, nao * sum(nocc) <= 4608 and naux * nao^2 * (sum(nocc) + nset)
+// <= 2^26 (option no_small_path disables it); everything larger takes the tensor-pipe kernels.
+#include "common.cuh"
+#include "ctx.h"
+
+namespace dfjk {
+
+constexpr int kSmThreads = 256;
+constexpr int kSmMaxNao = 96, kSmMaxElems = 4608;
+constexpr double kSmMaxWork = 67108864.0;
+
+struct SmallParams {
+  const double* Bp; size_t npair; int naux, nao;
+  const double* C; const double* occ;
+  double* J; double* K;                   // outputs (either may be nullptr)
+  double* Kpart; double* Jpart;           // [cta][set][nao*nao], [cta][set][npair]
+  unsigned int* ticket;                   // [0] arrivals at the grid barrier, [1] CTAs done (both zero between calls)
+  int ntot;                               // sum of nocc
+};
+
+// packed index -> (mu, nu), mu >= nu: float estimate, exact integer correction
+__device__ __forceinline__ void untri(int pr, int& mu, int& nu) {
+  int m = (int)((sqrtf(8.0f * (float)pr + 1.0f) - 1.0f) * 0.5f);
+  while ((m + 1) * (m + 2) / 2 <= pr) m++;
+  while (m * (m + 1) / 2 > pr) m--;
+  mu = m;
+  nu = pr - m * (m + 1) / 2;
+}
+
+// fixed-tree block sum of one value per thread; result valid in every thread
+__device__ __forceinline__ double block_sum(double v, double* red) {
+  const int tid = threadIdx.x;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  __syncthreads();
+  if ((tid & 31) == 0) red[tid >> 5] = v;
+  __syncthreads();
+  double t = 0.0;
+#pragma unroll
+  for (int w = 0; w < kSmThreads / 32; w++) t += red[w];
+  return t;
+}
+
+__global__ void __launch_bounds__(kSmThreads)
+k_small_fused(const __grid_constant__ SetInfo si, const __grid_constant__ SmallParams q) {
+  extern __shared__ __align__(16) double smem[];
+  const int nao = q.nao, ntot = q.ntot, ldb = nao + 1, tid = threadIdx.x;
+  double* Bs = smem;                      // [nao][nao + 1]   symmetric slice
+  double* Cs = Bs + nao * ldb;            // [nao][ntot]      C' = C sqrt|occ|
+  double* Xs = Cs + nao * ntot;           // [nao][ntot]
+  double* sg = Xs + nao * ntot;           // [ntot]           sign(occ)
+  double* red = sg + ntot;                // [8]
+  __shared__ int c0s[kMaxSets + 1];
+  const size_t n2 = (size_t)nao * nao;
+
+  // a1: C' and the signs; compact column c of set s = si.ooff[s] + i.  sg first holds sqrt|occ|, then sign(occ)
+  if (tid <= si.nset) c0s[tid] = tid < si.nset ? si.ooff[tid] : ntot;
+  for (int c = tid; c < ntot; c += kSmThreads) sg[c] = sqrt(fabs(q.occ[c]));
+  __syncthreads();
+  for (int s = 0; s < si.nset; s++) {
+    const int n = si.nocc[s], o = si.ooff[s];
+    for (int e = tid; e < nao * n; e += kSmThreads) {
+      const int lam = e / n, i = e - lam * n;
+      Cs[lam * ntot + o + i] = q.C[si.coff[s] + e] * sg[o + i];
+    }
+  }
+  __syncthreads();
+  for (int c = tid; c < ntot; c += kSmThreads) sg[c] = q.occ[c] < 0.0 ? -1.0 : 1.0;
+  __syncthreads();
+
+  double* Kp = q.Kpart + (size_t)blockIdx.x * si.nset * n2;
+  double* Jp = q.Jpart + (size_t)blockIdx.x * si.nset * q.npair;
+  bool first = true;
+  for (int P = blockIdx.x; P < q.naux; P += gridDim.x, first = false) {
+    const double* bp = q.Bp + (size_t)P * q.npair;
+    // a5: unpack the packed row into the symmetric slice (flat over the pairs: independent loads)
+    for (int pr = tid; pr < (int)q.npair; pr += kSmThreads) {
+      int mu, nu;
+      untri(pr, mu, nu);
+      const double v = ldg_stream1(bp + pr);
+      Bs[mu * ldb + nu] = v;
+      Bs[nu * ldb + mu] = v;
+    }
+    __syncthreads();
+    // a6: X[mu][c] = sum_lam b[mu][lam] C'[lam][c]; a thread owns column c = e % ntot of rows e / ntot
+    for (int e = tid; e < nao * ntot; e += kSmThreads) {
+      const int mu = e / ntot, c = e - mu * ntot;
+      const double* b = Bs + mu * ldb;
+      // four interleaved partial sums (fixed order): the dependent-DFMA chain is a quarter as long
+      double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;
+      int lam = 0;
+      for (; lam + 4 <= nao; lam += 4) {
+        t0 = fma(b[lam], Cs[lam * ntot + c], t0);
+        t1 = fma(b[lam + 1], Cs[(lam + 1) * ntot + c], t1);
+        t2 = fma(b[lam + 2], Cs[(lam + 2) * ntot + c], t2);
+        t3 = fma(b[lam + 3], Cs[(lam + 3) * ntot + c], t3);
+      }
+      for (; lam < nao; lam++) t0 = fma(b[lam], Cs[lam * ntot + c], t0);
+      Xs[e] = (t0 + t1) + (t2 + t3);
+    }
+    __syncthreads();
+    for (int s = 0; s < si.nset; s++) {
+      const int ca = c0s[s], cb = c0s[s + 1];
+      if (q.J) {
+        // a2 (fused): rho = sum_{mu, c in s} sign_c X[mu][c] C'[mu][c]; a3: J partial += rho * packed row
+        double t = 0.0;
+        for (int e = tid; e < nao * (cb - ca); e += kSmThreads) {
+          const int mu = e / (cb - ca), c = ca + e - mu * (cb - ca);
+          t = fma(Xs[mu * ntot + c] * sg[c], Cs[mu * ntot + c], t);
+        }
+        const double rho = block_sum(t, red);
+        double* jp = Jp + (size_t)s * q.npair;
+        for (size_t pr = tid; pr < q.npair; pr += kSmThreads) {
+          const double v = rho * ldg_stream1(bp + pr);
+          jp[pr] = first ? v : jp[pr] + v;
+        }
+      }
+      if (q.K) {
+        // a7: K partial[mu >= nu] += sum_{c in s} sign_c X[mu][c] X[nu][c]
+        double* kp = Kp + (size_t)s * n2;
+        for (int e = tid; e < nao * nao; e += kSmThreads) {
+          const int mu = e / nao, nu = e - mu * nao;
+          if (nu > mu) continue;
+          const double* xm = Xs + mu * ntot;
+          const double* xn = Xs + nu * ntot;
+          double t = 0.0;
+          for (int c = ca; c < cb; c++) t = fma(xm[c] * sg[c], xn[c], t);
+          kp[e] = first ? t : kp[e] + t;
+        }
+      }
+    }
+    __syncthreads();
+  }
+
+  // grid barrier: every partial is in global memory before anyone sums
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) {
+    atomicAdd(q.ticket, 1u);
+    while (*reinterpret_cast<volatile unsigned int*>(q.ticket) < gridDim.x) {}
+  }
+  __syncthreads();
+  __threadfence();
+  // a4 / a9: every output element = sum of the partials, written to both triangles.  Eight lanes share one
+  // element: lane k sums the partials k, k + 8, ... in ascending order, the eight sums are combined by a
+  // fixed shuffle tree -- the same order in every call
+  const int nparts = gridDim.x;
+  const size_t nout = (size_t)si.nset * q.npair;
+  const int sub = tid & 7;
+  for (size_t o0 = ((size_t)blockIdx.x * kSmThreads + tid) >> 3;; o0 += ((size_t)gridDim.x * kSmThreads) >> 3) {
+    const bool on = o0 < nout;
+    if (__syncthreads_or(on) == 0) break;
+    const size_t o = on ? o0 : 0;
+    const int s = (int)(o / q.npair);
+    const int pr = (int)(o - (size_t)s * q.npair);
+    int mu, nu;
+    untri(pr, mu, nu);
+    const size_t e = (size_t)mu * nao + nu, et = (size_t)nu * nao + mu;
+    double tk = 0.0, tj = 0.0;
+    if (on && q.K)
+      for (int g = sub; g < nparts; g += 8) tk += __ldcg(q.Kpart + ((size_t)g * si.nset + s) * n2 + e);
+    if (on && q.J)
+      for (int g = sub; g < nparts; g += 8) tj += __ldcg(q.Jpart + ((size_t)g * si.nset + s) * q.npair + pr);
+#pragma unroll
+    for (int off = 4; off > 0; off >>= 1) {
+      tk += __shfl_xor_sync(0xffffffffu, tk, off);
+      tj += __shfl_xor_sync(0xffffffffu, tj, off);
+    }
+    if (on && sub == 0) {
+      if (q.K) { q.K[(size_t)s * n2 + e] = tk; q.K[(size_t)s * n2 + et] = tk; }
+      if (q.J) { q.J[(size_t)s * n2 + e] = tj; q.J[(size_t)s * n2 + et] = tj; }
+    }
+  }
+  // the last CTA to finish re-arms the barrier for the next call (every CTA has passed it by then)
+  __syncthreads();
+  if (tid == 0 && atomicAdd(q.ticket + 1, 1u) == gridDim.x - 1) {
+    q.ticket[0] = 0;
+    q.ticket[1] = 0;
+  }
+}
+
+static size_t small_smem_bytes(int nao, int ntot) {
+  return ((size_t)nao * (nao + 1) + 2 * (size_t)nao * ntot + ntot + 16) * sizeof(double);
+}
+
+// 0 = not eligible, else the number of CTAs the fused kernel would use
+int small_path_ctas(const dfjk_ctx* h, const SetInfo& si) {
+  if (h->no_small_path || h->naux < 1 || h->nao > kSmMaxNao || h->k_emu_slices || h->ht_emu_slices) return 0;
+  int ntot = 0;
+  for (int s = 0; s < si.nset; s++) ntot += si.nocc[s];
+  if (ntot < 1 || (long long)h->nao * ntot > kSmMaxElems) return 0;
+  if ((double)h->naux * h->nao * h->nao * (ntot + si.nset) > kSmMaxWork) return 0;
+  // as many CTAs as aux rows, in equal rounds over the SMs (160 aux rows on 148 SMs: 80 CTAs x 2 rows)
+  const int rounds = cdiv(h->naux, h->num_sms);
+  int ctas = cdiv(h->naux, rounds);
+  // the private partials live in the X workspace
+  const size_t need = (size_t)ctas * si.nset * ((size_t)h->nao * h->nao + h->npair);
+  if (need > h->X_doubles) return 0;
+  return ctas;
+}
+
+int launch_small_fused(dfjk_ctx* h, const SetInfo& si, int ctas, const double* C, const double* occ, double* J_out,
+                       double* K_out, cudaStream_t st) {
+  int ntot = 0;
+  for (int s = 0; s < si.nset; s++) ntot += si.nocc[s];
+  const size_t smem = small_smem_bytes(h->nao, ntot);
+  static std::atomic<unsigned long long> attr_done{0};
+  if (ensure_dyn_smem(k_small_fused, (size_t)200 * 1024, h->device, attr_done) != cudaSuccess) return -1;
+  SmallParams p{h->B, h->npair, h->naux, h->nao, C, occ, J_out, K_out, h->X,
+                h->X + (size_t)ctas * si.nset * h->nao * h->nao, h->ticket, ntot};
+  prof_mark(h, DFJK_PHASE_HALF_TRANSFORM, st);
+  // cooperative launch: the grid barrier needs every CTA resident (ctas <= SMs, one CTA per SM fits)
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(ctas); cfg.blockDim = dim3(kSmThreads); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeCooperative;
+  attr[0].val.cooperative = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  if (cudaLaunchKernelEx(&cfg, k_small_fused, si, p) != cudaSuccess) return -1;
+  return 1;
+}
+
+}  // namespace dfjk

@@ -21,11 +21,23 @@ def torch_cuda():
     return torch
 
 
-@pytest.fixture(scope="module")
-def dfjk(torch_cuda):
+@pytest.fixture(scope="module", params=["default", "tiled"])
+def dfjk(request, torch_cuda):
+    """every test of this module runs twice: with the default dispatch (embedding-sized calls take the
+    single-launch path of csrc/small.cu) and with no_small_path=True (always the tensor-pipe kernels)"""
+    import types
     import paper_2505_03755_b200 as pkg
     pkg.load_library()
-    return pkg
+    if request.param == "default":
+        return pkg
+    proxy = types.SimpleNamespace(**{k: getattr(pkg, k) for k in dir(pkg) if not k.startswith("__")})
+
+    def tiled(*a, **kw):
+        kw.setdefault("no_small_path", True)
+        return pkg.DFJK(*a, **kw)
+    proxy.DFJK = tiled
+    proxy.small_path = False
+    return proxy
 
 
 def to_dev(torch, inp):
@@ -65,6 +77,57 @@ def test_dmma_fragment_mapping(dfjk):
 
 def test_tiny_config(torch_cuda, dfjk):
     check_against_oracle(torch_cuda, dfjk, dfjk_inputs.make_config("tiny"))
+
+
+def test_tiny_config_dispatch(torch_cuda, dfjk):
+    """tiny (nao=48, naux=160, nocc=12) is launch-latency bound: one launch by default, seven with
+    no_small_path; small (nao=300) always takes the tensor-pipe kernels"""
+    torch = torch_cuda
+    for name in ("tiny", "small"):
+        inp = dfjk_inputs.make_config(name)
+        B, Cs, occs = to_dev(torch, inp)
+        with dfjk.DFJK(B, inp.nao) as h:
+            h.get_jk(Cs, occs)
+            torch.cuda.synchronize()
+            one = h.last_launch_count == 1
+        assert one == (name == "tiny" and getattr(dfjk, "small_path", True))
+
+
+@pytest.mark.parametrize("nao,naux,nocc,seed,kw", [
+    (96, 20, [48], 171, {}),                                 # the largest basis and column count of the path
+    (80, 170, [40, 0, 8], 172, {}),                          # more aux rows than SMs, an empty set
+    (33, 9, [1] * 16 + [2] * 16, 173, dict(max_nset=32, max_nocc_total=48)),   # 32 sets
+    (1, 2, [1], 174, {}),                                    # a single AO
+    (64, 5, [64], 175, {}),                                  # nocc = nao, fewer aux rows than CTAs
+    (48, 300, [12], 176, {}),                                # ten aux rows per CTA
+])
+def test_single_launch_path(torch_cuda, dfjk, nao, naux, nocc, seed, kw):
+    """shapes inside the single-launch regime: J and K together, J alone, K alone, signed occupations,
+    two calls in a row (the arrival ticket is reset), against the oracle"""
+    import oracle
+    torch = torch_cuda
+    inp = dfjk_inputs.make_random(nao, naux, nocc, seed, L=max(3.0, nao / 6))
+    rs = np.random.default_rng(seed + 1)
+    for o in inp.occ:
+        o *= rs.choice([-1.0, 1.0], size=o.shape)
+    Jo, Ko = oracle.get_jk_inputs(inp)
+    B, Cs, occs = to_dev(torch, inp)
+    with dfjk.DFJK(B, inp.nao, **kw) as h:
+        J, K = h.get_jk(Cs, occs)
+        torch.cuda.synchronize()
+        assert (h.last_launch_count == 1) == getattr(dfjk, "small_path", True)
+        Jonly, _ = h.get_jk(Cs, occs, with_k=False)
+        _, Konly = h.get_jk(Cs, occs, with_j=False)
+        J2, K2 = h.get_jk(Cs, occs)
+        torch.cuda.synchronize()
+        assert torch.equal(J, J2) and torch.equal(K, K2) and torch.equal(K, Konly)
+    for s in range(inp.nset):
+        if nocc[s] == 0:
+            assert not J[s].any() and not K[s].any()
+            continue
+        assert rel(J[s].cpu().numpy(), Jo[s]) <= TOL and rel(K[s].cpu().numpy(), Ko[s]) <= TOL
+        assert rel(Jonly[s].cpu().numpy(), Jo[s]) <= TOL
+        assert torch.equal(J[s], J[s].T) and torch.equal(K[s], K[s].T)
 
 
 def test_small_config(torch_cuda, dfjk):
