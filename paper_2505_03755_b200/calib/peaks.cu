@@ -40,6 +40,31 @@ __global__ void k_dfma(double* out, int iters) {
   if (s == 123.456) out[0] = s;
 }
 
+// Do DMMA (tensor pipe) and DFMA (fp64 pipe) add up?  Even warps run the DMMA loop, odd warps the DFMA loop.
+__global__ void k_mixed(double* out, int iters) {
+  double acc[8][2], f[16];
+#pragma unroll
+  for (int i = 0; i < 8; i++) acc[i][0] = acc[i][1] = 0.0;
+#pragma unroll
+  for (int i = 0; i < 16; i++) f[i] = i;
+  const double a = 1.0 + threadIdx.x * 1e-3, b = 0.5, c = 1e-9;
+  if (((threadIdx.x >> 5) & 1) == 0) {
+    for (int it = 0; it < iters; it++)
+#pragma unroll
+      for (int i = 0; i < 8; i++) dmma(acc[i][0], acc[i][1], a, b);       // 8 x 512 flop per warp and iteration
+  } else {
+    for (int it = 0; it < iters; it++)
+#pragma unroll
+      for (int i = 0; i < 64; i++) f[i & 15] = fma(f[i & 15], a, c);      // 64 x 64 flop per warp and iteration
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 8; i++) s += acc[i][0] + acc[i][1];
+#pragma unroll
+  for (int i = 0; i < 16; i++) s += f[i];
+  if (s == 123.456) out[0] = s;
+}
+
 template <int U>
 __global__ void k_read(const double2* __restrict__ p, size_t n, double* out) {
   double s = 0.0;
@@ -72,6 +97,7 @@ static float time_ms(void (*launch)(void*), void* ctx) {
 struct Ctx { double* out; int warps; int iters; const double2* p; size_t n; int ctas; int threads; };
 template <int NACC> void l_dmma(void* c) { Ctx* x = (Ctx*)c; k_dmma<NACC><<<148, 32 * x->warps>>>(x->out, x->iters); }
 template <int NACC> void l_dfma(void* c) { Ctx* x = (Ctx*)c; k_dfma<NACC><<<148, 32 * x->warps>>>(x->out, x->iters); }
+void l_mixed(void* c) { Ctx* x = (Ctx*)c; k_mixed<<<148, 32 * x->warps>>>(x->out, x->iters); }
 template <int U> void l_read(void* c) { Ctx* x = (Ctx*)c; k_read<U><<<148 * x->ctas, x->threads>>>(x->p, x->n, x->out); }
 
 int main() {
@@ -92,6 +118,12 @@ int main() {
     }
     ms = time_ms(l_dfma<16>, &c);
     printf("dfma nacc=16 warps/SM=%2d  %7.3f ms  %6.2f TFLOP/s\n", warps, ms, 148.0 * warps * 32 * iters * 16 * 2.0 / ms * 1e-9);
+  }
+  for (int warps : {8, 16}) {                                           // half of the warps DMMA, the other half DFMA
+    c.warps = warps;
+    const float ms = time_ms(l_mixed, &c);
+    const double tm = 148.0 * (warps / 2) * iters * 8 * 512 / ms * 1e-9, tf = 148.0 * (warps / 2) * iters * 64 * 64 / ms * 1e-9;
+    printf("mixed warps/SM=%2d  %7.3f ms  dmma %6.2f + dfma %6.2f = %6.2f TFLOP/s\n", warps, ms, tm, tf, tm + tf);
   }
   c.warps = 16; c.iters = 40000 * 240;                                  // ~2.5 s: sustained
   float ms = time_ms(l_dmma<8>, &c);
