@@ -35,8 +35,9 @@ struct GemmTN {
   long long c_gstride = 0, c_nstride = 0;
 };
 
-// CTA tile (16 WTM) x (32 WTN); consumers 2 (M) x 4 (N), warp tile WTM x WTN MMA tiles (WTM = 4 in
-// the product: 64 x up to 352).
+// CTA tile (8 WTM WGM) x (8 WTN WGN), WGM x WGN = 8 consumer warps, warp tile WTM x WTN MMA tiles.  WGM = 2:
+// 2 (M) x 4 (N) warps, 64 or 128 rows x up to 352 columns; WGM = 8: all warps along M, 128 rows x 8 WTN columns
+// for tall and narrow products whose N is not a multiple of 32 (W of the active-first route, N = 36).
 // Shared-memory tiles are k-major, [16][TM + 4] and [16][TN + 4]: the row stride is 4 mod 16
 // doubles, so the fragment reads tile[k = l%4][row = l/4] hit 16 distinct banks per half-warp.
 // Producers: BULK = true -- both operands are plain k-major matrices whose rows start 16-byte aligned
@@ -45,10 +46,13 @@ struct GemmTN {
 // warp issue the 32 row copies of a stage, completion is counted in bytes.  Columns past M or N are
 // never stored, so tails need no zero fill.  BULK = false -- 8-byte cp.async gathers (any alignment,
 // grouped A rows, zero-fill past M, N, K).
-template <int WTM, int WTN, bool BULK>
+template <int WTM, int WTN, bool BULK, int WGM = 2>
 __global__ void __launch_bounds__(kGThreads, 1)
 k_gemm_tn(const __grid_constant__ GemmTN g) {
-  constexpr int TM = 16 * WTM, TN = 32 * WTN, LA = TM + 4, LB = TN + 4;
+  constexpr int WGN = 8 / WGM;
+  constexpr int TM = 8 * WTM * WGM, TN = 8 * WTN * WGN, LA = TM + 4, LB = TN + 4;
+  static_assert(LA % 16 == 4 || LA % 16 == 12, "A tile row stride must be +-4 mod 16 doubles");
+  static_assert(LB % 16 == 4 || LB % 16 == 12, "B tile row stride must be +-4 mod 16 doubles");
   constexpr int kStageDoubles = kGKC * (LA + LB);
   extern __shared__ __align__(128) double smem[];
   __shared__ __align__(8) unsigned long long bars[2 * kGStages];
@@ -73,7 +77,7 @@ k_gemm_tn(const __grid_constant__ GemmTN g) {
     // ===================== producer warpgroup =====================
     reg_dec<kProducerRegs>();
     const int tp = tid - 256;
-    if (BULK) {
+    if constexpr (BULK) {
       if (tp >= kGKC) return;               // lane k of the first producer warp owns k row k of every stage
       const int mrows = min(TM, g.M - m0), ncols = min(TN, g.N - n0);
       const uint32_t a_bytes = (uint32_t)mrows * 8u, b_bytes = (uint32_t)ncols * 8u;
@@ -93,7 +97,7 @@ k_gemm_tn(const __grid_constant__ GemmTN g) {
         }
       }
       return;
-    }
+    } else {
     // a thread keeps its columns for the whole kernel: one column m of the A tile (k rows tp / TM,
     // + 128 / TM, ...) and the columns tp, tp + 128, ... of the B tile; only k moves per chunk
     static_assert(128 % TM == 0 || TM % 128 == 0, "A tile width must divide or be a multiple of 128");
@@ -142,12 +146,13 @@ k_gemm_tn(const __grid_constant__ GemmTN g) {
       cp_async_mbar_arrive_noinc(full0 + 8 * stage);
     }
     return;
+    }
   }
 
   // ===================== consumer warpgroups =====================
   reg_inc<kConsumerRegs>();
   const int r = l >> 2, j = l & 3;
-  const int wm = w & 1, wn = w >> 1;
+  const int wm = w % WGM, wn = w / WGM;
   double acc[WTM][WTN][2];
 #pragma unroll
   for (int t = 0; t < WTM; t++)
@@ -202,16 +207,16 @@ __global__ void k_zero_ao(double* p, size_t n) {
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = 0.0;
 }
 
-template <int WTM, int WTN, bool BULK>
+template <int WTM, int WTN, bool BULK, int WGM = 2>
 static cudaError_t launch_gemm_tn_b(int device, const GemmTN& g, int batch, cudaStream_t st) {
-  constexpr int TM = 16 * WTM, TN = 32 * WTN;
+  constexpr int TM = 8 * WTM * WGM, TN = 8 * WTN * (8 / WGM);
   constexpr size_t smem = (size_t)kGStages * kGKC * (TM + 4 + TN + 4) * sizeof(double);
   static std::atomic<unsigned long long> attr_done{0};
-  cudaError_t e = ensure_dyn_smem(k_gemm_tn<WTM, WTN, BULK>, smem, device, attr_done);
+  cudaError_t e = ensure_dyn_smem(k_gemm_tn<WTM, WTN, BULK, WGM>, smem, device, attr_done);
   if (e != cudaSuccess) return e;
   if (g.M <= 0 || g.N <= 0 || batch <= 0) return cudaSuccess;
   dim3 grid(cdiv(g.M, TM), cdiv(g.N, TN), batch);
-  k_gemm_tn<WTM, WTN, BULK><<<grid, kGThreads, smem, st>>>(g);
+  k_gemm_tn<WTM, WTN, BULK, WGM><<<grid, kGThreads, smem, st>>>(g);
   return cudaSuccess;
 }
 
@@ -222,10 +227,10 @@ static bool gemm_tn_bulk_ok(const GemmTN& g) {
          even(g.sA) && even(g.sB) && even(g.M) && even(g.N) && (g.K & 3) == 0;
 }
 
-template <int WTM, int WTN>
+template <int WTM, int WTN, int WGM = 2>
 static cudaError_t launch_gemm_tn(int device, const GemmTN& g, int batch, cudaStream_t st) {
-  return gemm_tn_bulk_ok(g) ? launch_gemm_tn_b<WTM, WTN, true>(device, g, batch, st)
-                            : launch_gemm_tn_b<WTM, WTN, false>(device, g, batch, st);
+  return gemm_tn_bulk_ok(g) ? launch_gemm_tn_b<WTM, WTN, true, WGM>(device, g, batch, st)
+                            : launch_gemm_tn_b<WTM, WTN, false, WGM>(device, g, batch, st);
 }
 
 // CTA tile 64 x (32 WTN): the N tile is fitted to the problem (at most 352 columns per tile, the
@@ -233,6 +238,8 @@ static cudaError_t launch_gemm_tn(int device, const GemmTN& g, int batch, cudaSt
 static cudaError_t gemm_tn(int device, const GemmTN& g, int batch, cudaStream_t st) {
   const int n8 = cdiv(g.N > 0 ? g.N : 1, 8);
   const int ntn = cdiv(n8, 44), wtn = cdiv(n8, 4 * ntn);
+  if (g.N > 32 && g.N <= 40 && g.M >= 128 * 148)   // 36 packed (a1 >= a2) pairs of 8 active orbitals: 128 x 40 tiles
+    return launch_gemm_tn<2, 5, 8>(device, g, batch, st);
   if (wtn <= 2 && g.M >= 128 * 148) {       // narrow and tall (W of the active-first route): 128-row tiles
     return wtn == 1 ? launch_gemm_tn<8, 1>(device, g, batch, st) : launch_gemm_tn<8, 2>(device, g, batch, st);
   }
@@ -327,14 +334,32 @@ __global__ void k_copy_cols(const double* __restrict__ M, int nao, int nmo, int 
   }
 }
 
-// Wsq[e1][e2][a] = Wsq[e2][e1][a] = W[tri(e1) + e2][a], e1 >= e2
-__global__ void k_unpack_w(const double* __restrict__ W, int nao, int naa, double* __restrict__ Wsq) {
+// baat[P][tri(a1) + a2] = bpa[P][a0 + a1][a2], a1 >= a2: the active-active block of bmo^P is symmetric, so the
+// W contraction only needs its nact (nact + 1) / 2 distinct columns (zero padded to ldt)
+__global__ void k_pack_baa(const double* __restrict__ bpa, int naux, size_t npa, int a0, int nact, int ldt,
+                           double* __restrict__ baat) {
+  for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < (size_t)naux * ldt; e += (size_t)gridDim.x * blockDim.x) {
+    const size_t P = e / ldt;
+    const int t = (int)(e - P * ldt);
+    int a1 = 0;
+    while ((a1 + 1) * (a1 + 2) / 2 <= t) a1++;
+    const int a2 = t - a1 * (a1 + 1) / 2;
+    baat[e] = a1 < nact ? bpa[P * npa + (size_t)(a0 + a1) * nact + a2] : 0.0;
+  }
+}
+
+// Wsq[e1][e2][a1 nact + a2] = W[tri(max(e1,e2)) + min(e1,e2)][tri(max(a1,a2)) + min(a1,a2)]; W element (pair, t) sits at
+// pair * pstride + t * tstride (either orientation of the W product)
+__global__ void k_unpack_w(const double* __restrict__ W, int nao, int nact, long long pstride, long long tstride,
+                           double* __restrict__ Wsq) {
+  const int naa = nact * nact;
   const size_t n = (size_t)nao * nao * naa;
   for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
-    const int a = (int)(e % naa);
+    const int a = (int)(e % naa), a1 = a / nact, a2 = a - a1 * nact;
     const size_t ee = e / naa;
     const int e1 = (int)(ee / nao), e2 = (int)(ee % nao);
-    Wsq[e] = W[(e1 >= e2 ? tri(e1) + e2 : tri(e2) + e1) * naa + a];
+    const int t = a1 >= a2 ? a1 * (a1 + 1) / 2 + a2 : a2 * (a2 + 1) / 2 + a1;
+    Wsq[e] = W[(e1 >= e2 ? tri(e1) + e2 : tri(e2) + e1) * pstride + t * tstride];
   }
 }
 
@@ -343,7 +368,7 @@ __global__ void k_unpack_w(const double* __restrict__ W, int nao, int naa, doubl
 //      Z^P = b^P M_act (nao x nact),   bpa^P = M^T Z^P,
 // and Eq. 20 is contracted over P in the AO basis first (a Coulomb-like build with the nact^2
 // "densities" baa^P, Eq. 15's pattern), then transformed:
-//      W[e1 e2][a1 a2] = sum_P b^P[e1][e2] bpa^P[a0+a1][a2],
+//      W[e1 e2][a1 a2] = sum_P b^P[e1][e2] bpa^P[a0+a1][a2]      (only the a1 >= a2 columns: baa^P is symmetric),
 //      ppaa[p1][p2][a1 a2] = sum_{e1 e2} M[e1][p1] W[e1 e2][a1 a2] M[e2][p2].
 // Work 2 naux nao^2 nact + naux nao^2 nact^2 + small, against 2 naux nao nmo (nao + nmo) for the
 // printed order: 5x less at nmo = 340, nact = 8; the printed order wins for large active spaces.
@@ -386,19 +411,29 @@ static int launch_ao2mo_active_first(dfjk_ctx* h, int nmo, int a0, int nact, con
   }
   prof_mark(h, DFJK_PHASE_SYRK, st);
   if (ppaa_out) {
+    const int ldt = round_up(nact * (nact + 1) / 2, 2);
     double* W = h->X;
-    double* Wsq = W + h->npair * naa;
+    double* Wsq = W + h->npair * ldt;
     double* T = Wsq + (size_t)nao * nao * naa;
-    GemmTN gw{h->B, bpa_out + (size_t)a0 * nact, W, (int)h->npair, (int)naa, naux, (long long)h->npair,
-              (long long)npa, (long long)naa, 0, 0, 0, 0};
-    if (gemm_tn(h->device, gw, 1, st) != cudaSuccess) return -1;                                      // W = sum_P b^P (x) baa^P
-    k_unpack_w<<<1184, 256, 0, st>>>(W, nao, (int)naa, Wsq);
+    double* baat = T + (size_t)nmo * nao * naa;
+    k_pack_baa<<<148, 256, 0, st>>>(bpa_out, naux, npa, a0, nact, ldt, baat);
+    // W = sum_P b^P (x) baa^P.  With bulk-copyable operands the product runs transposed, Wt[t][pair] = baat^T B
+    // (40 x 256 tiles, 20 accumulator tiles per warp); otherwise as W[pair][t] = B^T baat
+    GemmTN gwt{baat, h->B, W, ldt, (int)h->npair, naux, (long long)ldt, (long long)h->npair, (long long)h->npair, 0, 0, 0, 0};
+    const bool wt = ldt > 32 && ldt <= 40 && gemm_tn_bulk_ok(gwt);
+    if (wt) {
+      if (launch_gemm_tn_b<5, 4, true, 1>(h->device, gwt, 1, st) != cudaSuccess) return -1;
+    } else {
+      GemmTN gw{h->B, baat, W, (int)h->npair, ldt, naux, (long long)h->npair, (long long)ldt, (long long)ldt, 0, 0, 0, 0};
+      if (gemm_tn(h->device, gw, 1, st) != cudaSuccess) return -1;
+    }
+    k_unpack_w<<<1184, 256, 0, st>>>(W, nao, nact, wt ? 1 : ldt, wt ? (long long)h->npair : 1LL, Wsq);
     GemmTN gt{M, Wsq, T, nmo, (int)(nao * naa), nao, nmo, (long long)(nao * naa), (long long)(nao * naa), 0, 0, 0, 0};
     if (gemm_tn(h->device, gt, 1, st) != cudaSuccess) return -1;                                      // T[p1][e2 a] = M^T W
     GemmTN gp{M, T, ppaa_out, nmo, (int)naa, nao, nmo, (long long)naa, (long long)naa, 0, (long long)(nao * naa),
               (long long)(nmo * naa), 0};
     if (gemm_tn(h->device, gp, nmo, st) != cudaSuccess) return -1;                                    // ppaa[p1][p2][a] = T_p1^T M
-    launches += 4;
+    launches += 5;
   }
   if (papa_out) {
     GemmTN g21{bpa_out, bpa_out, papa_out, (int)npa, (int)npa, naux, (long long)npa, (long long)npa,
@@ -422,9 +457,10 @@ int launch_ao2mo(dfjk_ctx* h, int nmo, int a0, int nact, const double* M, double
   }
   const double dn = nao, dm = nmo, da = nact;
   const double cost_printed = 2.0 * dn * dm * (dn + dm) + 2.0 * dm * dm * da * da;          // per aux row
-  const double cost_active = 2.0 * dn * dn * round_up(nact, 8) + 2.0 * dn * dm * 32.0 + dn * dn * da * da +
+  const double cost_active = 2.0 * dn * dn * round_up(nact, 8) + 2.0 * dn * dm * 32.0 + dn * dn * da * (da + 1.0) * 0.5 +
                              2.0 * dn * dm * da * da * (dn + dm) / (naux > 0 ? naux : 1);
-  const size_t need2 = h->npair * naa + (size_t)nao * nao * naa + (size_t)nmo * nao * naa;  // W, Wsq, T
+  const size_t need2 = h->npair * round_up(nact * (nact + 1) / 2, 2) + (size_t)nao * nao * naa + (size_t)nmo * nao * naa +
+                       (size_t)naux * round_up(nact * (nact + 1) / 2, 2);                     // W, Wsq, T, packed baa
   const size_t need1 = (size_t)round_up(nao * nact, 2) + (size_t)nao * round_up(nact, 8);   // Mact + one row of Z
   const bool fits = nact > 0 && need2 <= h->X_doubles && need1 <= h->X_doubles && (double)nao * naa < 2e9 &&
                     round_up(nact, 8) <= h->nocc_pad_cap;
