@@ -150,6 +150,7 @@ int launch_small_fused(dfjk_ctx* h, const SetInfo& si, int ctas, const double* C
 bool symm_thin_ok(const dfjk_ctx* h, int ncols);
 int launch_symm_thin(dfjk_ctx* h, const double* M, int ldm, int ncols, int p_first, int nb, double* X, int ldx,
                      cudaStream_t st);
+int launch_symm_thin_jk(dfjk_ctx* h, int ncols, int p_first, int nb, double* X, double* rho, cudaStream_t st);
 size_t retile_doubles_per_aux_row(int nao);
 cudaError_t launch_retile(const double* Bp, size_t npair, int nao, int naux, double* Bt);
 int run_dmma_selftest();

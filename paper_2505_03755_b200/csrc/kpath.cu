@@ -918,6 +918,7 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
   }
 
   const bool emu_ht = h->ht_emu_slices > 0;
+  const bool thin = !emu && !emu_ht && si.nset == 1 && ldx == 8 && symm_thin_ok(h, si.nocc[0]);
   if (emu_ht) {
     prof_mark(h, DFJK_PHASE_PREP, st);
     launches += launch_emu_slice_ct(h, ldx, st);
@@ -934,7 +935,10 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
     for (int s = 0; s <= si.nset; s++) a.col0[s] = si.col0[s];
     const long long ht_tiles = (long long)nb * ntm_ht * ntn;
     const int ht_grid = (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid);
-    if (emu_ht) {
+    if (thin) {
+      // one set of at most 8 columns: one pass over the packed triangle (symm.cu), rho written directly
+      if (launch_symm_thin_jk(h, si.nocc[0], p0, nb, h->X, want_rho ? h->rho : nullptr, st) != 0) return -1;
+    } else if (emu_ht) {
       if (launch_emu_ht(h, ldx, p0, nb, h->X, nch, st) < 0) return -1;
     } else if (dispatch_ht(h->device, wn, want_rho ? 1 : 0, ht_grid, st, a) != cudaSuccess) {
       return -1;
@@ -966,7 +970,7 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
     k_k_epilogue<<<ge, be, 0, st>>>(h->Kpart + n2 * s, ksplit, split_stride, nao, K_out + n2 * s);
     launches++;
   }
-  if (want_rho) {
+  if (want_rho && !thin) {
     prof_mark(h, DFJK_PHASE_J1, st);
     dim3 gr(cdiv(naux, 128), si.nset);
     k_rho_reduce<<<gr, 128, 0, st>>>(h->rho_ht, ntm_ht * ntn * 8, si.nset, naux, h->rho);

@@ -66,10 +66,17 @@ __device__ __forceinline__ int sy_invperm(int a) { return (int)((0x37621540u >> 
 struct SymmParams {
   const double* Bp; size_t npair; size_t b_elems;   // packed tensor (16-byte aligned), elements it holds
   int nao;
-  const double* M; int ldm, ncols;                  // right-hand side M[lam * ldm + a], a < ncols <= 8
-  double* X; int ldx, xrows;                        // out, row-major: X[(pl * xrows + mu) * ldx + a], a < 8
+  // right-hand side, element (lam, a), a < ncols <= 8, at M[(lam >> m_sh) * m_hi + (lam & m_msk) * m_lo + a * m_a]:
+  // row-major M[lam * ldm + a] (AO2MO), or the k-tiled C'^T of k_prep_ct (JK call on one thin set)
+  const double* M; int ncols; int m_sh, m_msk; long long m_hi, m_lo, m_a;
+  double* X; long long x_pstride, x_rstride;        // out: X[pl * x_pstride + mu * x_rstride + a], a < 8 (strides even)
   int p_first, nb;                                  // aux rows [p_first, p_first + nb)
+  double* rho; const unsigned int* sgn;             // optional: rho[p_first + pl] = sum_{mu, a} sign_a Z[mu][a] M[mu][a] (Eq. 14, R16)
 };
+
+__device__ __forceinline__ double sy_m(const SymmParams& q, int lam, int a) {
+  return __ldg(q.M + (size_t)(lam >> q.m_sh) * q.m_hi + (size_t)(lam & q.m_msk) * q.m_lo + (size_t)a * q.m_a);
+}
 
 template <int NW, int G, int LC, int STAGES, bool MREG>
 __global__ void __launch_bounds__(32 * NW + 128, 1)
@@ -83,6 +90,7 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
   double* zd = smem + kSyStages * kSyStageDoubles;      // [2][8][kSyG][64]
   double* Mp = zd + Cfg::kZdDoubles;                    // !MREG: [column block][lane][h] = M[8 Jb + 4h + j][r]
   __shared__ __align__(8) unsigned long long bars[2 * kSyStages];
+  __shared__ double rho_red[NW];
   const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kSyStages]);
   const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
   const int nao = q.nao;
@@ -93,7 +101,7 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
   if (!MREG)
     for (int e = tid; e < Cfg::kMpDoubles; e += kSyThreads) {
       const int h = e & 1, ln = (e >> 1) & 31, lam = 8 * (e >> 6) + 4 * h + (ln & 3), a = ln >> 2;
-      Mp[e] = (a < q.ncols && lam < nao) ? __ldg(q.M + (size_t)lam * q.ldm + a) : 0.0;
+      Mp[e] = (a < q.ncols && lam < nao) ? sy_m(q, lam, a) : 0.0;
     }
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   if (tid == 0) {
@@ -164,7 +172,7 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
 #pragma unroll
       for (int h = 0; h < 2; h++) {
         const int lam = 8 * (NW * sl + w) + 4 * h + j;
-        Mf[sl][h] = (col_ok && lam < nao) ? __ldg(q.M + (size_t)lam * q.ldm + r) : 0.0;
+        Mf[sl][h] = (col_ok && lam < nao) ? sy_m(q, lam, r) : 0.0;
       }
   }
   const double* Mp_lane = Mp + (w * 32 + l) * 2;         // + 64 NW sl: this warp's column block NW sl + w
@@ -192,7 +200,7 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
 #pragma unroll
         for (int g = 0; g < 2; g++) {
           const int mu = sgx * kSyRows + 8 * gi + sy_perm(4 * g + j);
-          dst[gi][g] = (col_ok && mu < nao) ? __ldg(q.M + (size_t)mu * q.ldm + r) : 0.0;
+          dst[gi][g] = (col_ok && mu < nao) ? sy_m(q, mu, r) : 0.0;
         }
     };
     double tB[kSyG][2], tBn[kSyG][2];
@@ -280,7 +288,7 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
               const int lam = 8 * I + 4 * h + j;
               double a = gb[r * kSyS + (bpar ^ (r >> 2)) + 4 * h + j];
               if (4 * h + j > pr) a = 0.0;
-              const double b = (col_ok && lam < nao) ? __ldg(q.M + (size_t)lam * q.ldm + r) : 0.0;
+              const double b = (col_ok && lam < nao) ? sy_m(q, lam, r) : 0.0;
               dmma884(Zd[gi][0], Zd[gi][1], a, b);
             }
 #pragma unroll
@@ -323,11 +331,36 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
       }
     }
     // Z of this aux row: block Jb = 8 sl + w, rows 8 Jb + r, columns 2j, 2j + 1
-    double* Xp = q.X + (size_t)pl * q.xrows * q.ldx;
+    double* Xp = q.X + (size_t)pl * q.x_pstride;
 #pragma unroll
     for (int sl = 0; sl < kSyNSLOT; sl++) {
       const int mu = 8 * (NW * sl + w) + r;
-      if (mu < nao) *reinterpret_cast<double2*>(Xp + (size_t)mu * q.ldx + 2 * j) = make_double2(Zt[sl][0], Zt[sl][1]);
+      if (mu < nao) *reinterpret_cast<double2*>(Xp + (size_t)mu * q.x_rstride + 2 * j) = make_double2(Zt[sl][0], Zt[sl][1]);
+    }
+    if (q.rho) {
+      // rho_P = sum_{mu, a} sign_a Z[mu][a] M[mu][a]: lanes -> warp (xor tree), warps -> CTA in warp order
+      const unsigned int sw = __ldg(q.sgn) >> (2 * j);
+      const double s0 = (sw & 1u) ? -1.0 : 1.0, s1 = (sw & 2u) ? -1.0 : 1.0;
+      const bool c0_ok = 2 * j < q.ncols, c1_ok = 2 * j + 1 < q.ncols;
+      double t = 0.0;
+#pragma unroll
+      for (int sl = 0; sl < kSyNSLOT; sl++) {
+        const int mu = 8 * (NW * sl + w) + r;
+        if (mu < nao) {
+          if (c0_ok) t = fma(Zt[sl][0] * s0, sy_m(q, mu, 2 * j), t);
+          if (c1_ok) t = fma(Zt[sl][1] * s1, sy_m(q, mu, 2 * j + 1), t);
+        }
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+      if (l == 0) rho_red[w] = t;
+      asm volatile("bar.sync 1, %0;" ::"n"(32 * NW) : "memory");
+      if (w == 0 && l == 0) {
+        double v = 0.0;
+#pragma unroll
+        for (int ww = 0; ww < NW; ww++) v += rho_red[ww];
+        q.rho[q.p_first + pl] = v;
+      }
     }
   }
 }
@@ -348,14 +381,27 @@ bool symm_thin_ok(const dfjk_ctx* h, int ncols) {
   return !h->no_symm_thin && h->b_aligned16 && h->nao <= kSyMaxNao && ncols >= 1 && ncols <= 8 && h->naux > 0;
 }
 
-// Z[pl][mu][a] (row-major, row stride ldx >= 8, even) for the aux rows [p_first, p_first + nb)
-int launch_symm_thin(dfjk_ctx* h, const double* M, int ldm, int ncols, int p_first, int nb, double* X, int ldx,
-                     cudaStream_t st) {
-  SymmParams p{h->B, h->npair, (size_t)h->naux * h->npair, h->nao, M, ldm, ncols, X, ldx, h->nao, p_first, nb};
+static int launch_symm(dfjk_ctx* h, const SymmParams& p, int nb, cudaStream_t st) {
   const int grid = nb < h->num_sms ? nb : h->num_sms;
   // measured at nao = 1200, naux = 4000 (B200): 16 rows x 256 columns per stage, 3 stages, B fragments in shared
   // memory 4.3 ms; 32 x 128 x 3: 4.4; register-resident B fragments (32 x 128 x 5): 4.9-5.4; 16 consumer warps: 4.8
   return launch_symm_cfg<8, 2, 256, 3, false>(h, p, grid, st);
+}
+
+// AO2MO: Z[pl][mu][a] (row-major, row stride ldx >= 8, even) for the aux rows [p_first, p_first + nb), M row-major
+int launch_symm_thin(dfjk_ctx* h, const double* M, int ldm, int ncols, int p_first, int nb, double* X, int ldx,
+                     cudaStream_t st) {
+  SymmParams p{h->B, h->npair, (size_t)h->naux * h->npair, h->nao, M, ncols, 0, 0, ldm, 0, 1,
+               X, (long long)h->nao * ldx, ldx, p_first, nb, nullptr, nullptr};
+  return launch_symm(h, p, nb, st);
+}
+
+// JK call on one set of at most 8 columns: X k-tiled for k_syrk2 (one 32-column chunk), C' from the k-tiled Ct of
+// k_prep_ct, rho[P] (Eq. 14 through the half-transformed block, R16) when rho != nullptr
+int launch_symm_thin_jk(dfjk_ctx* h, int ncols, int p_first, int nb, double* X, double* rho, cudaStream_t st) {
+  SymmParams p{h->B, h->npair, (size_t)h->naux * h->npair, h->nao, h->Ct, ncols, 4, 15, (long long)h->ct_rows * kHtLd, 1, kHtLd,
+               X, (long long)h->mu_pad * kLdT, kLdT, p_first, nb, rho, h->sgnbits};
+  return launch_symm(h, p, nb, st);
 }
 
 }  // namespace dfjk

@@ -414,3 +414,39 @@ def test_error_codes(torch_cuda, dfjk):
     lib = dfjk.load_library()
     assert lib.dfjk_destroy(None) == 0
     assert lib.dfjk_strerror(4).decode().startswith("unsupported")
+
+
+@pytest.mark.parametrize("nao,naux,nocc,seed,opts", [
+    (130, 30, [5], 181, {}),                          # npair odd: odd aux rows start 8-byte aligned
+    (200, 170, [8], 182, {}),                         # more aux rows than SMs
+    (263, 21, [3], 183, dict(nblk=4)),                # several aux blocks: rho written block by block
+    (1203, 6, [7], 184, {}),                          # ragged, all 20 column blocks per warp
+    (520, 9, [8], 185, dict(two_pass_j=True)),        # rho from the two-pass J, X from the thin kernel
+])
+def test_one_thin_set_takes_the_one_pass_half_transform(torch_cuda, dfjk, nao, naux, nocc, seed, opts):
+    """a JK call on one set of at most 8 orbitals (a fragment's active space): the half-transform streams the
+    packed triangle once (k_symm_thin) and writes rho itself; signed occupations; against the oracle and
+    against the tiled kernel (no_symm_thin)"""
+    import oracle
+    torch = torch_cuda
+    inp = dfjk_inputs.make_random(nao, naux, nocc, seed, L=max(4.0, nao / 6))
+    inp.occ[0][::2] *= -1.0
+    Jo, Ko = oracle.get_jk_inputs(inp)
+    B, Cs, occs = to_dev(torch, inp)
+    res = []
+    for extra in ({}, dict(no_symm_thin=True)):
+        with dfjk.DFJK(B, inp.nao, **opts, **extra) as h:
+            J, K = h.get_jk(Cs, occs)
+            n_both = h.last_launch_count
+            _, Konly = h.get_jk(Cs, occs, with_j=False)
+            Jonly, _ = h.get_jk(Cs, occs, with_k=False)
+            torch.cuda.synchronize()
+            assert torch.equal(K, Konly)
+        assert rel(J[0].cpu().numpy(), Jo[0]) <= TOL and rel(K[0].cpu().numpy(), Ko[0]) <= TOL
+        assert rel(Jonly[0].cpu().numpy(), Jo[0]) <= TOL
+        assert torch.equal(J[0], J[0].T) and torch.equal(K[0], K[0].T)
+        res.append((J, K, n_both))
+    assert rel(res[0][0].cpu().numpy(), res[1][0].cpu().numpy()) <= 1e-12
+    assert rel(res[0][1].cpu().numpy(), res[1][1].cpu().numpy()) <= 1e-12
+    if not opts.get("two_pass_j"):
+        assert res[0][2] == res[1][2] - 1                    # no rho-reduce launch: the thin kernel writes rho
