@@ -54,6 +54,7 @@ struct dfjk_ctx {
   int ks_cache_nblk, ks_cache_ntiles, ks_cache_val;   // last answer of the split-K model
   int n_mtiles;              // 128-row tiles along nao
   int j1_chunks, j2_splits;
+  int j1_mma_min_sets;       // J pass 1: sets per group from which the DMMA kernel replaces the DFMA one
   int num_sms;
   int ht_grid;               // persistent half-transform: CTAs (= SMs)
   int ao2mo_route;           // option: 0 = cheaper route, 1 = Eq. 18-21 as printed, 2 = active first

@@ -2,10 +2,11 @@
 //   pass 1  rho[s][P]  = sum_pair B[P][pair] Dw_s[pair]        (one stream over packed B)
 //   pass 2  Jp_s[pair] = sum_P rho[s][P] B[P][pair]            (second stream over packed B)
 //   epilogue: fixed-order sum of the P-split partials and unpack to the full symmetric square.
-// Pass 1 is a bulk-copy (TMA engine) pipeline when npair is even (k_j1_tma); for odd npair, where
-// packed rows are only 8-byte aligned, k_j1 streams with plain loads: a (64 aux rows) x (<=8 sets)
-// x (pairs) contraction per warp on DMMA.8x8x4, whose row x set accumulators fall out of the MMA
-// fragments (no per-row shuffle reduction; one Dw fragment serves 8 row groups).
+// Pass 1 is a bulk-copy (TMA engine) pipeline when npair is even: k_j1_tma (DFMA) for one or two sets,
+// k_j1_mma (DMMA, the weighted densities fetched once per 64 aux rows) for three to eight; for odd
+// npair, where packed rows are only 8-byte aligned, k_j1 streams with plain loads: a (64 aux rows) x
+// (<=8 sets) x (pairs) contraction per warp on DMMA.8x8x4, whose row x set accumulators fall out of
+// the MMA fragments (no per-row shuffle reduction; one Dw fragment serves 8 row groups).
 #include "common.cuh"
 #include "ctx.h"
 #include "pipeline.cuh"
@@ -109,7 +110,7 @@ k_j1(const double* __restrict__ B, size_t npair, int naux, const double* __restr
 // shuffles and a fixed-order sum over the 8 warps once per row group.
 constexpr int kJ1tSC = 512;                       // pairs per stage
 constexpr int kJ1tThreads = 288;                  // 8 consumer warps + 1 producer warp
-__host__ __device__ constexpr int j1t_stages(int ns) { return ns <= 1 ? 6 : ns <= 2 ? 5 : ns <= 4 ? 4 : 3; }
+__host__ __device__ constexpr int j1t_stages(int ns) { return ns <= 1 ? 6 : 5; }
 
 template <int NS>
 __global__ void __launch_bounds__(kJ1tThreads, 1)
@@ -212,6 +213,135 @@ k_j1_tma(const double* __restrict__ B, size_t npair, int naux, const double* __r
   }
 }
 
+// Pass 1 for three and more sets, DMMA formulation of the same bulk-copy pipeline.  The DFMA kernel above
+// re-reads the NS weighted densities from L2 once per 8 aux rows (NS * 4 KB per 32 KB of B: 1.75x the HBM stream
+// at NS = 6, which then sits at the L2-to-SM rate) because its 8 x NS accumulators per lane only cover one row
+// group.  Here rho[row][set] is a GEMM over the pairs on the FP64 tensor pipe: one DMMA.8x8x4 takes 8 rows x 4
+// pairs x 8 sets, its accumulator tile is 2 registers per lane, so a warp keeps the tiles of all 8 row groups
+// of the CTA (64 aux rows) and the loop runs chunk-outer: the Dw chunk is fetched ONCE per 64 rows and its 16
+// B fragments stay in registers while the 8 row groups stream through the ring.  Rows land with a stride of
+// 516 doubles (4 mod 16): the fragment reads are bank-conflict free.
+constexpr int kJ1mLd = kJ1tSC + 4;                 // 516
+constexpr int kJ1mStages = 4;
+constexpr int kJ1mStageDoubles = 8 * kJ1mLd;       // 8 rows of one chunk
+constexpr int kJ1mDwDoubles = 8 * kJ1mLd;          // up to 8 sets of one chunk
+
+__global__ void __launch_bounds__(kJ1tThreads, 1)
+k_j1_mma(const double* __restrict__ B, size_t npair, int naux, const double* __restrict__ Dw, int ns,
+         double* __restrict__ part, int naux_pad) {
+  extern __shared__ __align__(128) double smem[];
+  double* ring = smem;                                          // kJ1mStages x 8 rows
+  double* dws = smem + kJ1mStages * kJ1mStageDoubles;           // 2 x ns rows
+  __shared__ __align__(8) unsigned long long bars[2 * kJ1mStages + 4];
+  const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kJ1mStages]);
+  const uint32_t dfull0 = smem_u32(&bars[2 * kJ1mStages]), dempty0 = smem_u32(&bars[2 * kJ1mStages + 2]);
+  const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
+  const int p0 = blockIdx.y * kJ1Rows;
+  const size_t kbeg = (size_t)blockIdx.x * kJ1Chunk;
+  const size_t kend = kbeg + kJ1Chunk < npair ? kbeg + kJ1Chunk : npair;
+  const int nchunk = (int)((kend - kbeg + kJ1tSC - 1) / kJ1tSC);
+  const int ngroups = min(8, (naux - p0 + 7) / 8);
+  for (int e = tid; e < kJ1mStages * kJ1mStageDoubles + 2 * kJ1mDwDoubles; e += kJ1tThreads) smem[e] = 0.0;   // stale slots stay finite
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  if (tid == 0) {
+    for (int s = 0; s < kJ1mStages; s++) {
+      mbar_init(full0 + 8 * s, 1);
+      mbar_init(empty0 + 8 * s, 8);
+    }
+    for (int s = 0; s < 2; s++) {
+      mbar_init(dfull0 + 8 * s, 1);
+      mbar_init(dempty0 + 8 * s, 8);
+    }
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  if (w == 8) {
+    if (l == 0) {
+      const uint32_t ring_u32 = smem_u32(ring), dws_u32 = smem_u32(dws);
+      int it = 0;
+      for (int c = 0; c < nchunk; c++) {
+        const size_t k0 = kbeg + (size_t)c * kJ1tSC;
+        const uint32_t bytes = (uint32_t)((kend - k0 < (size_t)kJ1tSC ? kend - k0 : (size_t)kJ1tSC) * 8);
+        const uint32_t dfull = dfull0 + 8 * (c & 1);
+        mbar_wait(dempty0 + 8 * (c & 1), ((c >> 1) & 1) ^ 1);
+        mbar_arrive_expect_tx(dfull, bytes * (uint32_t)ns);
+        for (int s = 0; s < ns; s++)
+          bulk_g2s(dws_u32 + (uint32_t)((c & 1) * kJ1mDwDoubles + s * kJ1mLd) * 8u, Dw + (size_t)s * npair + k0, bytes, dfull);
+        for (int rg = 0; rg < ngroups; rg++, it++) {
+          const int stage = it % kJ1mStages;
+          const uint32_t fullb = full0 + 8 * stage;
+          mbar_wait(empty0 + 8 * stage, ((it / kJ1mStages) & 1) ^ 1);
+          const int nrows = min(8, naux - (p0 + 8 * rg));
+          mbar_arrive_expect_tx(fullb, bytes * (uint32_t)nrows);
+          for (int g = 0; g < nrows; g++)
+            bulk_g2s(ring_u32 + (uint32_t)(stage * kJ1mStageDoubles + g * kJ1mLd) * 8u, B + (size_t)(p0 + 8 * rg + g) * npair + k0,
+                     bytes, fullb);
+        }
+      }
+    }
+    return;
+  }
+
+  const int r = l >> 2, j = l & 3;
+  double acc[8][2];
+#pragma unroll
+  for (int rg = 0; rg < 8; rg++) acc[rg][0] = acc[rg][1] = 0.0;
+  int it = 0;
+  for (int c = 0; c < nchunk; c++) {
+    const size_t k0 = kbeg + (size_t)c * kJ1tSC;
+    const int nvalid = (int)(kend - k0 < (size_t)kJ1tSC ? kend - k0 : (size_t)kJ1tSC);
+    // B fragments of this chunk: Dw[set r][pair 64 w + 4 i + j], zero for sets past ns and pairs past the end
+    double bf[16];
+    mbar_wait(dfull0 + 8 * (c & 1), (c >> 1) & 1);
+    const double* dp = dws + (c & 1) * kJ1mDwDoubles + r * kJ1mLd + 64 * w + j;
+#pragma unroll
+    for (int i = 0; i < 16; i++) bf[i] = (r < ns && 64 * w + 4 * i + j < nvalid) ? dp[4 * i] : 0.0;
+    __syncwarp();
+    if (l == 0) mbar_arrive(dempty0 + 8 * (c & 1));
+#pragma unroll
+    for (int rg = 0; rg < 8; rg++) {
+      if (rg < ngroups) {
+        const int stage = it % kJ1mStages;
+        mbar_wait(full0 + 8 * stage, (it / kJ1mStages) & 1);
+        const double* ap = ring + stage * kJ1mStageDoubles + r * kJ1mLd + 64 * w + j;
+        double a[16];
+#pragma unroll
+        for (int i = 0; i < 16; i++) a[i] = ap[4 * i];
+#pragma unroll
+        for (int i = 0; i < 16; i++) dmma884(acc[rg][0], acc[rg][1], a[i], bf[i]);
+        __syncwarp();
+        if (l == 0) mbar_arrive(empty0 + 8 * stage);
+        it++;
+      }
+    }
+  }
+  // warps -> CTA in warp order: lane (r, j) of warp w holds rho[row 8 rg + r][sets 2j, 2j + 1] over its pairs
+  asm volatile("bar.sync 1, 256;" ::: "memory");            // every stage has been consumed: the ring is free
+  double* red = ring;                                       // [8 warps][64 rows][8 sets]
+#pragma unroll
+  for (int rg = 0; rg < 8; rg++)
+    *reinterpret_cast<double2*>(red + (w * 64 + 8 * rg + r) * 8 + 2 * j) = make_double2(acc[rg][0], acc[rg][1]);
+  asm volatile("bar.sync 1, 256;" ::: "memory");
+  for (int e = tid; e < kJ1Rows * 8; e += 256) {
+    const int s = e / kJ1Rows, row = e % kJ1Rows;
+    double t = 0.0;
+#pragma unroll
+    for (int ww = 0; ww < 8; ww++) t += red[(ww * 64 + row) * 8 + s];
+    if (s < ns) part[((size_t)blockIdx.x * 8 + s) * naux_pad + p0 + row] = t;
+  }
+}
+
+static cudaError_t launch_j1_mma(int device, dim3 grid, cudaStream_t st, const double* B, size_t npair, int naux,
+                                 const double* Dw, int ns, double* part, int naux_pad) {
+  constexpr size_t smem = (size_t)(kJ1mStages * kJ1mStageDoubles + 2 * kJ1mDwDoubles) * sizeof(double);
+  static std::atomic<unsigned long long> attr_done{0};
+  cudaError_t e = ensure_dyn_smem(k_j1_mma, smem, device, attr_done);
+  if (e != cudaSuccess) return e;
+  k_j1_mma<<<grid, kJ1tThreads, smem, st>>>(B, npair, naux, Dw, ns, part, naux_pad);
+  return cudaSuccess;
+}
+
 template <int NS>
 static cudaError_t launch_j1_tma(int device, dim3 grid, cudaStream_t st, const double* B, size_t npair, int naux,
                                  const double* Dw, double* part, int naux_pad) {
@@ -228,8 +358,7 @@ static cudaError_t dispatch_j1_tma(int device, int ns, dim3 grid, cudaStream_t s
   switch (ns) {
 #define DFJK_J1T_CASE(N) \
   case N: return launch_j1_tma<N>(device, grid, st, B, npair, naux, Dw, part, naux_pad);
-    DFJK_J1T_CASE(1) DFJK_J1T_CASE(2) DFJK_J1T_CASE(3) DFJK_J1T_CASE(4)
-    DFJK_J1T_CASE(5) DFJK_J1T_CASE(6) DFJK_J1T_CASE(7) DFJK_J1T_CASE(8)
+    DFJK_J1T_CASE(1) DFJK_J1T_CASE(2)          // three and more sets take k_j1_mma
 #undef DFJK_J1T_CASE
     default: return cudaErrorInvalidValue;
   }
@@ -377,7 +506,10 @@ int launch_j_passes(dfjk_ctx* h, const SetInfo& si, double* J_out, bool rho_read
     if (naux > 0 && !rho_ready) {
       prof_mark(h, DFJK_PHASE_J1, st);
       dim3 g1(h->j1_chunks, naux_pad / kJ1Rows);
-      if (vec) {
+      if (vec && ns >= h->j1_mma_min_sets) {
+        if (launch_j1_mma(h->device, g1, st, h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad) != cudaSuccess)
+          return -1;
+      } else if (vec) {
         if (dispatch_j1_tma(h->device, ns, g1, st, h->B, npair, naux, h->Dw + (size_t)s0 * npair, h->rho_part, naux_pad) != cudaSuccess)
           return -1;
       } else {

@@ -450,3 +450,30 @@ def test_one_thin_set_takes_the_one_pass_half_transform(torch_cuda, dfjk, nao, n
     assert rel(res[0][1].cpu().numpy(), res[1][1].cpu().numpy()) <= 1e-12
     if not opts.get("two_pass_j"):
         assert res[0][2] == res[1][2] - 1                    # no rho-reduce launch: the thin kernel writes rho
+
+
+@pytest.mark.parametrize("nao,naux,nsets,seed", [
+    (67, 45, 3, 191),        # npair = 2278: four full chunks + 230 pairs (not a multiple of 4); 45 rows = 5 groups + 5
+    (183, 70, 6, 192),       # npair = 16836: a second CTA chunk of 452 pairs; two row blocks of 64
+    (200, 130, 8, 193),      # eight sets, three row blocks
+    (64, 9, 5, 194),         # two row groups, the second with one row
+])
+def test_j_pass_1_on_the_tensor_pipe(torch_cuda, dfjk, nao, naux, nsets, seed):
+    """three to eight sets: pass 1 runs as a GEMM over the pairs on DMMA.8x8x4 (k_j1_mma), the weighted densities
+    fetched once per 64 aux rows; J alone (two-pass J), signed occupations"""
+    import oracle
+    torch = torch_cuda
+    rs = np.random.default_rng(seed)
+    nocc = [int(rs.integers(1, 7)) for _ in range(nsets)]
+    inp = dfjk_inputs.make_random(nao, naux, nocc, seed, L=max(4.0, nao / 6))
+    inp.occ[0] *= -1.0
+    Jo, _ = oracle.get_jk_inputs(inp, with_k=False)
+    B, Cs, occs = to_dev(torch, inp)
+    with dfjk.DFJK(B, inp.nao, no_small_path=True) as h:
+        J, _ = h.get_jk(Cs, occs, with_k=False)
+        J2, _ = h.get_jk(Cs, occs, with_k=False)
+        torch.cuda.synchronize()
+        assert torch.equal(J, J2)
+    for s in range(nsets):
+        assert rel(J[s].cpu().numpy(), Jo[s]) <= TOL, (s, rel(J[s].cpu().numpy(), Jo[s]))
+        assert torch.equal(J[s], J[s].T)
