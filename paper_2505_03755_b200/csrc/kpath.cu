@@ -24,6 +24,7 @@
 #include "ctx.h"
 #include "pipeline.cuh"
 
+#include <algorithm>
 #include <functional>
 #include <queue>
 #include <vector>
@@ -567,11 +568,20 @@ __device__ __forceinline__ void syrk2_store(double* Kp, int nao, int mu0, int nu
 
 // grid: the n_off * ksplit off-diagonal CTAs first (blockIdx.x = g * n_off + t), then the
 // ntiles_m * ksplit cheaper diagonal ones, which fill the tail of the last wave.
+// the sets of one launch (blockIdx.y): columns [c0, c1) of X and the offset of K_s inside a partial slot; the
+// widest set comes first so that the thin ones fill the tail of the launch
+struct SyrkSets {
+  int c0[kMaxSets], c1[kMaxSets];
+  long long koff[kMaxSets];
+};
+
 template <int WM>
 __global__ void __launch_bounds__(kThreads, 1)
 k_syrk2(const double* __restrict__ X, const double* __restrict__ X2, const unsigned int* __restrict__ sgn, int nao,
-        int nch, int mu_pad, int c0, int c1, int nrows_blk, int rows_per_split, int ntiles_m, int ksplit,
-        double* __restrict__ Kpart_s, size_t split_stride, int first) {
+        int nch, int mu_pad, const __grid_constant__ SyrkSets sets, int nrows_blk, int rows_per_split, int ntiles_m, int ksplit,
+        double* __restrict__ Kpart, size_t split_stride, int first) {
+  const int c0 = sets.c0[blockIdx.y], c1 = sets.c1[blockIdx.y];
+  double* Kpart_s = Kpart + sets.koff[blockIdx.y];
   // X2 == nullptr: K += X X^T (SYRK).  Otherwise K += X X2^T for a product known to be symmetric
   // (density-matrix form, Eq. 16-17: X = B_P D, X2 = B_P): the column operand comes from X2, and
   // diagonal tiles fetch both operands.
@@ -761,7 +771,7 @@ static cudaError_t dispatch_ht(int device, int wn, int epi, int grid, cudaStream
 }
 
 struct SyrkArgs {
-  const double* X; int nao, nch, mu_pad, c0, c1, nrows_blk, rows_per_split, ntiles_m; double* Kpart_s;
+  const double* X; int nao, nch, mu_pad, nsets; SyrkSets sets; int nrows_blk, rows_per_split, ntiles_m; double* Kpart;
   size_t split_stride; int first;
   const double* X2 = nullptr;   // k_syrk2 only: column operand of the two-operand form
   const unsigned int* sgn = nullptr;   // sign bits of the occupations (C-form), nullptr for the two-operand form
@@ -772,9 +782,9 @@ static cudaError_t launch_syrk2(int device, int ksplit, cudaStream_t st, const S
   static std::atomic<unsigned long long> attr_done{0};
   cudaError_t e = ensure_dyn_smem(k_syrk2<WM>, syrk_smem_bytes(WM), device, attr_done);
   if (e != cudaSuccess) return e;
-  const int grid = a.ntiles_m * (a.ntiles_m + 1) / 2 * ksplit;
-  k_syrk2<WM><<<grid, kThreads, syrk_smem_bytes(WM), st>>>(a.X, a.X2, a.sgn, a.nao, a.nch, a.mu_pad, a.c0, a.c1, a.nrows_blk,
-                                                         a.rows_per_split, a.ntiles_m, ksplit, a.Kpart_s,
+  const dim3 grid(a.ntiles_m * (a.ntiles_m + 1) / 2 * ksplit, a.nsets);
+  k_syrk2<WM><<<grid, kThreads, syrk_smem_bytes(WM), st>>>(a.X, a.X2, a.sgn, a.nao, a.nch, a.mu_pad, a.sets, a.nrows_blk,
+                                                         a.rows_per_split, a.ntiles_m, ksplit, a.Kpart,
                                                          a.split_stride, a.first);
   return cudaSuccess;
 }
@@ -946,18 +956,28 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
     launches++;
     const int rps = cdiv(nb, ksplit);
     prof_mark(h, DFJK_PHASE_SYRK, st);
-    for (int s = 0; s < si.nset; s++) {
-      if (si.col0[s + 1] == si.col0[s]) continue;
-      if (emu) {
+    if (emu) {
+      for (int s = 0; s < si.nset; s++) {
+        if (si.col0[s + 1] == si.col0[s]) continue;
         const int k = launch_emu_syrk_set(h, h->X, nch, si.col0[s], si.col0[s] + si.nocc[s], nb, emu_xq, emu_scale,
                                           h->Kpart + n2 * s, split_stride, ksplit, p0 == 0 ? 1 : 0, st);
         if (k < 0) return -1;
         launches += k;
-        continue;
       }
-      // columns past nocc[s] (padding to the 8-column MMA tile) are zero: stop at the k4 step
-      SyrkArgs sa{h->X, nao, nch, h->mu_pad, si.col0[s], si.col0[s] + round_up(si.nocc[s], 4), nb, rps, ntm,
-                  h->Kpart + n2 * s, split_stride, p0 == 0 ? 1 : 0};
+    } else {
+      // all sets in ONE launch (grid.y): the widest first, the thin ones (rank-8 fragment sets) fill its tail.
+      // Columns past nocc[s] (padding to the 8-column MMA tile) are zero: stop at the k4 step
+      SyrkArgs sa{h->X, nao, nch, h->mu_pad, 0, {}, nb, rps, ntm, h->Kpart, split_stride, p0 == 0 ? 1 : 0};
+      int order[kMaxSets];
+      for (int s = 0; s < si.nset; s++)
+        if (si.col0[s + 1] != si.col0[s]) order[sa.nsets++] = s;
+      std::stable_sort(order, order + sa.nsets, [&](int a, int b) { return si.nocc[a] > si.nocc[b]; });
+      for (int q = 0; q < sa.nsets; q++) {
+        const int s = order[q];
+        sa.sets.c0[q] = si.col0[s];
+        sa.sets.c1[q] = si.col0[s] + round_up(si.nocc[s], 4);
+        sa.sets.koff[q] = (long long)(n2 * s);
+      }
       sa.sgn = h->sgnbits;
       if (dispatch_syrk2(h->device, wm_s, ksplit, st, sa) != cudaSuccess) return -1;
       launches++;
@@ -1074,8 +1094,8 @@ int launch_k_path_dm(dfjk_ctx* h, int nset, const double* D, double* K_out, cuda
       k_unpack_tiled<<<gu, 256, 0, st>>>(h->B, h->npair, nao, p0, nch, h->mu_pad, X2);
       launches += 2;
       prof_mark(h, DFJK_PHASE_SYRK, st);
-      SyrkArgs sa{X1, nao, nch, h->mu_pad, 0, round_up(nao, 4), nb, cdiv(nb, ksplit), ntm, h->Kpart + n2 * s,
-                  split_stride, p0 == 0 ? 1 : 0, X2};
+      SyrkArgs sa{X1, nao, nch, h->mu_pad, 1, {}, nb, cdiv(nb, ksplit), ntm, h->Kpart, split_stride, p0 == 0 ? 1 : 0, X2};
+      sa.sets.c0[0] = 0; sa.sets.c1[0] = round_up(nao, 4); sa.sets.koff[0] = (long long)(n2 * s);
       if (dispatch_syrk2(h->device, wm_s, ksplit, st, sa) != cudaSuccess) return -1;
       launches++;
     }

@@ -65,6 +65,19 @@ k_small_fused(const __grid_constant__ SetInfo si, const __grid_constant__ SmallP
   __shared__ int c0s[kMaxSets + 1];
   const size_t n2 = (size_t)nao * nao;
 
+  // the packed row of the next aux row is fetched into registers while the current one is processed
+  constexpr int kPre = (kSmMaxNao * (kSmMaxNao + 1) / 2 + kSmThreads - 1) / kSmThreads;     // 19
+  double pre[kPre];
+  auto prefetch = [&](int P) {
+    const double* bp = q.Bp + (size_t)P * q.npair;
+#pragma unroll
+    for (int k = 0; k < kPre; k++) {
+      const int pr = tid + k * kSmThreads;
+      pre[k] = (P < q.naux && pr < (int)q.npair) ? ldg_stream1(bp + pr) : 0.0;
+    }
+  };
+  prefetch(blockIdx.x);                  // in flight during the prologue
+
   // a1: C' and the signs; compact column c of set s = si.ooff[s] + i.  sg first holds sqrt|occ|, then sign(occ)
   if (tid <= si.nset) c0s[tid] = tid < si.nset ? si.ooff[tid] : ntot;
   for (int c = tid; c < ntot; c += kSmThreads) sg[c] = sqrt(fabs(q.occ[c]));
@@ -84,15 +97,18 @@ k_small_fused(const __grid_constant__ SetInfo si, const __grid_constant__ SmallP
   double* Jp = q.Jpart + (size_t)blockIdx.x * si.nset * q.npair;
   bool first = true;
   for (int P = blockIdx.x; P < q.naux; P += gridDim.x, first = false) {
-    const double* bp = q.Bp + (size_t)P * q.npair;
-    // a5: unpack the packed row into the symmetric slice (flat over the pairs: independent loads)
-    for (int pr = tid; pr < (int)q.npair; pr += kSmThreads) {
-      int mu, nu;
-      untri(pr, mu, nu);
-      const double v = ldg_stream1(bp + pr);
-      Bs[mu * ldb + nu] = v;
-      Bs[nu * ldb + mu] = v;
+    // a5: unpack the packed row into the symmetric slice
+#pragma unroll
+    for (int k = 0; k < kPre; k++) {
+      const int pr = tid + k * kSmThreads;
+      if (pr < (int)q.npair) {
+        int mu, nu;
+        untri(pr, mu, nu);
+        Bs[mu * ldb + nu] = pre[k];
+        Bs[nu * ldb + mu] = pre[k];
+      }
     }
+    prefetch(P + gridDim.x);
     __syncthreads();
     // a6: X[mu][c] = sum_lam b[mu][lam] C'[lam][c]; a thread owns column c = e % ntot of rows e / ntot
     for (int e = tid; e < nao * ntot; e += kSmThreads) {
@@ -122,8 +138,10 @@ k_small_fused(const __grid_constant__ SetInfo si, const __grid_constant__ SmallP
         }
         const double rho = block_sum(t, red);
         double* jp = Jp + (size_t)s * q.npair;
-        for (size_t pr = tid; pr < q.npair; pr += kSmThreads) {
-          const double v = rho * ldg_stream1(bp + pr);
+        for (int pr = tid; pr < (int)q.npair; pr += kSmThreads) {
+          int mu, nu;
+          untri(pr, mu, nu);
+          const double v = rho * Bs[mu * ldb + nu];
           jp[pr] = first ? v : jp[pr] + v;
         }
       }
@@ -195,6 +213,11 @@ static size_t small_smem_bytes(int nao, int ntot) {
   return ((size_t)nao * (nao + 1) + 2 * (size_t)nao * ntot + ntot + 16) * sizeof(double);
 }
 
+static cudaError_t small_attr(int device) {
+  static std::atomic<unsigned long long> attr_done{0};
+  return ensure_dyn_smem(k_small_fused, (size_t)200 * 1024, device, attr_done);
+}
+
 // 0 = not eligible, else the number of CTAs the fused kernel would use
 int small_path_ctas(const dfjk_ctx* h, const SetInfo& si) {
   if (h->no_small_path || h->naux < 1 || h->nao > kSmMaxNao || h->k_emu_slices || h->ht_emu_slices) return 0;
@@ -202,8 +225,17 @@ int small_path_ctas(const dfjk_ctx* h, const SetInfo& si) {
   for (int s = 0; s < si.nset; s++) ntot += si.nocc[s];
   if (ntot < 1 || (long long)h->nao * ntot > kSmMaxElems) return 0;
   if ((double)h->naux * h->nao * h->nao * (ntot + si.nset) > kSmMaxWork) return 0;
-  // as many CTAs as aux rows, in equal rounds over the SMs (160 aux rows on 148 SMs: 80 CTAs x 2 rows)
-  const int rounds = cdiv(h->naux, h->num_sms);
+  // as many CTAs as aux rows, in equal rounds over at most two resident CTAs per SM (more partials would make the
+  // final sum the long pole); the cooperative launch needs all of them resident
+  int occ = 0;
+  if (small_attr(h->device) != cudaSuccess) { cudaGetLastError(); return 0; }
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_small_fused, kSmThreads, small_smem_bytes(h->nao, ntot)) != cudaSuccess) {
+    cudaGetLastError();
+    return 0;
+  }
+  if (occ < 1) return 0;
+  const int slots = h->num_sms * (occ < 2 ? occ : 2);
+  const int rounds = cdiv(h->naux, slots);
   int ctas = cdiv(h->naux, rounds);
   // the private partials live in the X workspace
   const size_t need = (size_t)ctas * si.nset * ((size_t)h->nao * h->nao + h->npair);
@@ -216,8 +248,7 @@ int launch_small_fused(dfjk_ctx* h, const SetInfo& si, int ctas, const double* C
   int ntot = 0;
   for (int s = 0; s < si.nset; s++) ntot += si.nocc[s];
   const size_t smem = small_smem_bytes(h->nao, ntot);
-  static std::atomic<unsigned long long> attr_done{0};
-  if (ensure_dyn_smem(k_small_fused, (size_t)200 * 1024, h->device, attr_done) != cudaSuccess) return -1;
+  if (small_attr(h->device) != cudaSuccess) return -1;
   SmallParams p{h->B, h->npair, h->naux, h->nao, C, occ, J_out, K_out, h->X,
                 h->X + (size_t)ctas * si.nset * h->nao * h->nao, h->ticket, ntot};
   prof_mark(h, DFJK_PHASE_HALF_TRANSFORM, st);

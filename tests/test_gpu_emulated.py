@@ -57,7 +57,7 @@ def test_emulated_k_against_the_oracle_and_the_stated_bound(nao, naux, nocc, see
     B = torch.from_numpy(inp.B_packed).cuda()
     Cs = [torch.from_numpy(c).cuda() for c in inp.C]
     occs = [torch.from_numpy(o).cuda() for o in inp.occ]
-    with dfjk.DFJK(B, nao) as h:
+    with dfjk.DFJK(B, nao, no_small_path=True) as h:               # the same J kernels as the emulated handles
         Jn, Kn = h.get_jk(Cs, occs)
         torch.cuda.synchronize()
     errs = {}
