@@ -182,9 +182,9 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
       one_row += emu_bytes_per_aux_row(nao, cdiv(h->nocc_pad_cap, kBK) + 1, h->k_emu_slices, h->k_emu_pgroup) / sizeof(double) + 1024;
     size_t dbl = cap / sizeof(double);
     if (o.nblk > 0) dbl = (size_t)o.nblk * one_row;
-    if (dbl < one_row) dbl = one_row;
+    if (dbl < 2 * one_row) dbl = 2 * one_row;     // the density-matrix form keeps two operands per aux row
     const size_t all_rows = (size_t)(naux > 0 ? naux : 1) * one_row;
-    if (dbl > all_rows) dbl = all_rows;
+    if (dbl > all_rows && all_rows >= 2 * one_row) dbl = all_rows;
     h->X_doubles = dbl;
     h->nblk = (int)(dbl / one_row);
   }
