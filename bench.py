@@ -36,8 +36,8 @@ FP64_DMMA_PEAK_TFLOPS = 37.1
 FP64_CUBLAS_TFLOPS = 35.47
 HBM_READ_STREAM_GBS = 7430.0
 # ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum of k_half_transform<19,1> at `large`:
-# 9.10 + 3.26 GB per 1122-aux-row launch (profiles/r01_ncu_large_v3.md; the re-tiled Bt is 1.35x the packed bytes)
-HT_DRAM_BYTES_PER_AUX_ROW_LARGE = 12.36e9 / 1122
+# 8.95 + 3.26 GB per 1122-aux-row launch (profiles/r02_ncu_large.md; the re-tiled Bt is 1.35x the packed bytes)
+HT_DRAM_BYTES_PER_AUX_ROW_LARGE = 12.21e9 / 1122
 
 
 def measured_peaks():
@@ -527,7 +527,7 @@ def main():
                      "peak": FP64_DMMA_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ht_tflops / FP64_DMMA_PEAK_TFLOPS,
                      "traffic": (HT_DRAM_BYTES_PER_AUX_ROW_LARGE * naux * args.steps / max(ht_n, 1)
                                  if (nao, sum(nocc)) == (1200, 300) else None),
-                     "traffic_unit": "bytes per launch (ncu dram read + write, profiles/r01_ncu_large_v3.md)",
+                     "traffic_unit": "bytes per launch (constant from one ncu --set full capture: dram read + write, profiles/r02_ncu_large.md)",
                      "algorithmic_bytes_per_launch": (npair_bytes + nao * sum(nocc) * 8.0) * naux * args.steps / max(ht_n, 1),
                      "launches": ht_n, "avg_launch_ms": ht_ms / max(ht_n, 1),
                      "algorithmic_flops_per_step": fb["ht"],
