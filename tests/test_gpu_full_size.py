@@ -108,3 +108,26 @@ def test_ao2mo_at_bench_size_sampled():
     assert np.abs(ppaa - ppaa.transpose(1, 0, 2, 3)).max() <= 1e-12 * s20
     assert np.abs(ppaa - ppaa.transpose(0, 1, 3, 2)).max() <= 1e-12 * s20
     assert np.abs(papa - papa.transpose(2, 3, 0, 1)).max() <= 1e-12 * s21
+
+
+def test_basis_beyond_the_bench_sizes_every_element():
+    """nao = 2000 (system C of the paper has 1378 AOs): 32 row blocks, 508 padded columns in two N
+    tiles of the half-transform, 25 x 25 SYRK tiles, a thin second set; AO2MO's active-first route with the tiled
+    half-transform (the one-pass kernel stops at nao = 1280).  Every element against the oracle."""
+    import oracle
+    import torch
+    import paper_2505_03755_b200 as dfjk
+    nao, naux = 2000, 40
+    inp = dfjk_inputs.make_random(nao, naux, [500, 8], 601, L=120.0)
+    inp.occ[1][::2] *= -1.0
+    B = torch.from_numpy(inp.B_packed).cuda()
+    J, K, plan = _gpu_jk(inp, B)
+    Jo, Ko = oracle.get_jk_inputs(inp)
+    _assert_every_element(inp, J, K, Jo, Ko, plan)
+    M = np.ascontiguousarray(np.linalg.qr(np.random.default_rng(602).standard_normal((nao, 64)))[0])
+    with dfjk.DFJK(B, nao, ao2mo_route=2) as h:
+        bpa, ppaa, papa = h.ao2mo(torch.from_numpy(M).cuda(), 50, 6)
+        torch.cuda.synchronize()
+    o_bpa, o_ppaa, o_papa = oracle.ao2mo(inp.B_packed, nao, M, 50, 6)
+    for a, b in ((bpa, o_bpa), (ppaa, o_ppaa), (papa, o_papa)):
+        assert np.abs(a.cpu().numpy() - b).max() <= TOL * np.abs(b).max()
