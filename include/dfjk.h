@@ -83,7 +83,8 @@ typedef struct {
   int no_symm_thin;           /* 0 = a half-transform with at most 8 columns (the active columns of dfjk_ao2mo's
                                  "active first" route; a dfjk_get_jk call on ONE set of at most 8 orbitals) streams
                                  the packed triangle once and uses every stored element for both Z[mu] and Z[lam]
-                                 (needs a 16-byte aligned B and nao <= 1280); 1 = always the tiled half-transform */
+                                 (needs a 16-byte aligned B; one launch per 1280 columns of the basis); 1 = always
+                                 the tiled half-transform */
   int no_small_path;          /* 0 = an embedding-sized dfjk_get_jk (nao <= 96, nao * sum(nocc) <= 4608 and
                                  naux * nao^2 * (sum(nocc) + nset) <= 2^26) runs as ONE kernel launch: the call is
                                  launch-latency bound there ("called thousands of times");

@@ -19,8 +19,8 @@
 // (row group I, column block Jb < I) it issues four DMMA.8x8x4:
 //   direct      Zd[I]  += T   (8 x 8)  M[8 Jb ..]      (A fragment: lane (r, j) reads T[r][4h + j])
 //   transposed  Zt[Jb] += T^T (8 x 8)  M[8 I ..]       (A fragment: lane (r, j) reads T[rows(g)[j]][r])
-// Zt (all the warp's blocks: 20 accumulator tiles for nao <= 1280 and 8 warps) lives in registers for
-// the whole aux row; the B fragments of the direct products (rows of M of the warp's own column
+// Zt (all the warp's blocks of a panel of 1280 columns: 20 accumulator tiles with 8 warps) lives in registers
+// for the whole aux row (a larger basis takes one launch per panel, SymmParams::cb0); the B fragments of the direct products (rows of M of the warp's own column
 // blocks) sit in shared memory as ready fragment pairs (or in registers, MREG); the B fragments of
 // the transposed products (rows of M of the current row group) are loaded one super-group ahead.
 // The direct accumulators Zd are partial over the warp's column blocks: after every super-group the
@@ -72,6 +72,10 @@ struct SymmParams {
   double* X; long long x_pstride, x_rstride;        // out: X[pl * x_pstride + mu * x_rstride + a], a < 8 (strides even)
   int p_first, nb;                                  // aux rows [p_first, p_first + nb)
   double* rho; const unsigned int* sgn;             // optional: rho[p_first + pl] = sum_{mu, a} sign_a Z[mu][a] M[mu][a] (Eq. 14, R16)
+  // column panel of this launch: the column blocks [cb0, cb0 + 160) (1280 columns: what a warp's register-resident
+  // accumulators cover).  A basis beyond 1280 takes one launch per panel, in ascending order on one stream; panel 0
+  // writes every row of Z (rows past its columns: the direct sums alone), later panels add to it
+  int cb0;
 };
 
 __device__ __forceinline__ double sy_m(const SymmParams& q, int lam, int a) {
@@ -96,11 +100,15 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
   const int nao = q.nao;
   const int nsg = (nao + kSyRows - 1) / kSyRows;
   const int ngroups = (nao + 7) >> 3;
+  const int cb0 = q.cb0, col_base = 8 * cb0;           // first column block / column of this panel
+  const int sg0 = col_base / kSyRows;                  // rows above the panel's first column hold none of its columns
+  const bool first_panel = cb0 == 0;
+  constexpr int kPanelBlocks = kSyMaxNao / 8;
 
   for (int e = tid; e < kSyStages * kSyStageDoubles; e += kSyThreads) ring[e] = 0.0;   // stale slots must hold finite numbers
   if (!MREG)
     for (int e = tid; e < Cfg::kMpDoubles; e += kSyThreads) {
-      const int h = e & 1, ln = (e >> 1) & 31, lam = 8 * (e >> 6) + 4 * h + (ln & 3), a = ln >> 2;
+      const int h = e & 1, ln = (e >> 1) & 31, lam = col_base + 8 * (e >> 6) + 4 * h + (ln & 3), a = ln >> 2;
       Mp[e] = (a < q.ncols && lam < nao) ? sy_m(q, lam, a) : 0.0;
     }
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -125,9 +133,9 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
     int it = 0;
     for (int pl = blockIdx.x; pl < q.nb; pl += gridDim.x) {
       const size_t rowbase = (size_t)(q.p_first + pl) * q.npair;
-      for (int sg = 0; sg < nsg; sg++) {
+      for (int sg = sg0; sg < nsg; sg++) {
         const int mu = sg * kSyRows + rr;
-        const int nch = (sg * kSyRows + kSyRows + kSyLC - 1) / kSyLC;
+        const int nch = (min(sg * kSyRows + kSyRows, col_base + kSyMaxNao) - col_base + kSyLC - 1) / kSyLC;
         const size_t trimu = tri(mu);
         for (int cc = 0; cc < nch; cc++, it++) {
           const int stage = it % kSyStages;
@@ -137,7 +145,7 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
           uint32_t bytes = 0;
           size_t as2 = 0;
           if (lane_on && mu < nao) {
-            const int c0 = cc * kSyLC;                     // c0 <= first row of the super-group <= mu: never empty
+            const int c0 = col_base + cc * kSyLC;          // c0 <= first row of the super-group <= mu: never empty
             const size_t as = rowbase + trimu + c0, ae = rowbase + trimu + min(c0 + kSyLC, mu + 1);
             as2 = as & ~(size_t)1;
             const size_t ae2 = (ae + 1) & ~(size_t)1;
@@ -171,7 +179,7 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
     for (int sl = 0; sl < (MREG ? kSyNSLOT : 1); sl++)
 #pragma unroll
       for (int h = 0; h < 2; h++) {
-        const int lam = 8 * (NW * sl + w) + 4 * h + j;
+        const int lam = col_base + 8 * (NW * sl + w) + 4 * h + j;
         Mf[sl][h] = (col_ok && lam < nao) ? sy_m(q, lam, r) : 0.0;
       }
   }
@@ -204,10 +212,10 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
         }
     };
     double tB[kSyG][2], tBn[kSyG][2];
-    load_tB(0, tBn);
-    for (int sg = 0; sg < nsg; sg++, sgc++) {
+    load_tB(sg0, tBn);
+    for (int sg = sg0; sg < nsg; sg++, sgc++) {
       const int mu0 = sg * kSyRows;
-      const int nch = (mu0 + kSyRows + kSyLC - 1) / kSyLC;
+      const int nch = (min(mu0 + kSyRows, col_base + kSyMaxNao) - col_base + kSyLC - 1) / kSyLC;
 #pragma unroll
       for (int gi = 0; gi < kSyG; gi++) { tB[gi][0] = tBn[gi][0]; tB[gi][1] = tBn[gi][1]; }
       load_tB(sg + 1, tBn);                              // rows past nao give zeros
@@ -223,7 +231,7 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
           const int stage = it % kSyStages;
           mbar_wait(full0 + 8 * stage, (it / kSyStages) & 1);
           stage_ptr = ring + stage * kSyStageDoubles;
-          if (sg_full && (kSyLC / 8) * (cc + 1) <= kSyG * sg) {
+          if (sg_full && cb0 + (kSyLC / 8) * (cc + 1) <= kSyG * sg) {
             // every block of the chunk is a full stored block: straight-line code, two row groups at a time so
             // that consecutive DMMAs on one accumulator are four instructions apart
 #pragma unroll
@@ -252,7 +260,7 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
               const int I = kSyG * sg + gi;
 #pragma unroll
               for (int qq = 0; qq < kQ; qq++) {
-                const int sl = kQ * cc + qq, Jb = NW * sl + w;
+                const int sl = kQ * cc + qq, Jb = cb0 + NW * sl + w;
                 if (Jb < I && I < ngroups) {               // a full stored block (warp-uniform)
                   const double* gb = stage_ptr + gi * 8 * kSyS + 8 * NW * qq;
                   const double ad0 = gb[offD], ad1 = gb[offD + 4];
@@ -279,8 +287,8 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
 #pragma unroll
         for (int gi = 0; gi < kSyG; gi++) {
           const int I = kSyG * sg + gi;
-          if ((I & (NW - 1)) == w && I < ngroups) {
-            const int x0 = 8 * I - kSyLC * cl;
+          if ((I & (NW - 1)) == w && I < ngroups && I < cb0 + kPanelBlocks) {   // I >= cb0: rows start at the panel
+            const int x0 = 8 * I - col_base - kSyLC * cl;
             const double* gb = stage_ptr + gi * 8 * kSyS + x0;
 #pragma unroll
             for (int h = 0; h < 2; h++) {
@@ -323,29 +331,43 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
             s0 += v.x;
             s1 += v.y;
           }
-          const int slI = I / NW;
+          if (I < cb0 + kPanelBlocks) {
+            const int slI = (I - cb0) / NW;
 #pragma unroll
-          for (int sl = 0; sl < kSyNSLOT; sl++)
-            if (sl == slI) { Zt[sl][0] += s0; Zt[sl][1] += s1; }
+            for (int sl = 0; sl < kSyNSLOT; sl++)
+              if (sl == slI) { Zt[sl][0] += s0; Zt[sl][1] += s1; }
+          } else if (8 * I + r < nao) {
+            // a row group past this panel's columns: its Z tile lives in a later panel's registers; the direct sum goes
+            // to memory (the first panel writes, later panels add)
+            double2* zp = reinterpret_cast<double2*>(q.X + (size_t)pl * q.x_pstride + (size_t)(8 * I + r) * q.x_rstride + 2 * j);
+            if (first_panel) *zp = make_double2(s0, s1);
+            else { const double2 o = *zp; *zp = make_double2(o.x + s0, o.y + s1); }
+          }
         }
       }
     }
-    // Z of this aux row: block Jb = 8 sl + w, rows 8 Jb + r, columns 2j, 2j + 1
+    // Z of this aux row: block Jb = cb0 + NW sl + w, rows 8 Jb + r, columns 2j, 2j + 1 (later panels add to what
+    // the first one stored for their rows)
     double* Xp = q.X + (size_t)pl * q.x_pstride;
 #pragma unroll
     for (int sl = 0; sl < kSyNSLOT; sl++) {
-      const int mu = 8 * (NW * sl + w) + r;
-      if (mu < nao) *reinterpret_cast<double2*>(Xp + (size_t)mu * q.x_rstride + 2 * j) = make_double2(Zt[sl][0], Zt[sl][1]);
+      const int mu = 8 * (cb0 + NW * sl + w) + r;
+      if (mu < nao) {
+        double2* zp = reinterpret_cast<double2*>(Xp + (size_t)mu * q.x_rstride + 2 * j);
+        if (!first_panel) { const double2 o = *zp; Zt[sl][0] += o.x; Zt[sl][1] += o.y; }
+        *zp = make_double2(Zt[sl][0], Zt[sl][1]);
+      }
     }
     if (q.rho) {
-      // rho_P = sum_{mu, a} sign_a Z[mu][a] M[mu][a]: lanes -> warp (xor tree), warps -> CTA in warp order
+      // rho_P = sum_{mu, a} sign_a Z[mu][a] M[mu][a] over the rows of this panel: lanes -> warp (xor tree), warps -> CTA
+      // in warp order, panels in launch order
       const unsigned int sw = __ldg(q.sgn) >> (2 * j);
       const double s0 = (sw & 1u) ? -1.0 : 1.0, s1 = (sw & 2u) ? -1.0 : 1.0;
       const bool c0_ok = 2 * j < q.ncols, c1_ok = 2 * j + 1 < q.ncols;
       double t = 0.0;
 #pragma unroll
       for (int sl = 0; sl < kSyNSLOT; sl++) {
-        const int mu = 8 * (NW * sl + w) + r;
+        const int mu = 8 * (cb0 + NW * sl + w) + r;
         if (mu < nao) {
           if (c0_ok) t = fma(Zt[sl][0] * s0, sy_m(q, mu, 2 * j), t);
           if (c1_ok) t = fma(Zt[sl][1] * s1, sy_m(q, mu, 2 * j + 1), t);
@@ -359,14 +381,13 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
         double v = 0.0;
 #pragma unroll
         for (int ww = 0; ww < NW; ww++) v += rho_red[ww];
-        q.rho[q.p_first + pl] = v;
+        q.rho[q.p_first + pl] = first_panel ? v : q.rho[q.p_first + pl] + v;
       }
     }
   }
 }
 
-// usable when the packed tensor is 16-byte aligned, nao fits the register-resident accumulators and
-// the right-hand side has at most 8 columns
+// usable when the packed tensor is 16-byte aligned and the right-hand side has at most 8 columns
 template <int NW, int G, int LC, int STAGES, bool MREG>
 static int launch_symm_cfg(dfjk_ctx* h, const SymmParams& p, int grid, cudaStream_t st) {
   using Cfg = SyCfg<NW, G, LC, STAGES, MREG>;
@@ -378,21 +399,23 @@ static int launch_symm_cfg(dfjk_ctx* h, const SymmParams& p, int grid, cudaStrea
 }
 
 bool symm_thin_ok(const dfjk_ctx* h, int ncols) {
-  return !h->no_symm_thin && h->b_aligned16 && h->nao <= kSyMaxNao && ncols >= 1 && ncols <= 8 && h->naux > 0;
+  return !h->no_symm_thin && h->b_aligned16 && ncols >= 1 && ncols <= 8 && h->naux > 0;
 }
 
-static int launch_symm(dfjk_ctx* h, const SymmParams& p, int nb, cudaStream_t st) {
+static int launch_symm(dfjk_ctx* h, SymmParams p, int nb, cudaStream_t st) {
   const int grid = nb < h->num_sms ? nb : h->num_sms;
   // measured at nao = 1200, naux = 4000 (B200): 16 rows x 256 columns per stage, 3 stages, B fragments in shared
   // memory 4.3 ms; 32 x 128 x 3: 4.4; register-resident B fragments (32 x 128 x 5): 4.9-5.4; 16 consumer warps: 4.8
-  return launch_symm_cfg<8, 2, 256, 3, false>(h, p, grid, st);
+  for (p.cb0 = 0; 8 * p.cb0 < h->nao; p.cb0 += kSyMaxNao / 8)       // one launch per panel of 1280 columns
+    if (launch_symm_cfg<8, 2, 256, 3, false>(h, p, grid, st) != 0) return -1;
+  return 0;
 }
 
 // AO2MO: Z[pl][mu][a] (row-major, row stride ldx >= 8, even) for the aux rows [p_first, p_first + nb), M row-major
 int launch_symm_thin(dfjk_ctx* h, const double* M, int ldm, int ncols, int p_first, int nb, double* X, int ldx,
                      cudaStream_t st) {
   SymmParams p{h->B, h->npair, (size_t)h->naux * h->npair, h->nao, M, ncols, 0, 0, ldm, 0, 1,
-               X, (long long)h->nao * ldx, ldx, p_first, nb, nullptr, nullptr};
+               X, (long long)h->nao * ldx, ldx, p_first, nb, nullptr, nullptr, 0};
   return launch_symm(h, p, nb, st);
 }
 
@@ -400,7 +423,7 @@ int launch_symm_thin(dfjk_ctx* h, const double* M, int ldm, int ncols, int p_fir
 // k_prep_ct, rho[P] (Eq. 14 through the half-transformed block, R16) when rho != nullptr
 int launch_symm_thin_jk(dfjk_ctx* h, int ncols, int p_first, int nb, double* X, double* rho, cudaStream_t st) {
   SymmParams p{h->B, h->npair, (size_t)h->naux * h->npair, h->nao, h->Ct, ncols, 4, 15, (long long)h->ct_rows * kHtLd, 1, kHtLd,
-               X, (long long)h->mu_pad * kLdT, kLdT, p_first, nb, rho, h->sgnbits};
+               X, (long long)h->mu_pad * kLdT, kLdT, p_first, nb, rho, h->sgnbits, 0};
   return launch_symm(h, p, nb, st);
 }
 

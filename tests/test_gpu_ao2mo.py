@@ -141,9 +141,18 @@ def test_symm_thin_large_basis_every_block():
     run_case(1203, 150, 24, 8, 8, 307, L=0.0, ao2mo_route=2)
 
 
-def test_symm_thin_falls_back_past_its_basis_limit():
-    """nao = 1300 > 1280: the tiled half-transform serves route 2"""
-    run_case(1300, 3, 16, 4, 4, 308, L=100.0, ao2mo_route=2)
+@pytest.mark.parametrize("nao,naux,nmo,a0,nact,seed", [
+    (1300, 3, 16, 4, 4, 308),       # two column panels of 1280: 20 columns in the second
+    (1400, 4, 12, 2, 8, 311),       # the second panel holds 15 column blocks, ragged last row group (1400 = 175 x 8)
+    (2570, 2, 10, 1, 3, 312),       # three panels: the first two add direct sums for the rows of the third
+])
+def test_symm_thin_column_panels(nao, naux, nmo, a0, nact, seed):
+    """a basis beyond 1280 (system C of the paper: 1378 AOs) takes one launch per panel of 1280 columns; the first
+    panel stores every row of Z, later panels add; against the oracle and against the tiled half-transform"""
+    a = run_case(nao, naux, nmo, a0, nact, seed, L=100.0, ao2mo_route=2)
+    b = run_case(nao, naux, nmo, a0, nact, seed, L=100.0, ao2mo_route=2, no_symm_thin=True)
+    for x, y in zip(a, b):
+        assert rel(x, y) <= 1e-12
 
 
 def test_symm_thin_unaligned_tensor_falls_back():

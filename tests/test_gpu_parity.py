@@ -422,6 +422,7 @@ def test_error_codes(torch_cuda, dfjk):
     (263, 21, [3], 183, dict(nblk=4)),                # several aux blocks: rho written block by block
     (1203, 6, [7], 184, {}),                          # ragged, all 20 column blocks per warp
     (520, 9, [8], 185, dict(two_pass_j=True)),        # rho from the two-pass J, X from the thin kernel
+    (1400, 5, [6], 186, {}),                          # two column panels of the one-pass kernel: rho summed over both
 ])
 def test_one_thin_set_takes_the_one_pass_half_transform(torch_cuda, dfjk, nao, naux, nocc, seed, opts):
     """a JK call on one set of at most 8 orbitals (a fragment's active space): the half-transform streams the
