@@ -292,19 +292,18 @@ k_emu_syrk(const __grid_constant__ EmuSyrkParams q) {
       tc_fence_after();
 #pragma unroll
       for (int c0 = 0; c0 < kEmuTN; c0 += 8) {
-        double t[8];
-        int v[8];
-        tmem_ld8(lane_addr + (uint32_t)((S - 1) * kEmuTN + c0), v);
+        // the S accumulator groups of these 8 columns: all loads in flight, one wait
+        int v[S][8];
+#pragma unroll
+        for (int gq = 0; gq < S; gq++) tmem_ld8(lane_addr + (uint32_t)(gq * kEmuTN + c0), v[gq]);
         tmem_ld_wait();
+        double t[8];
 #pragma unroll
-        for (int i = 0; i < 8; i++) t[i] = (double)v[i];
+        for (int i = 0; i < 8; i++) t[i] = (double)v[S - 1][i];
 #pragma unroll
-        for (int gq = S - 2; gq >= 0; gq--) {
-          tmem_ld8(lane_addr + (uint32_t)(gq * kEmuTN + c0), v);
-          tmem_ld_wait();
+        for (int gq = S - 2; gq >= 0; gq--)
 #pragma unroll
-          for (int i = 0; i < 8; i++) t[i] = fma(t[i], 1.0 / 128.0, (double)v[i]);
-        }
+          for (int i = 0; i < 8; i++) t[i] = fma(t[i], 1.0 / 128.0, (double)v[gq][i]);
 #pragma unroll
         for (int i = 0; i < 8; i++) acc[c0 + i] = fma(t[i], rs * __ldg(sc + b0 + c0 + i), acc[c0 + i]);
       }
@@ -494,38 +493,38 @@ k_emu_ht(const __grid_constant__ EmuHtParams q) {
       const int pl = tile / tiles_per_p, rem = tile - pl * tiles_per_p;
       const int a0 = (rem / q.ntn) * kEmuTM, n0 = (rem % q.ntn) * kEmuTN;
       const int mu = a0 + 32 * quarter + l;
-      double t[kEmuTN];
+      const double rs = mu < q.nao ? q.bscale[(size_t)(q.p_first + pl) * q.mu_q + mu] * (1.0 / 4096.0) : 0.0;
+      double* Xp = q.X + (size_t)pl * q.nch * q.mu_pad * kLdT;
       mbar_wait(tfull, nt & 1);
       tc_fence_after();
 #pragma unroll
       for (int c0 = 0; c0 < kEmuTN; c0 += 8) {
-        int v[8];
-        tmem_ld8(lane_addr + (uint32_t)((S - 1) * kEmuTN + c0), v);
+        // the S accumulator groups of these 8 columns: all loads in flight, one wait; recombined, scaled and stored
+        // at once, so that the tensor memory is free again after ten round trips
+        int v[S][8];
+#pragma unroll
+        for (int gq = 0; gq < S; gq++) tmem_ld8(lane_addr + (uint32_t)(gq * kEmuTN + c0), v[gq]);
         tmem_ld_wait();
+        double t[8];
 #pragma unroll
-        for (int i = 0; i < 8; i++) t[c0 + i] = (double)v[i];
+        for (int i = 0; i < 8; i++) t[i] = (double)v[S - 1][i];
 #pragma unroll
-        for (int gq = S - 2; gq >= 0; gq--) {
-          tmem_ld8(lane_addr + (uint32_t)(gq * kEmuTN + c0), v);
-          tmem_ld_wait();
+        for (int gq = S - 2; gq >= 0; gq--)
 #pragma unroll
-          for (int i = 0; i < 8; i++) t[c0 + i] = fma(t[c0 + i], 1.0 / 128.0, (double)v[i]);
+          for (int i = 0; i < 8; i++) t[i] = fma(t[i], 1.0 / 128.0, (double)v[gq][i]);
+        if (mu < q.nao) {
+#pragma unroll
+          for (int i = 0; i < 8; i += 2) {
+            const int n = n0 + c0 + i;
+            if (n < q.nocc_pad)
+              *reinterpret_cast<double2*>(Xp + ((size_t)(n >> 5) * q.mu_pad + mu) * kLdT + (n & 31)) =
+                  make_double2(t[i] * (rs * __ldg(q.cscale + n)), t[i + 1] * (rs * __ldg(q.cscale + n + 1)));
+          }
         }
       }
       tc_fence_before();
       __syncwarp();
-      if (l == 0) mbar_arrive(tempty);          // the next tile's MMAs may start while this one is stored
-      if (mu < q.nao) {
-        const double rs = q.bscale[(size_t)(q.p_first + pl) * q.mu_q + mu] * (1.0 / 4096.0);
-        double* Xp = q.X + (size_t)pl * q.nch * q.mu_pad * kLdT;
-#pragma unroll
-        for (int c0 = 0; c0 < kEmuTN; c0 += 2) {
-          const int n = n0 + c0;
-          if (n < q.nocc_pad)
-            *reinterpret_cast<double2*>(Xp + ((size_t)(n >> 5) * q.mu_pad + mu) * kLdT + (n & 31)) =
-                make_double2(t[c0] * (rs * __ldg(q.cscale + n)), t[c0 + 1] * (rs * __ldg(q.cscale + n + 1)));
-        }
-      }
+      if (l == 0) mbar_arrive(tempty);          // the next tile's MMAs may start
     }
   }
   tc_fence_before();
