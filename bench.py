@@ -9,8 +9,9 @@ and K of the `large` config (nao=1200, naux=4000, nocc=300, ~23 GB packed B resi
 through dfjk_get_jk_host with pinned HOST buffers for C, occ, J, K (copies inside the timed
 region; B stays resident as the paper prescribes).  `roofline` describes the
 dominant kernel (the DMMA half-transform), `cpu_baseline` the oracle on the host cores on a
-bounded sample of aux rows.  The path does not shard in this build ("replicas only"):
-with --gpus N every rank runs an independent replica and the max over ranks is reported.
+bounded sample of aux rows.  north_star names no sharding ("replicas only"): with
+--gpus N every rank runs an independent replica and the max over ranks is reported; --shard-aux is the
+opt-in, unmeasured aux-sharded mode (one all-reduce of the partial J, K).
 """
 from __future__ import annotations
 

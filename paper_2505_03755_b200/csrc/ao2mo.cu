@@ -33,6 +33,9 @@ struct GemmTN {
   // whose rows are (P, a) and whose columns are p
   int c_group = 0;
   long long c_gstride = 0, c_nstride = 0;
+  // 1: C is known to be symmetric (Eq. 21: A == B): tiles that lie entirely above the diagonal are skipped and
+  // k_mirror_lower fills the upper triangle from the lower one afterwards
+  int lower_only = 0;
 };
 
 // CTA tile (8 WTM WGM) x (8 WTN WGN), WGM x WGN = 8 consumer warps, warp tile WTM x WTN MMA tiles.  WGM = 2:
@@ -59,6 +62,7 @@ k_gemm_tn(const __grid_constant__ GemmTN g) {
   const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kGStages]);
   const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
   const int m0 = blockIdx.x * TM, n0 = blockIdx.y * TN;
+  if (g.lower_only && n0 >= m0 + TM) return;          // every element of this tile has n > m
   const double* A = g.A + (size_t)blockIdx.z * g.sA;
   const double* B = g.B + (size_t)blockIdx.z * g.sB;
   double* C = g.C + (size_t)blockIdx.z * g.sC;
@@ -236,6 +240,7 @@ static cudaError_t launch_gemm_tn(int device, const GemmTN& g, int batch, cudaSt
 // CTA tile 64 x (32 WTN): the N tile is fitted to the problem (at most 352 columns per tile, the
 // fewest tiles that cover N, then the narrowest WTN that does), so that e.g. N = 340 pays 352.
 static cudaError_t gemm_tn(int device, const GemmTN& g, int batch, cudaStream_t st) {
+  if (g.lower_only) return launch_gemm_tn<8, 4>(device, g, batch, st);     // square 128 x 128 tiles: half of them run
   const int n8 = cdiv(g.N > 0 ? g.N : 1, 8);
   const int ntn = cdiv(n8, 44), wtn = cdiv(n8, 4 * ntn);
   if (g.N > 32 && g.N <= 40 && g.M >= 128 * 148)   // 36 packed (a1 >= a2) pairs of 8 active orbitals: 128 x 40 tiles
@@ -250,6 +255,23 @@ static cudaError_t gemm_tn(int device, const GemmTN& g, int batch, cudaStream_t 
     DFJK_GEMM_CASE(7) DFJK_GEMM_CASE(8) DFJK_GEMM_CASE(9) DFJK_GEMM_CASE(10) DFJK_GEMM_CASE(11)
 #undef DFJK_GEMM_CASE
     default: return cudaErrorInvalidValue;
+  }
+}
+
+// C[m][n] = C[n][m] for n > m (n x n, row stride ldc): completes a product computed on its lower tiles
+__global__ void k_mirror_lower(double* __restrict__ C, int n, long long ldc) {
+  __shared__ double t[32][33];
+  const int bi = blockIdx.x, bj = blockIdx.y;
+  if (bj > bi) return;
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  for (int r = ty; r < 32; r += 8) {
+    const int m = bi * 32 + r, c = bj * 32 + tx;
+    t[r][tx] = (m < n && c < n) ? C[(size_t)m * ldc + c] : 0.0;
+  }
+  __syncthreads();
+  for (int r = ty; r < 32; r += 8) {
+    const int row = bj * 32 + r, col = bi * 32 + tx;             // the mirrored tile (bj, bi): element (row, col) = lower (col, row)
+    if (row < n && col < n && col > row) C[(size_t)row * ldc + col] = t[tx][r];
   }
 }
 
@@ -320,8 +342,14 @@ static int launch_ao2mo_as_printed(dfjk_ctx* h, int nmo, int a0, int nact, const
     prof_mark(h, DFJK_PHASE_SYRK, st);
     GemmTN g21{bpa_out, bpa_out, papa_out, (int)npa, (int)npa, naux, (long long)npa, (long long)npa,
                (long long)npa, 0, 0, 0, 0};
+    g21.lower_only = 1;                                                                              // (p1 a1|p2 a2) = (p2 a2|p1 a1)
     if (gemm_tn(h->device, g21, 1, st) != cudaSuccess) return -1;                                    // Eq. 21
-    launches++;
+    {
+      const int nb32 = cdiv((int)npa, 32);
+      dim3 gm(nb32, nb32), bm(32, 8);
+      k_mirror_lower<<<gm, bm, 0, st>>>(papa_out, (int)npa, (long long)npa);
+    }
+    launches += 2;
   }
   return launches;
 }
@@ -438,8 +466,14 @@ static int launch_ao2mo_active_first(dfjk_ctx* h, int nmo, int a0, int nact, con
   if (papa_out) {
     GemmTN g21{bpa_out, bpa_out, papa_out, (int)npa, (int)npa, naux, (long long)npa, (long long)npa,
                (long long)npa, 0, 0, 0, 0};
+    g21.lower_only = 1;                                                                               // (p1 a1|p2 a2) = (p2 a2|p1 a1)
     if (gemm_tn(h->device, g21, 1, st) != cudaSuccess) return -1;                                     // Eq. 21
-    launches++;
+    {
+      const int nb32 = cdiv((int)npa, 32);
+      dim3 gm(nb32, nb32), bm(32, 8);
+      k_mirror_lower<<<gm, bm, 0, st>>>(papa_out, (int)npa, (long long)npa);
+    }
+    launches += 2;
   }
   return launches;
 }

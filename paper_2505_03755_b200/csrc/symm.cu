@@ -82,7 +82,10 @@ __device__ __forceinline__ double sy_m(const SymmParams& q, int lam, int a) {
   return __ldg(q.M + (size_t)(lam >> q.m_sh) * q.m_hi + (size_t)(lam & q.m_msk) * q.m_lo + (size_t)a * q.m_a);
 }
 
-template <int NW, int G, int LC, int STAGES, bool MREG>
+// PANELS: the basis needs more than one column panel (cb0 may be nonzero, outputs may be added to); RHO: rho is
+// wanted.  Both are compile-time so that the common single-panel AO2MO instance keeps its hot loop small (the
+// unrolled chunk loop is instruction-cache sensitive: 2800 vs 4100 instructions made 4.3 vs 4.8 ms)
+template <int NW, int G, int LC, int STAGES, bool MREG, bool PANELS, bool RHO>
 __global__ void __launch_bounds__(32 * NW + 128, 1)
 k_symm_thin(const __grid_constant__ SymmParams q) {
   using Cfg = SyCfg<NW, G, LC, STAGES, MREG>;
@@ -100,9 +103,9 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
   const int nao = q.nao;
   const int nsg = (nao + kSyRows - 1) / kSyRows;
   const int ngroups = (nao + 7) >> 3;
-  const int cb0 = q.cb0, col_base = 8 * cb0;           // first column block / column of this panel
+  const int cb0 = PANELS ? q.cb0 : 0, col_base = 8 * cb0;   // first column block / column of this panel
   const int sg0 = col_base / kSyRows;                  // rows above the panel's first column hold none of its columns
-  const bool first_panel = cb0 == 0;
+  const bool first_panel = !PANELS || cb0 == 0;
   constexpr int kPanelBlocks = kSyMaxNao / 8;
 
   for (int e = tid; e < kSyStages * kSyStageDoubles; e += kSyThreads) ring[e] = 0.0;   // stale slots must hold finite numbers
@@ -336,7 +339,7 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
 #pragma unroll
             for (int sl = 0; sl < kSyNSLOT; sl++)
               if (sl == slI) { Zt[sl][0] += s0; Zt[sl][1] += s1; }
-          } else if (8 * I + r < nao) {
+          } else if (PANELS && 8 * I + r < nao) {
             // a row group past this panel's columns: its Z tile lives in a later panel's registers; the direct sum goes
             // to memory (the first panel writes, later panels add)
             double2* zp = reinterpret_cast<double2*>(q.X + (size_t)pl * q.x_pstride + (size_t)(8 * I + r) * q.x_rstride + 2 * j);
@@ -358,7 +361,7 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
         *zp = make_double2(Zt[sl][0], Zt[sl][1]);
       }
     }
-    if (q.rho) {
+    if (RHO && q.rho) {
       // rho_P = sum_{mu, a} sign_a Z[mu][a] M[mu][a] over the rows of this panel: lanes -> warp (xor tree), warps -> CTA
       // in warp order, panels in launch order
       const unsigned int sw = __ldg(q.sgn) >> (2 * j);
@@ -388,13 +391,13 @@ k_symm_thin(const __grid_constant__ SymmParams q) {
 }
 
 // usable when the packed tensor is 16-byte aligned and the right-hand side has at most 8 columns
-template <int NW, int G, int LC, int STAGES, bool MREG>
+template <int NW, int G, int LC, int STAGES, bool MREG, bool PANELS, bool RHO>
 static int launch_symm_cfg(dfjk_ctx* h, const SymmParams& p, int grid, cudaStream_t st) {
   using Cfg = SyCfg<NW, G, LC, STAGES, MREG>;
   static_assert(Cfg::kSmemBytes + 1024 <= 227 * 1024, "shared memory");
   static std::atomic<unsigned long long> attr_done{0};
-  if (ensure_dyn_smem(k_symm_thin<NW, G, LC, STAGES, MREG>, Cfg::kSmemBytes, h->device, attr_done) != cudaSuccess) return -1;
-  k_symm_thin<NW, G, LC, STAGES, MREG><<<grid, Cfg::kThreads, Cfg::kSmemBytes, st>>>(p);
+  if (ensure_dyn_smem(k_symm_thin<NW, G, LC, STAGES, MREG, PANELS, RHO>, Cfg::kSmemBytes, h->device, attr_done) != cudaSuccess) return -1;
+  k_symm_thin<NW, G, LC, STAGES, MREG, PANELS, RHO><<<grid, Cfg::kThreads, Cfg::kSmemBytes, st>>>(p);
   return 0;
 }
 
@@ -406,8 +409,15 @@ static int launch_symm(dfjk_ctx* h, SymmParams p, int nb, cudaStream_t st) {
   const int grid = nb < h->num_sms ? nb : h->num_sms;
   // measured at nao = 1200, naux = 4000 (B200): 16 rows x 256 columns per stage, 3 stages, B fragments in shared
   // memory 4.3 ms; 32 x 128 x 3: 4.4; register-resident B fragments (32 x 128 x 5): 4.9-5.4; 16 consumer warps: 4.8
-  for (p.cb0 = 0; 8 * p.cb0 < h->nao; p.cb0 += kSyMaxNao / 8)       // one launch per panel of 1280 columns
-    if (launch_symm_cfg<8, 2, 256, 3, false>(h, p, grid, st) != 0) return -1;
+  const bool panels = h->nao > kSyMaxNao, rho = p.rho != nullptr;
+  for (p.cb0 = 0; 8 * p.cb0 < h->nao; p.cb0 += kSyMaxNao / 8) {     // one launch per panel of 1280 columns
+    int rc;
+    if (panels) rc = rho ? launch_symm_cfg<8, 2, 256, 3, false, true, true>(h, p, grid, st)
+                         : launch_symm_cfg<8, 2, 256, 3, false, true, false>(h, p, grid, st);
+    else rc = rho ? launch_symm_cfg<8, 2, 256, 3, false, false, true>(h, p, grid, st)
+                  : launch_symm_cfg<8, 2, 256, 3, false, false, false>(h, p, grid, st);
+    if (rc != 0) return -1;
+  }
   return 0;
 }
 
