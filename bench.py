@@ -381,8 +381,9 @@ def main():
         ht_ao_bytes = naux * (nao * (nao + 1) // 2 * 8.0 + nao * 8 * 8.0)
         ao_flops = (2.0 * naux * nao * nao * nmo + 2.0 * naux * nao * nmo * nmo
                     + 2.0 * naux * nmo * nmo * nact * nact + 2.0 * naux * (nmo * nact) ** 2)
-        ao_exec = (2.0 * naux * nao * nao * nact + 2.0 * naux * nao * nmo * nact + 2.0 * naux * (nao * (nao + 1) // 2) * (nact * (nact + 1) // 2)
-                   + 2.0 * nao * nmo * nact * nact * (nao + nmo) + 2.0 * naux * (nmo * nact) ** 2) if ao_route == 2 else ao_flops
+        ntri = nact * (nact + 1) // 2
+        ao_exec = (2.0 * naux * nao * nao * nact + 2.0 * naux * nao * nmo * nact + 2.0 * naux * (nao * (nao + 1) // 2) * ntri
+                   + 2.0 * nao * nmo * ntri * (nao + nmo) + 1.0 * naux * (nmo * nact) ** 2) if ao_route == 2 else ao_flops
         ao = {"ms": ms_ao, "nmo": nmo, "a0": a0, "nact": nact, "launches_per_call": ao_launches,
               "route": {1: "Eq. 18-21 in the printed order", 2: "active first (bmo never formed)"}.get(ao_route, "?"),
               "eq18_ms": ht_ao_ms, "contractions_ms": aprof["syrk"][0],

@@ -376,18 +376,26 @@ __global__ void k_pack_baa(const double* __restrict__ bpa, int naux, size_t npa,
   }
 }
 
-// Wsq[e1][e2][a1 nact + a2] = W[tri(max(e1,e2)) + min(e1,e2)][tri(max(a1,a2)) + min(a1,a2)]; W element (pair, t) sits at
-// pair * pstride + t * tstride (either orientation of the W product)
-__global__ void k_unpack_w(const double* __restrict__ W, int nao, int nact, long long pstride, long long tstride,
+// Wsq[e1][e2][t] = W[tri(max(e1,e2)) + min(e1,e2)][t], t < ldt (the packed active pairs a1 >= a2); W element (pair, t)
+// sits at pair * pstride + t * tstride (either orientation of the W product)
+__global__ void k_unpack_w(const double* __restrict__ W, int nao, int ldt, long long pstride, long long tstride,
                            double* __restrict__ Wsq) {
-  const int naa = nact * nact;
-  const size_t n = (size_t)nao * nao * naa;
+  const size_t n = (size_t)nao * nao * ldt;
   for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
-    const int a = (int)(e % naa), a1 = a / nact, a2 = a - a1 * nact;
-    const size_t ee = e / naa;
+    const int t = (int)(e % ldt);
+    const size_t ee = e / ldt;
     const int e1 = (int)(ee / nao), e2 = (int)(ee % nao);
-    const int t = a1 >= a2 ? a1 * (a1 + 1) / 2 + a2 : a2 * (a2 + 1) / 2 + a1;
     Wsq[e] = W[(e1 >= e2 ? tri(e1) + e2 : tri(e2) + e1) * pstride + t * tstride];
+  }
+}
+
+// ppaa[p1][p2][a1][a2] = Pt[p1][p2][tri(max(a1,a2)) + min(a1,a2)]
+__global__ void k_expand_ppaa(const double* __restrict__ Pt, size_t n2, int nact, int ldt, double* __restrict__ ppaa) {
+  const int naa = nact * nact;
+  for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n2 * naa; e += (size_t)gridDim.x * blockDim.x) {
+    const size_t pp = e / naa;
+    const int a = (int)(e - pp * naa), a1 = a / nact, a2 = a - a1 * nact;
+    ppaa[e] = Pt[pp * ldt + (a1 >= a2 ? a1 * (a1 + 1) / 2 + a2 : a2 * (a2 + 1) / 2 + a1)];
   }
 }
 
@@ -397,14 +405,14 @@ __global__ void k_unpack_w(const double* __restrict__ W, int nao, int nact, long
 // and Eq. 20 is contracted over P in the AO basis first (a Coulomb-like build with the nact^2
 // "densities" baa^P, Eq. 15's pattern), then transformed:
 //      W[e1 e2][a1 a2] = sum_P b^P[e1][e2] bpa^P[a0+a1][a2]      (only the a1 >= a2 columns: baa^P is symmetric),
-//      ppaa[p1][p2][a1 a2] = sum_{e1 e2} M[e1][p1] W[e1 e2][a1 a2] M[e2][p2].
+//      ppaa[p1][p2][a1 a2] = sum_{e1 e2} M[e1][p1] W[e1 e2][a1 a2] M[e2][p2]    (packed pairs a1 >= a2 throughout).
 // Work 2 naux nao^2 nact + naux nao^2 nact^2 + small, against 2 naux nao nmo (nao + nmo) for the
 // printed order: 5x less at nmo = 340, nact = 8; the printed order wins for large active spaces.
 static int launch_ao2mo_active_first(dfjk_ctx* h, int nmo, int a0, int nact, const double* M, double* bpa_out,
                                      double* ppaa_out, double* papa_out, cudaStream_t st) {
   int launches = 0;
   const int nao = h->nao, naux = h->naux;
-  const size_t npa = (size_t)nmo * nact, naa = (size_t)nact * nact;
+  const size_t npa = (size_t)nmo * nact;
   const int ldz = round_up(nact, 8);
   double* Mact = h->X;
   double* Z = h->X + round_up(nao * nact, 2);
@@ -441,27 +449,39 @@ static int launch_ao2mo_active_first(dfjk_ctx* h, int nmo, int a0, int nact, con
   if (ppaa_out) {
     const int ldt = round_up(nact * (nact + 1) / 2, 2);
     double* W = h->X;
-    double* Wsq = W + h->npair * ldt;
-    double* T = Wsq + (size_t)nao * nao * naa;
-    double* baat = T + (size_t)nmo * nao * naa;
+    double* Wsq = W + h->npair * ldt;                        // [e1][e2][t]
+    double* T = Wsq + (size_t)nao * nao * ldt;               // [p1][e2][t]
+    double* baat = T + (size_t)nmo * nao * ldt;              // [P][t]
+    double* Pt = baat + (size_t)naux * ldt;                  // [p1][p2][t]
     k_pack_baa<<<148, 256, 0, st>>>(bpa_out, naux, npa, a0, nact, ldt, baat);
     // W = sum_P b^P (x) baa^P.  With bulk-copyable operands the product runs transposed, Wt[t][pair] = baat^T B
-    // (40 x 256 tiles, 20 accumulator tiles per warp); otherwise as W[pair][t] = B^T baat
+    // (40..64 x 256 tiles, 20 to 32 accumulator tiles per warp); otherwise as W[pair][t] = B^T baat
     GemmTN gwt{baat, h->B, W, ldt, (int)h->npair, naux, (long long)ldt, (long long)h->npair, (long long)h->npair, 0, 0, 0, 0};
-    const bool wt = ldt > 32 && ldt <= 40 && gemm_tn_bulk_ok(gwt);
+    const bool wt = ldt > 32 && ldt <= 64 && gemm_tn_bulk_ok(gwt);         // 8 to 11 active orbitals: 36 to 66 pairs
     if (wt) {
-      if (launch_gemm_tn_b<5, 4, true, 1>(h->device, gwt, 1, st) != cudaSuccess) return -1;
+      cudaError_t e = cudaErrorInvalidValue;
+      switch (cdiv(ldt, 8)) {
+        case 5: e = launch_gemm_tn_b<5, 4, true, 1>(h->device, gwt, 1, st); break;
+        case 6: e = launch_gemm_tn_b<6, 4, true, 1>(h->device, gwt, 1, st); break;
+        case 7: e = launch_gemm_tn_b<7, 4, true, 1>(h->device, gwt, 1, st); break;
+        case 8: e = launch_gemm_tn_b<8, 4, true, 1>(h->device, gwt, 1, st); break;
+        default: break;
+      }
+      if (e != cudaSuccess) return -1;
     } else {
       GemmTN gw{h->B, baat, W, (int)h->npair, ldt, naux, (long long)h->npair, (long long)ldt, (long long)ldt, 0, 0, 0, 0};
       if (gemm_tn(h->device, gw, 1, st) != cudaSuccess) return -1;
     }
-    k_unpack_w<<<1184, 256, 0, st>>>(W, nao, nact, wt ? 1 : ldt, wt ? (long long)h->npair : 1LL, Wsq);
-    GemmTN gt{M, Wsq, T, nmo, (int)(nao * naa), nao, nmo, (long long)(nao * naa), (long long)(nao * naa), 0, 0, 0, 0};
-    if (gemm_tn(h->device, gt, 1, st) != cudaSuccess) return -1;                                      // T[p1][e2 a] = M^T W
-    GemmTN gp{M, T, ppaa_out, nmo, (int)naa, nao, nmo, (long long)naa, (long long)naa, 0, (long long)(nao * naa),
-              (long long)(nmo * naa), 0};
-    if (gemm_tn(h->device, gp, nmo, st) != cudaSuccess) return -1;                                    // ppaa[p1][p2][a] = T_p1^T M
-    launches += 5;
+    k_unpack_w<<<1184, 256, 0, st>>>(W, nao, ldt, wt ? 1 : ldt, wt ? (long long)h->npair : 1LL, Wsq);
+    // the two index transformations keep the packed active pairs: T[p1][e2 t] = M^T W, then ONE product over all
+    // (p1, t) rows, Pt[(p1 t)][p2] = sum_e2 T[p1][e2][t] M[e2][p2], stored as Pt[p1][p2][t]
+    GemmTN gt{M, Wsq, T, nmo, nao * ldt, nao, nmo, (long long)nao * ldt, (long long)nao * ldt, 0, 0, 0, 0};
+    if (gemm_tn(h->device, gt, 1, st) != cudaSuccess) return -1;
+    GemmTN gp{T, M, Pt, nmo * ldt, nmo, nao, ldt, nmo, 0, 0, 0, 0, 0,
+              ldt, (long long)nao * ldt, ldt, (long long)nmo * ldt, ldt};
+    if (gemm_tn(h->device, gp, 1, st) != cudaSuccess) return -1;
+    k_expand_ppaa<<<1184, 256, 0, st>>>(Pt, (size_t)nmo * nmo, nact, ldt, ppaa_out);
+    launches += 6;
   }
   if (papa_out) {
     GemmTN g21{bpa_out, bpa_out, papa_out, (int)npa, (int)npa, naux, (long long)npa, (long long)npa,
@@ -493,10 +513,10 @@ int launch_ao2mo(dfjk_ctx* h, int nmo, int a0, int nact, const double* M, double
   const double cost_printed = 2.0 * dn * dm * (dn + dm) + 2.0 * dm * dm * da * da;          // per aux row
   const double cost_active = 2.0 * dn * dn * round_up(nact, 8) + 2.0 * dn * dm * 32.0 + dn * dn * da * (da + 1.0) * 0.5 +
                              2.0 * dn * dm * da * da * (dn + dm) / (naux > 0 ? naux : 1);
-  const size_t need2 = h->npair * round_up(nact * (nact + 1) / 2, 2) + (size_t)nao * nao * naa + (size_t)nmo * nao * naa +
-                       (size_t)naux * round_up(nact * (nact + 1) / 2, 2);                     // W, Wsq, T, packed baa
+  const size_t ldt_ = (size_t)round_up(nact * (nact + 1) / 2, 2);
+  const size_t need2 = (h->npair + (size_t)nao * nao + (size_t)nmo * nao + (size_t)naux + (size_t)nmo * nmo) * ldt_;  // W, Wsq, T, baat, Pt
   const size_t need1 = (size_t)round_up(nao * nact, 2) + (size_t)nao * round_up(nact, 8);   // Mact + one row of Z
-  const bool fits = nact > 0 && need2 <= h->X_doubles && need1 <= h->X_doubles && (double)nao * naa < 2e9 &&
+  const bool fits = nact > 0 && need2 <= h->X_doubles && need1 <= h->X_doubles && (double)nao * ldt_ < 2e9 && (double)nmo * ldt_ < 2e9 &&
                     round_up(nact, 8) <= h->nocc_pad_cap;
   bool active = fits && cost_active < cost_printed;
   if (h->ao2mo_route == 1) active = false;

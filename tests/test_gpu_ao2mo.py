@@ -172,3 +172,17 @@ def test_symm_thin_unaligned_tensor_falls_back():
     o_bpa, o_ppaa, o_papa = oracle.ao2mo(inp.B_packed[1:], nao, M, 2, 6)
     assert rel(bpa.cpu().numpy(), o_bpa) <= TOL and rel(ppaa.cpu().numpy(), o_ppaa) <= TOL
     assert rel(papa.cpu().numpy(), o_papa) <= TOL
+
+
+@pytest.mark.parametrize("nao,naux,nmo,a0,nact,seed", [
+    (200, 40, 60, 5, 9, 321),       # 45 active pairs (padded to 46): 48-row tiles of the transposed W product
+    (203, 64, 70, 20, 10, 322),     # 55 pairs: 56-row tiles
+    (120, 72, 50, 3, 11, 323),      # 66 pairs: beyond 64, the W product runs in the other orientation
+    (200, 41, 60, 5, 8, 324),       # naux % 4 != 0: no bulk copies, the gather producer
+])
+def test_active_first_route_with_more_active_orbitals(nao, naux, nmo, a0, nact, seed):
+    """the W contraction over the packed active pairs a1 >= a2 in both orientations, the packed index transformations
+    and the lower-tile Eq. 21, for 8 to 11 active orbitals"""
+    bpa, ppaa, papa = run_case(nao, naux, nmo, a0, nact, seed, L=max(4.0, nao / 6), ao2mo_route=2)
+    assert np.array_equal(papa, papa.transpose(2, 3, 0, 1))                  # mirrored: bitwise symmetric
+    assert np.array_equal(ppaa, ppaa.transpose(0, 1, 3, 2))                  # one packed pair serves (a1, a2) and (a2, a1)
