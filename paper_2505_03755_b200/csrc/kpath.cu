@@ -836,6 +836,19 @@ static double syrk_makespan(int n_off, int n_diag, double diag_cost, int ksplit,
   return end;
 }
 
+// SYRK tile T = 16 * WM, WM in {4, 5, 6, 7}: the least modelled work over the lower triangle (ties -> the larger
+// tile); a diagonal CTA costs (WM + 1) / (2 WM) of an off-diagonal one
+static int pick_syrk_tile(int nao) {
+  int wm = 7;
+  double best = 1e300;
+  for (int wmc = 7; wmc >= 4; wmc--) {
+    const int T = 16 * wmc, nt = cdiv(nao, T);
+    const double area = (0.5 * nt * (nt - 1) + (wmc + 1) / (2.0 * wmc) * nt) * (double)T * T;
+    if (area < best * 0.995) { best = area; wm = wmc; }
+  }
+  return wm;
+}
+
 // Split-K factor of the SYRK for blocks of nblk aux rows: the split with the shortest modelled
 // makespan (one CTA per SM), 0.2 % per split for the extra partial tiles; remembered in the handle
 // because the model costs a few thousand heap operations.
@@ -899,17 +912,7 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
   const int n8 = ldx / 8;
   const int ntn = cdiv(n8, 2 * kHtMaxWN), wn = cdiv(n8, 2 * ntn);  // N tile = 16*wn columns
   const int ntm_ht = cdiv(nao, 64);
-  // SYRK tile T = 16*wm_s in {64,...,112}: least modelled work (ties -> larger tile); a diagonal
-  // CTA costs (WM+1)/(2 WM) of an off-diagonal one
-  int wm_s = 7;
-  {
-    double best = 1e300;
-    for (int wmc = 7; wmc >= 4; wmc--) {
-      const int T = 16 * wmc, nt = cdiv(nao, T);
-      const double area = (0.5 * nt * (nt - 1) + (wmc + 1) / (2.0 * wmc) * nt) * (double)T * T;
-      if (area < best * 0.995) { best = area; wm_s = wmc; }
-    }
-  }
+  const int wm_s = pick_syrk_tile(nao);
   const double diag_cost = (wm_s + 1) / (2.0 * wm_s);
   const int ntm = cdiv(nao, 16 * wm_s), ntiles = ntm * (ntm + 1) / 2;
   const int ksplit = emu ? emu_pick_ksplit(nao, cdiv((int)nblk, h->k_emu_pgroup), h->ksplit, h->num_sms)
@@ -1064,15 +1067,7 @@ int launch_k_path_dm(dfjk_ctx* h, int nset, const double* D, double* K_out, cuda
   const int n8 = ldx / 8;
   const int ntn = cdiv(n8, 2 * kHtMaxWN), wn = cdiv(n8, 2 * ntn);
   const int ntm_ht = cdiv(nao, 64);
-  int wm_s = 7;
-  {
-    double best = 1e300;
-    for (int wmc = 7; wmc >= 4; wmc--) {
-      const int T = 16 * wmc, nt = cdiv(nao, T);
-      const double area = (0.5 * nt * (nt - 1) + (wmc + 1) / (2.0 * wmc) * nt) * (double)T * T;
-      if (area < best * 0.995) { best = area; wm_s = wmc; }
-    }
-  }
+  const int wm_s = pick_syrk_tile(nao);
   const double diag_cost = (wm_s + 1) / (2.0 * wm_s);
   const int ntm = cdiv(nao, 16 * wm_s), ntiles = ntm * (ntm + 1) / 2;
   const int ksplit = pick_ksplit(h, (int)nblk, ntiles, ntm, diag_cost);
