@@ -198,7 +198,8 @@ size_t dfjk_workspace_bytes(dfjk_handle h);
 /* Plan of the last/next call, for tests and the bench: aux block size, SYRK split-K factor, padded
  * column capacity of X, and whether the half-transform reads the re-tiled private copy of B
  * (1) or gathers from the packed triangle (0: option no_retile, or the copy did not fit the
- * device memory at create).  Any pointer may be NULL. */
+ * device memory at create).  After a single-launch call (option no_small_path) nblk = naux and ksplit =
+ * the number of CTAs of that launch.  Any pointer may be NULL. */
 int dfjk_get_plan(dfjk_handle h, int* nblk, int* ksplit, int* nocc_pad_capacity, int* retiled);
 
 /* Number of kernel launches dfjk_get_jk enqueued in its last call on this handle. */

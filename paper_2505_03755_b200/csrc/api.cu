@@ -282,13 +282,16 @@ int dfjk_get_jk(dfjk_handle h, int nset, const int* nocc, const double* C, const
   int n = 0, k;
   // embedding-sized call: one launch does steps a1-a9 (small.cu)
   if (const int ctas = small_path_ctas(h, si)) {
-    if (launch_small_fused(h, si, ctas, C, occ, J_out, K_out, st) < 0) { set_err(h, "small path launch", cudaGetLastError()); return DFJK_ERR_CUDA; }
-    prof_mark(h, -1, st);
-    h->last_launches = 1;
-    h->plan_nblk = h->naux; h->plan_ksplit = ctas; h->plan_nblocks = 1;
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) { set_err(h, "kernel launch", e); return DFJK_ERR_CUDA; }
-    return DFJK_OK;
+    if (launch_small_fused(h, si, ctas, C, occ, J_out, K_out, st) >= 0) {
+      prof_mark(h, -1, st);
+      h->last_launches = 1;
+      h->plan_nblk = h->naux; h->plan_ksplit = ctas; h->plan_nblocks = 1;
+      cudaError_t e = cudaGetLastError();
+      if (e != cudaSuccess) { set_err(h, "kernel launch", e); return DFJK_ERR_CUDA; }
+      return DFJK_OK;
+    }
+    cudaGetLastError();          // the cooperative launch was refused (e.g. not every CTA can be resident): the tiled kernels serve the call
+    h->ev_n = 0;
   }
   n += launch_prep_ct(h, si, C, occ, st);
   // both outputs: rho falls out of the half-transform, so J needs one stream over B instead of two
