@@ -189,6 +189,7 @@ int dfjk_create(int naux, int nao, const double* B_packed, const dfjk_options* o
     h->nblk = (int)(dbl / one_row);
   }
   h->j1_chunks = (int)((h->npair + kJ1Chunk - 1) / kJ1Chunk);
+  h->j2_mma_min_sets = 1;   // measured at large: k_j2 (DFMA) 3.18 / 3.39 / 4.58 ms at 1 / 4 / 8 sets, k_j2_mma 3.13 / 3.20 / 3.35
   h->j1_mma_min_sets = 3;   // measured at large: DFMA kernel 3.27 / 3.41 / 3.81 ms at 1 / 2 / 4 sets, DMMA kernel 3.43 / 3.47 / 3.51 (3.65 at 8)
   {
     const long long xcols = (long long)((h->npair + 2 * kJ2Threads - 1) / (2 * kJ2Threads));

@@ -55,6 +55,7 @@ struct dfjk_ctx {
   int n_mtiles;              // 128-row tiles along nao
   int j1_chunks, j2_splits;
   int j1_mma_min_sets;       // J pass 1: sets per group from which the DMMA kernel replaces the DFMA one
+  int j2_mma_min_sets;       // J pass 2: likewise
   int num_sms;
   int ht_grid;               // persistent half-transform: CTAs (= SMs)
   int ao2mo_route;           // option: 0 = cheaper route, 1 = Eq. 18-21 as printed, 2 = active first

@@ -440,6 +440,97 @@ k_j2(const double* __restrict__ B, size_t npair, int naux, const double* __restr
   }
 }
 
+// Pass 2 on the FP64 tensor pipe (16-byte aligned packed rows; k_j2 serves the rest): Jp[set][pair] = sum_P rho[set][P] B[P][pair] is a GEMM over the
+// aux rows, one DMMA.8x8x4 takes 8 sets x 4 aux rows x 8 pairs.  CTA = one chunk of 512 pairs x one split of
+// the aux rows; a stage of the bulk-copy ring holds 8 aux rows of the chunk (row stride 516 doubles: conflict-
+// free fragments); warp w owns pairs [64 w, 64 w + 64) as 8 accumulator tiles (16 registers) for the whole
+// split.  k_j2 (DFMA, 2 NS FMAs per loaded pair) falls from 7.2 to 4.9 TB/s between one and eight sets; this
+// kernel does the same 16 LDS + 16 DMMA per stage and warp whatever the number of sets.
+constexpr int kJ2mStages = 5;
+
+__global__ void __launch_bounds__(kJ1tThreads, 1)
+k_j2_mma(const double* __restrict__ B, size_t npair, int naux, const double* __restrict__ rho, int ns,
+         double* __restrict__ part, size_t split_stride, int rows_per_split) {
+  extern __shared__ __align__(128) double smem[];
+  __shared__ __align__(8) unsigned long long bars[2 * kJ2mStages];
+  const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kJ2mStages]);
+  const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
+  const size_t k0 = (size_t)blockIdx.x * kJ1tSC;
+  const int nvalid = (int)(npair - k0 < (size_t)kJ1tSC ? npair - k0 : (size_t)kJ1tSC);
+  const int p_beg = blockIdx.y * rows_per_split;
+  const int p_end = min(naux, p_beg + rows_per_split);
+  const int nstage = p_end > p_beg ? (p_end - p_beg + 7) / 8 : 0;
+  for (int e = tid; e < kJ2mStages * kJ1mStageDoubles; e += kJ1tThreads) smem[e] = 0.0;      // stale slots stay finite
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  if (tid == 0) {
+    for (int s = 0; s < kJ2mStages; s++) {
+      mbar_init(full0 + 8 * s, 1);
+      mbar_init(empty0 + 8 * s, 8);
+    }
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  if (w == 8) {
+    if (l == 0) {
+      const uint32_t ring_u32 = smem_u32(smem);
+      const uint32_t bytes = (uint32_t)nvalid * 8u;
+      for (int it = 0; it < nstage; it++) {
+        const int stage = it % kJ2mStages;
+        const uint32_t fullb = full0 + 8 * stage;
+        mbar_wait(empty0 + 8 * stage, ((it / kJ2mStages) & 1) ^ 1);
+        const int nrows = min(8, p_end - (p_beg + 8 * it));
+        mbar_arrive_expect_tx(fullb, bytes * (uint32_t)nrows);
+        for (int g = 0; g < nrows; g++)
+          bulk_g2s(ring_u32 + (uint32_t)(stage * kJ1mStageDoubles + g * kJ1mLd) * 8u, B + (size_t)(p_beg + 8 * it + g) * npair + k0,
+                   bytes, fullb);
+      }
+    }
+    return;
+  }
+
+  const int r = l >> 2, j = l & 3;
+  double acc[8][2];
+#pragma unroll
+  for (int t = 0; t < 8; t++) acc[t][0] = acc[t][1] = 0.0;
+  const double* rp = rho + (size_t)(r < ns ? r : 0) * naux;
+  for (int it = 0; it < nstage; it++) {
+    const int stage = it % kJ2mStages;
+    // A fragments: rho[set r][P], P = p_beg + 8 it + 4 h + j (zero for sets past ns and rows past the split)
+    const int P0 = p_beg + 8 * it + j;
+    const double a0 = (r < ns && P0 < p_end) ? __ldg(rp + P0) : 0.0;
+    const double a1 = (r < ns && P0 + 4 < p_end) ? __ldg(rp + P0 + 4) : 0.0;
+    mbar_wait(full0 + 8 * stage, (it / kJ2mStages) & 1);
+    const double* bp = smem + stage * kJ1mStageDoubles + j * kJ1mLd + 64 * w + r;
+    double b0[8], b1[8];
+#pragma unroll
+    for (int t = 0; t < 8; t++) { b0[t] = bp[8 * t]; b1[t] = bp[4 * kJ1mLd + 8 * t]; }
+#pragma unroll
+    for (int t = 0; t < 8; t++) dmma884(acc[t][0], acc[t][1], a0, b0[t]);
+#pragma unroll
+    for (int t = 0; t < 8; t++) dmma884(acc[t][0], acc[t][1], a1, b1[t]);
+    __syncwarp();
+    if (l == 0) mbar_arrive(empty0 + 8 * stage);
+  }
+  // lane (r, j) holds Jp[set r][pairs 64 w + 8 t + 2 j, + 1]
+  if (r < ns) {
+    double* out = part + (size_t)blockIdx.y * split_stride + (size_t)r * npair + k0 + 64 * w + 2 * j;
+#pragma unroll
+    for (int t = 0; t < 8; t++)
+      if (64 * w + 8 * t + 2 * j < nvalid) *reinterpret_cast<double2*>(out + 8 * t) = make_double2(acc[t][0], acc[t][1]);
+  }
+}
+
+static cudaError_t launch_j2_mma(int device, dim3 grid, cudaStream_t st, const double* B, size_t npair, int naux,
+                                 const double* rho, int ns, double* part, size_t split_stride, int rows_per_split) {
+  constexpr size_t smem = (size_t)kJ2mStages * kJ1mStageDoubles * sizeof(double);
+  static std::atomic<unsigned long long> attr_done{0};
+  cudaError_t e = ensure_dyn_smem(k_j2_mma, smem, device, attr_done);
+  if (e != cudaSuccess) return e;
+  k_j2_mma<<<grid, kJ1tThreads, smem, st>>>(B, npair, naux, rho, ns, part, split_stride, rows_per_split);
+  return cudaSuccess;
+}
+
 // Step a4: J_s[mu][nu] = J_s[nu][mu] = sum_g part[g][s][tri(mu)+nu] (g ascending), 32x32 tiles,
 // the mirrored tile goes through shared memory so both global writes are row-contiguous.
 __global__ void __launch_bounds__(256)
@@ -521,6 +612,14 @@ int launch_j_passes(dfjk_ctx* h, const SetInfo& si, double* J_out, bool rho_read
     }
     prof_mark(h, DFJK_PHASE_J2, st);
     dim3 g2((unsigned)((npair + 2 * kJ2Threads - 1) / (2 * kJ2Threads)), h->j2_splits);
+    if (vec && ns >= h->j2_mma_min_sets) {
+      dim3 gm((unsigned)((npair + kJ1tSC - 1) / kJ1tSC), h->j2_splits);
+      if (launch_j2_mma(h->device, gm, st, h->B, npair, naux, h->rho + (size_t)s0 * naux, ns, h->Jp_part + (size_t)s0 * npair,
+                        split_stride, rows_per_split) != cudaSuccess)
+        return -1;
+      launches += 1;
+      continue;
+    }
     cudaError_t e2 = vec ? launch_j2<true>(ns, g2, st, h->B, npair, naux, h->rho + (size_t)s0 * naux, h->Jp_part + (size_t)s0 * npair, split_stride, rows_per_split)
                          : launch_j2<false>(ns, g2, st, h->B, npair, naux, h->rho + (size_t)s0 * naux, h->Jp_part + (size_t)s0 * npair, split_stride, rows_per_split);
     if (e2 != cudaSuccess) return -1;
