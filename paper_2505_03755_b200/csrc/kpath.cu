@@ -655,7 +655,24 @@ k_syrk2(const double* __restrict__ X, const double* __restrict__ X2, const unsig
   double* Kp = Kpart_s + (size_t)g * split_stride;
   double* red = smem;                                // reused after the main loop
   Syrk2Consumer q{sA, one_operand ? sA : sB, full0, empty0, nchunks, ch0, ch1, c0, c1, kTileDoubles, 0, 0, 0, sgn};
-  if (!diag) {
+  if (!diag && a0 + 8 * WM >= nao) {
+    // half-height tile of the last tile row: the rows of the lower block row (bm = 1) lie past the basis, so the two
+    // sub-partitions of a block column share the upper block 4-way: warp (sp, hh) takes the k4 steps
+    // (sp & 1) + 2 hh mod 4 of block (0, bn), bn = sp >> 1; half the DMMAs of a full tile on every sub-partition
+    const int bn = sp >> 1, part = (sp & 1) + 2 * hh;
+    q.row0 = 0; q.col0 = bn * 8 * WM; q.kidx = part;
+    double acc[WM][WM][2];
+    syrk2_mainloop<WM, false, 4>(q, l, acc);
+    consumer_bar_sync();
+    if (part != 0) syrk2_put<WM, false>(red, 3 * bn + part - 1, l, acc);
+    consumer_bar_sync();
+    if (part == 0) {
+      syrk2_add<WM, false>(red, 3 * bn, l, acc);
+      syrk2_add<WM, false>(red, 3 * bn + 1, l, acc);
+      syrk2_add<WM, false>(red, 3 * bn + 2, l, acc);
+      syrk2_store<WM, false>(Kp, nao, a0, b0 + q.col0, first, l, acc);
+    }
+  } else if (!diag) {
     // block (bm, bn) = (sp & 1, sp >> 1); pair split-K 2
     q.row0 = (sp & 1) * 8 * WM; q.col0 = (sp >> 1) * 8 * WM; q.kidx = hh;
     double acc[WM][WM][2];
@@ -837,13 +854,16 @@ static double syrk_makespan(int n_off, int n_diag, double diag_cost, int ksplit,
 }
 
 // SYRK tile T = 16 * WM, WM in {4, 5, 6, 7}: the least modelled work over the lower triangle (ties -> the larger
-// tile); a diagonal CTA costs (WM + 1) / (2 WM) of an off-diagonal one
+// tile); a diagonal CTA costs (WM + 1) / (2 WM) of an off-diagonal one, a half-height one 1/2
 static int pick_syrk_tile(int nao) {
   int wm = 7;
   double best = 1e300;
   for (int wmc = 7; wmc >= 4; wmc--) {
     const int T = 16 * wmc, nt = cdiv(nao, T);
-    const double area = (0.5 * nt * (nt - 1) + (wmc + 1) / (2.0 * wmc) * nt) * (double)T * T;
+    // the off-diagonal tiles of the last tile row cost half when at most T / 2 of its rows exist
+    const bool half_last = nao - (nt - 1) * T <= T / 2;
+    const double n_off = 0.5 * nt * (nt - 1) - (half_last ? 0.5 * (nt - 1) : 0.0);
+    const double area = (n_off + (wmc + 1) / (2.0 * wmc) * nt) * (double)T * T;
     if (area < best * 0.995) { best = area; wm = wmc; }
   }
   return wm;
