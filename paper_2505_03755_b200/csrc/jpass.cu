@@ -612,7 +612,10 @@ int launch_j_passes(dfjk_ctx* h, const SetInfo& si, double* J_out, bool rho_read
     }
     prof_mark(h, DFJK_PHASE_J2, st);
     dim3 g2((unsigned)((npair + 2 * kJ2Threads - 1) / (2 * kJ2Threads)), h->j2_splits);
-    if (vec && ns >= h->j2_mma_min_sets) {
+    // the tensor-pipe kernel wins on long streams (3.13 vs 3.18 ms at large) and whenever there are many sets; on
+    // short ones (medium: 0.47 vs 0.42 ms) its per-CTA ring set-up shows, and k_j2 stays
+    const bool long_stream = (double)naux * (double)npair * 8.0 >= 8e9;
+    if (vec && ns >= (long_stream ? h->j2_mma_min_sets : 7)) {
       dim3 gm((unsigned)((npair + kJ1tSC - 1) / kJ1tSC), h->j2_splits);
       if (launch_j2_mma(h->device, gm, st, h->B, npair, naux, h->rho + (size_t)s0 * naux, ns, h->Jp_part + (size_t)s0 * npair,
                         split_stride, rows_per_split) != cudaSuccess)
