@@ -78,3 +78,20 @@ def test_bench_work_model_matches_survey_table():
     fb = bench.flops_bytes(dfjk_inputs.CONFIGS["large"])
     assert abs(fb["ht"] - 3.456e12) < 1e9 and abs(fb["k"] - 5.185e12) / 5.185e12 < 1e-3
     assert abs(fb["b_bytes"] - 23.0592e9) < 1e6 and abs(fb["j_bytes"] - 46.12e9) / 46.12e9 < 1e-3
+
+
+def test_options_struct_matches_the_header_field_for_field():
+    """dfjk_options crosses the boundary by value layout: the ctypes mirror must list the same fields, in the
+    same order and with the same C types as include/dfjk.h, and DFJK.__init__ must take every one of them"""
+    import inspect
+    from paper_2505_03755_b200.api import DFJK, dfjk_options
+    txt = open(os.path.join(ROOT, "include", "dfjk.h")).read()
+    body = txt[txt.index("typedef struct {"):txt.index("} dfjk_options;")]
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    fields = re.findall(r"\b(size_t|int)\s+([A-Za-z_0-9]+)\s*;", body)
+    ctype = {"size_t": ct.c_size_t, "int": ct.c_int}
+    assert [(n, ctype[t]) for t, n in fields] == list(dfjk_options._fields_)
+    assert ct.sizeof(dfjk_options) == 8 + 4 * (len(fields) - 1) + (4 * (len(fields) - 1)) % 8
+    params = inspect.signature(DFJK.__init__).parameters
+    for _, n in fields:
+        assert n in params, n
