@@ -426,7 +426,8 @@ static int launch_ao2mo_active_first(dfjk_ctx* h, int nmo, int a0, int nact, con
   si.nset = 1; si.col0[0] = 0; si.nocc[0] = nact; si.coff[0] = 0; si.ooff[0] = 0;
   si.col0[1] = si.nocc_pad = ldz;
   // at most 8 active columns: one pass over the packed triangle, every stored element used twice (symm.cu)
-  // (two passes of the thin kernel for 9 to 16 columns were measured: 10.5 ms against 9.8 ms tiled at nact = 10)
+  // (9 to 16 columns were measured both as two passes of the thin kernel, 10.5 ms, and as two column groups on the
+  // same fragments, 10.2 ms, against 9.8 ms tiled at nact = 10: the thin kernel is bound by its DMMA issue)
   const bool thin = symm_thin_ok(h, nact) && ldz == 8;
   launches += 1;
   if (!thin) launches += launch_prep_ct(h, si, Mact, nullptr, st);
