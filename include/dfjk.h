@@ -169,7 +169,8 @@ int dfjk_get_jk_dm(dfjk_handle h, int nset, const double* D, double* J_out, doub
  *   bpa_out  DEVICE, naux x nmo x nact: bpa[P][p][a] = bmo^P[p][a0+a], the block the paper pulls
  *            back to the host.  Required (it is also the operand of Eq. 21).
  *   ppaa_out DEVICE, nmo x nmo x nact x nact, or NULL to skip Eq. 20.
- *   papa_out DEVICE, nmo x nact x nmo x nact, or NULL to skip Eq. 21 (the paper runs it on the CPU).
+ *   papa_out DEVICE, nmo x nact x nmo x nact, or NULL to skip Eq. 21 (the paper runs it on the CPU).  Computed on the
+ *            tiles at and below the diagonal of the (p1 a1) x (p2 a2) matrix and mirrored: bitwise symmetric.
  * Same conventions as dfjk_get_jk: enqueue-only on `stream`, no allocation, no host
  * synchronisation, outputs overwritten, deterministic.  The aux blocks share the X workspace of
  * the handle (per aux row nao*roundup(nmo,8) + nmo^2 + nact^2 doubles); if the cap
