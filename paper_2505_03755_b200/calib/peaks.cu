@@ -40,6 +40,26 @@ __global__ void k_dfma(double* out, int iters) {
   if (s == 123.456) out[0] = s;
 }
 
+// Issue rate of ONE warp per SM sub-partition as a function of operand reuse: 16 accumulators, DMMA i reads
+// a[i % NA] and b[(i / 2) % NB] (NA = NB = 1: both operands reused; NA = 16, NB = 8: every DMMA reads fresh registers)
+template <int NA, int NB>
+__global__ void k_dmma_ops(double* out, int iters) {
+  double acc[16][2], a[NA], b[NB];
+#pragma unroll
+  for (int i = 0; i < 16; i++) acc[i][0] = acc[i][1] = 0.0;
+#pragma unroll
+  for (int i = 0; i < NA; i++) a[i] = 1.0 + threadIdx.x * 1e-3 + i;
+#pragma unroll
+  for (int i = 0; i < NB; i++) b[i] = 0.5 + i * 0.25 + threadIdx.x;
+  for (int it = 0; it < iters; it++)
+#pragma unroll
+    for (int i = 0; i < 16; i++) dmma(acc[i][0], acc[i][1], a[i % NA], b[(i / 2) % NB]);
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 16; i++) s += acc[i][0] + acc[i][1];
+  if (s == 123.456) out[0] = s;
+}
+
 // Do DMMA (tensor pipe) and DFMA (fp64 pipe) add up?  Even warps run the DMMA loop, odd warps the DFMA loop.
 __global__ void k_mixed(double* out, int iters) {
   double acc[8][2], f[16];
@@ -97,6 +117,7 @@ static float time_ms(void (*launch)(void*), void* ctx) {
 struct Ctx { double* out; int warps; int iters; const double2* p; size_t n; int ctas; int threads; };
 template <int NACC> void l_dmma(void* c) { Ctx* x = (Ctx*)c; k_dmma<NACC><<<148, 32 * x->warps>>>(x->out, x->iters); }
 template <int NACC> void l_dfma(void* c) { Ctx* x = (Ctx*)c; k_dfma<NACC><<<148, 32 * x->warps>>>(x->out, x->iters); }
+template <int NA, int NB> void l_ops(void* c) { Ctx* x = (Ctx*)c; k_dmma_ops<NA, NB><<<148, 32 * x->warps>>>(x->out, x->iters); }
 void l_mixed(void* c) { Ctx* x = (Ctx*)c; k_mixed<<<148, 32 * x->warps>>>(x->out, x->iters); }
 template <int U> void l_read(void* c) { Ctx* x = (Ctx*)c; k_read<U><<<148 * x->ctas, x->threads>>>(x->p, x->n, x->out); }
 
@@ -118,6 +139,12 @@ int main() {
     }
     ms = time_ms(l_dfma<16>, &c);
     printf("dfma nacc=16 warps/SM=%2d  %7.3f ms  %6.2f TFLOP/s\n", warps, ms, 148.0 * warps * 32 * iters * 16 * 2.0 / ms * 1e-9);
+  }
+  for (int warps : {4, 8}) {                                            // operand reuse: one / two warps per sub-partition
+    c.warps = warps;
+    const double f = 148.0 * warps * iters * 16 * 512 * 1e-9;
+    printf("dmma operands warps/SM=%d  A,B reused %6.2f  A reused %6.2f  B reused %6.2f  none reused %6.2f TFLOP/s\n", warps,
+           f / time_ms(l_ops<1, 1>, &c), f / time_ms(l_ops<1, 8>, &c), f / time_ms(l_ops<16, 1>, &c), f / time_ms(l_ops<16, 8>, &c));
   }
   for (int warps : {8, 16}) {                                           // half of the warps DMMA, the other half DFMA
     c.warps = warps;
