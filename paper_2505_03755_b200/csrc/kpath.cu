@@ -66,12 +66,44 @@ struct HtParams {
   // (tile (mb, c), c < 4 (mb + 1), at image 2 mb (mb + 1) + c), so that the A operand of every chunk
   // is one bulk copy (a stored or diagonal tile) or four (the transpose: 16 rows of four images)
   const double* Bt; size_t bt_pstride;
+  // with Bt and 1 <= nao % 64 <= 32 the last 64-row block of an aux row is half empty: the last blocks of TWO aux
+  // rows then share one tile (rows 0-31: aux row pl, rows 32-63: aux row pl + 1), scheduled after the full tiles
+  int pair_last;
 };
+
+// tile index -> (aux row, 64-row block, N tile); paired: the tile holds the last blocks of aux rows pl and pl + 1
+struct HtTile { int pl, mb, nt; bool paired; };
+template <bool PAIR>
+__device__ __forceinline__ int ht_num_tiles(const HtParams& q) {
+  return PAIR ? q.nb * (q.ntm - 1) * q.ntn + ((q.nb + 1) >> 1) * q.ntn : q.nb * q.ntm * q.ntn;
+}
+template <bool PAIR>
+__device__ __forceinline__ HtTile ht_tile(const HtParams& q, int tile) {
+  HtTile t;
+  if (!PAIR) {
+    const int tiles_per_p = q.ntm * q.ntn;
+    t.pl = tile / tiles_per_p;
+    const int rem = tile - t.pl * tiles_per_p;
+    t.mb = rem / q.ntn; t.nt = rem % q.ntn; t.paired = false;
+    return t;
+  }
+  const int per_p = (q.ntm - 1) * q.ntn, nfull = q.nb * per_p;
+  if (tile < nfull) {
+    t.pl = tile / per_p;
+    const int rem = tile - t.pl * per_p;
+    t.mb = rem / q.ntn; t.nt = rem - t.mb * q.ntn; t.paired = false;
+  } else {
+    const int t2 = tile - nfull;
+    t.pl = 2 * (t2 / q.ntn); t.nt = t2 % q.ntn; t.mb = q.ntm - 1; t.paired = true;
+  }
+  return t;
+}
 
 // EPI = 0: X k-tiled for k_syrk2.  EPI = 1: the same, plus rho[s][P] = sum_{mu,i in s} X[mu][i] C'[mu][i]
 // (= sum_{mu,lam} B_P[mu][lam] D_s[lam][mu], Eq. 14) as per-warp partials, so that a get_jk call that
 // wants both J and K streams B twice instead of three times.  EPI = 2: X row-major (AO2MO, Eq. 18).
-template <int WN, int EPI>
+// PAIR (compile-time, so that the unpaired instances keep their register budget): HtParams::pair_last
+template <int WN, int EPI, bool PAIR>
 __global__ void __launch_bounds__(kThreads, 1)
 k_half_transform(const __grid_constant__ HtParams q) {
   extern __shared__ __align__(128) double smem[];
@@ -86,7 +118,7 @@ k_half_transform(const __grid_constant__ HtParams q) {
   const int nao = q.nao;
   const int nk4 = (nao + 3) >> 2;                  // k4 steps that carry data
   const int nchunks = (nk4 + 3) >> 2;
-  const int tiles_per_p = q.ntm * q.ntn, ntiles = q.nb * tiles_per_p;
+  const int tiles_per_p = q.ntm * q.ntn, ntiles = ht_num_tiles<PAIR>(q);
 
   if (tid == 0) {
     for (int s = 0; s < kS; s++) {
@@ -108,17 +140,22 @@ k_half_transform(const __grid_constant__ HtParams q) {
       constexpr uint32_t kImgBytes = 64 * kHtLd * 8, kPieceBytes = 16 * kHtLd * 8;
       int g = 0;
       for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const int pl = tile / tiles_per_p, rem = tile - pl * tiles_per_p;
-        const int mb = rem / q.ntn, n0 = (rem % q.ntn) * NT;
+        const HtTile ht = ht_tile<PAIR>(q, tile);
+        const int pl = ht.pl, mb = ht.mb, n0 = ht.nt * NT;
         const double* BtP = q.Bt + (size_t)(q.p_first + pl) * q.bt_pstride;
+        const bool second = (PAIR && ht.paired) && pl + 1 < q.nb;
         for (int c = 0; c < nchunks; c++, g++) {
           const int stage = g % kS;
           const uint32_t fullb = full0 + 8 * stage;
           mbar_wait(empty0 + 8 * stage, ((g / kS) & 1) ^ 1);
-          mbar_arrive_expect_tx(fullb, kBBytes + kImgBytes);
+          mbar_arrive_expect_tx(fullb, kBBytes + ((PAIR && ht.paired) && !second ? kImgBytes / 2 : kImgBytes));
           bulk_g2s(sB_u32 + (uint32_t)stage * kBBytes, q.Ct + ((size_t)c * q.ct_rows + n0) * kHtLd, kBBytes, fullb);
           const uint32_t a_base = sA_u32 + (uint32_t)(stage * kHtATile) * 8u;
-          if (c < 4 * (mb + 1)) {                    // stored or diagonal tile: its image as it is
+          if ((PAIR && ht.paired)) {                           // rows 0-31 of the last block's image of two aux rows (always stored / diagonal)
+            const size_t img = (size_t)(2 * mb * (mb + 1) + c) * (64 * kHtLd);
+            bulk_g2s(a_base, BtP + img, kImgBytes / 2, fullb);
+            if (second) bulk_g2s(a_base + kImgBytes / 2, BtP + q.bt_pstride + img, kImgBytes / 2, fullb);
+          } else if (c < 4 * (mb + 1)) {             // stored or diagonal tile: its image as it is
             bulk_g2s(a_base, BtP + (size_t)(2 * mb * (mb + 1) + c) * (64 * kHtLd), kImgBytes, fullb);
           } else {                                   // transpose: rows 16 (c % 4) .. + 15 of the images (c / 4, 4 mb + qq)
             const int mbl = c >> 2;
@@ -137,8 +174,8 @@ k_half_transform(const __grid_constant__ HtParams q) {
     const uint32_t a_dst_d = (uint32_t)(md * kHtLd + kd) * 8u, a_dst_t = (uint32_t)(kt * kHtLdT + mt) * 8u;
     int g = 0;                                     // chunk counter across tiles
     for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-      const int pl = tile / tiles_per_p, rem = tile - pl * tiles_per_p;
-      const int m0 = (rem / q.ntn) * 64, n0 = (rem % q.ntn) * NT;
+      const HtTile ht = ht_tile<PAIR>(q, tile);
+      const int pl = ht.pl, m0 = ht.mb * 64, n0 = ht.nt * NT;
       const double* BpP = q.Bp + (size_t)(q.p_first + pl) * q.npair;
       const bool okt = m0 + mt < nao;
       for (int c = 0; c < nchunks; c++, g++) {
@@ -192,9 +229,12 @@ k_half_transform(const __grid_constant__ HtParams q) {
 
   int g = 0;
   for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-    const int pl = tile / tiles_per_p, rem = tile - pl * tiles_per_p;
-    const int mb = rem / q.ntn, nt = rem % q.ntn;
+    const HtTile ht = ht_tile<PAIR>(q, tile);
+    const int mb = ht.mb, nt = ht.nt, rem = PAIR ? mb * q.ntn + nt : tile - ht.pl * tiles_per_p;
     const int m0 = mb * 64, n0 = nt * NT;
+    // rows of this warp: 16 wm.. of aux row pl; in a paired tile rows 16 (wm & 1).. of aux row pl + (wm >> 1)
+    const int pl = (PAIR && ht.paired) ? ht.pl + (wm >> 1) : ht.pl;
+    const int mrow0 = (PAIR && ht.paired) ? m0 + (wm & 1) * 16 : m0 + wm * 16;
 #pragma unroll
     for (int t = 0; t < 2; t++)
 #pragma unroll
@@ -246,12 +286,13 @@ k_half_transform(const __grid_constant__ HtParams q) {
       __syncwarp();
       if (l == 0) mbar_arrive(empty0 + 8 * stage);
     }
-    // epilogue: lane owns X[mu][n], X[mu][n+1] with mu = m0 + 16 wm + 8t + r, n = n0 + 8 (wn WN + u) + 2j
+    // epilogue: lane owns X[mu][n], X[mu][n+1] with mu = mrow0 + 8t + r, n = n0 + 8 (wn WN + u) + 2j
+    if (PAIR && pl >= q.nb) continue;             // second half of a paired tile past the last aux row
     if (EPI == 2) {
       double* Xp = q.X + (size_t)pl * q.xrows * q.ldx;
 #pragma unroll
       for (int t = 0; t < 2; t++) {
-        const int mu = m0 + wm * 16 + 8 * t + r;
+        const int mu = mrow0 + 8 * t + r;
         if (mu >= nao) continue;
 #pragma unroll
         for (int u = 0; u < WN; u++) {
@@ -264,7 +305,7 @@ k_half_transform(const __grid_constant__ HtParams q) {
       double* Xp = q.X + (size_t)pl * q.nch * q.mu_pad * kLdT;
 #pragma unroll
       for (int t = 0; t < 2; t++) {
-        const int mu = m0 + wm * 16 + 8 * t + r;
+        const int mu = mrow0 + 8 * t + r;
         if (mu >= nao) continue;
 #pragma unroll
         for (int u = 0; u < WN; u++) {
@@ -282,6 +323,8 @@ k_half_transform(const __grid_constant__ HtParams q) {
       const int nslots = tiles_per_p * 8;
       double* slot = q.rho_ht + ((size_t)(q.p_first + pl) * nslots + (size_t)rem * 8 + w) * q.nset;
       for (int s = l; s < q.nset; s += 32) slot[s] = 0.0;
+      if ((PAIR && ht.paired))                                     // the slots of the warps that serve the other aux row stay empty
+        for (int s = l; s < q.nset; s += 32) (slot + ((w ^ 2) - w) * q.nset)[s] = 0.0;
       int myset = -1;
       if (l < WN) {
         const int col = n0 + 8 * (wn * WN + l);
@@ -304,7 +347,7 @@ k_half_transform(const __grid_constant__ HtParams q) {
             const int n = n0 + 8 * (wn * WN + u0 + uu) + 2 * j;
 #pragma unroll
             for (int t = 0; t < 2; t++) {
-              const int mu = min(m0 + wm * 16 + 8 * t + r, nao - 1);     // rows past nao hold acc = 0
+              const int mu = min(mrow0 + 8 * t + r, nao - 1);     // rows past nao hold acc = 0
               const double* cp = q.Ct + ((size_t)(mu >> 4) * q.ct_rows + n) * kHtLd + (mu & 15);
               cv[uu][t][0] = __ldg(cp);
               cv[uu][t][1] = __ldg(cp + kHtLd);
@@ -356,7 +399,7 @@ k_half_transform(const __grid_constant__ HtParams q) {
           const int n = n0 + 8 * (wn * WN + u0 + uu) + 2 * j;
 #pragma unroll
           for (int t = 0; t < 2; t++) {
-            const int mu = m0 + wm * 16 + 8 * t + r;
+            const int mu = mrow0 + 8 * t + r;
             const bool ok = su[uu] >= 0 && mu < nao;
             const double* cp = q.Ct + ((size_t)(ok ? (mu >> 4) : 0) * q.ct_rows + (ok ? n : 0)) * kHtLd + (mu & 15);
             cv[uu][t][0] = ok ? __ldg(cp) : 0.0;
@@ -754,13 +797,20 @@ __global__ void k_zero(double* p, size_t n) {
 static size_t ht_smem_bytes(int wn) { return (size_t)ht_stages(wn) * (kHtATile + 16 * wn * kHtLd) * sizeof(double); }
 static size_t syrk_smem_bytes(int wm) { return (size_t)kStages * 2 * (16 * wm * kLdT) * sizeof(double); }
 
+template <int WN, int EPI, bool PAIR>
+static cudaError_t launch_ht_p(int device, int grid, cudaStream_t st, const HtParams& a) {
+  static std::atomic<unsigned long long> attr_done{0};   // per instantiation, one bit per device
+  cudaError_t e = ensure_dyn_smem(k_half_transform<WN, EPI, PAIR>, ht_smem_bytes(WN), device, attr_done);
+  if (e != cudaSuccess) return e;
+  k_half_transform<WN, EPI, PAIR><<<grid, kThreads, ht_smem_bytes(WN), st>>>(a);
+  return cudaSuccess;
+}
+
+// the paired variant exists for the k-tiled epilogues (JK path, density-matrix form); row-major X (AO2MO) is unpaired
 template <int WN, int EPI>
 static cudaError_t launch_ht(int device, int grid, cudaStream_t st, const HtParams& a) {
-  static std::atomic<unsigned long long> attr_done{0};   // per instantiation, one bit per device
-  cudaError_t e = ensure_dyn_smem(k_half_transform<WN, EPI>, ht_smem_bytes(WN), device, attr_done);
-  if (e != cudaSuccess) return e;
-  k_half_transform<WN, EPI><<<grid, kThreads, ht_smem_bytes(WN), st>>>(a);
-  return cudaSuccess;
+  if (EPI != 2 && a.pair_last) return launch_ht_p<WN, EPI, EPI != 2>(device, grid, st, a);
+  return launch_ht_p<WN, EPI, false>(device, grid, st, a);
 }
 
 template <int EPI>
@@ -776,6 +826,9 @@ static cudaError_t dispatch_ht_wn(int device, int wn, int grid, cudaStream_t st,
     default: return cudaErrorInvalidValue;
   }
 }
+
+// the last 64-row block holds at most 32 rows and the re-tiled copy exists: two aux rows share its tiles
+static int ht_pair_last(const dfjk_ctx* h) { return h->Bt != nullptr && (h->nao & 63) >= 1 && (h->nao & 63) <= 32 ? 1 : 0; }
 
 // epi: 0 = k-tiled X, 1 = k-tiled X + rho partials, 2 = row-major X
 static cudaError_t dispatch_ht(int device, int wn, int epi, int grid, cudaStream_t st, const HtParams& a) {
@@ -824,9 +877,9 @@ int launch_half_transform_rowmajor(dfjk_ctx* h, const SetInfo& si, int p_first, 
   const int ntn = cdiv(n8, 2 * kHtMaxWN), wn = cdiv(n8, 2 * ntn);
   const int ntm_ht = cdiv(h->nao, 64);
   HtParams a;
-  a.Bt = h->Bt; a.bt_pstride = h->bt_pstride; a.Bp = h->B; a.npair = h->npair; a.nao = h->nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = si.nocc_pad;
+  a.Bt = h->Bt; a.bt_pstride = h->bt_pstride; a.pair_last = ht_pair_last(h); a.Bp = h->B; a.npair = h->npair; a.nao = h->nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = si.nocc_pad;
   a.X = X; a.nch = 0; a.mu_pad = 0; a.p_first = p_first; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
-  a.rho_ht = nullptr; a.nset = 0; a.ldx = ldx; a.xrows = h->nao; a.sgnbits = nullptr;
+  a.rho_ht = nullptr; a.nset = 0; a.ldx = ldx; a.xrows = h->nao; a.sgnbits = nullptr; a.pair_last = 0;
   a.col0[0] = 0;
   const long long ht_tiles = (long long)nb * ntm_ht * ntn;
   const int ht_grid = (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid);
@@ -962,7 +1015,7 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
     const int nb = (int)(naux - p0 < nblk ? naux - p0 : nblk);
     prof_mark(h, DFJK_PHASE_HALF_TRANSFORM, st);
     HtParams a;
-    a.Bt = h->Bt; a.bt_pstride = h->bt_pstride; a.Bp = h->B; a.npair = h->npair; a.nao = nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = ldx;
+    a.Bt = h->Bt; a.bt_pstride = h->bt_pstride; a.pair_last = ht_pair_last(h); a.Bp = h->B; a.npair = h->npair; a.nao = nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = ldx;
     a.X = h->X; a.nch = nch; a.mu_pad = h->mu_pad; a.p_first = p0; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
     a.rho_ht = h->rho_ht; a.nset = si.nset; a.ldx = 0; a.xrows = 0; a.sgnbits = h->sgnbits;
     for (int s = 0; s <= si.nset; s++) a.col0[s] = si.col0[s];
@@ -1100,7 +1153,7 @@ int launch_k_path_dm(dfjk_ctx* h, int nset, const double* D, double* K_out, cuda
       const int nb = (int)(naux - p0 < nblk ? naux - p0 : nblk);
       prof_mark(h, DFJK_PHASE_HALF_TRANSFORM, st);
       HtParams a;
-      a.Bt = h->Bt; a.bt_pstride = h->bt_pstride; a.Bp = h->B; a.npair = h->npair; a.nao = nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = ldx;
+      a.Bt = h->Bt; a.bt_pstride = h->bt_pstride; a.pair_last = ht_pair_last(h); a.Bp = h->B; a.npair = h->npair; a.nao = nao; a.Ct = h->Ct; a.ct_rows = h->ct_rows; a.nocc_pad = ldx;
       a.X = X1; a.nch = nch; a.mu_pad = h->mu_pad; a.p_first = p0; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
       a.rho_ht = nullptr; a.nset = 0; a.ldx = 0; a.xrows = 0; a.col0[0] = 0; a.sgnbits = nullptr;
       const long long ht_tiles = (long long)nb * ntm_ht * ntn;
