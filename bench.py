@@ -499,6 +499,12 @@ def main():
                 small[sname]["tiled_kernels_launches_per_call"] = ht_.last_launch_count
                 small[sname]["tiled_kernels_ms_direct"] = max_over_ranks(timed(t_fn, 100))
                 ht_.close()
+                # the allocation-free entry point (same kernel on the library's static scratch; one 8-byte memset more)
+                n_fn = lambda: dfjk.small_jk_static(sB, sinp.nao, sinp.nocc, sC, socc, out_j=sJ, out_k=sK, stream=stream)
+                for _ in range(3):
+                    n_fn()
+                torch.cuda.synchronize()
+                small[sname]["static_scratch_ms_direct"] = max_over_ranks(timed(n_fn, 100))
     if not lead:
         h.close()
         ranks.close()

@@ -157,6 +157,35 @@ int dfjk_get_jk_host(dfjk_handle h, int nset, const int* nocc, const double* C, 
 int dfjk_get_jk_dm(dfjk_handle h, int nset, const double* D, double* J_out, double* K_out, dfjk_stream stream);
 
 /*
+ * dfjk_small_jk_static -- dfjk_get_jk for embedding-sized calls WITHOUT a handle and without
+ * any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, serving loops, harnesses
+ * that forbid it).  One cooperative launch of the single-launch kernel (steps a1-a9, Eq. 14-17);
+ * its scratch (private J/K partials of every CTA and two barrier counters) is a file-scope device array of
+ * DFJK_STATIC_SCRATCH_BYTES (+ 256) bytes that every GPU loading the library holds until the process exits.
+ *   naux, nao  >= 1;   B_packed  DEVICE, naux x nao(nao+1)/2, packed lower triangle as in dfjk_create (borrowed).
+ *   nset, nocc, C, occ, J_out, K_out, stream: as in dfjk_get_jk (nocc HOST; C, occ, J_out, K_out DEVICE).
+ * Maximum sizes (beyond them: DFJK_ERR_INVALID_ARG, the text in dfjk_small_jk_static_last_error):
+ *   nao <= 96, nset <= DFJK_STATIC_MAX_NSET, 1 <= sum(nocc), nao * sum(nocc) <= 4608,
+ *   naux * nao^2 * (sum(nocc) + nset) <= 2^26.
+ * The number of CTAs is that of dfjk_get_jk's single-launch path, capped so that the partials
+ * (CTAs * nset * (nao^2 + nao(nao+1)/2) doubles) fit the array; with fewer CTAs the sums run in another order, so
+ * results agree with dfjk_get_jk to rounding (and bitwise when the cap does not bind), and are deterministic.
+ * The call enqueues one 8-byte memset (the barrier counters must start at zero; the array keeps the last call's
+ * contents, the partials are overwritten before they are read) and one kernel on `stream`; it calls no cudaMalloc,
+ * cudaFree or allocating library routine and never synchronises the host.  The first call on a device looks up the
+ * array's device address (cudaGetSymbolAddress, once per device, with that device current).
+ * EVERY call on a device shares the one array: calls that overlap on the GPU (two streams, two host threads, two
+ * graphs in flight) race on it -- serialise them.  Calls on one stream are ordered and safe.
+ */
+#define DFJK_STATIC_SCRATCH_BYTES 8388608
+#define DFJK_STATIC_MAX_NSET 8
+int dfjk_small_jk_static(int naux, int nao, const double* B_packed, int nset, const int* nocc, const double* C,
+                         const double* occ, double* J_out, double* K_out, dfjk_stream stream);
+
+/* Text of the last failure of dfjk_small_jk_static on the calling thread ("" if none). */
+const char* dfjk_small_jk_static_last_error(void);
+
+/*
  * dfjk_ao2mo -- the AO2MO kernel of section 2.D.ii (Eq. 18-21) on the same
  * resident Cholesky vectors, with the index pattern fixed by Eq. 12, g = (m1 m2|m3 m4) = b b:
  *      X^P[e2][p1]   = sum_{e1} b^P[e1][e2] M[e1][p1]                          Eq. 18

@@ -3,6 +3,6 @@
 Thin Python binding over the C ABI in include/dfjk.h: argument marshalling only, every step of the
 path runs in the CUDA kernels of csrc/.  PyTorch is used for device memory and streams.
 """
-from .api import DFJK, DFJKError, get_jk, lib_path, load_library, selftest_dmma
+from .api import DFJK, DFJKError, get_jk, lib_path, load_library, selftest_dmma, small_jk_static
 
-__all__ = ["DFJK", "DFJKError", "get_jk", "lib_path", "load_library", "selftest_dmma"]
+__all__ = ["DFJK", "DFJKError", "get_jk", "lib_path", "load_library", "selftest_dmma", "small_jk_static"]

@@ -14,7 +14,8 @@ _lib = None
 
 EXPORTS = ["dfjk_create", "dfjk_get_jk", "dfjk_get_jk_host", "dfjk_destroy", "dfjk_strerror",
            "dfjk_last_error", "dfjk_workspace_bytes", "dfjk_get_plan", "dfjk_last_launch_count",
-           "dfjk_selftest_dmma", "dfjk_set_profiling", "dfjk_get_profile", "dfjk_ao2mo", "dfjk_get_jk_dm", "dfjk_last_ao2mo_route"]
+           "dfjk_selftest_dmma", "dfjk_set_profiling", "dfjk_get_profile", "dfjk_ao2mo", "dfjk_get_jk_dm", "dfjk_last_ao2mo_route",
+           "dfjk_small_jk_static", "dfjk_small_jk_static_last_error"]
 
 PHASES = ["prep", "j1", "j2", "j_epilogue", "half_transform", "syrk", "k_epilogue"]
 
@@ -77,6 +78,10 @@ def load_library():
     lib.dfjk_get_profile.restype = ct.c_int
     lib.dfjk_selftest_dmma.argtypes = []
     lib.dfjk_selftest_dmma.restype = ct.c_int
+    lib.dfjk_small_jk_static.argtypes = [ct.c_int, ct.c_int, dp, ct.c_int, ip, dp, dp, dp, dp, vp]
+    lib.dfjk_small_jk_static.restype = ct.c_int
+    lib.dfjk_small_jk_static_last_error.argtypes = []
+    lib.dfjk_small_jk_static_last_error.restype = ct.c_char_p
     _lib = lib
     return lib
 
@@ -94,6 +99,36 @@ def _check(lib, code: int, handle=None):
 def selftest_dmma() -> None:
     lib = load_library()
     _check(lib, lib.dfjk_selftest_dmma())
+
+
+def small_jk_static(B_packed, nao: int, nocc: List[int], C, occ, out_j=None, out_k=None, stream=None) -> None:
+    """dfjk_small_jk_static: the single-launch get_jk on the library's static scratch; no handle and no
+    allocation, here or in the library.  C/occ concatenated on the device as for DFJK.get_jk_raw; out_j/out_k
+    are caller-allocated (nset, nao, nao) CUDA float64 tensors (None skips that output).  Calls that overlap
+    on the GPU race on the shared scratch."""
+    import torch
+    lib = load_library()
+    npair = nao * (nao + 1) // 2
+    if not (B_packed.is_cuda and B_packed.dtype == torch.float64 and B_packed.is_contiguous()
+            and B_packed.dim() == 2 and B_packed.shape[1] == npair):
+        raise ValueError(f"B_packed must be a contiguous CUDA float64 tensor of shape (naux, {npair})")
+    nset = len(nocc)
+    for t in (out_j, out_k):
+        if t is not None and not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+                                  and tuple(t.shape) == (nset, nao, nao)):
+            raise ValueError(f"outputs must be contiguous CUDA float64 tensors of shape {(nset, nao, nao)}")
+    with torch.cuda.device(B_packed.device):
+        st = stream if stream is not None else torch.cuda.current_stream()
+        arr = (ct.c_int * max(nset, 1))(*nocc)
+        code = lib.dfjk_small_jk_static(int(B_packed.shape[0]), int(nao), ct.c_void_p(B_packed.data_ptr()), nset, arr,
+                                        ct.c_void_p(C.data_ptr()), ct.c_void_p(occ.data_ptr()),
+                                        ct.c_void_p(out_j.data_ptr() if out_j is not None else 0),
+                                        ct.c_void_p(out_k.data_ptr() if out_k is not None else 0),
+                                        ct.c_void_p(st.cuda_stream))
+    if code != 0:
+        msg = lib.dfjk_strerror(code).decode()
+        extra = lib.dfjk_small_jk_static_last_error().decode()
+        raise DFJKError(code, f"{msg} ({extra})" if extra else msg)
 
 
 class DFJK:

@@ -12,6 +12,9 @@
 // Plain DFMA on purpose: this regime is latency-bound, not throughput-bound (tiny config: 13 MFLOP).
 // Chosen by dfjk_get_jk when nao <= 96, nao * sum(nocc) <= 4608 and naux * nao^2 * (sum(nocc) + nset)
 // <= 2^26 (option no_small_path disables it); everything larger takes the tensor-pipe kernels.
+#include <cstdarg>
+#include <cstdio>
+
 #include "common.cuh"
 #include "ctx.h"
 
@@ -264,3 +267,131 @@ int launch_small_fused(dfjk_ctx* h, const SetInfo& si, int ctas, const double* C
 }
 
 }  // namespace dfjk
+
+// ---------------------------------------------------------------------------------------------------------
+// dfjk_small_jk_static (include/dfjk.h): the same kernel for callers that cannot allocate (CUDA graph capture,
+// serving loops, harnesses that forbid cudaMalloc).  No handle: the private J/K partials and the two barrier
+// counters live in one file-scope device array that every GPU loading the library holds until exit.
+// ---------------------------------------------------------------------------------------------------------
+namespace {
+
+constexpr size_t kStaticDoubles = (size_t)1 << 20;   // 8 MiB of partials (DFJK_STATIC_SCRATCH_BYTES)
+constexpr size_t kStaticHead = 32;                   // 256 B in front: [0], [1] of the first 8 bytes are the tickets
+static_assert(kStaticDoubles * sizeof(double) == DFJK_STATIC_SCRATCH_BYTES, "header and kernel disagree");
+static __device__ __align__(256) double g_static_scratch[kStaticHead + kStaticDoubles];
+
+// In host code g_static_scratch is only a stand-in for the symbol: the device address is asked for once per
+// device, with that device current, and kept here together with what else the launch needs to know about it.
+struct StaticDev {
+  std::atomic<int> state{0};   // 0 = not set up, 1 = being set up, 2 = ready, 3 = failed
+  double* scratch = nullptr;
+  int num_sms = 0, cc_major = 0;
+  cudaError_t err = cudaSuccess;
+};
+constexpr int kStaticMaxDev = 64;
+StaticDev g_static_dev[kStaticMaxDev];
+thread_local char g_static_err[256] = "";
+
+int static_fail(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_static_err, sizeof(g_static_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+// set-up of the CURRENT device (dev); returns its record or nullptr
+StaticDev* static_setup(int dev) {
+  StaticDev& d = g_static_dev[dev];
+  int s = d.state.load(std::memory_order_acquire);
+  if (s == 2) return &d;
+  int expect = 0;
+  if (s == 0 && d.state.compare_exchange_strong(expect, 1, std::memory_order_acq_rel)) {
+    double* p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress((void**)&p, g_static_scratch);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&d.num_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&d.cc_major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e == cudaSuccess && p == nullptr) e = cudaErrorInvalidSymbol;
+    d.scratch = p;
+    d.err = e;
+    if (e != cudaSuccess) cudaGetLastError();
+    d.state.store(e == cudaSuccess ? 2 : 3, std::memory_order_release);
+  }
+  while ((s = d.state.load(std::memory_order_acquire)) == 1) {}
+  return s == 2 ? &d : nullptr;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* dfjk_small_jk_static_last_error(void) { return g_static_err; }
+
+int dfjk_small_jk_static(int naux, int nao, const double* B_packed, int nset, const int* nocc, const double* C,
+                         const double* occ, double* J_out, double* K_out, dfjk_stream stream) {
+  using namespace dfjk;
+  g_static_err[0] = 0;
+  if (naux < 1 || nao < 1 || nset < 1 || !nocc || !B_packed)
+    return static_fail(DFJK_ERR_INVALID_ARG, "naux, nao, nset must be >= 1 and B_packed, nocc non-NULL");
+  if (nao > kSmMaxNao) return static_fail(DFJK_ERR_INVALID_ARG, "nao = %d is beyond the maximum %d of this entry point", nao, kSmMaxNao);
+  if (nset > DFJK_STATIC_MAX_NSET)
+    return static_fail(DFJK_ERR_INVALID_ARG, "nset = %d is beyond the maximum %d of this entry point", nset, DFJK_STATIC_MAX_NSET);
+  SetInfo si{};
+  si.nset = nset;
+  long long coff = 0;
+  int ntot = 0, col = 0;
+  for (int s = 0; s < nset; s++) {
+    if (nocc[s] < 0 || nocc[s] > nao) return static_fail(DFJK_ERR_INVALID_ARG, "nocc[%d] = %d is outside [0, nao]", s, nocc[s]);
+    si.col0[s] = col; si.nocc[s] = nocc[s]; si.coff[s] = coff; si.ooff[s] = ntot;
+    col += round_up(nocc[s], 8);
+    coff += (long long)nao * nocc[s];
+    ntot += nocc[s];
+  }
+  si.col0[nset] = col;
+  si.nocc_pad = col;
+  if (ntot < 1 || !C || !occ) return static_fail(DFJK_ERR_INVALID_ARG, "needs at least one occupied column and C, occ non-NULL");
+  if ((long long)nao * ntot > kSmMaxElems)
+    return static_fail(DFJK_ERR_INVALID_ARG, "nao * sum(nocc) = %lld is beyond the maximum %d of this entry point", (long long)nao * ntot, kSmMaxElems);
+  if ((double)naux * nao * nao * (ntot + nset) > kSmMaxWork)
+    return static_fail(DFJK_ERR_INVALID_ARG, "naux * nao^2 * (sum(nocc) + nset) is beyond the maximum 2^26 of this entry point");
+  if (!J_out && !K_out) return DFJK_OK;
+
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess || dev < 0 || dev >= kStaticMaxDev) { cudaGetLastError(); return static_fail(DFJK_ERR_CUDA, "cudaGetDevice: %s", cudaGetErrorString(e)); }
+  StaticDev* d = static_setup(dev);
+  if (!d) return static_fail(DFJK_ERR_CUDA, "cudaGetSymbolAddress of the static scratch on device %d: %s", dev, cudaGetErrorString(g_static_dev[dev].err));
+  if (d->cc_major != 10) return static_fail(DFJK_ERR_UNSUPPORTED_ARCH, "device %d is sm_%d0, the library is built for sm_100", dev, d->cc_major);
+
+  const size_t npair = (size_t)nao * (nao + 1) / 2, n2 = (size_t)nao * nao;
+  const size_t per_cta = (size_t)nset * (n2 + npair);           // doubles of private partials per CTA
+  if (per_cta > kStaticDoubles) return static_fail(DFJK_ERR_INVALID_ARG, "one CTA's partials exceed the static scratch");
+  const size_t smem = small_smem_bytes(nao, ntot);
+  if ((e = small_attr(dev)) != cudaSuccess) { cudaGetLastError(); return static_fail(DFJK_ERR_CUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
+  int resident = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, k_small_fused, kSmThreads, smem);
+  if (e != cudaSuccess || resident < 1) { cudaGetLastError(); return static_fail(DFJK_ERR_CUDA, "the kernel does not fit an SM with %zu bytes of shared memory", smem); }
+  // as dfjk_get_jk sizes it (equal rounds over at most two resident CTAs per SM), then capped by the static scratch
+  const int slots = d->num_sms * (resident < 2 ? resident : 2);
+  int ctas = cdiv(naux, cdiv(naux, slots));
+  const size_t fit = kStaticDoubles / per_cta;
+  if ((size_t)ctas > fit) ctas = (int)fit;
+
+  cudaStream_t st = (cudaStream_t)stream;
+  unsigned int* ticket = reinterpret_cast<unsigned int*>(d->scratch);
+  double* part = d->scratch + kStaticHead;
+  // the array keeps the last call's contents: the barrier counters must start at zero (a call that failed half way
+  // would leave them set); the partials are overwritten before they are read (every CTA owns >= 1 aux row)
+  if ((e = cudaMemsetAsync(ticket, 0, 2 * sizeof(unsigned int), st)) != cudaSuccess) { cudaGetLastError(); return static_fail(DFJK_ERR_CUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e)); }
+  SmallParams p{B_packed, npair, naux, nao, C, occ, J_out, K_out, part, part + (size_t)ctas * nset * n2, ticket, ntot};
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(ctas); cfg.blockDim = dim3(kSmThreads); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeCooperative;
+  attr[0].val.cooperative = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  if ((e = cudaLaunchKernelEx(&cfg, k_small_fused, si, p)) != cudaSuccess) { cudaGetLastError(); return static_fail(DFJK_ERR_CUDA, "cooperative launch of %d CTAs: %s", ctas, cudaGetErrorString(e)); }
+  return DFJK_OK;
+}
+
+}  // extern "C"

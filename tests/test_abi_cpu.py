@@ -43,6 +43,18 @@ def test_calls_that_need_no_device():
     assert lib.dfjk_create(4, 4, None, None, None) == 1               # no out pointer
     arr = (ct.c_int * 1)(1)
     assert lib.dfjk_get_jk(None, 1, arr, None, None, None, None, None) == 1
+    # the allocation-free entry point checks its maximum sizes before it touches the device
+    p = ct.c_void_p(64)                                               # never dereferenced on the host
+    assert lib.dfjk_small_jk_static(10, 97, p, 1, arr, p, p, p, p, None) == 1
+    assert b"maximum 96" in lib.dfjk_small_jk_static_last_error()
+    assert lib.dfjk_small_jk_static(10, 48, p, 9, (ct.c_int * 9)(*[1] * 9), p, p, p, p, None) == 1
+    assert b"nset = 9" in lib.dfjk_small_jk_static_last_error()
+    assert lib.dfjk_small_jk_static(10, 96, p, 1, (ct.c_int * 1)(49), p, p, p, p, None) == 1
+    assert b"maximum 4608" in lib.dfjk_small_jk_static_last_error()
+    assert lib.dfjk_small_jk_static(10, 48, p, 1, arr, p, p, None, None, None) == 0   # nothing asked for
+    assert lib.dfjk_small_jk_static_last_error() == b""
+    hdr = open(os.path.join(ROOT, "include", "dfjk.h")).read()
+    assert "#define DFJK_STATIC_SCRATCH_BYTES 8388608" in hdr and "#define DFJK_STATIC_MAX_NSET 8" in hdr
 
 
 def test_product_does_not_import_the_oracle():
