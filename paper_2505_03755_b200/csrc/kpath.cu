@@ -66,16 +66,17 @@ struct HtParams {
   // (tile (mb, c), c < 4 (mb + 1), at image 2 mb (mb + 1) + c), so that the A operand of every chunk
   // is one bulk copy (a stored or diagonal tile) or four (the transpose: 16 rows of four images)
   const double* Bt; size_t bt_pstride;
-  // with Bt and 1 <= nao % 64 <= 32 the last 64-row block of an aux row is half empty: the last blocks of TWO aux
-  // rows then share one tile (rows 0-31: aux row pl, rows 32-63: aux row pl + 1), scheduled after the full tiles
+  // with Bt and 1 <= nao % 64 <= 48 the last 64-row block of an aux row holds v = pair_last < 4 pieces of 16 rows:
+  // the nb * v pieces of the last blocks of consecutive aux rows are then packed four to a tile (piece k of the
+  // block range is rows 16 (k % v).. of aux row k / v), scheduled after the full tiles.  0 = off
   int pair_last;
 };
 
-// tile index -> (aux row, 64-row block, N tile); paired: the tile holds the last blocks of aux rows pl and pl + 1
+// tile index -> (aux row, 64-row block, N tile); paired: the tile holds the pieces pl .. pl + 3 of the last blocks
 struct HtTile { int pl, mb, nt; bool paired; };
 template <bool PAIR>
 __device__ __forceinline__ int ht_num_tiles(const HtParams& q) {
-  return PAIR ? q.nb * (q.ntm - 1) * q.ntn + ((q.nb + 1) >> 1) * q.ntn : q.nb * q.ntm * q.ntn;
+  return PAIR ? q.nb * (q.ntm - 1) * q.ntn + ((q.nb * q.pair_last + 3) >> 2) * q.ntn : q.nb * q.ntm * q.ntn;
 }
 template <bool PAIR>
 __device__ __forceinline__ HtTile ht_tile(const HtParams& q, int tile) {
@@ -94,7 +95,7 @@ __device__ __forceinline__ HtTile ht_tile(const HtParams& q, int tile) {
     t.mb = rem / q.ntn; t.nt = rem - t.mb * q.ntn; t.paired = false;
   } else {
     const int t2 = tile - nfull;
-    t.pl = 2 * (t2 / q.ntn); t.nt = t2 % q.ntn; t.mb = q.ntm - 1; t.paired = true;
+    t.pl = 4 * (t2 / q.ntn); t.nt = t2 % q.ntn; t.mb = q.ntm - 1; t.paired = true;
   }
   return t;
 }
@@ -114,7 +115,10 @@ k_half_transform(const __grid_constant__ HtParams q) {
   double* sB = smem + kS * kHtATile;          // kS x NT*kHtLd
   __shared__ __align__(8) unsigned long long bars[2 * kS];
   const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kS]);
-  const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
+  const int tid = threadIdx.x, l = tid & 31;
+  // PAIR: the warp index read from lane 0, so that the compiler sees the per-warp row assignment (and the branch
+  // that skips a piece past the last aux row) as warp-uniform
+  const int w = PAIR ? __shfl_sync(0xffffffffu, tid >> 5, 0) : tid >> 5;
   const int nao = q.nao;
   const int nk4 = (nao + 3) >> 2;                  // k4 steps that carry data
   const int nchunks = (nk4 + 3) >> 2;
@@ -142,19 +146,30 @@ k_half_transform(const __grid_constant__ HtParams q) {
       for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const HtTile ht = ht_tile<PAIR>(q, tile);
         const int pl = ht.pl, mb = ht.mb, n0 = ht.nt * NT;
-        const double* BtP = q.Bt + (size_t)(q.p_first + pl) * q.bt_pstride;
-        const bool second = (PAIR && ht.paired) && pl + 1 < q.nb;
+        const double* BtP = q.Bt + (size_t)(q.p_first + ((PAIR && ht.paired) ? 0 : pl)) * q.bt_pstride;
+        // packed tile: number of pieces that exist, aux row and piece-in-block of the first one
+        int npc = 0, pk0 = 0, ik0 = 0;
+        if (PAIR && ht.paired) {
+          npc = min(4, q.nb * q.pair_last - pl);
+          pk0 = pl / q.pair_last;
+          ik0 = pl - pk0 * q.pair_last;
+        }
         for (int c = 0; c < nchunks; c++, g++) {
           const int stage = g % kS;
           const uint32_t fullb = full0 + 8 * stage;
           mbar_wait(empty0 + 8 * stage, ((g / kS) & 1) ^ 1);
-          mbar_arrive_expect_tx(fullb, kBBytes + ((PAIR && ht.paired) && !second ? kImgBytes / 2 : kImgBytes));
+          mbar_arrive_expect_tx(fullb, kBBytes + ((PAIR && ht.paired) ? (uint32_t)npc * kPieceBytes : kImgBytes));
           bulk_g2s(sB_u32 + (uint32_t)stage * kBBytes, q.Ct + ((size_t)c * q.ct_rows + n0) * kHtLd, kBBytes, fullb);
           const uint32_t a_base = sA_u32 + (uint32_t)(stage * kHtATile) * 8u;
-          if ((PAIR && ht.paired)) {                           // rows 0-31 of the last block's image of two aux rows (always stored / diagonal)
+          if ((PAIR && ht.paired)) {                           // 16-row pieces of the last block's image (always stored / diagonal)
             const size_t img = (size_t)(2 * mb * (mb + 1) + c) * (64 * kHtLd);
-            bulk_g2s(a_base, BtP + img, kImgBytes / 2, fullb);
-            if (second) bulk_g2s(a_base + kImgBytes / 2, BtP + q.bt_pstride + img, kImgBytes / 2, fullb);
+            // consecutive pieces of one aux row are contiguous on both sides: one copy per aux row in the tile
+            const double* src = BtP + (size_t)pk0 * q.bt_pstride + img;
+            for (int k = 0, ik = ik0; k < npc; ik = 0, src += q.bt_pstride) {
+              const int run = min(q.pair_last - ik, npc - k);
+              bulk_g2s(a_base + (uint32_t)k * kPieceBytes, src + (size_t)ik * 16 * kHtLd, (uint32_t)run * kPieceBytes, fullb);
+              k += run;
+            }
           } else if (c < 4 * (mb + 1)) {             // stored or diagonal tile: its image as it is
             bulk_g2s(a_base, BtP + (size_t)(2 * mb * (mb + 1) + c) * (64 * kHtLd), kImgBytes, fullb);
           } else {                                   // transpose: rows 16 (c % 4) .. + 15 of the images (c / 4, 4 mb + qq)
@@ -232,9 +247,6 @@ k_half_transform(const __grid_constant__ HtParams q) {
     const HtTile ht = ht_tile<PAIR>(q, tile);
     const int mb = ht.mb, nt = ht.nt, rem = PAIR ? mb * q.ntn + nt : tile - ht.pl * tiles_per_p;
     const int m0 = mb * 64, n0 = nt * NT;
-    // rows of this warp: 16 wm.. of aux row pl; in a paired tile rows 16 (wm & 1).. of aux row pl + (wm >> 1)
-    const int pl = (PAIR && ht.paired) ? ht.pl + (wm >> 1) : ht.pl;
-    const int mrow0 = (PAIR && ht.paired) ? m0 + (wm & 1) * 16 : m0 + wm * 16;
 #pragma unroll
     for (int t = 0; t < 2; t++)
 #pragma unroll
@@ -287,6 +299,10 @@ k_half_transform(const __grid_constant__ HtParams q) {
       if (l == 0) mbar_arrive(empty0 + 8 * stage);
     }
     // epilogue: lane owns X[mu][n], X[mu][n+1] with mu = mrow0 + 8t + r, n = n0 + 8 (wn WN + u) + 2j
+    // rows of this warp: 16 wm.. of aux row pl; in a paired tile piece ht.pl + wm = rows 16 ip.. of aux row pl
+    const int pl = (PAIR && ht.paired) ? (ht.pl + wm) / q.pair_last : ht.pl;
+    const int ip = (PAIR && ht.paired) ? ht.pl + wm - pl * q.pair_last : wm;
+    const int mrow0 = m0 + ip * 16;
     if (PAIR && pl >= q.nb) continue;             // second half of a paired tile past the last aux row
     if (EPI == 2) {
       double* Xp = q.X + (size_t)pl * q.xrows * q.ldx;
@@ -321,10 +337,11 @@ k_half_transform(const __grid_constant__ HtParams q) {
       // 8-column tile belongs to one set; a warp's tiles of one set are contiguous).  One slot of
       // nset doubles per (aux row, tile, warp); k_rho_reduce sums the slots in fixed order.
       const int nslots = tiles_per_p * 8;
-      double* slot = q.rho_ht + ((size_t)(q.p_first + pl) * nslots + (size_t)rem * 8 + w) * q.nset;
+      double* slot = q.rho_ht + ((size_t)(q.p_first + pl) * nslots + (size_t)rem * 8 + (ip + 4 * wn)) * q.nset;
       for (int s = l; s < q.nset; s += 32) slot[s] = 0.0;
-      if ((PAIR && ht.paired))                                     // the slots of the warps that serve the other aux row stay empty
-        for (int s = l; s < q.nset; s += 32) (slot + ((w ^ 2) - w) * q.nset)[s] = 0.0;
+      if ((PAIR && ht.paired) && ip == 0)                          // the slots of the pieces the last block does not have stay empty
+        for (int i2 = q.pair_last; i2 < 4; i2++)
+          for (int s = l; s < q.nset; s += 32) (slot + i2 * q.nset)[s] = 0.0;
       int myset = -1;
       if (l < WN) {
         const int col = n0 + 8 * (wn * WN + l);
@@ -828,7 +845,7 @@ static cudaError_t dispatch_ht_wn(int device, int wn, int grid, cudaStream_t st,
 }
 
 // the last 64-row block holds at most 32 rows and the re-tiled copy exists: two aux rows share its tiles
-static int ht_pair_last(const dfjk_ctx* h) { return h->Bt != nullptr && (h->nao & 63) >= 1 && (h->nao & 63) <= 32 ? 1 : 0; }
+static int ht_pair_last(const dfjk_ctx* h) { return h->Bt != nullptr && (h->nao & 63) >= 1 && (h->nao & 63) <= 48 ? ((h->nao & 63) + 15) >> 4 : 0; }
 
 // epi: 0 = k-tiled X, 1 = k-tiled X + rho partials, 2 = row-major X
 static cudaError_t dispatch_ht(int device, int wn, int epi, int grid, cudaStream_t st, const HtParams& a) {
