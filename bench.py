@@ -37,8 +37,8 @@ FP64_DMMA_PEAK_TFLOPS = 37.1
 FP64_CUBLAS_TFLOPS = 35.47
 HBM_READ_STREAM_GBS = 7430.0
 # ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum of k_half_transform<19,1> at `large`:
-# 8.95 + 3.26 GB per 1122-aux-row launch (profiles/r02_ncu_large.md; the re-tiled Bt is 1.35x the packed bytes)
-HT_DRAM_BYTES_PER_AUX_ROW_LARGE = 12.21e9 / 1122
+# 9.41 + 3.26 GB per 1122-aux-row launch (profiles/r02_ncu_large.md; the re-tiled Bt is 1.35x the packed bytes)
+HT_DRAM_BYTES_PER_AUX_ROW_LARGE = 12.66e9 / 1122
 
 
 def measured_peaks():

@@ -115,7 +115,7 @@ __host__ __device__ constexpr int j1t_stages(int ns) { return ns <= 1 ? 6 : 5; }
 template <int NS>
 __global__ void __launch_bounds__(kJ1tThreads, 1)
 k_j1_tma(const double* __restrict__ B, size_t npair, int naux, const double* __restrict__ Dw,
-         double* __restrict__ part, int naux_pad) {
+         double* __restrict__ part, int naux_pad, int rows_cta) {
   constexpr int STAGES = j1t_stages(NS);
   constexpr int kStageDoubles = (8 + NS) * kJ1tSC;
   extern __shared__ __align__(128) double smem[];
@@ -123,11 +123,11 @@ k_j1_tma(const double* __restrict__ B, size_t npair, int naux, const double* __r
   __shared__ double red[8][8][NS];
   const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[STAGES]);
   const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
-  const int p0 = blockIdx.y * kJ1Rows;
+  const int p0 = blockIdx.y * rows_cta;          // rows_cta = 8, 16, 32 or 64 aux rows per CTA (launch_j_passes)
   const size_t kbeg = (size_t)blockIdx.x * kJ1Chunk;
   const size_t kend = kbeg + kJ1Chunk < npair ? kbeg + kJ1Chunk : npair;
   const int nchunk = (int)((kend - kbeg + kJ1tSC - 1) / kJ1tSC);
-  const int ngroups = min(8, (naux - p0 + 7) / 8);
+  const int ngroups = min(rows_cta >> 3, (naux - p0 + 7) / 8);
   const int nstage = ngroups * nchunk;
   if (tid == 0) {
     for (int s = 0; s < STAGES; s++) {
@@ -344,20 +344,20 @@ static cudaError_t launch_j1_mma(int device, dim3 grid, cudaStream_t st, const d
 
 template <int NS>
 static cudaError_t launch_j1_tma(int device, dim3 grid, cudaStream_t st, const double* B, size_t npair, int naux,
-                                 const double* Dw, double* part, int naux_pad) {
+                                 const double* Dw, double* part, int naux_pad, int rows_cta) {
   constexpr size_t smem = (size_t)j1t_stages(NS) * (8 + NS) * kJ1tSC * sizeof(double);
   static std::atomic<unsigned long long> attr_done{0};
   cudaError_t e = ensure_dyn_smem(k_j1_tma<NS>, smem, device, attr_done);
   if (e != cudaSuccess) return e;
-  k_j1_tma<NS><<<grid, kJ1tThreads, smem, st>>>(B, npair, naux, Dw, part, naux_pad);
+  k_j1_tma<NS><<<grid, kJ1tThreads, smem, st>>>(B, npair, naux, Dw, part, naux_pad, rows_cta);
   return cudaSuccess;
 }
 
 static cudaError_t dispatch_j1_tma(int device, int ns, dim3 grid, cudaStream_t st, const double* B, size_t npair,
-                                   int naux, const double* Dw, double* part, int naux_pad) {
+                                   int naux, const double* Dw, double* part, int naux_pad, int rows_cta) {
   switch (ns) {
 #define DFJK_J1T_CASE(N) \
-  case N: return launch_j1_tma<N>(device, grid, st, B, npair, naux, Dw, part, naux_pad);
+  case N: return launch_j1_tma<N>(device, grid, st, B, npair, naux, Dw, part, naux_pad, rows_cta);
     DFJK_J1T_CASE(1) DFJK_J1T_CASE(2)          // three and more sets take k_j1_mma
 #undef DFJK_J1T_CASE
     default: return cudaErrorInvalidValue;
@@ -601,7 +601,18 @@ int launch_j_passes(dfjk_ctx* h, const SetInfo& si, double* J_out, bool rho_read
         if (launch_j1_mma(h->device, g1, st, h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad) != cudaSuccess)
           return -1;
       } else if (vec) {
-        if (dispatch_j1_tma(h->device, ns, g1, st, h->B, npair, naux, h->Dw + (size_t)s0 * npair, h->rho_part, naux_pad) != cudaSuccess)
+        // aux rows per CTA: 64 on long streams; short ones (small: 48 CTAs of 64 rows, medium: 2.6 waves) take the
+        // split that needs the least time in whole waves of one CTA per SM, a CTA costing its rows plus a fixed
+        // set-up (ring fill; about one row's worth)
+        int rows_cta = kJ1Rows;
+        double best = 0.0;
+        for (int rc = kJ1Rows; rc >= 8; rc >>= 1) {
+          const long long ctas = (long long)h->j1_chunks * cdiv(naux, rc);
+          const double cost = (double)((ctas + h->num_sms - 1) / h->num_sms) * (rc + 1.0);
+          if (rc == kJ1Rows || cost < 0.97 * best) { best = cost; rows_cta = rc; }
+        }
+        dim3 g1t(h->j1_chunks, cdiv(naux, rows_cta));
+        if (dispatch_j1_tma(h->device, ns, g1t, st, h->B, npair, naux, h->Dw + (size_t)s0 * npair, h->rho_part, naux_pad, rows_cta) != cudaSuccess)
           return -1;
       } else {
         k_j1<<<g1, kJ1Warps * 32, 0, st>>>(h->B, npair, naux, h->Dw + (size_t)s0 * npair, ns, h->rho_part, naux_pad);
