@@ -22,9 +22,10 @@
 
 namespace dfjk {
 
-constexpr int kEmuMinS = 3, kEmuMaxS = 6;   // S * 80 accumulator columns must fit the 512 TMEM columns
+constexpr int kEmuMaxS = 6;          // slices (dfjk_create takes 3..6): S * 80 accumulator columns must fit the 512 TMEM columns
 constexpr int kEmuTM = 128;          // tile rows   = UMMA M (one TMEM lane per row)
 constexpr int kEmuTN = 80;           // tile columns = UMMA N; S accumulator groups x 80 columns <= 512 TMEM columns for S <= 6
+static_assert(kEmuMaxS * kEmuTN <= 512, "the accumulator groups of all slices must fit the TMEM columns");
 constexpr int kEmuStages = 4;
 constexpr int kEmuThreads = 192;     // warp 0: bulk-copy producer, warp 1: MMA issuer, warps 2-5: epilogue (TMEM lane quarters 2,3,0,1)
 
