@@ -34,9 +34,14 @@ namespace dfjk {
 constexpr int kStages = 3;
 // Pipeline depth of the half-transform by N tile width: 3 stages of 59 KB at 304 columns; a thin
 // tile (AO2MO's active columns, small sets) is bandwidth-bound and keeps up to 8 stages in flight.
+// Narrow tiles (at most 96 columns: the `small` config, fragment-sized sets) run TWO CTAs per SM: a tile is
+// only nao/16 short chunks, so its epilogue (X stores, rho) is a sizeable share of it, and with a second
+// resident CTA the tensor pipe has the other tile's chunks to work on meanwhile.  Register budget then:
+// 80 per thread at launch, 40 for the producer warpgroup, 96 for the consumers.
+__host__ __device__ constexpr int ht_ctas_per_sm(int wn) { return wn <= 6 ? 2 : 1; }
 __host__ __device__ constexpr int ht_stages(int wn) {
   const int stage_bytes = (64 * kHtLd + 16 * wn * kHtLd) * 8;
-  const int fit = (200 * 1024) / stage_bytes;
+  const int fit = ((ht_ctas_per_sm(wn) == 2 ? 100 : 200) * 1024) / stage_bytes;
   return fit < 3 ? 3 : (fit > 8 ? 8 : fit);
 }
 constexpr int kThreads = 384;             // 2 consumer warpgroups + 1 producer warpgroup
@@ -105,7 +110,7 @@ __device__ __forceinline__ HtTile ht_tile(const HtParams& q, int tile) {
 // wants both J and K streams B twice instead of three times.  EPI = 2: X row-major (AO2MO, Eq. 18).
 // PAIR (compile-time, so that the unpaired instances keep their register budget): HtParams::pair_last
 template <int WN, int EPI, bool PAIR>
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __launch_bounds__(kThreads, ht_ctas_per_sm(WN))
 k_half_transform(const __grid_constant__ HtParams q) {
   extern __shared__ __align__(128) double smem[];
   constexpr int NT = 16 * WN;
@@ -237,7 +242,7 @@ k_half_transform(const __grid_constant__ HtParams q) {
   }
 
   // ===================== consumer warpgroups =====================
-  reg_inc<kConsumerRegs>();
+  reg_inc<ht_ctas_per_sm(WN) == 2 ? 96 : kConsumerRegs>();
   const int r = l >> 2, j = l & 3;
   const int wm = w & 3, wn = w >> 2;
   double acc[2][WN][2];
@@ -899,7 +904,8 @@ int launch_half_transform_rowmajor(dfjk_ctx* h, const SetInfo& si, int p_first, 
   a.rho_ht = nullptr; a.nset = 0; a.ldx = ldx; a.xrows = h->nao; a.sgnbits = nullptr; a.pair_last = 0;
   a.col0[0] = 0;
   const long long ht_tiles = (long long)nb * ntm_ht * ntn;
-  const int ht_grid = (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid);
+  const long long ht_slots = (long long)h->ht_grid * ht_ctas_per_sm(wn);   // persistent: one or two CTAs per SM
+  const int ht_grid = (int)(ht_tiles < ht_slots ? ht_tiles : ht_slots);
   return dispatch_ht(h->device, wn, 2, ht_grid, st, a) == cudaSuccess ? 0 : -1;
 }
 
@@ -1037,7 +1043,8 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
     a.rho_ht = h->rho_ht; a.nset = si.nset; a.ldx = 0; a.xrows = 0; a.sgnbits = h->sgnbits;
     for (int s = 0; s <= si.nset; s++) a.col0[s] = si.col0[s];
     const long long ht_tiles = (long long)nb * ntm_ht * ntn;
-    const int ht_grid = (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid);
+    const long long ht_slots = (long long)h->ht_grid * ht_ctas_per_sm(wn);   // persistent: one or two CTAs per SM
+  const int ht_grid = (int)(ht_tiles < ht_slots ? ht_tiles : ht_slots);
     if (thin) {
       // one set of at most 8 columns: one pass over the packed triangle (symm.cu), rho written directly
       if (launch_symm_thin_jk(h, si.nocc[0], p0, nb, h->X, want_rho ? h->rho : nullptr, st) != 0) return -1;
@@ -1174,7 +1181,8 @@ int launch_k_path_dm(dfjk_ctx* h, int nset, const double* D, double* K_out, cuda
       a.X = X1; a.nch = nch; a.mu_pad = h->mu_pad; a.p_first = p0; a.nb = nb; a.ntm = ntm_ht; a.ntn = ntn;
       a.rho_ht = nullptr; a.nset = 0; a.ldx = 0; a.xrows = 0; a.col0[0] = 0; a.sgnbits = nullptr;
       const long long ht_tiles = (long long)nb * ntm_ht * ntn;
-      if (dispatch_ht(h->device, wn, 0, (int)(ht_tiles < h->ht_grid ? ht_tiles : h->ht_grid), st, a) != cudaSuccess) return -1;
+      const long long ht_slots = (long long)h->ht_grid * ht_ctas_per_sm(wn);
+      if (dispatch_ht(h->device, wn, 0, (int)(ht_tiles < ht_slots ? ht_tiles : ht_slots), st, a) != cudaSuccess) return -1;
       dim3 gu(nch, nb);
       k_unpack_tiled<<<gu, 256, 0, st>>>(h->B, h->npair, nao, p0, nch, h->mu_pad, X2);
       launches += 2;
