@@ -308,7 +308,7 @@ k_half_transform(const __grid_constant__ HtParams q) {
     const int pl = (PAIR && ht.paired) ? (ht.pl + wm) / q.pair_last : ht.pl;
     const int ip = (PAIR && ht.paired) ? ht.pl + wm - pl * q.pair_last : wm;
     const int mrow0 = m0 + ip * 16;
-    if (PAIR && pl >= q.nb) continue;             // second half of a paired tile past the last aux row
+    if (PAIR && pl >= q.nb) continue;             // a piece slot of the last packed tile past the last aux row
     if (EPI == 2) {
       double* Xp = q.X + (size_t)pl * q.xrows * q.ldx;
 #pragma unroll
@@ -828,7 +828,7 @@ static cudaError_t launch_ht_p(int device, int grid, cudaStream_t st, const HtPa
   return cudaSuccess;
 }
 
-// the paired variant exists for the k-tiled epilogues (JK path, density-matrix form); row-major X (AO2MO) is unpaired
+// the packed-piece variant exists for the k-tiled epilogues (JK path, density-matrix form); row-major X (AO2MO) has none
 template <int WN, int EPI>
 static cudaError_t launch_ht(int device, int grid, cudaStream_t st, const HtParams& a) {
   if (EPI != 2 && a.pair_last) return launch_ht_p<WN, EPI, EPI != 2>(device, grid, st, a);
@@ -849,7 +849,7 @@ static cudaError_t dispatch_ht_wn(int device, int wn, int grid, cudaStream_t st,
   }
 }
 
-// the last 64-row block holds at most 32 rows and the re-tiled copy exists: two aux rows share its tiles
+// pieces (16 rows) in the last 64-row block when it is part-empty and the re-tiled copy exists: packed tiles (HtParams::pair_last)
 static int ht_pair_last(const dfjk_ctx* h) { return h->Bt != nullptr && (h->nao & 63) >= 1 && (h->nao & 63) <= 48 ? ((h->nao & 63) + 15) >> 4 : 0; }
 
 // epi: 0 = k-tiled X, 1 = k-tiled X + rho partials, 2 = row-major X
