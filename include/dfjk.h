@@ -173,7 +173,8 @@ int dfjk_get_jk_dm(dfjk_handle h, int nset, const double* D, double* J_out, doub
  * The call enqueues one 8-byte memset (the barrier counters must start at zero; the array keeps the last call's
  * contents, the partials are overwritten before they are read) and one kernel on `stream`; it calls no cudaMalloc,
  * cudaFree or allocating library routine and never synchronises the host.  The first call on a device looks up the
- * array's device address (cudaGetSymbolAddress, once per device, with that device current).
+ * array's device address (cudaGetSymbolAddress, once per device, with that device current) and opts the kernel in to
+ * its shared memory: make one call before starting a stream capture, later calls can be captured and replayed.
  * EVERY call on a device shares the one array: calls that overlap on the GPU (two streams, two host threads, two
  * graphs in flight) race on it -- serialise them.  Calls on one stream are ordered and safe.
  */

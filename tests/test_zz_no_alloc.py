@@ -126,6 +126,38 @@ def test_static_scratch_entry_one_output_at_a_time(torch_cuda):
     assert torch.equal(J, J2) and torch.equal(K, K2), "J-only and K-only calls give the bits of the joint call"
 
 
+def test_static_scratch_entry_in_a_cuda_graph(torch_cuda):
+    """the stated use: after one call outside the capture (set-up: address of the static array, function
+    attribute) the entry point only enqueues a memset node and a kernel node, so it can be captured and replayed
+    on new orbitals"""
+    torch = torch_cuda
+    import paper_2505_03755_b200 as pkg
+    a = dfjk_inputs.make_random(60, 35, [13, 5], seed=7201, L=9.0)
+    b = dfjk_inputs.make_random(60, 35, [13, 5], seed=7202, L=9.0)           # other orbitals, same shapes
+    B, C, occ = device_inputs(torch, a)
+    refs = []
+    for inp in (a, b):
+        _, Ci, oi = device_inputs(torch, inp)
+        refs.append(handle_path(torch, pkg, inp, B, Ci, oi))
+    J = torch.empty((2, 60, 60), dtype=torch.float64, device="cuda")
+    K = torch.empty_like(J)
+    pkg.small_jk_static(B, 60, a.nocc, C, occ, out_j=J, out_k=K)             # set-up happens here
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        pkg.small_jk_static(B, 60, a.nocc, C, occ, out_j=J, out_k=K, stream=torch.cuda.current_stream())
+    for inp, (Jr, Kr) in ((b, refs[1]), (a, refs[0]), (b, refs[1])):
+        _, Ci, oi = device_inputs(torch, inp)
+        C.copy_(Ci)
+        occ.copy_(oi)
+        J.fill_(float("nan"))
+        K.fill_(float("nan"))
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(J, Jr) and torch.equal(K, Kr)
+    del g
+
+
 def test_static_scratch_entry_allocates_no_device_memory(torch_cuda):
     """free device memory as the driver reports it does not shrink over a call (after one warm-up call, which
     loads the kernel and looks up the address of the static array)"""
