@@ -31,6 +31,8 @@
 
 namespace dfjk {
 
+static inline long long cdiv_ll(long long a, long long b) { return (a + b - 1) / b; }
+
 constexpr int kStages = 3;
 // Pipeline depth of the half-transform by N tile width: 3 stages of 59 KB at 304 columns; a thin
 // tile (AO2MO's active columns, small sets) is bandwidth-bound and keeps up to 8 stages in flight.
@@ -1008,6 +1010,25 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
   const int n8 = ldx / 8;
   const int ntn = cdiv(n8, 2 * kHtMaxWN), wn = cdiv(n8, 2 * ntn);  // N tile = 16*wn columns
   const int ntm_ht = cdiv(nao, 64);
+  // equal blocks: the same number of launches, but no short last block (3 x 1122 + 634 rows at `large` become
+  // 4 x 1000); then up to 15 rows more per block if that saves a round of half-transform tiles over the persistent
+  // grid (1002, 1002, 1002, 994 rows: 127 + 127 + 127 + 126 rounds of 148 tiles, the minimum, instead of 4 x 127)
+  if (!emu && h->nblk_forced <= 0) {
+    const long long cap = nblk, nblocks = cdiv_ll(naux, cap), slots = (long long)h->ht_grid * ht_ctas_per_sm(wn);
+    const int v = ht_pair_last(h);
+    auto tiles = [&](long long nb) {
+      return v ? (nb * (ntm_ht - 1) + ((nb * v + 3) >> 2)) * ntn : nb * ntm_ht * ntn;
+    };
+    const long long bal = cdiv_ll(naux, nblocks);
+    long long best_nb = bal, best_rounds = -1;
+    for (long long nb = bal; nb <= cap && nb < bal + 16; nb++) {
+      const long long last = naux - (nblocks - 1) * nb;
+      if (last < 1) break;
+      const long long rounds = (nblocks - 1) * cdiv_ll(tiles(nb), slots) + cdiv_ll(tiles(last), slots);
+      if (best_rounds < 0 || rounds < best_rounds) { best_rounds = rounds; best_nb = nb; }
+    }
+    nblk = best_nb;
+  }
   const int wm_s = pick_syrk_tile(nao);
   const double diag_cost = (wm_s + 1) / (2.0 * wm_s);
   const int ntm = cdiv(nao, 16 * wm_s), ntiles = ntm * (ntm + 1) / 2;
