@@ -969,6 +969,24 @@ static int pick_ksplit(dfjk_ctx* h, int nblk, int ntiles, int ntm, double diag_c
   return ksplit < 1 ? 1 : ksplit;
 }
 
+// Rows per aux block under a cap: the fewest blocks that fit, made equal (no short last block: 3 x 1122 + 634 rows at
+// `large` become 4 x 1000), then up to 15 rows more per block if that saves a round of half-transform tiles over the
+// persistent grid (1002, 1002, 1002, 994 rows: 127 + 127 + 127 + 126 rounds of 148 tiles, the minimum, not 4 x 127)
+static long long pick_block_rows(const dfjk_ctx* h, long long cap, int naux, int ntm_ht, int ntn, int wn) {
+  const long long nblocks = cdiv_ll(naux, cap), slots = (long long)h->ht_grid * ht_ctas_per_sm(wn);
+  const int v = ht_pair_last(h);
+  auto tiles = [&](long long nb) { return v ? (nb * (ntm_ht - 1) + ((nb * v + 3) >> 2)) * ntn : nb * ntm_ht * ntn; };
+  const long long bal = cdiv_ll(naux, nblocks);
+  long long best_nb = bal, best_rounds = -1;
+  for (long long nb = bal; nb <= cap && nb < bal + 16; nb++) {
+    const long long last = naux - (nblocks - 1) * nb;
+    if (last < 1) break;
+    const long long rounds = (nblocks - 1) * cdiv_ll(tiles(nb), slots) + cdiv_ll(tiles(last), slots);
+    if (best_rounds < 0 || rounds < best_rounds) { best_rounds = rounds; best_nb = nb; }
+  }
+  return best_nb;
+}
+
 // Aux-block scheduler: cap the X workspace, pick the split-K factor, enqueue
 // half-transform and SYRK block after block on one stream.  No allocation, no host sync.
 // With want_rho the half-transform also produces rho (step a2 fused): the
@@ -1010,25 +1028,7 @@ int launch_k_path(dfjk_ctx* h, const SetInfo& si, double* K_out, bool want_rho, 
   const int n8 = ldx / 8;
   const int ntn = cdiv(n8, 2 * kHtMaxWN), wn = cdiv(n8, 2 * ntn);  // N tile = 16*wn columns
   const int ntm_ht = cdiv(nao, 64);
-  // equal blocks: the same number of launches, but no short last block (3 x 1122 + 634 rows at `large` become
-  // 4 x 1000); then up to 15 rows more per block if that saves a round of half-transform tiles over the persistent
-  // grid (1002, 1002, 1002, 994 rows: 127 + 127 + 127 + 126 rounds of 148 tiles, the minimum, instead of 4 x 127)
-  if (!emu && h->nblk_forced <= 0) {
-    const long long cap = nblk, nblocks = cdiv_ll(naux, cap), slots = (long long)h->ht_grid * ht_ctas_per_sm(wn);
-    const int v = ht_pair_last(h);
-    auto tiles = [&](long long nb) {
-      return v ? (nb * (ntm_ht - 1) + ((nb * v + 3) >> 2)) * ntn : nb * ntm_ht * ntn;
-    };
-    const long long bal = cdiv_ll(naux, nblocks);
-    long long best_nb = bal, best_rounds = -1;
-    for (long long nb = bal; nb <= cap && nb < bal + 16; nb++) {
-      const long long last = naux - (nblocks - 1) * nb;
-      if (last < 1) break;
-      const long long rounds = (nblocks - 1) * cdiv_ll(tiles(nb), slots) + cdiv_ll(tiles(last), slots);
-      if (best_rounds < 0 || rounds < best_rounds) { best_rounds = rounds; best_nb = nb; }
-    }
-    nblk = best_nb;
-  }
+  if (!emu && h->nblk_forced <= 0) nblk = pick_block_rows(h, nblk, naux, ntm_ht, ntn, wn);
   const int wm_s = pick_syrk_tile(nao);
   const double diag_cost = (wm_s + 1) / (2.0 * wm_s);
   const int ntm = cdiv(nao, 16 * wm_s), ntiles = ntm * (ntm + 1) / 2;
@@ -1180,11 +1180,12 @@ int launch_k_path_dm(dfjk_ctx* h, int nset, const double* D, double* K_out, cuda
   if (nblk > naux) nblk = naux;
   if (nblk > 32768) nblk = 32768;
   if (nblk < 1) return -2;
-  double* X1 = h->X;
-  double* X2 = h->X + (size_t)nblk * row_doubles;
   const int n8 = ldx / 8;
   const int ntn = cdiv(n8, 2 * kHtMaxWN), wn = cdiv(n8, 2 * ntn);
   const int ntm_ht = cdiv(nao, 64);
+  if (h->nblk_forced <= 0) nblk = pick_block_rows(h, nblk, naux, ntm_ht, ntn, wn);
+  double* X1 = h->X;
+  double* X2 = h->X + (size_t)nblk * row_doubles;
   const int wm_s = pick_syrk_tile(nao);
   const double diag_cost = (wm_s + 1) / (2.0 * wm_s);
   const int ntm = cdiv(nao, 16 * wm_s), ntiles = ntm * (ntm + 1) / 2;
