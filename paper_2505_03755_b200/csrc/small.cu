@@ -60,10 +60,11 @@ __global__ void __launch_bounds__(kSmThreads)
 k_small_fused(const __grid_constant__ SetInfo si, const __grid_constant__ SmallParams q) {
   extern __shared__ __align__(16) double smem[];
   const int nao = q.nao, ntot = q.ntot, ldb = nao + 1, tid = threadIdx.x;
+  const int ldxs = ntot | 1;              // odd row stride of Xs: the K loop reads X[nu][c] with nu along the lanes
   double* Bs = smem;                      // [nao][nao + 1]   symmetric slice
   double* Cs = Bs + nao * ldb;            // [nao][ntot]      C' = C sqrt|occ|
-  double* Xs = Cs + nao * ntot;           // [nao][ntot]
-  double* sg = Xs + nao * ntot;           // [ntot]           sign(occ)
+  double* Xs = Cs + nao * ntot;           // [nao][ldxs]
+  double* sg = Xs + nao * ldxs;           // [ntot]           sign(occ)
   double* red = sg + ntot;                // [8]
   __shared__ int c0s[kMaxSets + 1];
   const size_t n2 = (size_t)nao * nao;
@@ -127,7 +128,7 @@ k_small_fused(const __grid_constant__ SetInfo si, const __grid_constant__ SmallP
         t3 = fma(b[lam + 3], Cs[(lam + 3) * ntot + c], t3);
       }
       for (; lam < nao; lam++) t0 = fma(b[lam], Cs[lam * ntot + c], t0);
-      Xs[e] = (t0 + t1) + (t2 + t3);
+      Xs[mu * ldxs + c] = (t0 + t1) + (t2 + t3);
     }
     __syncthreads();
     for (int s = 0; s < si.nset; s++) {
@@ -137,7 +138,7 @@ k_small_fused(const __grid_constant__ SetInfo si, const __grid_constant__ SmallP
         double t = 0.0;
         for (int e = tid; e < nao * (cb - ca); e += kSmThreads) {
           const int mu = e / (cb - ca), c = ca + e - mu * (cb - ca);
-          t = fma(Xs[mu * ntot + c] * sg[c], Cs[mu * ntot + c], t);
+          t = fma(Xs[mu * ldxs + c] * sg[c], Cs[mu * ntot + c], t);
         }
         const double rho = block_sum(t, red);
         double* jp = Jp + (size_t)s * q.npair;
@@ -154,8 +155,8 @@ k_small_fused(const __grid_constant__ SetInfo si, const __grid_constant__ SmallP
         for (int e = tid; e < nao * nao; e += kSmThreads) {
           const int mu = e / nao, nu = e - mu * nao;
           if (nu > mu) continue;
-          const double* xm = Xs + mu * ntot;
-          const double* xn = Xs + nu * ntot;
+          const double* xm = Xs + mu * ldxs;
+          const double* xn = Xs + nu * ldxs;
           double t = 0.0;
           for (int c = ca; c < cb; c++) t = fma(xm[c] * sg[c], xn[c], t);
           kp[e] = first ? t : kp[e] + t;
@@ -213,7 +214,7 @@ k_small_fused(const __grid_constant__ SetInfo si, const __grid_constant__ SmallP
 }
 
 static size_t small_smem_bytes(int nao, int ntot) {
-  return ((size_t)nao * (nao + 1) + 2 * (size_t)nao * ntot + ntot + 16) * sizeof(double);
+  return ((size_t)nao * (nao + 1) + (size_t)nao * ntot + (size_t)nao * (ntot | 1) + ntot + 16) * sizeof(double);
 }
 
 static cudaError_t small_attr(int device) {
