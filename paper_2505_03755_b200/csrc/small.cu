@@ -9,7 +9,8 @@
 //   grid barrier (the kernel is launched cooperatively: all CTAs are resident);
 //   phase 2, all CTAs: every output element is the sum of the partials in CTA order, written to both
 //     triangles of J and K (deterministic: the assignment of aux rows to CTAs is fixed).
-// Plain DFMA on purpose: this regime is latency-bound, not throughput-bound (tiny config: 13 MFLOP).
+// The two products of phase 1 run as 8 x 8 x 4 DMMA tiles out of shared memory (a scalar DFMA version spent 40 % of its
+// time on the instructions of the K loop at nao = 80); rho, the J partial and phase 2 are plain DFMA / DADD.
 // Chosen by dfjk_get_jk when nao <= 96, nao * sum(nocc) <= 4608 and naux * nao^2 * (sum(nocc) + nset)
 // <= 2^26 (option no_small_path disables it); everything larger takes the tensor-pipe kernels.
 #include <cstdarg>
@@ -60,18 +61,30 @@ __global__ void __launch_bounds__(kSmThreads)
 k_small_fused(const __grid_constant__ SetInfo si, const __grid_constant__ SmallParams q) {
   extern __shared__ __align__(16) double smem[];
   const int nao = q.nao, ntot = q.ntot, ldb = nao + 1, tid = threadIdx.x;
-  const int ldxs = ntot | 1;              // odd row stride of Xs: the K loop reads X[nu][c] with nu along the lanes
-  double* Bs = smem;                      // [nao][nao + 1]   symmetric slice
-  double* Cs = Bs + nao * ldb;            // [nao][ntot]      C' = C sqrt|occ|
-  double* Xs = Cs + nao * ntot;           // [nao][ldxs]
+  const int ldxs = ntot | 1;              // odd row stride of Xs: the fragment loads of the K product walk its rows
+  const int nao4 = (nao + 3) & ~3;        // C' rows padded to the k step of the MMA (zero rows)
+  double* Bs = smem;                      // [nao][nao + 1]   symmetric slice (column nao stays zero)
+  double* Cs = Bs + nao * ldb;            // [nao4][ntot]     C' = C sqrt|occ|
+  double* Xs = Cs + nao4 * ntot;          // [nao][ldxs]
   double* sg = Xs + nao * ldxs;           // [ntot]           sign(occ)
-  double* red = sg + ntot;                // [8]
+  double* red = sg + ntot;                // [16]
   __shared__ int c0s[kMaxSets + 1];
   const size_t n2 = (size_t)nao * nao;
+  const int w = tid >> 5, l = tid & 31, r = l >> 2, jj = l & 3;      // DMMA.8x8x4 fragment coordinates
+  const int mt = (nao + 7) >> 3;          // 8-row blocks of the basis
 
-  // the packed row of the next aux row is fetched into registers while the current one is processed
+  // the packed row of the next aux row is fetched into registers while the current one is processed;
+  // (mu, nu) of the packed elements a thread owns are the same for every row: worked out once
   constexpr int kPre = (kSmMaxNao * (kSmMaxNao + 1) / 2 + kSmThreads - 1) / kSmThreads;     // 19
   double pre[kPre];
+  int mn[kPre];
+#pragma unroll
+  for (int k = 0; k < kPre; k++) {
+    const int pr = tid + k * kSmThreads;
+    int mu = 0, nu = 0;
+    if (pr < (int)q.npair) untri(pr, mu, nu);
+    mn[k] = (mu << 8) | nu;
+  }
   auto prefetch = [&](int P) {
     const double* bp = q.Bp + (size_t)P * q.npair;
 #pragma unroll
@@ -82,6 +95,11 @@ k_small_fused(const __grid_constant__ SetInfo si, const __grid_constant__ SmallP
   };
   prefetch(blockIdx.x);                  // in flight during the prologue
 
+  // every pad (column nao of Bs, rows nao.. of C', the odd column of Xs) is zero, and nothing a fragment load can
+  // touch is uninitialised: a pad meets a zero in the other operand, and rows or columns past the end only feed
+  // results that are not stored
+  for (int i = tid; i < nao * ldb + nao4 * ntot + nao * ldxs + ntot + 16; i += kSmThreads) smem[i] = 0.0;
+  __syncthreads();
   // a1: C' and the signs; compact column c of set s = si.ooff[s] + i.  sg first holds sqrt|occ|, then sign(occ)
   if (tid <= si.nset) c0s[tid] = tid < si.nset ? si.ooff[tid] : ntot;
   for (int c = tid; c < ntot; c += kSmThreads) sg[c] = sqrt(fabs(q.occ[c]));
@@ -104,31 +122,31 @@ k_small_fused(const __grid_constant__ SetInfo si, const __grid_constant__ SmallP
     // a5: unpack the packed row into the symmetric slice
 #pragma unroll
     for (int k = 0; k < kPre; k++) {
-      const int pr = tid + k * kSmThreads;
-      if (pr < (int)q.npair) {
-        int mu, nu;
-        untri(pr, mu, nu);
+      if (tid + k * kSmThreads < (int)q.npair) {
+        const int mu = mn[k] >> 8, nu = mn[k] & 255;
         Bs[mu * ldb + nu] = pre[k];
         Bs[nu * ldb + mu] = pre[k];
       }
     }
     prefetch(P + gridDim.x);
     __syncthreads();
-    // a6: X[mu][c] = sum_lam b[mu][lam] C'[lam][c]; a thread owns column c = e % ntot of rows e / ntot
-    for (int e = tid; e < nao * ntot; e += kSmThreads) {
-      const int mu = e / ntot, c = e - mu * ntot;
-      const double* b = Bs + mu * ldb;
-      // four interleaved partial sums (fixed order): the dependent-DFMA chain is a quarter as long
-      double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;
-      int lam = 0;
-      for (; lam + 4 <= nao; lam += 4) {
-        t0 = fma(b[lam], Cs[lam * ntot + c], t0);
-        t1 = fma(b[lam + 1], Cs[(lam + 1) * ntot + c], t1);
-        t2 = fma(b[lam + 2], Cs[(lam + 2) * ntot + c], t2);
-        t3 = fma(b[lam + 3], Cs[(lam + 3) * ntot + c], t3);
+    // a6: X = b C' in 8 x 8 tiles on the FP64 tensor pipe, a warp takes every eighth tile.  A[row][k] = b[mu][lam],
+    // B[k][col] = C'[lam][c]; rows past nao are clamped (their results are not stored), lam past nao meets the
+    // zero rows of C', columns past ntot run into finite data and are not stored
+    {
+      const int nt = (ntot + 7) >> 3;
+      for (int t = w; t < mt * nt; t += kSmThreads / 32) {
+        const int i = t / nt, j = t - i * nt;
+        const double* ap = Bs + min(8 * i + r, nao - 1) * ldb + jj;
+        const double* bp = Cs + jj * ntot + 8 * j + r;
+        double d0 = 0.0, d1 = 0.0;
+        for (int k0 = 0; k0 < nao; k0 += 4) dmma884(d0, d1, ap[k0], bp[k0 * ntot]);
+        const int row = 8 * i + r, col = 8 * j + 2 * jj;
+        if (row < nao) {
+          if (col < ntot) Xs[row * ldxs + col] = d0;
+          if (col + 1 < ntot) Xs[row * ldxs + col + 1] = d1;
+        }
       }
-      for (; lam < nao; lam++) t0 = fma(b[lam], Cs[lam * ntot + c], t0);
-      Xs[mu * ldxs + c] = (t0 + t1) + (t2 + t3);
     }
     __syncthreads();
     for (int s = 0; s < si.nset; s++) {
@@ -142,25 +160,42 @@ k_small_fused(const __grid_constant__ SetInfo si, const __grid_constant__ SmallP
         }
         const double rho = block_sum(t, red);
         double* jp = Jp + (size_t)s * q.npair;
-        for (int pr = tid; pr < (int)q.npair; pr += kSmThreads) {
-          int mu, nu;
-          untri(pr, mu, nu);
-          const double v = rho * Bs[mu * ldb + nu];
-          jp[pr] = first ? v : jp[pr] + v;
+#pragma unroll
+        for (int k = 0; k < kPre; k++) {
+          const int pr = tid + k * kSmThreads;
+          if (pr < (int)q.npair) {
+            const double v = rho * Bs[(mn[k] >> 8) * ldb + (mn[k] & 255)];
+            jp[pr] = first ? v : jp[pr] + v;
+          }
         }
       }
-      if (q.K) {
-        // a7: K partial[mu >= nu] += sum_{c in s} sign_c X[mu][c] X[nu][c]
+      if (q.K && cb > ca) {
+        // a7: K partial[mu >= nu] += sum_{c in s} sign_c X[mu][c] X[nu][c], the lower 8 x 8 tiles (i >= j) on the tensor
+        // pipe: A[row][k] = X[mu][c], B[k][col] = sign_c X[nu][c], zero past the last column of the set
         double* kp = Kp + (size_t)s * n2;
-        for (int e = tid; e < nao * nao; e += kSmThreads) {
-          const int mu = e / nao, nu = e - mu * nao;
-          if (nu > mu) continue;
-          const double* xm = Xs + mu * ldxs;
-          const double* xn = Xs + nu * ldxs;
-          double t = 0.0;
-          for (int c = ca; c < cb; c++) t = fma(xm[c] * sg[c], xn[c], t);
-          kp[e] = first ? t : kp[e] + t;
+        const int nk = (cb - ca + 3) >> 2;
+        for (int t = w; t < mt * (mt + 1) / 2; t += kSmThreads / 32) {
+          int i, j;
+          untri(t, i, j);
+          const double* ap = Xs + min(8 * i + r, nao - 1) * ldxs + ca + jj;
+          const double* bp = Xs + min(8 * j + r, nao - 1) * ldxs + ca + jj;
+          double d0 = 0.0, d1 = 0.0;
+          for (int k = 0; k < nk; k++) {
+            const int c = ca + 4 * k + jj;
+            const double b = c < cb ? bp[4 * k] * sg[c] : 0.0;
+            dmma884(d0, d1, ap[4 * k], b);
+          }
+          const int row = 8 * i + r, col = 8 * j + 2 * jj;
+          if (row < nao) {
+            double* o = kp + (size_t)row * nao + col;
+            if (col <= row) o[0] = first ? d0 : o[0] + d0;
+            if (col + 1 <= row) o[1] = first ? d1 : o[1] + d1;
+          }
         }
+      } else if (q.K && first) {
+        // a set without columns: its partial is zero
+        double* kp = Kp + (size_t)s * n2;
+        for (int e = tid; e < nao * nao; e += kSmThreads) kp[e] = 0.0;
       }
     }
     __syncthreads();
@@ -214,7 +249,7 @@ k_small_fused(const __grid_constant__ SetInfo si, const __grid_constant__ SmallP
 }
 
 static size_t small_smem_bytes(int nao, int ntot) {
-  return ((size_t)nao * (nao + 1) + (size_t)nao * ntot + (size_t)nao * (ntot | 1) + ntot + 16) * sizeof(double);
+  return ((size_t)nao * (nao + 1) + (size_t)((nao + 3) & ~3) * ntot + (size_t)nao * (ntot | 1) + ntot + 16) * sizeof(double);
 }
 
 static cudaError_t small_attr(int device) {
