@@ -86,7 +86,7 @@ typedef struct {
                                  (needs a 16-byte aligned B; one launch per 1280 columns of the basis); 1 = always
                                  the tiled half-transform */
   int no_small_path;          /* 0 = an embedding-sized dfjk_get_jk (nao <= 96, nao * sum(nocc) <= 4608 and
-                                 naux * nao^2 * (sum(nocc) + nset) <= 2^26) runs as ONE kernel launch: the call is
+                                 naux * nao^2 * (sum(nocc) + nset) <= 2^26, 2^27 for one set) runs as ONE kernel launch: the call is
                                  launch-latency bound there ("called thousands of times");
                                  dfjk_last_launch_count then returns 1.  1 = always the tiled kernels */
 } dfjk_options;

@@ -12,7 +12,7 @@
 // The two products of phase 1 run as 8 x 8 x 4 DMMA tiles out of shared memory (a scalar DFMA version spent 40 % of its
 // time on the instructions of the K loop at nao = 80); rho, the J partial and phase 2 are plain DFMA / DADD.
 // Chosen by dfjk_get_jk when nao <= 96, nao * sum(nocc) <= 4608 and naux * nao^2 * (sum(nocc) + nset)
-// <= 2^26 (option no_small_path disables it); everything larger takes the tensor-pipe kernels.
+// <= 2^26 (2^27 for one set; option no_small_path disables it); everything larger takes the tiled tensor-pipe kernels.
 #include <cstdarg>
 #include <cstdio>
 
@@ -23,7 +23,8 @@ namespace dfjk {
 
 constexpr int kSmThreads = 256;
 constexpr int kSmMaxNao = 96, kSmMaxElems = 4608;
-constexpr double kSmMaxWork = 67108864.0;
+constexpr double kSmMaxWork = 67108864.0;           // 2^26; one set: twice that (measured crossover with the tiled kernels:
+                                                    // 2^27.5 for one set, below 2^26.6 for four thin sets)
 
 struct SmallParams {
   const double* Bp; size_t npair; int naux, nao;
@@ -263,7 +264,7 @@ int small_path_ctas(const dfjk_ctx* h, const SetInfo& si) {
   int ntot = 0;
   for (int s = 0; s < si.nset; s++) ntot += si.nocc[s];
   if (ntot < 1 || (long long)h->nao * ntot > kSmMaxElems) return 0;
-  if ((double)h->naux * h->nao * h->nao * (ntot + si.nset) > kSmMaxWork) return 0;
+  if ((double)h->naux * h->nao * h->nao * (ntot + si.nset) > (si.nset == 1 ? 2.0 : 1.0) * kSmMaxWork) return 0;
   // as many CTAs as aux rows, in equal rounds over at most two resident CTAs per SM (more partials would make the
   // final sum the long pole); the cooperative launch needs all of them resident
   int occ = 0;
