@@ -5,7 +5,9 @@
 //   phase 1, per CTA, for its aux rows P (round-robin, one or two each):
 //     b^P unpacked into shared memory, X = b^P C' (Eq. 16), rho_s = <X_s, C'_s sign> (Eq. 14,
 //     DESIGN.md R16), K partial += X_s sign X_s^T (Eq. 17, lower triangle), J partial += rho_s b^P (Eq. 15),
-//     both partials private to the CTA (no atomics on data);
+//     both partials private to the CTA and every element owned by one thread: the first aux row of the CTA stores,
+//     later ones add with a reduction that returns nothing (no load to wait for; one thread per address in program
+//     order, so the sum is the same double as a load-add-store and the result stays deterministic);
 //   grid barrier (the kernel is launched cooperatively: all CTAs are resident);
 //   phase 2, all CTAs: every output element is the sum of the partials in CTA order, written to both
 //     triangles of J and K (deterministic: the assignment of aux rows to CTAs is fixed).
@@ -166,7 +168,7 @@ k_small_fused(const __grid_constant__ SetInfo si, const __grid_constant__ SmallP
           const int pr = tid + k * kSmThreads;
           if (pr < (int)q.npair) {
             const double v = rho * Bs[(mn[k] >> 8) * ldb + (mn[k] & 255)];
-            jp[pr] = first ? v : jp[pr] + v;
+            if (first) jp[pr] = v; else atomicAdd(jp + pr, v);
           }
         }
       }
@@ -189,8 +191,8 @@ k_small_fused(const __grid_constant__ SetInfo si, const __grid_constant__ SmallP
           const int row = 8 * i + r, col = 8 * j + 2 * jj;
           if (row < nao) {
             double* o = kp + (size_t)row * nao + col;
-            if (col <= row) o[0] = first ? d0 : o[0] + d0;
-            if (col + 1 <= row) o[1] = first ? d1 : o[1] + d1;
+            if (col <= row) { if (first) o[0] = d0; else atomicAdd(o, d0); }
+            if (col + 1 <= row) { if (first) o[1] = d1; else atomicAdd(o + 1, d1); }
           }
         }
       } else if (q.K && first) {
