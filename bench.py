@@ -458,8 +458,12 @@ def main():
     small = None
     if not args.no_small_calls:
         small = {}
-        for sname in ("tiny", "small"):
-            sinp = dfjk_inputs.make_config(sname)
+        # the two small configs of BASELINE.json and one fragment-sized call with two sets (nao 80, naux 300: the
+        # embedding-sized regime of PAPER.md:84-86 between them)
+        frag = dict(nao=80, naux=300, nocc=[10, 8])
+        for sname in ("tiny", "fragment", "small"):
+            sinp = (dfjk_inputs.make_random(frag["nao"], frag["naux"], frag["nocc"], seed=8080, L=12.0)
+                    if sname == "fragment" else dfjk_inputs.make_config(sname))
             sB = torch.from_numpy(sinp.B_packed).cuda()
             sC = torch.from_numpy(sinp.C_concat()).cuda()
             socc = torch.from_numpy(sinp.occ_concat()).cuda()
@@ -482,7 +486,7 @@ def main():
             graph.replay()
             torch.cuda.synchronize()
             ms_graph = max_over_ranks(timed(graph.replay, 100))
-            sfb = flops_bytes(dfjk_inputs.CONFIGS[sname])
+            sfb = flops_bytes(frag if sname == "fragment" else dfjk_inputs.CONFIGS[sname])
             small[sname] = {"nao": sinp.nao, "naux": sinp.naux, "nocc": sinp.nocc, "l2": "L2-warm",
                             "launches_per_call": s_launches, "ms_direct": ms_direct, "ms_cuda_graph": ms_graph,
                             "k_tflops_graph": sfb["k"] / (ms_graph * 1e-3) * 1e-12}
