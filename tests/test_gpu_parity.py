@@ -99,7 +99,9 @@ def test_tiny_config_dispatch(torch_cuda, dfjk):
     (33, 9, [1] * 16 + [2] * 16, 173, dict(max_nset=32, max_nocc_total=48)),   # 32 sets
     (1, 2, [1], 174, {}),                                    # a single AO
     (64, 5, [64], 175, {}),                                  # nocc = nao, fewer aux rows than CTAs
-    (48, 300, [12], 176, {}),                                # ten aux rows per CTA
+    (48, 300, [12], 176, {}),                                # two aux rows per CTA: the second adds to the partials
+    (64, 700, [16, 5], 177, {}),                             # three aux rows per CTA, two sets, a ragged last tile of columns
+    (90, 310, [21], 178, {}),                                # nao not a multiple of 8: clamped rows in the 8 x 8 tiles
 ])
 def test_single_launch_path(torch_cuda, dfjk, nao, naux, nocc, seed, kw):
     """shapes inside the single-launch regime: J and K together, J alone, K alone, signed occupations,
